@@ -1,0 +1,14 @@
+"""CPU oracle (TEST INFRASTRUCTURE — see oracle/tpt_oracle.h).
+
+Importable only from tests/, __graft_entry__.smoke() and bench.py's cpu_baseline/--impl reference legs.
+"""
+from .binding import (  # noqa: F401
+    OraclePlan,
+    apply_operator_flux,
+    dense_solve_3d,
+    eig_1d,
+    num_threads,
+    operator_1d,
+    residual_norms,
+    symmetrize_1d,
+)
