@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the tensor-product–Thomas solver on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config c3|c4|c5|c2|c1]
+
+A "step" is one pass of the whole hot path (forward x, forward y, Thomas z, inverse y, inverse x) over one
+right-hand side of the workload: BASELINE.json's metric workload, config c3 = FP64 Poisson, 512^3 cells,
+tanh beta = 2 in all three directions, all-Neumann (singular), uniform[-1,1] rhs (seed 2) with its
+volume-weighted mean removed.  Prints ONE JSON line (rank 0).
+
+  value       whole-job Gpts/s with the rhs already resident in HBM (N>1: N independent replicas, §8(e))
+  e2e         the same metric through the C-ABI call tpt_solve_host with pinned HOST buffers (H2D + D2H inside)
+  roofline    dominant kernel (forward-x DMMA GEMM): algorithmic flops / CUDA-event duration vs FP64 peak
+  cpu_baseline the oracle (as it stands) timed on the host cores on a bounded z-slab sample of the workload
+  --impl reference  times the oracle alone (rank 0 only)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2603_09528_b200 import inputs as I  # noqa: E402
+
+METRIC = "FP64 stretched-grid Poisson solve Gpts/s at 512^3 (one tensor-product-Thomas solve per step)"
+UNIT = "Gpts/s"
+# FP64 peak of one B200: 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1.965 GHz; the DMMA and
+# DFMA microbenchmarks of the library are reported next to it.
+SM_COUNT, FP64_FMA_PER_CLK_SM = 148, 64
+ORACLE_SAMPLE_NZ = 64
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def _workload(name: str):
+    probs = I.CONFIGS[name]
+    return probs
+
+
+def _config_json(name: str, probs, extra=None):
+    P = probs[0]
+    cfg = {
+        "workload": f"BASELINE.json configs[{int(name[1]) - 1}] ({name}): " + ", ".join(p.name for p in probs),
+        "grid": list(P.n), "tanh_beta": list(P.beta), "bc": ["N" if b == 0 else "D" for b in P.bc],
+        "solves_per_step": len(probs), "helmholtz_alpha": [p.alpha for p in probs],
+        "points_per_step": sum(p.points for p in probs),
+        "cache": "each array (>= 1 GiB at 512^3) exceeds the 126 MB L2; no flush needed between steps",
+    }
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {
+        0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+        0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+        0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index = index
+        self.stop_flag = threading.Event()
+        self.sm, self.power, self.mask, self.sm_max = [], [], 0, None
+        self.ok = False
+
+    def run(self):
+        try:
+            import pynvml as nv
+
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            self.ok = True
+            while not self.stop_flag.is_set():
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                    self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                except Exception:
+                    pass
+                time.sleep(0.02)
+        except Exception:
+            self.ok = False
+
+    def summary(self):
+        if not self.ok or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["unavailable"]}
+        reasons = [n for b, n in self.REASONS.items() if self.mask & b and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.sm_max, "reasons": reasons,
+                "power_w_max": max(self.power) if self.power else None, "samples": len(self.sm)}
+
+
+BAD_REASONS = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+
+
+def _oracle_sample(probs, steps: int, warmup: int):
+    """Times the oracle's solve (plan excluded, like the GPU's) on a z-slab sample of each problem."""
+    import oracle   # test infrastructure; allowed here (cpu_baseline / --impl reference)
+
+    plans, rhs, pts = [], [], 0
+    for P in probs:
+        S = P.thin_z(min(ORACLE_SAMPLE_NZ, P.n[2]))
+        xf, yf, zf = S.faces()
+        plans.append(oracle.OraclePlan(xf, yf, zf, S.bc, S.alpha))
+        rhs.append(S.rhs())
+        pts += S.points
+    for _ in range(warmup):
+        for pl, f in zip(plans, rhs):
+            pl.solve(f)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        for pl, f in zip(plans, rhs):
+            pl.solve(f)
+    dt = (time.perf_counter() - t0) / steps
+    P = probs[0]
+    sample = (f"oracle solve on a z-slab of each problem: {P.n[0]}x{P.n[1]}x{min(ORACLE_SAMPLE_NZ, P.n[2])} cells "
+              f"(same x/y grids and eigenbases, {min(ORACLE_SAMPLE_NZ, P.n[2])}/{P.n[2]} of the points; per-point "
+              f"transform work identical); plan (eigendecomposition) excluded")
+    return {"value": pts / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample,
+            "ms_per_sample_step": dt * 1e3, "sample_points": pts}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    probs = _workload(args.config)
+    steps = max(1, min(args.steps, 5))
+    base = _oracle_sample(probs, steps, min(args.warmup, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": base["ms_per_sample_step"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": _config_json(args.config, probs, {"note": "CPU oracle on the host cores; a step is the bounded sample"}),
+        "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_gpu(args):
+    import torch
+
+    from paper_2603_09528_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        dist = dist_mod
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        torch.cuda.set_device(0)
+    dev_index = torch.cuda.current_device()
+    api.lib()   # fails loudly if the CUDA library is missing
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # replicas only (§8(e)): every rank solves its own copy of the workload (seed offset by rank)
+    probs = _workload(args.config)
+    plans, d_rhs, d_out, h_rhs = [], [], [], []
+    plan_cache = {}
+    for P in probs:
+        xf, yf, zf = P.faces()
+        key = (P.n, P.bc, P.alpha, P.beta, P.length)
+        if key not in plan_cache:
+            plan_cache[key] = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
+        plans.append(plan_cache[key])
+        import dataclasses
+
+        f = dataclasses.replace(P, seed=P.seed + 1000 * rank).rhs()
+        h_rhs.append(f)
+        d_rhs.append(torch.from_numpy(f).cuda())
+        d_out.append(torch.empty_like(d_rhs[-1]))
+    pts_step = sum(P.points for P in probs)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for pl, r, o in zip(plans, d_rhs, d_out):
+            api.solve(pl, r, o, stream)
+
+    def timed_region():
+        for _ in range(args.warmup):
+            step()
+        barrier()
+        sampler = ClockSampler(dev_index)
+        sampler.start()
+        for pl in plan_cache.values():
+            pl.set_profiling(True)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        ev[0].record(stream)
+        for s in range(args.steps):
+            step()
+            ev[s + 1].record(stream)
+        barrier()
+        sampler.stop_flag.set()
+        sampler.join()
+        total_ms = ev[0].elapsed_time(ev[-1])
+        per_step = sorted(ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps))
+        kt = {}
+        launches = 0
+        for key, pl in plan_cache.items():
+            ms, n_launch, n_solves = pl.kernel_times()
+            pl.set_profiling(False)
+            kt[key] = (ms, n_solves)
+            launches += n_launch
+        return total_ms, per_step, kt, launches, sampler.summary()
+
+    total_ms, per_step, kt, launches, clocks = timed_region()
+    if BAD_REASONS & set(clocks["reasons"]):          # rejected: re-measure once
+        total_ms, per_step, kt, launches, clocks = timed_region()
+        clocks["remeasured"] = True
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * pts_step * args.steps / (total_ms * 1e-3) / 1e9
+
+    # ---- e2e: the C-ABI call with pinned HOST buffers, copies inside the timed region
+    e2e_steps = max(1, min(args.steps, 5))
+    pin_in = [torch.from_numpy(f).pin_memory() for f in h_rhs]
+    pin_out = [torch.empty_like(t).pin_memory() for t in pin_in]
+    for pl, a, b in zip(plans, pin_in, pin_out):
+        api.solve_host(pl, a, b, stream)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        for pl, a, b in zip(plans, pin_in, pin_out):
+            api.solve_host(pl, a, b, stream)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = world * pts_step * e2e_steps / e2e_s / 1e9
+    e2e_ok = all(np.array_equal(b.numpy(), o.cpu().numpy()) for b, o in zip(pin_out, d_out))
+
+    if rank == 0:
+        peaks, peak_kind = _peaks()
+        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+        fp64_peak = SM_COUNT * FP64_FMA_PER_CLK_SM * 2 * sm_max * 1e6 / 1e12
+        dmma_meas, dfma_meas = api.fp64_peak(1), api.fp64_peak(0)
+        # per-kernel: mean event durations over the timed region (dominant plan = first)
+        key0 = next(iter(kt))
+        ms0, _ = kt[key0]
+        P0 = probs[0]
+        nx, ny, nz = P0.n
+        pts = P0.points
+        flops = {"fwd_x": 2.0 * nx * pts, "fwd_y": 2.0 * ny * pts, "inv_y": 2.0 * ny * pts, "inv_x": 2.0 * nx * pts}
+        kernels = {}
+        for slot, name in enumerate(api.KERNEL_NAMES):
+            entry = {"ms": ms0[slot]}
+            if name == "thomas":
+                gbs = 16.0 * pts / (ms0[slot] * 1e-3) / 1e9
+                entry.update({"bound": "hbm", "achieved_gbs_16B_per_pt": gbs, "frac_of_hbm_peak": gbs / peaks["hbm_gbs"]})
+            else:
+                tf = flops[name] / (ms0[slot] * 1e-3) / 1e12
+                entry.update({"bound": "tensor", "achieved_tflops": tf, "frac_of_fp64_peak": tf / fp64_peak})
+            kernels[name] = entry
+        dom = max(("fwd_x", "fwd_y", "inv_y", "inv_x"), key=lambda n: kernels[n]["ms"])
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(args.config, {}).get(dom)
+        roofline = {
+            "kernel": f"gemm_dmma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
+            "peak": fp64_peak, "unit": "TFLOP/s", "frac": kernels[dom]["achieved_tflops"] / fp64_peak, "traffic": traffic,
+            "peak_source": f"148 SMs x 64 FP64 FMA/clk x 2 x {sm_max:.0f} MHz ({peak_kind} sm_max_mhz); FP64 is absent from "
+                           "MEASURED_PEAKS.json",
+            "peak_measured_dmma_loop": dmma_meas, "peak_measured_dfma_loop": dfma_meas,
+            "frac_of_measured_dmma_loop": kernels[dom]["achieved_tflops"] / dmma_meas,
+            "algorithmic_flops_per_launch": flops[dom],
+        }
+        cpu = _oracle_sample(probs, 1, 1)
+        n20 = per_step[: min(20, len(per_step))]
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": _config_json(args.config, probs, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * pts_step, "d2h_bytes_per_step": 8 * pts_step,
+                    "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3, "matches_device_result": bool(e2e_ok)},
+            "gpu_launches": launches,
+            "roofline": roofline,
+            "kernels": kernels,
+            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "solve_ms_mean_20_fastest": float(np.mean(n20)) / len(probs), "solve_ms_min": per_step[0] / len(probs),
+            "hbm_peak_gbs": peaks["hbm_gbs"], "peaks": peak_kind,
+        }
+        print(json.dumps(line), flush=True)
+    for pl in plan_cache.values():
+        pl.destroy()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c3", choices=sorted(I.CONFIGS))
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,136 @@
+/*
+ * tpt.h — C ABI of the B200 (sm_100a) tensor-product–Thomas Poisson/Helmholtz solver.
+ *
+ * The library solves, in FP64 on one GPU,
+ *      T phi = f                  (Poisson,   helmholtz_alpha == 0)      PAPER.md:139, Eq. 7
+ *      (I - alpha T) u = f        (Helmholtz, helmholtz_alpha  > 0)      PAPER.md:68,  Eq. 2b
+ * with T = Tx (x) Iy (x) Iz + Ix (x) Ty (x) Iz + Ix (x) Iy (x) Tz the second-order finite-difference
+ * Laplacian of Eq. 3–4 on a staggered, non-uniform Cartesian grid, by the paper's
+ * tensor-product–Thomas procedure (steps 1.1–1.3 at plan time, 2.1–2.5 per solve).
+ *
+ * Conventions (all entry points):
+ *   - plain C, no torch types; every function returns a tpt status code (0 = TPT_OK) and never
+ *     throws or aborts across the ABI.  tpt_strerror() names a code.
+ *   - fields are FP64 arrays of nx*ny*nz elements, element (i,j,k) at  i + nx*(j + ny*k)
+ *     (x contiguous, z slowest — the paper's "leading dimension N_x").
+ *   - "HOST" / "DEVICE" below says where a pointer must live.  Device pointers must be 16-byte
+ *     aligned (any cudaMalloc / torch allocation is).
+ *   - the CUDA device is the one current at tpt_plan_create; the same device must be current in
+ *     later calls on that plan.  There is no CPU fallback: without a usable CUDA device
+ *     tpt_plan_create fails with TPT_ECUDA.
+ */
+#ifndef TPT_H
+#define TPT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tpt_plan tpt_plan; /* opaque */
+
+enum { TPT_BC_NEUMANN = 0, TPT_BC_DIRICHLET = 1 }; /* homogeneous, same at both ends of a direction */
+
+enum {
+    TPT_OK = 0,
+    TPT_EINVAL = -1,   /* bad argument (sizes, faces, bc, alpha, null/misaligned pointer) */
+    TPT_ENOMEM = -2,   /* host or device allocation failed */
+    TPT_ECUDA = -3,    /* CUDA runtime error (no device, launch failure, ...) */
+    TPT_ENUMERIC = -4  /* plan-time eigen-solver did not reach its accuracy rule */
+};
+
+/* Kernel slots, in execution order (used by tpt_plan_get_kernel_times / tpt_stage). */
+enum {
+    TPT_K_FWD_X = 0,  /* step 2.1, Eq. 10a */
+    TPT_K_FWD_Y = 1,  /* step 2.2, Eq. 10b */
+    TPT_K_THOMAS = 2, /* step 2.3, PAPER.md:183 (+ null-mode gauge) */
+    TPT_K_INV_Y = 3,  /* step 2.4, Eq. 12a */
+    TPT_K_INV_X = 4,  /* step 2.5, Eq. 12b */
+    TPT_K_COUNT = 5
+};
+
+/*
+ * tpt_plan_create — initialisation, steps 1.1–1.3.  Untimed, synchronous.
+ *   For x and y: build T_d (Eq. 3–4 with boundary rows), symmetrise T~ = D^{1/2} T D^{-1/2} (Eq. 5),
+ *   eigendecompose T~ = Q~ Lambda Q~^T on the host (implicit-shift QL + guarded factored-form
+ *   refinement), form the pre-scaled transform matrices Q^{-1} = Q~^T D^{1/2}, Q = D^{-1/2} Q~
+ *   (Eq. 6) and upload them; for z: the tridiagonal coefficients of T_z.
+ *   nx, ny, nz >= 2 cells.  xf, yf, zf: HOST, face coordinates, lengths nx+1, ny+1, nz+1, finite and
+ *   strictly increasing.  bc: HOST, {bc_x, bc_y, bc_z}.  helmholtz_alpha: 0 selects Poisson, > 0
+ *   Helmholtz; negative / non-finite is TPT_EINVAL.
+ *   All three bc Neumann with alpha == 0 gives a SINGULAR plan: tpt_solve then returns the solution
+ *   with zero cell-volume-weighted mean; following PAPER.md:219 the last z-equation of mode (0,0)
+ *   is replaced by "unknown = 0", so an incompatible rhs is not projected.
+ *   Ownership: the plan owns its device matrices, coefficient vectors and ONE field-sized
+ *   workspace (nx*ny*nz doubles).  *plan_out is untouched on failure.
+ */
+int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz,
+                    const double *xf, const double *yf, const double *zf,
+                    const int bc[3], double helmholtz_alpha);
+
+/*
+ * tpt_solve — steps 2.1–2.5: five kernels (+ one tiny gauge kernel on a singular
+ * plan) enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
+ * Asynchronous: returns after enqueueing; no host synchronisation, no allocation.
+ *   rhs_dev: DEVICE, nx*ny*nz doubles, read only (unless rhs_dev == out_dev, which is allowed).
+ *   out_dev: DEVICE, nx*ny*nz doubles, overwritten with phi (or u).
+ * A plan is not re-entrant (one workspace): order concurrent solves on one stream or use two plans.
+ */
+int tpt_solve(tpt_plan *plan, const double *rhs_dev, double *out_dev, void *cuda_stream);
+
+/*
+ * tpt_solve_host — the same solve for HOST buffers: copies rhs to the device (into a plan-owned
+ * staging field allocated on first use), runs tpt_solve, copies the result back and synchronises
+ * `cuda_stream` before returning.  rhs_host / out_host: HOST, nx*ny*nz doubles each (pinned memory
+ * makes the copies asynchronous and fast; pageable memory works).  May alias.
+ */
+int tpt_solve_host(tpt_plan *plan, const double *rhs_host, double *out_host, void *cuda_stream);
+
+/* tpt_plan_destroy — frees everything the plan owns (synchronises the device). NULL is a no-op. */
+int tpt_plan_destroy(tpt_plan *plan);
+
+/* ---- inspection / test entry points ------------------------------------------------------------ */
+
+/* Eigen-decomposition of direction dir (0 = x, 1 = y) as used by the plan: lambda_host[n]
+ * (descending, mode 0 smoothest) and qtilde_host[n*n] row-major, qtilde[i*n + m] = component i of
+ * mode m of the orthogonal Q~ (Eq. 5).  Either output may be NULL.  HOST pointers. */
+int tpt_plan_get_eigen(const tpt_plan *plan, int dir, double *lambda_host, double *qtilde_host);
+
+/* 1 if the plan is singular (all-Neumann Poisson), 0 if not, < 0 on error. */
+int tpt_plan_is_singular(const tpt_plan *plan);
+
+/* Bytes of device memory owned by the plan (matrices + vectors + workspace [+ staging]). */
+int tpt_plan_device_bytes(const tpt_plan *plan, size_t *bytes_out);
+
+/* Run ONE kernel slot (TPT_K_*) of the pipeline: in_dev -> out_dev (the Thomas slot works in place on
+ * out_dev after copying in_dev to it if they differ; it uses the plan workspace as scratch).
+ * For stage-by-stage comparison with the oracle.  DEVICE pointers, asynchronous on cuda_stream. */
+int tpt_stage(tpt_plan *plan, int slot, const double *in_dev, double *out_dev, void *cuda_stream);
+
+/* Per-kernel timing: while enabled, every tpt_solve brackets each kernel slot with CUDA events on the
+ * launching stream (no host synchronisation is added to the solve).  tpt_plan_get_kernel_times
+ * synchronises on the last profiled solve, returns the MEAN duration of each slot in milliseconds
+ * over the profiled solves since the previous read-out (ms_host[TPT_K_COUNT], HOST), the total
+ * number of kernel launches those solves made and how many solves they were, then resets the
+ * accumulation.  At most 4096 solves may accumulate between read-outs (TPT_EINVAL beyond). */
+int tpt_plan_set_profiling(tpt_plan *plan, int enabled);
+int tpt_plan_get_kernel_times(tpt_plan *plan, float *ms_host, int *launches_out, int *solves_out);
+
+/* Select the GEMM kernel for the transforms: 0 = generic FP64-FMA tile kernel (any shape),
+ * 1 = DMMA (mma.sync m8n8k4 f64) pipelined kernel where the shape allows (default).  For A/B
+ * measurement and tests; both are this library's own sm_100a kernels. */
+int tpt_plan_set_gemm_variant(tpt_plan *plan, int variant);
+
+/* FP64 arithmetic-pipe microbenchmarks used as roofline denominators: kind 0 = register-resident
+ * DFMA loop, kind 1 = register-resident DMMA (m8n8k4) loop.  Runs on the current device, returns
+ * achieved TFLOP/s (2 flop per FMA) in *tflops_out.  Synchronous. */
+int tpt_fp64_peak(int kind, double *tflops_out);
+
+const char *tpt_strerror(int status);
+const char *tpt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPT_H */

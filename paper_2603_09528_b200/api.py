@@ -1,0 +1,229 @@
+"""Thin ctypes binding of libtpt.so (include/tpt.h).  Argument marshalling only — every step of the
+solve runs in the library's CUDA kernels.  PyTorch is used for device memory and streams.
+
+    plan = plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha)
+    solve(plan, rhs, out)            # torch.float64 CUDA tensors of nx*ny*nz elements
+    plan_destroy(plan)
+
+Fails loudly (RuntimeError) if the library has not been built or a call returns a non-zero status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libtpt.so")
+
+NEUMANN, DIRICHLET = 0, 1
+K_FWD_X, K_FWD_Y, K_THOMAS, K_INV_Y, K_INV_X, K_COUNT = 0, 1, 2, 3, 4, 5
+KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")
+
+# every symbol include/tpt.h declares (tests check the library exports exactly these)
+SYMBOLS = (
+    "tpt_plan_create", "tpt_solve", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
+    "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
+    "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
+)
+
+_dp = C.POINTER(C.c_double)
+_lib = None
+
+
+class TptError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        super().__init__(f"{what}: status {status} ({strerror(status)})")
+
+
+def lib():
+    """Load libtpt.so.  No fallback: a missing library is an error."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2603_09528_b200.build` "
+                "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i, d = C.c_void_p, C.c_int, C.c_double
+        L.tpt_plan_create.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d]
+        L.tpt_solve.argtypes = [vp, vp, vp, vp]
+        L.tpt_solve_host.argtypes = [vp, vp, vp, vp]
+        L.tpt_plan_destroy.argtypes = [vp]
+        L.tpt_plan_get_eigen.argtypes = [vp, i, _dp, _dp]
+        L.tpt_plan_is_singular.argtypes = [vp]
+        L.tpt_plan_device_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+        L.tpt_stage.argtypes = [vp, i, vp, vp, vp]
+        L.tpt_plan_set_profiling.argtypes = [vp, i]
+        L.tpt_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i), C.POINTER(i)]
+        L.tpt_plan_set_gemm_variant.argtypes = [vp, i]
+        L.tpt_fp64_peak.argtypes = [i, _dp]
+        L.tpt_strerror.argtypes = [i]
+        L.tpt_strerror.restype = C.c_char_p
+        L.tpt_version.argtypes = []
+        L.tpt_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return lib().tpt_strerror(int(status)).decode()
+
+
+def version() -> str:
+    return lib().tpt_version().decode()
+
+
+def _check(status: int, what: str):
+    if status != 0:
+        raise TptError(status, what)
+
+
+def _faces(x):
+    a = np.ascontiguousarray(x, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def _stream_handle(stream) -> C.c_void_p:
+    if stream is None:
+        import torch
+
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+
+
+def _dev_ptr(t, count: int, what: str) -> C.c_void_p:
+    import torch
+
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+            and t.numel() == count):
+        raise ValueError(f"{what}: need a contiguous CUDA float64 tensor of {count} elements")
+    return C.c_void_p(t.data_ptr())
+
+
+class Plan:
+    """Handle of a tpt_plan.  Fields are float64 CUDA tensors of shape (nz, ny, nx) (x contiguous)."""
+
+    def __init__(self, handle, nx, ny, nz):
+        self._h = handle
+        self.nx, self.ny, self.nz = nx, ny, nz
+
+    @property
+    def shape(self):
+        return (self.nz, self.ny, self.nx)
+
+    @property
+    def points(self) -> int:
+        return self.nx * self.ny * self.nz
+
+    @property
+    def singular(self) -> bool:
+        r = lib().tpt_plan_is_singular(self._h)
+        if r < 0:
+            raise TptError(r, "tpt_plan_is_singular")
+        return bool(r)
+
+    def eigen(self, direction: int):
+        n = self.nx if direction == 0 else self.ny
+        lam, q = np.empty(n), np.empty((n, n))
+        _check(lib().tpt_plan_get_eigen(self._h, direction, lam.ctypes.data_as(_dp), q.ctypes.data_as(_dp)),
+               "tpt_plan_get_eigen")
+        return lam, q
+
+    def device_bytes(self) -> int:
+        b = C.c_size_t()
+        _check(lib().tpt_plan_device_bytes(self._h, C.byref(b)), "tpt_plan_device_bytes")
+        return int(b.value)
+
+    def solve(self, rhs, out, stream=None):
+        return solve(self, rhs, out, stream)
+
+    def solve_host(self, rhs_host, out_host, stream=None):
+        return solve_host(self, rhs_host, out_host, stream)
+
+    def stage(self, slot: int, inp, out, stream=None):
+        _check(lib().tpt_stage(self._h, slot, _dev_ptr(inp, self.points, "in"), _dev_ptr(out, self.points, "out"),
+                               _stream_handle(stream)), "tpt_stage")
+        return out
+
+    def set_profiling(self, enabled: bool):
+        _check(lib().tpt_plan_set_profiling(self._h, int(bool(enabled))), "tpt_plan_set_profiling")
+
+    def kernel_times(self):
+        """(mean ms per kernel slot [5], total launches, solves) over the profiled solves since the last
+        read-out; synchronises on the last of them and resets the accumulation."""
+        ms = (C.c_float * K_COUNT)()
+        n, k = C.c_int(), C.c_int()
+        _check(lib().tpt_plan_get_kernel_times(self._h, ms, C.byref(n), C.byref(k)), "tpt_plan_get_kernel_times")
+        return [float(v) for v in ms], int(n.value), int(k.value)
+
+    def set_gemm_variant(self, variant: int):
+        _check(lib().tpt_plan_set_gemm_variant(self._h, int(variant)), "tpt_plan_set_gemm_variant")
+
+    def destroy(self):
+        if self._h is not None:
+            h, self._h = self._h, None
+            _check(lib().tpt_plan_destroy(h), "tpt_plan_destroy")
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0) -> Plan:
+    xa, xp = _faces(xf)
+    ya, yp = _faces(yf)
+    za, zp = _faces(zf)
+    if (xa.size, ya.size, za.size) != (nx + 1, ny + 1, nz + 1):
+        raise ValueError("face arrays must have n+1 entries per direction")
+    bca = (C.c_int * 3)(*[int(b) for b in bc])
+    h = C.c_void_p()
+    _check(lib().tpt_plan_create(C.byref(h), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha)), "tpt_plan_create")
+    return Plan(h, nx, ny, nz)
+
+
+def solve(plan: Plan, rhs, out, stream=None):
+    """Enqueue one solve on `stream` (default: torch's current stream).  Asynchronous."""
+    _check(lib().tpt_solve(plan._h, _dev_ptr(rhs, plan.points, "rhs"), _dev_ptr(out, plan.points, "out"),
+                           _stream_handle(stream)), "tpt_solve")
+    return out
+
+
+def solve_host(plan: Plan, rhs_host, out_host, stream=None):
+    """Solve with HOST buffers (numpy float64 arrays or CPU torch tensors, ideally pinned)."""
+    def hp(a, what):
+        if isinstance(a, np.ndarray):
+            if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"] or a.size != plan.points:
+                raise ValueError(f"{what}: need a contiguous float64 array of {plan.points} elements")
+            return C.c_void_p(a.ctypes.data)
+        import torch
+
+        if not (isinstance(a, torch.Tensor) and not a.is_cuda and a.dtype == torch.float64 and a.is_contiguous()
+                and a.numel() == plan.points):
+            raise ValueError(f"{what}: need a contiguous CPU float64 tensor of {plan.points} elements")
+        return C.c_void_p(a.data_ptr())
+
+    _check(lib().tpt_solve_host(plan._h, hp(rhs_host, "rhs"), hp(out_host, "out"), _stream_handle(stream)),
+           "tpt_solve_host")
+    return out_host
+
+
+def plan_destroy(plan: Plan):
+    plan.destroy()
+
+
+def fp64_peak(kind: int) -> float:
+    """Measured FP64 pipe throughput in TFLOP/s: kind 0 = DFMA loop, 1 = DMMA loop."""
+    v = C.c_double()
+    _check(lib().tpt_fp64_peak(int(kind), C.byref(v)), "tpt_fp64_peak")
+    return float(v.value)

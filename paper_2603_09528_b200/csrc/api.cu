@@ -1,0 +1,362 @@
+// api.cu — the C ABI declared in include/tpt.h.  No torch types; plain pointers and sizes.
+#include "../../include/tpt.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "kernels.cuh"
+#include "plan_host.hpp"
+
+struct tpt_plan {
+    int nx = 0, ny = 0, nz = 0;
+    int bc[3] = {0, 0, 0};
+    double alpha = 0.0;
+    int singular = 0;
+    int device = 0;
+    double shift0 = 0.0;          // 0 (Poisson) or -1/alpha (Helmholtz, A5)
+    int gemm_variant = 1;
+    int profiling = 0;
+    int launches_last = 0;
+    std::vector<double> lamx, lamy, qx, qy;   // host copies (inspection)
+    // device: pre-scaled transform matrices, all row-major
+    double *d_xfwd = nullptr;   // [i][m]  = s * sqrt(wx_i) Q~x[i][m]      B-operand of step 2.1
+    double *d_xinv = nullptr;   // [m][i]  = Q~x[i][m] / sqrt(wx_i)         B-operand of step 2.5
+    double *d_yfwd = nullptr;   // [m][j]  = sqrt(wy_j) Q~y[j][m]           A-operand of step 2.2
+    double *d_yinv = nullptr;   // [j][m]  = Q~y[j][m] / sqrt(wy_j)         A-operand of step 2.4
+    double *d_vec = nullptr;    // lamx | lamy | az | bz | cz | wz
+    double *d_lamx = nullptr, *d_lamy = nullptr, *d_az = nullptr, *d_bz = nullptr, *d_cz = nullptr, *d_wz = nullptr;
+    double *d_work = nullptr;   // one field
+    double *d_stage = nullptr;  // staging field for tpt_solve_host (lazy)
+    // profiling: one set of TPT_K_COUNT+1 events per profiled solve since the last read-out
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;           // events handed out since the last read-out
+    long launches_accum = 0;
+    size_t points() const { return (size_t)nx * ny * nz; }
+};
+
+namespace {
+
+bool bc_valid(int b) { return b == TPT_BC_NEUMANN || b == TPT_BC_DIRICHLET; }
+
+void free_plan(tpt_plan *p) {
+    if (!p) return;
+    cudaFree(p->d_xfwd);
+    cudaFree(p->d_xinv);
+    cudaFree(p->d_yfwd);
+    cudaFree(p->d_yinv);
+    cudaFree(p->d_vec);
+    cudaFree(p->d_work);
+    cudaFree(p->d_stage);
+    for (auto &e : p->ev_pool) cudaEventDestroy(e);
+    delete p;
+}
+
+int upload(double **dst, const std::vector<double> &src) {
+    cudaError_t e = cudaMalloc(dst, src.size() * sizeof(double));
+    if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
+    e = cudaMemcpy(*dst, src.data(), src.size() * sizeof(double), cudaMemcpyHostToDevice);
+    return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *mat) {
+    // steps 2.1 / 2.5: all N_y*N_z lines at once, out[r][:] = in[r][:] * mat
+    tpt::GemmArgs g{};
+    g.A = in; g.B = mat; g.C = out;
+    g.M = p->ny * p->nz; g.N = p->nx; g.K = p->nx;
+    g.lda = p->nx; g.ldb = p->nx; g.ldc = p->nx;
+    g.strideA = g.strideB = g.strideC = 0;
+    g.batch = 1;
+    return g;
+}
+
+tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat) {
+    // steps 2.2 / 2.4: per z-plane, out_k = mat * in_k  (strided-batched, no transposes)
+    tpt::GemmArgs g{};
+    g.A = mat; g.B = in; g.C = out;
+    g.M = p->ny; g.N = p->nx; g.K = p->ny;
+    g.lda = p->ny; g.ldb = p->nx; g.ldc = p->nx;
+    g.strideA = 0; g.strideB = (int64_t)p->nx * p->ny; g.strideC = (int64_t)p->nx * p->ny;
+    g.batch = p->nz;
+    return g;
+}
+
+// Runs one slot; *launches incremented by the number of kernels enqueued.
+int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches) {
+    cudaError_t e = cudaSuccess;
+    switch (slot) {
+        case TPT_K_FWD_X: e = tpt::launch_gemm(gemm_x(p, in, out, p->d_xfwd), p->gemm_variant, st); ++*launches; break;
+        case TPT_K_INV_X: e = tpt::launch_gemm(gemm_x(p, in, out, p->d_xinv), p->gemm_variant, st); ++*launches; break;
+        case TPT_K_FWD_Y: e = tpt::launch_gemm(gemm_y(p, in, out, p->d_yfwd), p->gemm_variant, st); ++*launches; break;
+        case TPT_K_INV_Y: e = tpt::launch_gemm(gemm_y(p, in, out, p->d_yinv), p->gemm_variant, st); ++*launches; break;
+        case TPT_K_THOMAS:
+            // in place on `out`; the plan workspace holds c'
+            e = tpt::launch_thomas(out, p->d_work, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
+                                   p->shift0, p->singular, st);
+            ++*launches;
+            if (e == cudaSuccess && p->singular) {
+                e = tpt::launch_gauge(out, p->d_wz, p->nx, p->ny, p->nz, st);
+                ++*launches;
+            }
+            break;
+        default: return TPT_EINVAL;
+    }
+    return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+bool aligned16(const void *q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
+                    const double *zf, const int bc[3], double helmholtz_alpha) {
+    if (!plan_out || !bc) return TPT_EINVAL;
+    if (!tpt::faces_valid(nx, xf) || !tpt::faces_valid(ny, yf) || !tpt::faces_valid(nz, zf)) return TPT_EINVAL;
+    if (!bc_valid(bc[0]) || !bc_valid(bc[1]) || !bc_valid(bc[2])) return TPT_EINVAL;
+    if (!(helmholtz_alpha >= 0.0) || !std::isfinite(helmholtz_alpha)) return TPT_EINVAL;
+    if ((double)nx * ny * nz > 4.0e9) return TPT_EINVAL;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
+    int cc_major = 0;
+    if (cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return TPT_ECUDA;
+    }
+    if (cc_major != 10) return TPT_ECUDA;   // sm_100a binary only; no fallback
+
+    tpt_plan *p = new (std::nothrow) tpt_plan();
+    if (!p) return TPT_ENOMEM;
+    p->nx = nx; p->ny = ny; p->nz = nz;
+    p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
+    p->alpha = helmholtz_alpha;
+    p->device = dev;
+    p->singular = (helmholtz_alpha == 0.0 && bc[0] == TPT_BC_NEUMANN && bc[1] == TPT_BC_NEUMANN &&
+                   bc[2] == TPT_BC_NEUMANN) ? 1 : 0;
+    // Helmholtz (I - alpha T) u = f  <=>  (T - I/alpha) u = -f/alpha: same z kernel with a constant
+    // extra shift, the -1/alpha scale folded into the forward-x matrix ("constant shift").
+    const double rhs_scale = helmholtz_alpha > 0.0 ? -1.0 / helmholtz_alpha : 1.0;
+    p->shift0 = helmholtz_alpha > 0.0 ? -1.0 / helmholtz_alpha : 0.0;
+
+    int rc = TPT_OK;
+    try {
+        tpt::Operator1D ox, oy, oz;
+        tpt::build_operator(nx, xf, bc[0], ox);
+        tpt::build_operator(ny, yf, bc[1], oy);
+        tpt::build_operator(nz, zf, bc[2], oz);
+        if (tpt::eigen_decompose(ox, p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
+        if (rc == TPT_OK) {
+            bool same = (nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
+            if (same) { p->lamy = p->lamx; p->qy = p->qx; }
+            else if (tpt::eigen_decompose(oy, p->lamy, p->qy) != 0) rc = TPT_ENUMERIC;
+        }
+        if (rc == TPT_OK) {
+            std::vector<double> m((size_t)nx * nx);
+            for (int i = 0; i < nx; ++i) {
+                const double s = rhs_scale * std::sqrt(ox.w[i]);
+                for (int k = 0; k < nx; ++k) m[(size_t)i * nx + k] = s * p->qx[(size_t)i * nx + k];
+            }
+            rc = upload(&p->d_xfwd, m);
+            if (rc == TPT_OK) {
+                for (int i = 0; i < nx; ++i) {
+                    const double s = 1.0 / std::sqrt(ox.w[i]);
+                    for (int k = 0; k < nx; ++k) m[(size_t)k * nx + i] = s * p->qx[(size_t)i * nx + k];
+                }
+                rc = upload(&p->d_xinv, m);
+            }
+            m.assign((size_t)ny * ny, 0.0);
+            if (rc == TPT_OK) {
+                for (int j = 0; j < ny; ++j) {
+                    const double s = std::sqrt(oy.w[j]);
+                    for (int k = 0; k < ny; ++k) m[(size_t)k * ny + j] = s * p->qy[(size_t)j * ny + k];
+                }
+                rc = upload(&p->d_yfwd, m);
+            }
+            if (rc == TPT_OK) {
+                for (int j = 0; j < ny; ++j) {
+                    const double s = 1.0 / std::sqrt(oy.w[j]);
+                    for (int k = 0; k < ny; ++k) m[(size_t)j * ny + k] = s * p->qy[(size_t)j * ny + k];
+                }
+                rc = upload(&p->d_yinv, m);
+            }
+        }
+        if (rc == TPT_OK) {
+            std::vector<double> v;
+            v.reserve((size_t)nx + ny + 4 * (size_t)nz + 8);
+            auto pad2 = [&]() { if (v.size() & 1) v.push_back(0.0); };
+            size_t o_lamx = v.size(); v.insert(v.end(), p->lamx.begin(), p->lamx.end()); pad2();
+            size_t o_lamy = v.size(); v.insert(v.end(), p->lamy.begin(), p->lamy.end()); pad2();
+            size_t o_az = v.size(); v.insert(v.end(), oz.a.begin(), oz.a.end()); pad2();
+            size_t o_bz = v.size(); v.insert(v.end(), oz.b.begin(), oz.b.end()); pad2();
+            size_t o_cz = v.size(); v.insert(v.end(), oz.c.begin(), oz.c.end()); pad2();
+            size_t o_wz = v.size(); v.insert(v.end(), oz.w.begin(), oz.w.end()); pad2();
+            rc = upload(&p->d_vec, v);
+            p->d_lamx = p->d_vec + o_lamx; p->d_lamy = p->d_vec + o_lamy;
+            p->d_az = p->d_vec + o_az; p->d_bz = p->d_vec + o_bz; p->d_cz = p->d_vec + o_cz; p->d_wz = p->d_vec + o_wz;
+        }
+    } catch (const std::bad_alloc &) {
+        rc = TPT_ENOMEM;
+    } catch (...) {
+        rc = TPT_ECUDA;
+    }
+    if (rc == TPT_OK) {
+        cudaError_t e = cudaMalloc(&p->d_work, p->points() * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); rc = (e == cudaErrorMemoryAllocation) ? TPT_ENOMEM : TPT_ECUDA; }
+    }
+    if (rc == TPT_OK && tpt::gemm_configure() != cudaSuccess) { cudaGetLastError(); rc = TPT_ECUDA; }
+    if (rc != TPT_OK) { free_plan(p); return rc; }
+    *plan_out = p;
+    return TPT_OK;
+}
+
+int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_stream) {
+    if (!p || !rhs_dev || !out_dev || !aligned16(rhs_dev) || !aligned16(out_dev)) return TPT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0;
+    const bool prof = p->profiling != 0;
+    cudaEvent_t *ev = nullptr;
+    if (prof) {
+        const size_t need = p->ev_used + TPT_K_COUNT + 1;
+        if (need > 4096 * (TPT_K_COUNT + 1)) return TPT_EINVAL;   // read the times out first
+        try {
+            while (p->ev_pool.size() < need) {
+                cudaEvent_t e;
+                if (cudaEventCreate(&e) != cudaSuccess) return TPT_ECUDA;
+                p->ev_pool.push_back(e);
+            }
+        } catch (const std::bad_alloc &) { return TPT_ENOMEM; }
+        ev = p->ev_pool.data() + p->ev_used;
+        p->ev_used = need;
+    }
+    // rhs -> W -> out -> [Thomas in place on out, c' in W] -> W -> out
+    const double *ins[TPT_K_COUNT] = {rhs_dev, p->d_work, out_dev, out_dev, p->d_work};
+    double *outs[TPT_K_COUNT] = {p->d_work, out_dev, out_dev, p->d_work, out_dev};
+    if (prof && cudaEventRecord(ev[0], st) != cudaSuccess) return TPT_ECUDA;
+    for (int s = 0; s < TPT_K_COUNT; ++s) {
+        int rc = run_slot(p, s, ins[s], outs[s], st, &launches);
+        if (rc != TPT_OK) return rc;
+        if (prof && cudaEventRecord(ev[s + 1], st) != cudaSuccess) return TPT_ECUDA;
+    }
+    p->launches_last = launches;
+    if (prof) p->launches_accum += launches;
+    return TPT_OK;
+}
+
+int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *cuda_stream) {
+    if (!p || !rhs_host || !out_host) return TPT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t bytes = p->points() * sizeof(double);
+    if (!p->d_stage) {
+        cudaError_t e = cudaMalloc(&p->d_stage, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); p->d_stage = nullptr; return e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
+    }
+    if (cudaMemcpyAsync(p->d_stage, rhs_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TPT_ECUDA;
+    int rc = tpt_solve(p, p->d_stage, p->d_stage, st);
+    if (rc != TPT_OK) return rc;
+    if (cudaMemcpyAsync(out_host, p->d_stage, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TPT_ECUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+int tpt_plan_destroy(tpt_plan *p) {
+    if (!p) return TPT_OK;
+    cudaError_t e = cudaDeviceSynchronize();
+    free_plan(p);
+    return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+int tpt_plan_get_eigen(const tpt_plan *p, int dir, double *lambda_host, double *qtilde_host) {
+    if (!p || (dir != 0 && dir != 1)) return TPT_EINVAL;
+    const std::vector<double> &l = dir == 0 ? p->lamx : p->lamy;
+    const std::vector<double> &q = dir == 0 ? p->qx : p->qy;
+    if (lambda_host) std::memcpy(lambda_host, l.data(), l.size() * sizeof(double));
+    if (qtilde_host) std::memcpy(qtilde_host, q.data(), q.size() * sizeof(double));
+    return TPT_OK;
+}
+
+int tpt_plan_is_singular(const tpt_plan *p) { return p ? p->singular : TPT_EINVAL; }
+
+int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
+    if (!p || !bytes_out) return TPT_EINVAL;
+    size_t b = 2 * ((size_t)p->nx * p->nx + (size_t)p->ny * p->ny) * sizeof(double);
+    b += ((size_t)p->nx + p->ny + 4 * (size_t)p->nz + 8) * sizeof(double);
+    b += p->points() * sizeof(double) * (p->d_stage ? 2 : 1);
+    *bytes_out = b;
+    return TPT_OK;
+}
+
+int tpt_stage(tpt_plan *p, int slot, const double *in_dev, double *out_dev, void *cuda_stream) {
+    if (!p || !in_dev || !out_dev || slot < 0 || slot >= TPT_K_COUNT) return TPT_EINVAL;
+    if (!aligned16(in_dev) || !aligned16(out_dev)) return TPT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0;
+    if (slot == TPT_K_THOMAS) {
+        if (in_dev != out_dev &&
+            cudaMemcpyAsync(out_dev, in_dev, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+            return TPT_ECUDA;
+    } else if (in_dev == out_dev) {
+        return TPT_EINVAL;   // the transforms are out of place
+    }
+    return run_slot(p, slot, in_dev, out_dev, st, &launches);
+}
+
+int tpt_plan_set_profiling(tpt_plan *p, int enabled) {
+    if (!p) return TPT_EINVAL;
+    p->profiling = enabled ? 1 : 0;
+    return TPT_OK;
+}
+
+int tpt_plan_get_kernel_times(tpt_plan *p, float *ms_host, int *launches_out, int *solves_out) {
+    if (!p || !ms_host) return TPT_EINVAL;
+    const size_t per = TPT_K_COUNT + 1;
+    const size_t solves = p->ev_used / per;
+    if (solves == 0) return TPT_EINVAL;
+    if (cudaEventSynchronize(p->ev_pool[p->ev_used - 1]) != cudaSuccess) return TPT_ECUDA;
+    double sum[TPT_K_COUNT] = {0, 0, 0, 0, 0};
+    for (size_t q = 0; q < solves; ++q)
+        for (int s = 0; s < TPT_K_COUNT; ++s) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, p->ev_pool[q * per + s], p->ev_pool[q * per + s + 1]) != cudaSuccess)
+                return TPT_ECUDA;
+            sum[s] += ms;
+        }
+    for (int s = 0; s < TPT_K_COUNT; ++s) ms_host[s] = (float)(sum[s] / (double)solves);
+    if (launches_out) *launches_out = (int)p->launches_accum;
+    if (solves_out) *solves_out = (int)solves;
+    p->ev_used = 0;
+    p->launches_accum = 0;
+    return TPT_OK;
+}
+
+int tpt_plan_set_gemm_variant(tpt_plan *p, int variant) {
+    if (!p || (variant != 0 && variant != 1)) return TPT_EINVAL;
+    p->gemm_variant = variant;
+    return TPT_OK;
+}
+
+int tpt_fp64_peak(int kind, double *tflops_out) {
+    if (!tflops_out || (kind != 0 && kind != 1)) return TPT_EINVAL;
+    cudaError_t e = tpt::run_fp64_peak(kind, tflops_out);
+    if (e != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
+    return TPT_OK;
+}
+
+const char *tpt_strerror(int status) {
+    switch (status) {
+        case TPT_OK: return "ok";
+        case TPT_EINVAL: return "invalid argument";
+        case TPT_ENOMEM: return "out of memory";
+        case TPT_ECUDA: return "CUDA error (no sm_100 device, or a runtime/launch failure)";
+        case TPT_ENUMERIC: return "plan-time eigen-decomposition missed its accuracy rule";
+        default: return "unknown status";
+    }
+}
+
+const char *tpt_version(void) { return "tpt 0.1 (sm_100a)"; }
+
+}  // extern "C"

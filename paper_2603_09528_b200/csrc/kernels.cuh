@@ -1,0 +1,41 @@
+// kernels.cuh — launch wrappers of the sm_100a kernels (definitions in kernels.cu).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+namespace tpt {
+
+// Row-major batched GEMM  C[b] = A[b] * B[b],  A: M x K (lda), B: K x N (ldb), C: M x N (ldc),
+// batch strides in elements (0 = operand shared by all batches).
+struct GemmArgs {
+    const double *A;
+    const double *B;
+    double *C;
+    int M, N, K;
+    int64_t lda, ldb, ldc;
+    int64_t strideA, strideB, strideC;
+    int batch;
+};
+
+// variant 0: generic FP64-FMA tile kernel, any shape.  variant 1: DMMA pipelined kernel when the
+// shape allows (falls back to the generic kernel otherwise).  Returns the launch's cudaError_t.
+cudaError_t launch_gemm(const GemmArgs &g, int variant, cudaStream_t stream);
+bool gemm_dmma_supported(const GemmArgs &g);
+cudaError_t gemm_configure();   // one-time cudaFuncSetAttribute for the dynamic-smem kernels
+
+// z sweep (step 2.3): in place on x (nx*ny*nz), cprime = field-sized scratch.
+// Solves (T_z + (lamx[i] + lamy[j] + shift0) I) x = rhs for each column; on a singular plan the
+// column (0,0) gets "last unknown = 0".
+cudaError_t launch_thomas(double *x, double *cprime, const double *az, const double *bz, const double *cz,
+                          const double *lamx, const double *lamy, int nx, int ny, int nz, double shift0,
+                          int singular, cudaStream_t stream);
+
+// Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean).
+cudaError_t launch_gauge(double *x, const double *wz, int nx, int ny, int nz, cudaStream_t stream);
+
+// FP64 pipe microbenchmarks (kind 0: DFMA, 1: DMMA).  Returns TFLOP/s.
+cudaError_t run_fp64_peak(int kind, double *tflops);
+
+}  // namespace tpt

@@ -1,0 +1,269 @@
+// plan_host.cpp — see plan_host.hpp.  Host-only C++ (compiled by nvcc's host compiler).
+#include "plan_host.hpp"
+
+#include <algorithm>
+#include <cfloat>
+#include <cmath>
+#include <cstddef>
+#include <numeric>
+
+namespace tpt {
+
+bool faces_valid(int n, const double *xf) {
+    if (n < 2 || xf == nullptr) return false;
+    for (int i = 0; i <= n; ++i)
+        if (!std::isfinite(xf[i])) return false;
+    for (int i = 0; i < n; ++i)
+        if (!(xf[i + 1] > xf[i])) return false;
+    return true;
+}
+
+// Eq. 3: (1/w_i) [ (phi_{i+1}-phi_i)/delta_{i+1} - (phi_i-phi_{i-1})/delta_i ].
+// Face-first reading: unknowns sit at the midpoints of the given faces, so the distance between
+// neighbouring unknowns across face i is half the sum of the two adjacent widths; at a boundary
+// the mirror ghost cell gives delta = w of the boundary cell.  Neumann: ghost = +phi (row loses its
+// outward coupling); Dirichlet at the face: ghost = -phi (outward coupling doubles onto the diagonal).
+void build_operator(int n, const double *xf, int bc, Operator1D &op) {
+    op.n = n;
+    op.bc = bc;
+    op.w.resize(n);
+    op.delta.resize(n + 1);
+    op.a.assign(n, 0.0);
+    op.b.assign(n, 0.0);
+    op.c.assign(n, 0.0);
+    for (int i = 0; i < n; ++i) op.w[i] = xf[i + 1] - xf[i];
+    for (int i = 1; i < n; ++i) op.delta[i] = 0.5 * (xf[i + 1] - xf[i - 1]);
+    op.delta[0] = op.w[0];
+    op.delta[n] = op.w[n - 1];
+    for (int i = 0; i < n; ++i) {
+        const double lo = 1.0 / (op.w[i] * op.delta[i]);      // coupling through the lower face
+        const double hi = 1.0 / (op.w[i] * op.delta[i + 1]);  // coupling through the upper face
+        double diag = 0.0;
+        if (i > 0) { op.a[i] = lo; diag -= lo; }
+        else if (bc == 1) diag -= 2.0 * lo;                   // Dirichlet ghost
+        if (i < n - 1) { op.c[i] = hi; diag -= hi; }
+        else if (bc == 1) diag -= 2.0 * hi;
+        op.b[i] = diag;
+    }
+}
+
+namespace {
+
+// Implicit-shift QL iteration on a symmetric tridiagonal matrix (diagonal d, off-diagonal e with
+// e[i] coupling i and i+1), accumulating the rotations into zt (rows of zt = eigenvectors).
+// The classical EISPACK tql2 scheme restated; deflation test is the local relative one,
+// |e_m| <= eps (|d_m| + |d_{m+1}|).
+int ql_implicit(int n, std::vector<double> &d, std::vector<double> &e, std::vector<double> &zt) {
+    e.resize(n, 0.0);
+    e[n - 1] = 0.0;
+    for (int l = 0; l < n; ++l) {
+        int iter = 0;
+        int m;
+        do {
+            for (m = l; m < n - 1; ++m) {
+                const double dd = std::fabs(d[m]) + std::fabs(d[m + 1]);
+                if (std::fabs(e[m]) <= DBL_EPSILON * dd) break;
+            }
+            if (m != l) {
+                if (iter++ == 80) return -1;
+                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                double r = std::hypot(g, 1.0);
+                g = d[m] - d[l] + e[l] / (g + std::copysign(r, g));
+                double s = 1.0, c = 1.0, p = 0.0;
+                int i;
+                for (i = m - 1; i >= l; --i) {
+                    double f = s * e[i];
+                    const double bb = c * e[i];
+                    r = std::hypot(f, g);
+                    e[i + 1] = r;
+                    if (r == 0.0) {
+                        d[i + 1] -= p;
+                        e[m] = 0.0;
+                        break;
+                    }
+                    s = f / r;
+                    c = g / r;
+                    g = d[i + 1] - p;
+                    r = (d[i] - g) * s + 2.0 * c * bb;
+                    p = s * r;
+                    d[i + 1] = g + p;
+                    g = c * r - bb;
+                    double *zi = &zt[(size_t)i * n];
+                    double *zj = &zt[(size_t)(i + 1) * n];
+                    for (int k = 0; k < n; ++k) {
+                        f = zj[k];
+                        zj[k] = s * zi[k] + c * f;
+                        zi[k] = c * zi[k] - s * f;
+                    }
+                }
+                if (r == 0.0 && i >= l) continue;
+                d[l] -= p;
+                e[l] = g;
+                e[m] = 0.0;
+            }
+        } while (m != l);
+    }
+    return 0;
+}
+
+// Y = B X where -T~ = B^T B is the flux factorisation: one row per face that carries a flux.
+// X, Y row-major with n columns.  Returns the number of rows of Y.
+int apply_flux_factor(const Operator1D &op, const std::vector<double> &X, std::vector<double> &Y) {
+    const int n = op.n;
+    std::vector<double> isw(n);
+    for (int i = 0; i < n; ++i) isw[i] = 1.0 / std::sqrt(op.w[i]);
+    int rows = 0;
+    auto boundary_row = [&](int cell) {
+        const double s = std::sqrt(2.0) / op.w[cell];
+        for (int m = 0; m < n; ++m) Y[(size_t)rows * n + m] = s * X[(size_t)cell * n + m];
+        ++rows;
+    };
+    if (op.bc == 1) boundary_row(0);
+    for (int f = 1; f < n; ++f) {
+        const double isd = 1.0 / std::sqrt(op.delta[f]);
+        const double up = isw[f] * isd, dn = isw[f - 1] * isd;
+        const double *xu = &X[(size_t)f * n], *xd = &X[(size_t)(f - 1) * n];
+        double *y = &Y[(size_t)rows * n];
+        for (int m = 0; m < n; ++m) y[m] = xu[m] * up - xd[m] * dn;
+        ++rows;
+    }
+    if (op.bc == 1) boundary_row(n - 1);
+    return rows;
+}
+
+// G = P^T P, P is rows x n row-major.
+void gram_matrix(int rows, int n, const std::vector<double> &P, std::vector<double> &G) {
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < n; ++i) {
+        double *g = &G[(size_t)i * n];
+        std::fill(g, g + n, 0.0);
+        for (int r = 0; r < rows; ++r) {
+            const double *p = &P[(size_t)r * n];
+            const double t = p[i];
+            for (int j = 0; j < n; ++j) g[j] += t * p[j];
+        }
+    }
+}
+
+struct RefineState {
+    double orth_defect;   // ||I - X^T X||_F
+    double corr_norm;     // ||E||_F
+};
+
+// One Ogita–Aishima evaluation in factored form: fills lam (Rayleigh
+// quotients -||B x_i||^2/||x_i||^2) and E (correction; X <- X + X E).  Pairs whose eigenvalues agree
+// to within tau*max|lambda| are treated as a cluster (E_ij = R_ij/2: re-orthogonalise only).
+RefineState refine_evaluate(const Operator1D &op, const std::vector<double> &X, std::vector<double> &Y,
+                            std::vector<double> &S, std::vector<double> &E, std::vector<double> &lam) {
+    const int n = op.n;
+    const int rows = apply_flux_factor(op, X, Y);
+    gram_matrix(rows, n, Y, S);   // S = (BX)^T (BX) = -X^T T~ X
+    gram_matrix(n, n, X, E);      // E = X^T X for now
+    for (int i = 0; i < n; ++i) lam[i] = -S[(size_t)i * n + i] / E[(size_t)i * n + i];
+    const double tau = 1e6 * n * DBL_EPSILON;
+    double sumR = 0.0, sumE = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : sumR, sumE)
+    for (int i = 0; i < n; ++i) {
+        for (int j = 0; j < n; ++j) {
+            const double rij = (i == j ? 1.0 : 0.0) - E[(size_t)i * n + j];
+            const double sij = -S[(size_t)i * n + j];
+            const double scale = std::max(std::fabs(lam[i]), std::fabs(lam[j]));
+            const double gap = lam[j] - lam[i];
+            double eij;
+            if (i != j && std::fabs(gap) > tau * scale) eij = (sij + lam[j] * rij) / gap;
+            else eij = 0.5 * rij;
+            E[(size_t)i * n + j] = eij;
+            sumR += rij * rij;
+            sumE += eij * eij;
+        }
+    }
+    return {std::sqrt(sumR), std::sqrt(sumE)};
+}
+
+void refine_apply(int n, const std::vector<double> &X, const std::vector<double> &E, std::vector<double> &Xn) {
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < n; ++r) {
+        const double *x = &X[(size_t)r * n];
+        double *o = &Xn[(size_t)r * n];
+        std::copy(x, x + n, o);
+        for (int i = 0; i < n; ++i) {
+            const double t = x[i];
+            const double *e = &E[(size_t)i * n];
+            for (int j = 0; j < n; ++j) o[j] += t * e[j];
+        }
+    }
+}
+
+}  // namespace
+
+int eigen_decompose(const Operator1D &op, std::vector<double> &lambda, std::vector<double> &q) {
+    const int n = op.n;
+    const size_t nn = (size_t)n * n;
+    // Step 1.1: T~ = D^{1/2} T D^{-1/2}: diagonal b_i, off-diagonal sqrt(c_i a_{i+1}).
+    std::vector<double> d(op.b), e(n, 0.0);
+    for (int i = 0; i + 1 < n; ++i) e[i] = std::sqrt(op.c[i] * op.a[i + 1]);
+    // Step 1.2: base solver.
+    std::vector<double> zt(nn, 0.0);
+    for (int i = 0; i < n; ++i) zt[(size_t)i * n + i] = 1.0;
+    if (ql_implicit(n, d, e, zt) != 0) return -1;
+    std::vector<double> X(nn), Xprev, Y((size_t)(n + 1) * n), S(nn), E(nn), lam(n), lamprev(n);
+    for (int m = 0; m < n; ++m)
+        for (int i = 0; i < n; ++i) X[(size_t)i * n + m] = zt[(size_t)m * n + i];
+    zt.clear();
+    zt.shrink_to_fit();
+    // Accuracy rule: two guarded refinement steps; an update that worsens orthogonality (above
+    // rounding level) is undone.
+    const int steps = 2;
+    double prev_defect = HUGE_VAL;
+    RefineState st{};
+    for (int step = 0;; ++step) {
+        st = refine_evaluate(op, X, Y, S, E, lam);
+        if (step > 0 && !(st.orth_defect <= prev_defect || st.orth_defect <= 1e-12 * n)) {
+            X.swap(Xprev);
+            lam = lamprev;
+            st.orth_defect = prev_defect;
+            break;
+        }
+        if (step == steps) break;
+        lamprev = lam;
+        Xprev.resize(nn);
+        refine_apply(n, X, E, Xprev);
+        X.swap(Xprev);   // X = refined, Xprev = previous
+        prev_defect = st.orth_defect;
+    }
+    if (!(st.orth_defect <= 1e-11 * n)) return -2;
+
+    // Order descending (mode 0 = smoothest), normalise columns.
+    std::vector<int> order(n);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return lam[x] > lam[y]; });
+    lambda.resize(n);
+    q.resize(nn);
+    for (int m = 0; m < n; ++m) {
+        const int src = order[m];
+        lambda[m] = lam[src];
+        double nrm = 0.0;
+        for (int i = 0; i < n; ++i) nrm += X[(size_t)i * n + src] * X[(size_t)i * n + src];
+        nrm = 1.0 / std::sqrt(nrm);
+        for (int i = 0; i < n; ++i) q[(size_t)i * n + m] = X[(size_t)i * n + src] * nrm;
+    }
+    const double L = std::accumulate(op.w.begin(), op.w.end(), 0.0);
+    if (op.bc == 0) {   // Neumann–Neumann: exact null pair (T 1 = 0 => T~ D^{1/2} 1 = 0)
+        lambda[0] = 0.0;
+        for (int i = 0; i < n; ++i) q[(size_t)i * n] = std::sqrt(op.w[i] / L);
+    }
+    for (int m = 0; m < n; ++m) {   // sign convention
+        double s = 0.0;
+        for (int i = 0; i < n; ++i) s += q[(size_t)i * n + m] * std::sqrt(op.w[i]);
+        bool flip = false;
+        if (std::fabs(s) > 1e-8 * std::sqrt(L)) flip = s < 0.0;
+        else
+            for (int i = 0; i < n; ++i)
+                if (std::fabs(q[(size_t)i * n + m]) > 1e-8) { flip = q[(size_t)i * n + m] < 0.0; break; }
+        if (flip)
+            for (int i = 0; i < n; ++i) q[(size_t)i * n + m] = -q[(size_t)i * n + m];
+    }
+    return 0;
+}
+
+}  // namespace tpt
