@@ -122,6 +122,11 @@ int tpt_plan_get_kernel_times(tpt_plan *plan, float *ms_host, int *launches_out,
  * measurement and tests; both are this library's own sm_100a kernels. */
 int tpt_plan_set_gemm_variant(tpt_plan *plan, int variant);
 
+/* Select the z-sweep kernel: 1 = on-chip partitioned Thomas kernel (column tiles resident in shared memory,
+ * 16 B/pt of HBM traffic; used where nx*ny % 16 == 0 and nz <= 768, default), 0 = streaming one-thread-per-column
+ * kernel that spills c' to the plan workspace (any shape).  Both solve step 2.3 exactly. */
+int tpt_plan_set_thomas_variant(tpt_plan *plan, int variant);
+
 /* FP64 arithmetic-pipe microbenchmarks used as roofline denominators: kind 0 = register-resident
  * DFMA loop, kind 1 = register-resident DMMA (m8n8k4) loop.  Runs on the current device, returns
  * achieved TFLOP/s (2 flop per FMA) in *tflops_out.  Synchronous. */

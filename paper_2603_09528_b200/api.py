@@ -25,7 +25,7 @@ KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")
 SYMBOLS = (
     "tpt_plan_create", "tpt_solve", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
-    "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
+    "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -59,6 +59,7 @@ def lib():
         L.tpt_plan_set_profiling.argtypes = [vp, i]
         L.tpt_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i), C.POINTER(i)]
         L.tpt_plan_set_gemm_variant.argtypes = [vp, i]
+        L.tpt_plan_set_thomas_variant.argtypes = [vp, i]
         L.tpt_fp64_peak.argtypes = [i, _dp]
         L.tpt_strerror.argtypes = [i]
         L.tpt_strerror.restype = C.c_char_p
@@ -161,6 +162,9 @@ class Plan:
 
     def set_gemm_variant(self, variant: int):
         _check(lib().tpt_plan_set_gemm_variant(self._h, int(variant)), "tpt_plan_set_gemm_variant")
+
+    def set_thomas_variant(self, variant: int):
+        _check(lib().tpt_plan_set_thomas_variant(self._h, int(variant)), "tpt_plan_set_thomas_variant")
 
     def destroy(self):
         if self._h is not None:

@@ -20,6 +20,8 @@ struct tpt_plan {
     int device = 0;
     double shift0 = 0.0;          // 0 (Poisson) or -1/alpha (Helmholtz, A5)
     int gemm_variant = 1;
+    int thomas_variant = 1;       // 1 = on-chip partitioned kernel where supported, 0 = streaming kernel
+    int sms = 0;
     int profiling = 0;
     int launches_last = 0;
     std::vector<double> lamx, lamy, qx, qy;   // host copies (inspection)
@@ -29,6 +31,7 @@ struct tpt_plan {
     double *d_yfwd = nullptr;   // [m][j]  = sqrt(wy_j) Q~y[j][m]           A-operand of step 2.2
     double *d_yinv = nullptr;   // [j][m]  = Q~y[j][m] / sqrt(wy_j)         A-operand of step 2.4
     double *d_vec = nullptr;    // lamx | lamy | az | bz | cz | wz
+    double *d_abc = nullptr;    // [a,b,c,0] per z row, identity-padded to nz + 64 rows (on-chip Thomas kernel)
     double *d_lamx = nullptr, *d_lamy = nullptr, *d_az = nullptr, *d_bz = nullptr, *d_cz = nullptr, *d_wz = nullptr;
     double *d_work = nullptr;   // one field
     double *d_stage = nullptr;  // staging field for tpt_solve_host (lazy)
@@ -50,6 +53,7 @@ void free_plan(tpt_plan *p) {
     cudaFree(p->d_yfwd);
     cudaFree(p->d_yinv);
     cudaFree(p->d_vec);
+    cudaFree(p->d_abc);
     cudaFree(p->d_work);
     cudaFree(p->d_stage);
     for (auto &e : p->ev_pool) cudaEventDestroy(e);
@@ -94,9 +98,12 @@ int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t 
         case TPT_K_FWD_Y: e = tpt::launch_gemm(gemm_y(p, in, out, p->d_yfwd), p->gemm_variant, st); ++*launches; break;
         case TPT_K_INV_Y: e = tpt::launch_gemm(gemm_y(p, in, out, p->d_yinv), p->gemm_variant, st); ++*launches; break;
         case TPT_K_THOMAS:
-            // in place on `out`; the plan workspace holds c'
-            e = tpt::launch_thomas(out, p->d_work, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
-                                   p->shift0, p->singular, st);
+            if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz))
+                e = tpt::launch_thomas_onchip(out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
+                                              p->singular, p->sms, st);
+            else   // streaming kernel: in place on `out`; the plan workspace holds c'
+                e = tpt::launch_thomas(out, p->d_work, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny,
+                                       p->nz, p->shift0, p->singular, st);
             ++*launches;
             if (e == cudaSuccess && p->singular) {
                 e = tpt::launch_gauge(out, p->d_wz, p->nx, p->ny, p->nz, st);
@@ -130,6 +137,11 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
         return TPT_ECUDA;
     }
     if (cc_major != 10) return TPT_ECUDA;   // sm_100a binary only; no fallback
+    int sm_count = 0;
+    if (cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sm_count < 1) {
+        cudaGetLastError();
+        return TPT_ECUDA;
+    }
 
     tpt_plan *p = new (std::nothrow) tpt_plan();
     if (!p) return TPT_ENOMEM;
@@ -137,6 +149,7 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
     p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
     p->alpha = helmholtz_alpha;
     p->device = dev;
+    p->sms = sm_count;
     p->singular = (helmholtz_alpha == 0.0 && bc[0] == TPT_BC_NEUMANN && bc[1] == TPT_BC_NEUMANN &&
                    bc[2] == TPT_BC_NEUMANN) ? 1 : 0;
     // Helmholtz (I - alpha T) u = f  <=>  (T - I/alpha) u = -f/alpha: same z kernel with a constant
@@ -199,6 +212,12 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
             rc = upload(&p->d_vec, v);
             p->d_lamx = p->d_vec + o_lamx; p->d_lamy = p->d_vec + o_lamy;
             p->d_az = p->d_vec + o_az; p->d_bz = p->d_vec + o_bz; p->d_cz = p->d_vec + o_cz; p->d_wz = p->d_vec + o_wz;
+        }
+        if (rc == TPT_OK) {
+            std::vector<double> t(4 * ((size_t)nz + 64), 0.0);
+            for (size_t k = 0; k < (size_t)nz + 64; ++k) t[4 * k + 1] = 1.0;
+            for (int k = 0; k < nz; ++k) { t[4 * k] = oz.a[k]; t[4 * k + 1] = oz.b[k]; t[4 * k + 2] = oz.c[k]; }
+            rc = upload(&p->d_abc, t);
         }
     } catch (const std::bad_alloc &) {
         rc = TPT_ENOMEM;
@@ -336,6 +355,12 @@ int tpt_plan_get_kernel_times(tpt_plan *p, float *ms_host, int *launches_out, in
 int tpt_plan_set_gemm_variant(tpt_plan *p, int variant) {
     if (!p || (variant != 0 && variant != 1)) return TPT_EINVAL;
     p->gemm_variant = variant;
+    return TPT_OK;
+}
+
+int tpt_plan_set_thomas_variant(tpt_plan *p, int variant) {
+    if (!p || (variant != 0 && variant != 1)) return TPT_EINVAL;
+    p->thomas_variant = variant;
     return TPT_OK;
 }
 

@@ -9,30 +9,16 @@
 //   thomas_kernel        step 2.3: one thread per (kx,ky) column, coalesced along x.
 //   gauge_kernel         null-mode gauge of a singular plan (A7).
 #include "kernels.cuh"
+#include "ptx.cuh"
 
 #include <cstdio>
 
 namespace tpt {
 
-// ------------------------------------------------------------------------------------------------
-// small PTX helpers
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
-}
-// D(8x8) += A(8x4, row) * B(4x8, col), FP64.  Fragment ownership (lane = 4*g + t):
-//   a = A[g][t],  b = B[t][g],  {c0,c1} = C[g][2t], C[g][2t+1].
-__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-        : "+d"(c0), "+d"(c1)
-        : "d"(a), "d"(b));
-}
+using ptx::cp_async16;
+using ptx::cp_async_commit;
+using ptx::cp_async_wait;
+using ptx::dmma884;
 
 // ------------------------------------------------------------------------------------------------
 // DMMA GEMM.  CTA tile BM x BN, k-slab BK = 16, warp tile WM x WN made of (WM/8) x (WN/8) m8n8k4 tiles.

@@ -170,6 +170,46 @@ def test_stage_by_stage_against_oracle(tpt, torch, orc, alpha):
     plan.destroy()
 
 
+THOMAS_SHAPES = [
+    # nx, ny, nz, bc_z, alpha, singular?      on-chip kernel configuration it exercises
+    (32, 16, 16, D_, 0.0),       # M = 8, S = 2
+    (64, 32, 50, N_, 0.0),       # M = 8, ragged last segment, S = 8 (padded), singular
+    (16, 16, 2, D_, 0.0),        # shortest column
+    (128, 64, 200, D_, 1e-3),    # M = 16, ragged, Helmholtz
+    (128, 64, 256, N_, 0.0),     # M = 16, S = 16, singular
+    (64, 48, 300, D_, 0.0),      # M = 32, S = 10
+    (64, 32, 512, N_, 0.0),      # M = 32, S = 16 (the bench configuration), singular
+    (64, 32, 768, D_, 5e-4),     # M = 32, S = 24, two-slot ring
+    (48, 24, 700, N_, 0.0),      # M = 32, ragged, S = 22, singular
+    (40, 6, 33, D_, 0.0),        # nx*ny % 16 == 0 with nx % 16 != 0: tiles straddle y rows
+]
+
+
+@pytest.mark.parametrize("shape", THOMAS_SHAPES, ids=[f"{s[0]}x{s[1]}x{s[2]}" for s in THOMAS_SHAPES])
+def test_thomas_onchip_matches_streaming_and_oracle(tpt, torch, orc, shape):
+    nx, ny, nz, bcz, alpha = shape
+    P = I.Problem("thomas", (nx, ny, nz), (1.0, 2.0, 1.0), (2.0, 1.5, 3.0), (N_, N_, bcz), alpha, 77 + nz)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, alpha)
+    oplan = orc.OraclePlan(xf, yf, zf, P.bc, alpha)
+    phat = I.uniform_pm1(123 + nz, P.points).reshape(nz, ny, nx)
+    if P.singular:
+        phat[:, 0, 0] -= (np.diff(zf) * phat[:, 0, 0]).sum() / np.diff(zf).sum()     # compatible null column
+    scale = 1.0 if alpha == 0.0 else -1.0 / alpha                                   # [A5]
+    d_in = torch.from_numpy(np.ascontiguousarray(scale * phat)).cuda()
+    outs = []
+    for variant in (0, 1):
+        plan.set_thomas_variant(variant)
+        d_out = torch.empty_like(d_in)
+        plan.stage(tpt.K_THOMAS, d_in, d_out)
+        torch.cuda.synchronize()
+        outs.append(d_out.cpu().numpy())
+    ref = oplan.thomas_z(phat)
+    assert _rel(outs[1], ref) <= 5e-11 and _rel(outs[0], ref) <= 5e-11
+    assert _rel(outs[1], outs[0]) <= 5e-11
+    plan.destroy()
+
+
 def test_gemm_variants_agree_and_transforms_invert(tpt, torch):
     P = I.Problem("inv", (256, 128, 10), (1.0, 1.0, 1.0), (3.0, 2.0, 1.0), (N_, D_, D_), 0.0, 5)
     xf, yf, zf = P.faces()
