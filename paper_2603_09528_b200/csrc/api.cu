@@ -31,7 +31,7 @@ struct tpt_plan {
     double *d_yfwd = nullptr;   // [m][j]  = sqrt(wy_j) Q~y[j][m]           A-operand of step 2.2
     double *d_yinv = nullptr;   // [j][m]  = Q~y[j][m] / sqrt(wy_j)         A-operand of step 2.4
     double *d_vec = nullptr;    // lamx | lamy | az | bz | cz | wz
-    double *d_abc = nullptr;    // [a,b,c,0] per z row, identity-padded to nz + 64 rows (on-chip Thomas kernel)
+    double *d_abc = nullptr;    // coefficient tables of the on-chip Thomas kernel (thomas_onchip_tables)
     double *d_lamx = nullptr, *d_lamy = nullptr, *d_az = nullptr, *d_bz = nullptr, *d_cz = nullptr, *d_wz = nullptr;
     double *d_work = nullptr;   // one field
     double *d_stage = nullptr;  // staging field for tpt_solve_host (lazy)
@@ -214,9 +214,8 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
             p->d_az = p->d_vec + o_az; p->d_bz = p->d_vec + o_bz; p->d_cz = p->d_vec + o_cz; p->d_wz = p->d_vec + o_wz;
         }
         if (rc == TPT_OK) {
-            std::vector<double> t(4 * ((size_t)nz + 64), 0.0);
-            for (size_t k = 0; k < (size_t)nz + 64; ++k) t[4 * k + 1] = 1.0;
-            for (int k = 0; k < nz; ++k) { t[4 * k] = oz.a[k]; t[4 * k + 1] = oz.b[k]; t[4 * k + 2] = oz.c[k]; }
+            std::vector<double> t;
+            tpt::thomas_onchip_tables(nz, oz.a.data(), oz.b.data(), oz.c.data(), t);
             rc = upload(&p->d_abc, t);
         }
     } catch (const std::bad_alloc &) {

@@ -20,6 +20,8 @@
 // dominant so no pivoting is needed, A13).  c'_t and g_t stay in registers, d_t / x_t in the tile.
 #include <cuda.h>
 
+#include <vector>
+
 #include "kernels.cuh"
 #include "ptx.cuh"
 
@@ -32,11 +34,12 @@ constexpr int ROW_BYTES = TCOLS * (int)sizeof(double);
 
 template <int M, int MAXT>
 __global__ void __launch_bounds__(MAXT)
-thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__restrict__ abc,
-                     const double *__restrict__ lamx, const double *__restrict__ lamy, int nx, int nz, int S, int nbuf,
-                     int box_rows, int nbox, double shift0, int singular, int ntiles) {
+thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__restrict__ tab_reg,
+                     const double *__restrict__ tab_null, const double *__restrict__ lamx,
+                     const double *__restrict__ lamy, int nx, int nz, int S, int nbuf, int box_rows, int nbox,
+                     int buf_rows, double shift0, int singular, int ntiles) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const size_t tile_elems = (size_t)box_rows * nbox * TCOLS;      // >= nz rows; rows past nz are zero-filled
+    const size_t tile_elems = (size_t)buf_rows * TCOLS;             // buf_rows = max(S*M, nbox*box_rows) >= nz
     double *bufs = reinterpret_cast<double *>(smem_raw);            // nbuf x tile_elems
     double *scratch = bufs + (size_t)nbuf * tile_elems;             // 2 sets x 3 x S x 16
     uint64_t *full = reinterpret_cast<uint64_t *>(scratch + 6 * S * TCOLS);
@@ -50,11 +53,15 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__r
         for (int b = 0; b < nbuf; ++b) ptx::mbar_init(&full[b], 1);
         ptx::fence_mbar_init();
     }
+    // rows the TMA boxes never reach (past nbox*box_rows) must read as zero: identity rows with p = 0
+    for (int b = 0; b < nbuf; ++b)
+        for (int e = nbox * box_rows * TCOLS + tid; e < (int)tile_elems; e += blockDim.x)
+            bufs[(size_t)b * tile_elems + e] = 0.0;
     __syncthreads();
 
     auto issue_load = [&](int tile, int b) {      // one thread: nbox boxes of box_rows x 16 doubles
         if (tid != 0) return;
-        ptx::mbar_arrive_expect_tx(&full[b], (uint32_t)(tile_elems * sizeof(double)));
+        ptx::mbar_arrive_expect_tx(&full[b], (uint32_t)((size_t)nbox * box_rows * ROW_BYTES));
         double *dst = bufs + (size_t)b * tile_elems;
         for (int q = 0; q < nbox; ++q)
             ptx::tma_load_2d(dst + (size_t)q * box_rows * TCOLS, &tmap, tile * TCOLS, q * box_rows, &full[b]);
@@ -65,57 +72,54 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__r
     for (int p = 0; p < nbuf - 1 && p < n_my; ++p) issue_load(first + p * (int)gridDim.x, p);
 
     const int k0 = seg * M;
+    const int me = seg * TCOLS + col;
+    const int STR = S * TCOLS;
+    double *const set0 = scratch, *const set1 = scratch + 3 * STR;
     int b = 0;
     uint32_t parity = 0;
     for (int it = 0; it < n_my; ++it) {
         const int tile = first + it * (int)gridDim.x;
-        double *buf = bufs + (size_t)b * tile_elems + col;
+        double *buf = bufs + (size_t)b * tile_elems + (size_t)k0 * TCOLS + col;   // my segment, my column
         const int gcol = tile * TCOLS + col;
         const double s = __ldg(lamx + gcol % nx) + __ldg(lamy + gcol / nx) + shift0;
+        // the null column of a singular plan reads a table whose last row is "-x = p", and zeroes p
         const bool null_col = singular && gcol == 0;
+        const double2 *tab = reinterpret_cast<const double2 *>(null_col ? tab_null : tab_reg) + 2 * k0;
 
-        ptx::bulk_wait_read<0>();              // my rows of the previous tile's store have left shared memory
+        ptx::bulk_wait_read<0>();              // (thread 0) the previous tile's store has left shared memory
         ptx::mbar_wait(&full[b], parity);
+        if (null_col && (nz - 1) / M == seg) buf[((nz - 1) - k0) * TCOLS] = 0.0;
 
         // ---- 1. cold forward elimination of rows k0 .. k0+M-1 ------------------------------------
         double cp[M], g[M];
-        double pi = 1.0, DD = 0.0, GG = 0.0, dprev = 0.0;
+        double pi = 1.0, DD = 0.0, GG = 0.0, dprev = 0.0, rprev = 0.0;
 #pragma unroll
         for (int t = 0; t < M; ++t) {
-            const int k = k0 + t;
-            const double2 ab = __ldg(reinterpret_cast<const double2 *>(abc) + 2 * k);
-            const double c = __ldg(abc + 4 * k + 2);
-            double a = ab.x;
-            double bb = k < nz ? ab.y + s : 1.0;
-            double p = k < nz ? buf[k * TCOLS] : 0.0;
-            if (null_col && k == nz - 1) {     // vanishing final pivot: unknown := 0
-                a = 0.0;
-                bb = 1.0;
-                p = 0.0;
-            }
-            const double den = t == 0 ? bb : fma(-a, cp[t - 1], bb);
+            const double2 t0 = __ldg(tab + 2 * t);         // { a_k c_{k-1}, b_k }
+            const double2 t1 = __ldg(tab + 2 * t + 1);     // { a_k, c_k }
+            const double p = buf[t * TCOLS];
+            const double bb = t0.y + s;
+            const double den = t == 0 ? bb : fma(-t0.x, rprev, bb);
             const double r = ptx::fast_rcp(den);
-            cp[t] = c * r;
-            const double d = (t == 0 ? p : fma(-a, dprev, p)) * r;
-            g[t] = (t == 0 ? a : -a * g[t - 1]) * r;
-            if (k < nz) buf[k * TCOLS] = d;
+            cp[t] = t1.y * r;
+            const double d = (t == 0 ? p : fma(-t1.x, dprev, p)) * r;
+            g[t] = (t == 0 ? t1.x : -t1.x * g[t - 1]) * r;
+            buf[t * TCOLS] = d;
             if (t < M - 1) {
                 DD = fma(pi, d, DD);
                 GG = fma(pi, g[t], GG);
                 pi = -pi * cp[t];
             }
             dprev = d;
+            rprev = r;
         }
         // ---- 2. reduced system for the last unknown X of each segment ------------------------------
         //   g_last X_{s-1} + (1 - c'_last GG_{s+1}) X_s + (c'_last PI_{s+1}) X_{s+1} = d_last - c'_last DD_{s+1}
-        double *set0 = scratch, *set1 = scratch + 3 * S * TCOLS;
-        const int me = seg * TCOLS + col;
-        const int STR = S * TCOLS;
         set0[me] = DD;
         set0[STR + me] = GG;
         set0[2 * STR + me] = pi;
         __syncthreads();
-        // every thread has passed bulk_wait_read: the ring slot stored from in the previous iteration is free
+        // thread 0 has passed bulk_wait_read: the ring slot stored from in the previous iteration is free
         if (it + nbuf - 1 < n_my) {
             int nb = b + nbuf - 1;
             if (nb >= nbuf) nb -= nbuf;
@@ -126,10 +130,10 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__r
             double Bd = 1.0;
             if (seg + 1 < S) {
                 const double cl = cp[M - 1];
-                const int nx_ = me + TCOLS;
-                Bd = fma(-cl, set0[STR + nx_], 1.0);
-                C = cl * set0[2 * STR + nx_];
-                D = fma(-cl, set0[nx_], D);
+                const int nb_ = me + TCOLS;
+                Bd = fma(-cl, set0[STR + nb_], 1.0);
+                C = cl * set0[2 * STR + nb_];
+                D = fma(-cl, set0[nb_], D);
             }
             const double rB = ptx::fast_rcp(Bd);
             A *= rB;
@@ -169,13 +173,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__r
         const double xl = seg > 0 ? wr[me - TCOLS] : 0.0;
         // ---- 3. back substitution -------------------------------------------------------------------
         double xk = D;
-        if (k0 + M - 1 < nz) buf[(k0 + M - 1) * TCOLS] = xk;
+        buf[(M - 1) * TCOLS] = xk;
 #pragma unroll
         for (int t = M - 2; t >= 0; --t) {
-            const int k = k0 + t;
-            const double d = k < nz ? buf[k * TCOLS] : 0.0;
-            xk = fma(-cp[t], xk, fma(-g[t], xl, d));
-            if (k < nz) buf[k * TCOLS] = xk;
+            xk = fma(-cp[t], xk, fma(-g[t], xl, buf[t * TCOLS]));
+            buf[t * TCOLS] = xk;
         }
         ptx::fence_proxy_async();
         __syncthreads();
@@ -224,13 +226,14 @@ bool make_field_map(CUtensorMap *map, double *x, size_t plane, int nz, int box_r
 }
 
 template <int M, int MAXT>
-cudaError_t launch_m(double *x, const double *abc, const double *lamx, const double *lamy, int nx, int ny, int nz,
+cudaError_t launch_m(double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny, int nz,
                      double shift0, int singular, int sms, cudaStream_t stream) {
     int S = (nz + M - 1) / M;
     if (S & 1) ++S;                                          // whole warps: 2 segments x 16 columns
     const int nbox = (nz + 255) / 256;                       // TMA boxes are at most 256 rows tall
     const int box_rows = (nz + nbox - 1) / nbox;
-    const size_t tile_bytes = (size_t)box_rows * nbox * ROW_BYTES;
+    const int buf_rows = S * M > nbox * box_rows ? S * M : nbox * box_rows;
+    const size_t tile_bytes = (size_t)buf_rows * ROW_BYTES;
     const size_t fixed = (size_t)6 * S * TCOLS * sizeof(double) + 64;
     int nbuf = (int)((220 * 1024 - fixed) / tile_bytes);
     if (nbuf > 3) nbuf = 3;
@@ -261,8 +264,9 @@ cudaError_t launch_m(double *x, const double *abc, const double *lamx, const dou
     const int ntiles = (int)(((size_t)nx * ny) / TCOLS);
     int grid = sms * per_sm_cache[1];
     if (grid > ntiles) grid = ntiles;
-    thomas_onchip_kernel<M, MAXT><<<grid, threads, smem, stream>>>(tmap, abc, lamx, lamy, nx, nz, S, nbuf, box_rows, nbox,
-                                                                  shift0, singular, ntiles);
+    thomas_onchip_kernel<M, MAXT><<<grid, threads, smem, stream>>>(
+        tmap, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf, box_rows, nbox, buf_rows, shift0,
+        singular, ntiles);
     return cudaGetLastError();
 }
 
@@ -272,13 +276,34 @@ bool thomas_onchip_supported(int nx, int ny, int nz) {
     return ((size_t)nx * ny) % TCOLS == 0 && nz >= 2 && nz <= 768;
 }
 
-cudaError_t launch_thomas_onchip(double *x, const double *abc, const double *lamx, const double *lamy, int nx, int ny,
+cudaError_t launch_thomas_onchip(double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
                                  int nz, double shift0, int singular, int sms, cudaStream_t stream) {
     if (!thomas_onchip_supported(nx, ny, nz)) return cudaErrorInvalidValue;
-    if (nz <= 64) return launch_m<8, 128>(x, abc, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    if (nz <= 256) return launch_m<16, 256>(x, abc, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    if (nz <= 512) return launch_m<32, 256>(x, abc, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    return launch_m<32, 384>(x, abc, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+    if (nz <= 128) return launch_m<8, 256>(x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+    if (nz <= 512) return launch_m<16, 512>(x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+    return launch_m<32, 384>(x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+}
+
+// Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows
+// [0, -1, 0, 0] (pivot -1 + s < 0 for every mode since s <= 0); the second table is the null column's, with the
+// last equation replaced by "-x = p" (the kernel zeroes p there): PAPER.md:219.
+void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out) {
+    const size_t rows = (size_t)nz + THOMAS_TABLE_PAD;
+    out.assign(8 * rows, 0.0);
+    for (int v = 0; v < 2; ++v) {
+        double *t = out.data() + (size_t)v * 4 * rows;
+        for (size_t k = 0; k < rows; ++k) t[4 * k + 1] = -1.0;
+        for (int k = 0; k < nz; ++k) {
+            t[4 * k] = k > 0 ? a[k] * c[k - 1] : 0.0;
+            t[4 * k + 1] = b[k];
+            t[4 * k + 2] = a[k];
+            t[4 * k + 3] = c[k];
+        }
+        if (v == 1) {
+            double *last = t + 4 * (size_t)(nz - 1);
+            last[0] = 0.0; last[1] = -1.0; last[2] = 0.0; last[3] = 0.0;
+        }
+    }
 }
 
 }  // namespace tpt
