@@ -10,7 +10,7 @@ volume-weighted mean removed.  Prints ONE JSON line (rank 0).
 
   value       whole-job Gpts/s with the rhs already resident in HBM (N>1: N independent replicas, §8(e))
   e2e         the same metric through the C-ABI call tpt_solve_host with pinned HOST buffers (H2D + D2H inside)
-  roofline    dominant kernel (forward-x DMMA GEMM): algorithmic flops / CUDA-event duration vs FP64 peak
+  roofline    dominant kernel (the slowest of the four DMMA GEMM transforms): algorithmic flops / CUDA-event duration vs FP64 peak
   cpu_baseline the oracle (as it stands) timed on the host cores on a bounded z-slab sample of the workload
   --impl reference  times the oracle alone (rank 0 only)
 """
@@ -293,7 +293,7 @@ def run_gpu(args):
             with open(tpath) as fh:
                 traffic = json.load(fh).get(args.config, {}).get(dom)
         roofline = {
-            "kernel": f"gemm_dmma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
+            "kernel": f"gemm_tma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
             "peak": fp64_peak, "unit": "TFLOP/s", "frac": kernels[dom]["achieved_tflops"] / fp64_peak, "traffic": traffic,
             "peak_source": f"148 SMs x 64 FP64 FMA/clk x 2 x {sm_max:.0f} MHz ({peak_kind} sm_max_mhz); FP64 is absent from "
                            "MEASURED_PEAKS.json",

@@ -117,9 +117,10 @@ int tpt_stage(tpt_plan *plan, int slot, const double *in_dev, double *out_dev, v
 int tpt_plan_set_profiling(tpt_plan *plan, int enabled);
 int tpt_plan_get_kernel_times(tpt_plan *plan, float *ms_host, int *launches_out, int *solves_out);
 
-/* Select the GEMM kernel for the transforms: 0 = generic FP64-FMA tile kernel (any shape),
- * 1 = DMMA (mma.sync m8n8k4 f64) pipelined kernel where the shape allows (default).  For A/B
- * measurement and tests; both are this library's own sm_100a kernels. */
+/* Select the GEMM kernel for the transforms: 2 = persistent warp-specialised DMMA kernel fed by TMA through an
+ * mbarrier ring (default; used where M and N are multiples of 128 and K of 16), 1 = cp.async-pipelined DMMA kernel
+ * (M, N multiples of 64), 0 = generic FP64-FMA tile kernel (any shape).  A variant falls back to the next lower one
+ * for shapes it does not take.  For A/B measurement and tests; all are this library's own sm_100a kernels. */
 int tpt_plan_set_gemm_variant(tpt_plan *plan, int variant);
 
 /* Select the z-sweep kernel: 1 = on-chip partitioned Thomas kernel (column tiles resident in shared memory,

@@ -19,7 +19,7 @@ struct tpt_plan {
     int singular = 0;
     int device = 0;
     double shift0 = 0.0;          // 0 (Poisson) or -1/alpha (Helmholtz, A5)
-    int gemm_variant = 1;
+    int gemm_variant = 2;
     int thomas_variant = 1;       // 1 = on-chip partitioned kernel where supported, 0 = streaming kernel
     int sms = 0;
     int profiling = 0;
@@ -89,14 +89,20 @@ tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const dou
     return g;
 }
 
+// variant 2 = persistent TMA/mbarrier DMMA kernel where the shape allows, else the variant-1 / generic kernels
+cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st) {
+    if (p->gemm_variant == 2 && tpt::gemm_tma_supported(g)) return tpt::launch_gemm_tma(g, p->sms, st);
+    return tpt::launch_gemm(g, p->gemm_variant >= 1 ? 1 : 0, st);
+}
+
 // Runs one slot; *launches incremented by the number of kernels enqueued.
 int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches) {
     cudaError_t e = cudaSuccess;
     switch (slot) {
-        case TPT_K_FWD_X: e = tpt::launch_gemm(gemm_x(p, in, out, p->d_xfwd), p->gemm_variant, st); ++*launches; break;
-        case TPT_K_INV_X: e = tpt::launch_gemm(gemm_x(p, in, out, p->d_xinv), p->gemm_variant, st); ++*launches; break;
-        case TPT_K_FWD_Y: e = tpt::launch_gemm(gemm_y(p, in, out, p->d_yfwd), p->gemm_variant, st); ++*launches; break;
-        case TPT_K_INV_Y: e = tpt::launch_gemm(gemm_y(p, in, out, p->d_yinv), p->gemm_variant, st); ++*launches; break;
+        case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd), st); ++*launches; break;
+        case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv), st); ++*launches; break;
+        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd), st); ++*launches; break;
+        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv), st); ++*launches; break;
         case TPT_K_THOMAS:
             if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz))
                 e = tpt::launch_thomas_onchip(out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
@@ -227,7 +233,10 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
         cudaError_t e = cudaMalloc(&p->d_work, p->points() * sizeof(double));
         if (e != cudaSuccess) { cudaGetLastError(); rc = (e == cudaErrorMemoryAllocation) ? TPT_ENOMEM : TPT_ECUDA; }
     }
-    if (rc == TPT_OK && tpt::gemm_configure() != cudaSuccess) { cudaGetLastError(); rc = TPT_ECUDA; }
+    if (rc == TPT_OK && (tpt::gemm_configure() != cudaSuccess || tpt::gemm_tma_configure() != cudaSuccess)) {
+        cudaGetLastError();
+        rc = TPT_ECUDA;
+    }
     if (rc != TPT_OK) { free_plan(p); return rc; }
     *plan_out = p;
     return TPT_OK;
@@ -352,7 +361,7 @@ int tpt_plan_get_kernel_times(tpt_plan *p, float *ms_host, int *launches_out, in
 }
 
 int tpt_plan_set_gemm_variant(tpt_plan *p, int variant) {
-    if (!p || (variant != 0 && variant != 1)) return TPT_EINVAL;
+    if (!p || variant < 0 || variant > 2) return TPT_EINVAL;
     p->gemm_variant = variant;
     return TPT_OK;
 }

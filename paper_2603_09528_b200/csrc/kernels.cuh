@@ -26,6 +26,12 @@ cudaError_t launch_gemm(const GemmArgs &g, int variant, cudaStream_t stream);
 bool gemm_dmma_supported(const GemmArgs &g);
 cudaError_t gemm_configure();   // one-time cudaFuncSetAttribute for the dynamic-smem kernels
 
+// variant 2 (gemm_tma.cu): persistent warp-specialised DMMA kernel fed by TMA through an mbarrier ring.
+// M % 128 == N % 128 == 0, K % 16 == 0, batched operands densely stacked.  sms = SM count.
+bool gemm_tma_supported(const GemmArgs &g);
+cudaError_t gemm_tma_configure();
+cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream);
+
 // z sweep (step 2.3): in place on x (nx*ny*nz), cprime = field-sized scratch.
 // Solves (T_z + (lamx[i] + lamy[j] + shift0) I) x = rhs for each column; on a singular plan the
 // column (0,0) gets "last unknown = 0".

@@ -35,7 +35,7 @@ def _rel(a, b):
     return float(np.abs(a - b).max() / np.abs(b).max())
 
 
-def _gpu_solve(tpt, torch, P, variant=1, inplace=False, stream=None):
+def _gpu_solve(tpt, torch, P, variant=2, inplace=False, stream=None):
     xf, yf, zf = P.faces()
     f = P.rhs()
     plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
@@ -68,7 +68,7 @@ SMALL = [
 
 
 @pytest.mark.parametrize("case", SMALL, ids=[c[0] for c in SMALL])
-@pytest.mark.parametrize("variant", [1, 0])
+@pytest.mark.parametrize("variant", [2, 1, 0])
 def test_parity_small_cases(tpt, torch, orc, case, variant):
     name, n, L, beta, bc, alpha = case
     P = I.Problem(name, n, L, beta, bc, alpha, seed=len(name) + n[0])
@@ -216,7 +216,7 @@ def test_gemm_variants_agree_and_transforms_invert(tpt, torch):
     f = torch.from_numpy(P.rhs()).cuda()
     plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0)
     outs = {}
-    for v in (0, 1):
+    for v in (0, 1, 2):
         plan.set_gemm_variant(v)
         a, b = torch.empty_like(f), torch.empty_like(f)
         plan.stage(tpt.K_FWD_X, f, a)
@@ -227,6 +227,7 @@ def test_gemm_variants_agree_and_transforms_invert(tpt, torch):
         plan.stage(tpt.K_INV_Y, a, b)
         assert float((b - f).abs().max()) < 1e-12
     assert float((outs[0] - outs[1]).abs().max()) < 1e-12 * float(outs[0].abs().max()) * 128
+    assert float((outs[0] - outs[2]).abs().max()) < 1e-12 * float(outs[0].abs().max()) * 128
     plan.destroy()
 
 
