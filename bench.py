@@ -37,6 +37,9 @@ UNIT = "Gpts/s"
 # DFMA microbenchmarks of the library are reported next to it.
 SM_COUNT, FP64_FMA_PER_CLK_SM = 148, 64
 ORACLE_SAMPLE_NZ = 64
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (gemm_tma_kernel), from the one
+# `ncu --set full` capture summarised in profiles/r1b_tma_gemm_onchip_thomas.md (config c3; bytes).  Other configs: null.
+NCU_TRAFFIC_BYTES = {"c3": 1.076042e9 + 1.030894e9}
 
 
 def _peaks():
@@ -287,11 +290,7 @@ def run_gpu(args):
                 entry.update({"bound": "tensor", "achieved_tflops": tf, "frac_of_fp64_peak": tf / fp64_peak})
             kernels[name] = entry
         dom = max(("fwd_x", "fwd_y", "inv_y", "inv_x"), key=lambda n: kernels[n]["ms"])
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            with open(tpath) as fh:
-                traffic = json.load(fh).get(args.config, {}).get(dom)
+        traffic = NCU_TRAFFIC_BYTES.get(args.config)
         roofline = {
             "kernel": f"gemm_tma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
             "peak": fp64_peak, "unit": "TFLOP/s", "frac": kernels[dom]["achieved_tflops"] / fp64_peak, "traffic": traffic,
@@ -299,7 +298,8 @@ def run_gpu(args):
                            "MEASURED_PEAKS.json",
             "peak_measured_dmma_loop": dmma_meas, "peak_measured_dfma_loop": dfma_meas,
             "frac_of_measured_dmma_loop": kernels[dom]["achieved_tflops"] / dmma_meas,
-            "algorithmic_flops_per_launch": flops[dom],
+            "algorithmic_flops_per_launch": flops[dom], "algorithmic_dram_bytes_per_launch": 16.0 * pts,
+            "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1b_*.md)",
         }
         cpu = _oracle_sample(probs, 1, 1)
         n20 = per_step[: min(20, len(per_step))]
