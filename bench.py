@@ -161,6 +161,29 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def replica_problem(P, rank: int):
+    """Replicas only: rank r solves its own copy of the workload, rhs seed offset by 1000 r."""
+    import dataclasses
+
+    return dataclasses.replace(P, seed=P.seed + 1000 * rank)
+
+
+def max_over_ranks(dist, value: float, device="cpu") -> float:
+    """Timing rule for N > 1: the job takes as long as its slowest rank."""
+    if dist is None:
+        return float(value)
+    import torch
+
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, pts_step: int, steps: int, seconds: float) -> float:
+    """Gpts/s over all replicas: every rank processed pts_step * steps points in `seconds` (max over ranks)."""
+    return world * pts_step * steps / seconds / 1e9
+
+
 def run_gpu(args):
     import torch
 
@@ -196,9 +219,7 @@ def run_gpu(args):
         if key not in plan_cache:
             plan_cache[key] = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
         plans.append(plan_cache[key])
-        import dataclasses
-
-        f = dataclasses.replace(P, seed=P.seed + 1000 * rank).rhs()
+        f = replica_problem(P, rank).rhs()
         h_rhs.append(f)
         d_rhs.append(torch.from_numpy(f).cuda())
         d_out.append(torch.empty_like(d_rhs[-1]))
@@ -240,12 +261,9 @@ def run_gpu(args):
     if BAD_REASONS & set(clocks["reasons"]):          # rejected: re-measure once
         total_ms, per_step, kt, launches, clocks = timed_region()
         clocks["remeasured"] = True
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(dist, total_ms, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * pts_step * args.steps / (total_ms * 1e-3) / 1e9
+    value = whole_job_value(world, pts_step, args.steps, total_ms * 1e-3)
 
     # ---- e2e: the C-ABI call with pinned HOST buffers, copies inside the timed region
     e2e_steps = max(1, min(args.steps, 5))
@@ -260,11 +278,8 @@ def run_gpu(args):
             api.solve_host(pl, a, b, stream)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_val = world * pts_step * e2e_steps / e2e_s / 1e9
+    e2e_s = max_over_ranks(dist, e2e_s, "cuda")
+    e2e_val = whole_job_value(world, pts_step, e2e_steps, e2e_s)
     e2e_ok = all(np.array_equal(b.numpy(), o.cpu().numpy()) for b, o in zip(pin_out, d_out))
 
     if rank == 0:
