@@ -80,10 +80,13 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz,
 int tpt_solve(tpt_plan *plan, const double *rhs_dev, double *out_dev, void *cuda_stream);
 
 /*
- * tpt_solve_host — the same solve for HOST buffers: copies rhs to the device (into a plan-owned
- * staging field allocated on first use), runs tpt_solve, copies the result back and synchronises
- * `cuda_stream` before returning.  rhs_host / out_host: HOST, nx*ny*nz doubles each (pinned memory
- * makes the copies asynchronous and fast; pageable memory works).  May alias.
+ * tpt_solve_host — the same solve for HOST buffers, synchronous: returns after the result is in out_host.
+ * The transforms act plane by plane in z (Eq. 10, 12 at PAPER.md:154–169), so the field crosses the bus in up to
+ * 16 z-slabs: slab s is transformed (steps 2.1, 2.2) while slab s+1 is still being copied in, the sweep (2.3) runs
+ * once every slab has arrived, and slab s is copied out while slab s+1 is transformed back (2.4, 2.5).  The copies
+ * run on two plan-owned streams ordered after earlier work on `cuda_stream`; the kernels run on `cuda_stream`.
+ * Uses a plan-owned staging field allocated on first use.  rhs_host / out_host: HOST, nx*ny*nz doubles each
+ * (pinned memory makes the copies asynchronous and fast; pageable memory works).  May alias.
  */
 int tpt_solve_host(tpt_plan *plan, const double *rhs_host, double *out_host, void *cuda_stream);
 

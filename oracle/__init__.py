@@ -3,6 +3,9 @@
 Importable only from tests/, __graft_entry__.smoke() and bench.py's cpu_baseline/--impl reference legs.
 """
 from .binding import (  # noqa: F401
+    DIRS_XYZ,
+    DIRS_YZ,
+    DIRS_Z,
     OraclePlan,
     apply_operator_flux,
     dense_solve_3d,

@@ -7,6 +7,8 @@ import numpy as np
 
 from . import build as _build
 
+DIRS_Z, DIRS_YZ, DIRS_XYZ = 4, 6, 7   # implicitly treated directions: bit 0 = x, 1 = y, 2 = z
+
 _lib = None
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -43,6 +45,13 @@ def lib():
         L.orc_apply_operator_flux.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, _dp, _dp]
         L.orc_residual_norms.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, _dp, _dp, _dp]
         L.orc_dense_solve_3d.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, _dp, _dp]
+        L.orc_plan_set_implicit_dirs.argtypes = [C.c_void_p, C.c_int]
+        L.orc_apply_operator_flux_dirs.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, C.c_int,
+                                                   _dp, _dp]
+        L.orc_residual_norms_dirs.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, C.c_int, _dp,
+                                              _dp, _dp]
+        L.orc_dense_solve_3d_dirs.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, C.c_int, _dp,
+                                              _dp]
         L.orc_num_threads.argtypes = []
         _lib = L
     return _lib
@@ -96,7 +105,7 @@ def eig_1d(xf, bc, refine_steps: int = 2, cache: bool = True):
 class OraclePlan:
     """orc_plan handle.  Fields are numpy float64 arrays of shape (nz, ny, nx)."""
 
-    def __init__(self, xf, yf, zf, bc, alpha: float = 0.0, refine_steps: int = 2):
+    def __init__(self, xf, yf, zf, bc, alpha: float = 0.0, refine_steps: int = 2, dirs: int = DIRS_XYZ):
         self.xf, self.yf, self.zf = _faces(xf), _faces(yf), _faces(zf)
         self.nx, self.ny, self.nz = self.xf.size - 1, self.yf.size - 1, self.zf.size - 1
         self.bc = tuple(int(b) for b in bc)
@@ -108,6 +117,9 @@ class OraclePlan:
                                               _ptr(self.zf), _bc(self.bc), self.alpha, _ptr(lamx), _ptr(qx),
                                               _ptr(lamy), _ptr(qy)), "plan_create")
         self._h = h
+        self.dirs = int(dirs)
+        if self.dirs != DIRS_XYZ:
+            _check(lib().orc_plan_set_implicit_dirs(self._h, self.dirs), "plan_set_implicit_dirs")
 
     def close(self):
         if getattr(self, "_h", None):
@@ -160,32 +172,32 @@ class OraclePlan:
         return phi
 
 
-def apply_operator_flux(xf, yf, zf, bc, alpha, phi):
+def apply_operator_flux(xf, yf, zf, bc, alpha, phi, dirs: int = DIRS_XYZ):
     xf, yf, zf = _faces(xf), _faces(yf), _faces(zf)
     nx, ny, nz = xf.size - 1, yf.size - 1, zf.size - 1
     phi = np.ascontiguousarray(phi, dtype=np.float64).reshape(nz, ny, nx)
     out = np.empty_like(phi)
-    _check(lib().orc_apply_operator_flux(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha), _ptr(phi),
-                                         _ptr(out)), "apply_operator_flux")
+    _check(lib().orc_apply_operator_flux_dirs(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha),
+                                              int(dirs), _ptr(phi), _ptr(out)), "apply_operator_flux")
     return out
 
 
-def residual_norms(xf, yf, zf, bc, alpha, f, phi) -> dict:
+def residual_norms(xf, yf, zf, bc, alpha, f, phi, dirs: int = DIRS_XYZ) -> dict:
     xf, yf, zf = _faces(xf), _faces(yf), _faces(zf)
     nx, ny, nz = xf.size - 1, yf.size - 1, zf.size - 1
     f = np.ascontiguousarray(f, dtype=np.float64).reshape(nz, ny, nx)
     phi = np.ascontiguousarray(phi, dtype=np.float64).reshape(nz, ny, nx)
     norms = np.empty(4)
-    _check(lib().orc_residual_norms(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha), _ptr(f),
-                                    _ptr(phi), _ptr(norms)), "residual_norms")
+    _check(lib().orc_residual_norms_dirs(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha), int(dirs),
+                                         _ptr(f), _ptr(phi), _ptr(norms)), "residual_norms")
     return {"rel2": norms[0], "relL2vol": norms[1], "relmax": norms[2], "backward": norms[3]}
 
 
-def dense_solve_3d(xf, yf, zf, bc, alpha, f):
+def dense_solve_3d(xf, yf, zf, bc, alpha, f, dirs: int = DIRS_XYZ):
     xf, yf, zf = _faces(xf), _faces(yf), _faces(zf)
     nx, ny, nz = xf.size - 1, yf.size - 1, zf.size - 1
     f = np.ascontiguousarray(f, dtype=np.float64).reshape(nz, ny, nx)
     phi = np.empty_like(f)
-    _check(lib().orc_dense_solve_3d(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha), _ptr(f),
-                                    _ptr(phi)), "dense_solve_3d")
+    _check(lib().orc_dense_solve_3d_dirs(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha), int(dirs),
+                                         _ptr(f), _ptr(phi)), "dense_solve_3d")
     return phi

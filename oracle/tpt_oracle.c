@@ -345,6 +345,7 @@ struct orc_plan {
     int bc[3];
     double alpha;
     int singular;
+    int dirs;              /* implicitly treated directions of L_I: bit 0 = x, 1 = y, 2 = z; 7 = the full operator */
     double *wx, *wy, *wz;
     double *az, *bz, *cz;
     double *lamx, *lamy;
@@ -375,6 +376,7 @@ int orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
     orc_plan *p = (orc_plan *)calloc(1, sizeof(orc_plan));
     if (!p) return ORC_ENOMEM;
     p->nx = nx; p->ny = ny; p->nz = nz; p->alpha = alpha;
+    p->dirs = ORC_DIRS_XYZ;
     p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
     /* [A7] structural detection of the null mode: all-Neumann and Poisson. */
     p->singular = (alpha == 0.0 && bc[0] == ORC_BC_NEUMANN && bc[1] == ORC_BC_NEUMANN && bc[2] == ORC_BC_NEUMANN);
@@ -414,6 +416,15 @@ int orc_plan_create(orc_plan **out, int nx, int ny, int nz,
 }
 
 int orc_plan_is_singular(const orc_plan *p) { return p ? p->singular : ORC_EINVAL; }
+
+/* L_I = L_z ("z"), L_y + L_z ("yz") or L ("xyz").  The partial choices exist for the Helmholtz
+ * problem of Eq. 2b only (the pressure Poisson equation always carries the full Laplacian, Eq. 2c). */
+int orc_plan_set_implicit_dirs(orc_plan *p, int dirs) {
+    if (!p || (dirs != ORC_DIRS_XYZ && dirs != ORC_DIRS_YZ && dirs != ORC_DIRS_Z)) return ORC_EINVAL;
+    if (dirs != ORC_DIRS_XYZ && !(p->alpha > 0.0)) return ORC_EINVAL;
+    p->dirs = dirs;
+    return ORC_OK;
+}
 
 int orc_plan_get_eigen(const orc_plan *p, int dir, double *lambda, double *qtilde) {
     if (!p || (dir != 0 && dir != 1)) return ORC_EINVAL;
@@ -533,7 +544,9 @@ int orc_thomas_z(const orc_plan *p, double *field) {
                 if (!ok) continue;
                 double *d = field + (size_t)j * nx;           /* d[k*plane + i] */
                 for (int i = 0; i < nx; ++i) {
-                    double sigma = p->lamx[i] + p->lamy[j];
+                    /* Eq. 9 restricted to the diagonalised directions ("the yz option omits the x
+                     * transforms, and the z option performs only the tridiagonal solve") */
+                    double sigma = ((p->dirs & 1) ? p->lamx[i] : 0.0) + ((p->dirs & 2) ? p->lamy[j] : 0.0);
                     double shift = (alpha == 0.0) ? sigma : -alpha * sigma;
                     int null_col = p->singular && i == 0 && j == 0;
                     /* forward elimination */
@@ -579,11 +592,12 @@ int orc_thomas_z(const orc_plan *p, double *field) {
 
 int orc_solve(const orc_plan *p, const double *f, double *phi, double *work) {
     if (!p || !f || !phi || !work || f == phi) return ORC_EINVAL;
-    orc_forward_x(p, f, work);        /* 2.1 */
-    orc_forward_y(p, work, phi);      /* 2.2 */
-    int rc = orc_thomas_z(p, phi);    /* 2.3 */
-    orc_inverse_y(p, phi, work);      /* 2.4 */
-    orc_inverse_x(p, work, phi);      /* 2.5 */
+    const size_t bytes = sizeof(double) * (size_t)p->nx * p->ny * p->nz;
+    if (p->dirs & 1) orc_forward_x(p, f, work); else memcpy(work, f, bytes);       /* 2.1 */
+    if (p->dirs & 2) orc_forward_y(p, work, phi); else memcpy(phi, work, bytes);   /* 2.2 */
+    int rc = orc_thomas_z(p, phi);                                                 /* 2.3 */
+    if (p->dirs & 2) orc_inverse_y(p, phi, work); else memcpy(work, phi, bytes);   /* 2.4 */
+    if (p->dirs & 1) orc_inverse_x(p, work, phi); else memcpy(phi, work, bytes);   /* 2.5 */
     return rc;
 }
 
@@ -608,6 +622,18 @@ static double lap1d_flux(const double *xf, int n, int bc, int i, double um, doub
 
 int orc_apply_operator_flux(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
                             const int bc[3], double alpha, const double *phi, double *out) {
+    return orc_apply_operator_flux_dirs(nx, ny, nz, xf, yf, zf, bc, alpha, ORC_DIRS_XYZ, phi, out);
+}
+
+static int dirs_ok(int dirs, double alpha) {
+    if (dirs == ORC_DIRS_XYZ) return 1;
+    return (dirs == ORC_DIRS_YZ || dirs == ORC_DIRS_Z) && alpha > 0.0;
+}
+
+/* (I - alpha L_I) phi with L_I the sum of the 1-D Laplacians of the directions in `dirs`. */
+int orc_apply_operator_flux_dirs(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
+                                 const int bc[3], double alpha, int dirs, const double *phi, double *out) {
+    if (!dirs_ok(dirs, alpha)) return ORC_EINVAL;
     if (!faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf) || !bc || !phi || !out) return ORC_EINVAL;
     const size_t plane = (size_t)nx * ny;
 #pragma omp parallel for schedule(static)
@@ -619,7 +645,7 @@ int orc_apply_operator_flux(int nx, int ny, int nz, const double *xf, const doub
                 double lx = lap1d_flux(xf, nx, bc[0], i, i > 0 ? phi[id - 1] : 0.0, u0, i < nx - 1 ? phi[id + 1] : 0.0);
                 double ly = lap1d_flux(yf, ny, bc[1], j, j > 0 ? phi[id - nx] : 0.0, u0, j < ny - 1 ? phi[id + nx] : 0.0);
                 double lz = lap1d_flux(zf, nz, bc[2], k, k > 0 ? phi[id - plane] : 0.0, u0, k < nz - 1 ? phi[id + plane] : 0.0);
-                double lap = lx + ly + lz;
+                double lap = ((dirs & 1) ? lx : 0.0) + ((dirs & 2) ? ly : 0.0) + lz;
                 out[id] = (alpha == 0.0) ? lap : u0 - alpha * lap;
             }
     return ORC_OK;
@@ -627,11 +653,17 @@ int orc_apply_operator_flux(int nx, int ny, int nz, const double *xf, const doub
 
 int orc_residual_norms(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
                        const int bc[3], double alpha, const double *f, const double *phi, double norms[4]) {
+    return orc_residual_norms_dirs(nx, ny, nz, xf, yf, zf, bc, alpha, ORC_DIRS_XYZ, f, phi, norms);
+}
+
+int orc_residual_norms_dirs(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
+                            const int bc[3], double alpha, int dirs, const double *f, const double *phi,
+                            double norms[4]) {
     if (!f || !norms) return ORC_EINVAL;
     size_t n = (size_t)nx * ny * nz;
     double *op = (double *)malloc(sizeof(double) * n);
     if (!op) return ORC_ENOMEM;
-    int rc = orc_apply_operator_flux(nx, ny, nz, xf, yf, zf, bc, alpha, phi, op);
+    int rc = orc_apply_operator_flux_dirs(nx, ny, nz, xf, yf, zf, bc, alpha, dirs, phi, op);
     if (rc != ORC_OK) { free(op); return rc; }
     double r2 = 0, f2 = 0, rv = 0, fv = 0, rmax = 0, fmax = 0, pmax = 0;
     const size_t plane = (size_t)nx * ny;
@@ -655,6 +687,7 @@ int orc_residual_norms(int nx, int ny, int nz, const double *xf, const double *y
     const double *ff[3] = {xf, yf, zf};
     int nn[3] = {nx, ny, nz};
     for (int d = 0; d < 3; ++d) {
+        if (!(dirs & (1 << d))) continue;
         int m = nn[d];
         double *w = malloc(sizeof(double) * m), *a = malloc(sizeof(double) * m), *b = malloc(sizeof(double) * m),
                *c = malloc(sizeof(double) * m);
@@ -677,6 +710,12 @@ int orc_residual_norms(int nx, int ny, int nz, const double *xf, const double *y
  * partial pivoting. */
 int orc_dense_solve_3d(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
                        const int bc[3], double alpha, const double *f, double *phi) {
+    return orc_dense_solve_3d_dirs(nx, ny, nz, xf, yf, zf, bc, alpha, ORC_DIRS_XYZ, f, phi);
+}
+
+int orc_dense_solve_3d_dirs(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
+                            const int bc[3], double alpha, int dirs, const double *f, double *phi) {
+    if (!dirs_ok(dirs, alpha)) return ORC_EINVAL;
     if (!faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf) || !bc || !f || !phi) return ORC_EINVAL;
     long n = (long)nx * ny * nz;
     if (n > 4096) return ORC_EINVAL;
@@ -697,6 +736,7 @@ int orc_dense_solve_3d(int nx, int ny, int nz, const double *xf, const double *y
                 int id[3] = {i, j, k};
                 long st[3] = {1, nx, (long)nx * ny};
                 for (int d = 0; d < 3; ++d) {
+                    if (!(dirs & (1 << d))) continue;
                     int q = id[d];
                     row[r] += co[d][2][q];
                     if (q > 0) row[r - st[d]] += co[d][1][q];

@@ -34,6 +34,8 @@ extern "C" {
 #endif
 
 enum { ORC_BC_NEUMANN = 0, ORC_BC_DIRICHLET = 1 };
+/* Implicitly treated directions L_I of the Helmholtz problem, Eq. 2b: bit 0 = x, 1 = y, 2 = z. */
+enum { ORC_DIRS_Z = 4, ORC_DIRS_YZ = 6, ORC_DIRS_XYZ = 7 };
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ENUMERIC = -4 };
 
 typedef struct orc_plan orc_plan;
@@ -68,6 +70,9 @@ int  orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
 void orc_plan_destroy(orc_plan *p);
 int  orc_plan_is_singular(const orc_plan *p);
 int  orc_plan_get_eigen(const orc_plan *p, int dir, double *lambda, double *qtilde);
+/* Partial implicit diffusion: (I - alpha L_I) u = f with L_I = L_z (ORC_DIRS_Z: only the tridiagonal
+ * solve), L_y + L_z (ORC_DIRS_YZ: the x transforms are omitted) or L (default).  Helmholtz plans only. */
+int  orc_plan_set_implicit_dirs(orc_plan *p, int dirs);
 
 void orc_forward_x(const orc_plan *p, const double *in, double *out);   /* Eq. 10a */
 void orc_forward_y(const orc_plan *p, const double *in, double *out);   /* Eq. 10b */
@@ -86,6 +91,11 @@ int  orc_apply_operator_flux(int nx, int ny, int nz,
                              const double *xf, const double *yf, const double *zf,
                              const int bc[3], double alpha, const double *phi, double *out);
 
+/* The same for a partial operator I - alpha L_I, L_I = sum of the 1-D Laplacians of the directions in `dirs`. */
+int  orc_apply_operator_flux_dirs(int nx, int ny, int nz,
+                                  const double *xf, const double *yf, const double *zf,
+                                  const int bc[3], double alpha, int dirs, const double *phi, double *out);
+
 /* Residual r = f - Op(phi) in flux form; norms[0] = ||r||2/||f||2, norms[1] = volume-weighted
  * L2 ratio, norms[2] = max|r|/max|f|, norms[3] = normwise backward error
  * max|r| / (||Op||_inf max|phi| + max|f|). */
@@ -94,12 +104,21 @@ int  orc_residual_norms(int nx, int ny, int nz,
                         const int bc[3], double alpha, const double *f, const double *phi,
                         double norms[4]);
 
+int  orc_residual_norms_dirs(int nx, int ny, int nz,
+                             const double *xf, const double *yf, const double *zf,
+                             const int bc[3], double alpha, int dirs, const double *f, const double *phi,
+                             double norms[4]);
+
 /* Brute force: assemble the dense operator of Eq. 7 (n = nx*ny*nz <= 4096) and solve by
  * Gaussian elimination with partial pivoting.  Singular (all-Neumann Poisson): bordered system
  * [T v; v^T 0] with v = cell volumes (zero volume-weighted mean). */
 int  orc_dense_solve_3d(int nx, int ny, int nz,
                         const double *xf, const double *yf, const double *zf,
                         const int bc[3], double alpha, const double *f, double *phi);
+
+int  orc_dense_solve_3d_dirs(int nx, int ny, int nz,
+                             const double *xf, const double *yf, const double *zf,
+                             const int bc[3], double alpha, int dirs, const double *f, double *phi);
 
 int  orc_num_threads(void);
 

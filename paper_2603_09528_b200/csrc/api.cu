@@ -35,6 +35,10 @@ struct tpt_plan {
     double *d_lamx = nullptr, *d_lamy = nullptr, *d_az = nullptr, *d_bz = nullptr, *d_cz = nullptr, *d_wz = nullptr;
     double *d_work = nullptr;   // one field
     double *d_stage = nullptr;  // staging field for tpt_solve_host (lazy)
+    // tpt_solve_host pipeline (lazy): copy streams and per-slab events
+    cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_done = nullptr;
+    std::vector<cudaEvent_t> ev_slab;   // 2 per z-slab: slab arrived, slab ready to leave
     // profiling: one set of TPT_K_COUNT+1 events per profiled solve since the last read-out
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;           // events handed out since the last read-out
@@ -57,6 +61,11 @@ void free_plan(tpt_plan *p) {
     cudaFree(p->d_work);
     cudaFree(p->d_stage);
     for (auto &e : p->ev_pool) cudaEventDestroy(e);
+    for (auto &e : p->ev_slab) cudaEventDestroy(e);
+    if (p->ev_start) cudaEventDestroy(p->ev_start);
+    if (p->ev_done) cudaEventDestroy(p->ev_done);
+    if (p->st_h2d) cudaStreamDestroy(p->st_h2d);
+    if (p->st_d2h) cudaStreamDestroy(p->st_d2h);
     delete p;
 }
 
@@ -67,25 +76,27 @@ int upload(double **dst, const std::vector<double> &src) {
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
 }
 
-tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *mat) {
-    // steps 2.1 / 2.5: all N_y*N_z lines at once, out[r][:] = in[r][:] * mat
+// The transforms act plane by plane in z, so a solve may be issued on z-slabs [k0, k0 + nk) (tpt_solve_host
+// overlaps the slabs' copies with their transforms); in / out point at plane k0.
+tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *mat, int nk) {
+    // steps 2.1 / 2.5: all N_y*nk lines at once, out[r][:] = in[r][:] * mat
     tpt::GemmArgs g{};
     g.A = in; g.B = mat; g.C = out;
-    g.M = p->ny * p->nz; g.N = p->nx; g.K = p->nx;
+    g.M = p->ny * nk; g.N = p->nx; g.K = p->nx;
     g.lda = p->nx; g.ldb = p->nx; g.ldc = p->nx;
     g.strideA = g.strideB = g.strideC = 0;
     g.batch = 1;
     return g;
 }
 
-tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat) {
+tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat, int nk) {
     // steps 2.2 / 2.4: per z-plane, out_k = mat * in_k  (strided-batched, no transposes)
     tpt::GemmArgs g{};
     g.A = mat; g.B = in; g.C = out;
     g.M = p->ny; g.N = p->nx; g.K = p->ny;
     g.lda = p->ny; g.ldb = p->nx; g.ldc = p->nx;
     g.strideA = 0; g.strideB = (int64_t)p->nx * p->ny; g.strideC = (int64_t)p->nx * p->ny;
-    g.batch = p->nz;
+    g.batch = nk;
     return g;
 }
 
@@ -95,14 +106,16 @@ cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st)
     return tpt::launch_gemm(g, p->gemm_variant >= 1 ? 1 : 0, st);
 }
 
-// Runs one slot; *launches incremented by the number of kernels enqueued.
-int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches) {
+// Runs one slot (the transforms on nk z-planes starting at in / out; the sweep always on the whole field);
+// *launches incremented by the number of kernels enqueued.
+int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int nk = -1) {
     cudaError_t e = cudaSuccess;
+    if (nk < 0) nk = p->nz;
     switch (slot) {
-        case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd), st); ++*launches; break;
-        case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv), st); ++*launches; break;
-        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd), st); ++*launches; break;
-        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv), st); ++*launches; break;
+        case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd, nk), st); ++*launches; break;
+        case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv, nk), st); ++*launches; break;
+        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd, nk), st); ++*launches; break;
+        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv, nk), st); ++*launches; break;
         case TPT_K_THOMAS:
             if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz))
                 e = tpt::launch_thomas_onchip(out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
@@ -275,6 +288,16 @@ int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_st
     return TPT_OK;
 }
 
+// z-slabs of a host solve: about 32 MiB each, at most 16 (the transforms of a slab hide under the next slab's copy)
+static int host_slabs(const tpt_plan *p) {
+    const size_t bytes = p->points() * sizeof(double);
+    size_t n = bytes / ((size_t)32 << 20);
+    if (n < 1) n = 1;
+    if (n > 16) n = 16;
+    if (n > (size_t)p->nz) n = (size_t)p->nz;
+    return (int)n;
+}
+
 int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *cuda_stream) {
     if (!p || !rhs_host || !out_host) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -283,10 +306,53 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
         cudaError_t e = cudaMalloc(&p->d_stage, bytes);
         if (e != cudaSuccess) { cudaGetLastError(); p->d_stage = nullptr; return e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
     }
-    if (cudaMemcpyAsync(p->d_stage, rhs_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TPT_ECUDA;
-    int rc = tpt_solve(p, p->d_stage, p->d_stage, st);
+    const int ns = host_slabs(p);
+    if (!p->st_h2d) {
+        if (cudaStreamCreateWithFlags(&p->st_h2d, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) != cudaSuccess)
+            return TPT_ECUDA;
+        try {
+            p->ev_slab.resize(2 * 16, nullptr);
+        } catch (const std::bad_alloc &) { return TPT_ENOMEM; }
+        for (auto &e : p->ev_slab)
+            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return TPT_ECUDA;
+    }
+    // Slab pipeline: the transforms act plane by plane, so slab s is transformed (2.1, 2.2) while slab s+1 is still
+    // on the bus; after the sweep (which needs every plane) slab s leaves while slab s+1 is transformed back.
+    const size_t plane = (size_t)p->nx * p->ny;
+    auto k_lo = [&](int s) { return (int)((long long)p->nz * s / ns); };
+    int launches = 0;
+    if (cudaEventRecord(p->ev_start, st) != cudaSuccess) return TPT_ECUDA;          // order after earlier work on st
+    if (cudaStreamWaitEvent(p->st_h2d, p->ev_start, 0) != cudaSuccess) return TPT_ECUDA;
+    for (int s = 0; s < ns; ++s) {
+        const int k0 = k_lo(s), nk = k_lo(s + 1) - k0;
+        const size_t off = plane * k0, cnt = plane * nk;
+        if (cudaMemcpyAsync(p->d_stage + off, rhs_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, p->st_h2d) != cudaSuccess ||
+            cudaEventRecord(p->ev_slab[2 * s], p->st_h2d) != cudaSuccess ||
+            cudaStreamWaitEvent(st, p->ev_slab[2 * s], 0) != cudaSuccess)
+            return TPT_ECUDA;
+        int rc = run_slot(p, TPT_K_FWD_X, p->d_stage + off, p->d_work + off, st, &launches, nk);
+        if (rc == TPT_OK) rc = run_slot(p, TPT_K_FWD_Y, p->d_work + off, p->d_stage + off, st, &launches, nk);
+        if (rc != TPT_OK) return rc;
+    }
+    int rc = run_slot(p, TPT_K_THOMAS, p->d_stage, p->d_stage, st, &launches);
     if (rc != TPT_OK) return rc;
-    if (cudaMemcpyAsync(out_host, p->d_stage, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TPT_ECUDA;
+    for (int s = 0; s < ns; ++s) {
+        const int k0 = k_lo(s), nk = k_lo(s + 1) - k0;
+        const size_t off = plane * k0, cnt = plane * nk;
+        rc = run_slot(p, TPT_K_INV_Y, p->d_stage + off, p->d_work + off, st, &launches, nk);
+        if (rc == TPT_OK) rc = run_slot(p, TPT_K_INV_X, p->d_work + off, p->d_stage + off, st, &launches, nk);
+        if (rc != TPT_OK) return rc;
+        if (cudaEventRecord(p->ev_slab[2 * s + 1], st) != cudaSuccess ||
+            cudaStreamWaitEvent(p->st_d2h, p->ev_slab[2 * s + 1], 0) != cudaSuccess ||
+            cudaMemcpyAsync(out_host + off, p->d_stage + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, p->st_d2h) != cudaSuccess)
+            return TPT_ECUDA;
+    }
+    if (cudaEventRecord(p->ev_done, p->st_d2h) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_done, 0) != cudaSuccess)
+        return TPT_ECUDA;
+    p->launches_last = launches;
     return cudaStreamSynchronize(st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
 }
 
