@@ -32,6 +32,9 @@ typedef struct tpt_plan tpt_plan; /* opaque */
 
 enum { TPT_BC_NEUMANN = 0, TPT_BC_DIRICHLET = 1 }; /* homogeneous, same at both ends of a direction */
 
+/* Implicitly treated directions L_I of the Helmholtz problem, Eq. 2b: bit 0 = x, 1 = y, 2 = z. */
+enum { TPT_DIRS_Z = 4, TPT_DIRS_YZ = 6, TPT_DIRS_XYZ = 7 };
+
 enum {
     TPT_OK = 0,
     TPT_EINVAL = -1,   /* bad argument (sizes, faces, bc, alpha, null/misaligned pointer) */
@@ -70,6 +73,19 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz,
                     const int bc[3], double helmholtz_alpha);
 
 /*
+ * tpt_plan_create_dirs — the same with a choice of the implicitly treated directions L_I of Eq. 2b
+ * (PAPER.md:59 "four choices for L_I", :209): the plan then solves (I - alpha L_I) u = f with
+ *   TPT_DIRS_XYZ  L_I = L                 all five steps (what tpt_plan_create builds),
+ *   TPT_DIRS_YZ   L_I = L_y + L_z         "the yz option omits the x transforms": steps 2.2, 2.3, 2.4,
+ *   TPT_DIRS_Z    L_I = L_z               "the z option performs only the tridiagonal solve": step 2.3.
+ * The partial choices need helmholtz_alpha > 0 (the pressure equation, Eq. 2c, always carries the full
+ * Laplacian): TPT_EINVAL otherwise.  No eigendecomposition is made for a direction that is not diagonalised.
+ */
+int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz,
+                         const double *xf, const double *yf, const double *zf,
+                         const int bc[3], double helmholtz_alpha, int implicit_dirs);
+
+/*
  * tpt_solve — steps 2.1–2.5: five kernels (+ one tiny gauge kernel on a singular
  * plan) enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
  * Asynchronous: returns after enqueueing; no host synchronisation, no allocation.
@@ -78,6 +94,18 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz,
  * A plan is not re-entrant (one workspace): order concurrent solves on one stream or use two plans.
  */
 int tpt_solve(tpt_plan *plan, const double *rhs_dev, double *out_dev, void *cuda_stream);
+
+/*
+ * tpt_solve_batch — nrhs right-hand sides of the same plan in one call ("the resulting eigenvalues and forward/inverse
+ * transform matrices are reused for every right-hand side"; the three velocity components of Eq. 2b):
+ * fields stacked densely, field r at rhs_dev + r*nx*ny*nz.  Each transform runs as ONE launch over all fields of a
+ * chunk (the stack is just a longer z axis for steps 2.1, 2.2, 2.4, 2.5); the sweep runs once per field.  A chunk is
+ * as many fields as the workspace holds: 1 unless tpt_plan_reserve_batch grew it.  Same rules as tpt_solve
+ * (asynchronous, no allocation, rhs_dev == out_dev allowed).
+ * tpt_plan_reserve_batch — grows the plan workspace to nrhs fields (synchronises the device; never shrinks).
+ */
+int tpt_solve_batch(tpt_plan *plan, const double *rhs_dev, double *out_dev, int nrhs, void *cuda_stream);
+int tpt_plan_reserve_batch(tpt_plan *plan, int nrhs);
 
 /*
  * tpt_solve_host — the same solve for HOST buffers, synchronous: returns after the result is in out_host.

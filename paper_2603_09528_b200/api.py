@@ -18,12 +18,13 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libtpt.so")
 
 NEUMANN, DIRICHLET = 0, 1
+DIRS_Z, DIRS_YZ, DIRS_XYZ = 4, 6, 7   # implicitly treated directions of Eq. 2b: bit 0 = x, 1 = y, 2 = z
 K_FWD_X, K_FWD_Y, K_THOMAS, K_INV_Y, K_INV_X, K_COUNT = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")
 
 # every symbol include/tpt.h declares (tests check the library exports exactly these)
 SYMBOLS = (
-    "tpt_plan_create", "tpt_solve", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
+    "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
 )
@@ -49,7 +50,10 @@ def lib():
         L = C.CDLL(LIB_PATH)
         vp, i, d = C.c_void_p, C.c_int, C.c_double
         L.tpt_plan_create.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d]
+        L.tpt_plan_create_dirs.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i]
         L.tpt_solve.argtypes = [vp, vp, vp, vp]
+        L.tpt_solve_batch.argtypes = [vp, vp, vp, i, vp]
+        L.tpt_plan_reserve_batch.argtypes = [vp, i]
         L.tpt_solve_host.argtypes = [vp, vp, vp, vp]
         L.tpt_plan_destroy.argtypes = [vp]
         L.tpt_plan_get_eigen.argtypes = [vp, i, _dp, _dp]
@@ -144,6 +148,12 @@ class Plan:
     def solve_host(self, rhs_host, out_host, stream=None):
         return solve_host(self, rhs_host, out_host, stream)
 
+    def solve_batch(self, rhs, out, stream=None):
+        return solve_batch(self, rhs, out, stream)
+
+    def reserve_batch(self, nrhs: int):
+        _check(lib().tpt_plan_reserve_batch(self._h, int(nrhs)), "tpt_plan_reserve_batch")
+
     def stage(self, slot: int, inp, out, stream=None):
         _check(lib().tpt_stage(self._h, slot, _dev_ptr(inp, self.points, "in"), _dev_ptr(out, self.points, "out"),
                                _stream_handle(stream)), "tpt_stage")
@@ -184,7 +194,7 @@ class Plan:
             pass
 
 
-def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0) -> Plan:
+def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0, dirs: int = DIRS_XYZ) -> Plan:
     xa, xp = _faces(xf)
     ya, yp = _faces(yf)
     za, zp = _faces(zf)
@@ -192,7 +202,8 @@ def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0) -> Pla
         raise ValueError("face arrays must have n+1 entries per direction")
     bca = (C.c_int * 3)(*[int(b) for b in bc])
     h = C.c_void_p()
-    _check(lib().tpt_plan_create(C.byref(h), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha)), "tpt_plan_create")
+    _check(lib().tpt_plan_create_dirs(C.byref(h), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha), int(dirs)),
+           "tpt_plan_create_dirs")
     return Plan(h, nx, ny, nz)
 
 
@@ -200,6 +211,16 @@ def solve(plan: Plan, rhs, out, stream=None):
     """Enqueue one solve on `stream` (default: torch's current stream).  Asynchronous."""
     _check(lib().tpt_solve(plan._h, _dev_ptr(rhs, plan.points, "rhs"), _dev_ptr(out, plan.points, "out"),
                            _stream_handle(stream)), "tpt_solve")
+    return out
+
+
+def solve_batch(plan: Plan, rhs, out, stream=None):
+    """Enqueue nrhs solves of stacked fields: rhs / out are CUDA float64 tensors of nrhs * nx*ny*nz elements."""
+    nrhs, rem = divmod(rhs.numel(), plan.points)
+    if rem or nrhs < 1:
+        raise ValueError("rhs must hold a whole number of fields")
+    _check(lib().tpt_solve_batch(plan._h, _dev_ptr(rhs, nrhs * plan.points, "rhs"), _dev_ptr(out, nrhs * plan.points, "out"),
+                                 nrhs, _stream_handle(stream)), "tpt_solve_batch")
     return out
 
 

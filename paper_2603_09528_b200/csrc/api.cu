@@ -17,6 +17,8 @@ struct tpt_plan {
     int bc[3] = {0, 0, 0};
     double alpha = 0.0;
     int singular = 0;
+    int dirs = TPT_DIRS_XYZ;      // implicitly treated directions: bit 0 = x, 1 = y, 2 = z
+    int work_fields = 1;          // fields the workspace holds (tpt_plan_reserve_batch)
     int device = 0;
     double shift0 = 0.0;          // 0 (Poisson) or -1/alpha (Helmholtz, A5)
     int gemm_variant = 2;
@@ -106,8 +108,27 @@ cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st)
     return tpt::launch_gemm(g, p->gemm_variant >= 1 ? 1 : 0, st);
 }
 
-// Runs one slot (the transforms on nk z-planes starting at in / out; the sweep always on the whole field);
-// *launches incremented by the number of kernels enqueued.
+// Step 2.3 on one field: in -> out (in == out allowed); `scratch` is a free field (used by the streaming kernel only).
+int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches) {
+    cudaError_t e;
+    if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) {
+        e = tpt::launch_thomas_onchip(in, out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
+                                      p->singular, p->sms, st);
+    } else {   // streaming kernel: in place on `out`, c' spilled to `scratch`
+        if (in != out && cudaMemcpyAsync(out, in, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+            return TPT_ECUDA;
+        e = tpt::launch_thomas(out, scratch, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
+                               p->shift0, p->singular, st);
+    }
+    ++*launches;
+    if (e == cudaSuccess && p->singular) {
+        e = tpt::launch_gauge(out, p->d_wz, p->nx, p->ny, p->nz, st);
+        ++*launches;
+    }
+    return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+// Runs one transform slot on nk z-planes starting at in / out; *launches incremented by the kernels enqueued.
 int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int nk = -1) {
     cudaError_t e = cudaSuccess;
     if (nk < 0) nk = p->nz;
@@ -116,22 +137,44 @@ int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t 
         case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv, nk), st); ++*launches; break;
         case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd, nk), st); ++*launches; break;
         case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv, nk), st); ++*launches; break;
-        case TPT_K_THOMAS:
-            if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz))
-                e = tpt::launch_thomas_onchip(out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
-                                              p->singular, p->sms, st);
-            else   // streaming kernel: in place on `out`; the plan workspace holds c'
-                e = tpt::launch_thomas(out, p->d_work, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny,
-                                       p->nz, p->shift0, p->singular, st);
-            ++*launches;
-            if (e == cudaSuccess && p->singular) {
-                e = tpt::launch_gauge(out, p->d_wz, p->nx, p->ny, p->nz, st);
-                ++*launches;
-            }
-            break;
         default: return TPT_EINVAL;
     }
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+bool slot_active(const tpt_plan *p, int slot) {
+    if (slot == TPT_K_FWD_X || slot == TPT_K_INV_X) return (p->dirs & 1) != 0;
+    if (slot == TPT_K_FWD_Y || slot == TPT_K_INV_Y) return (p->dirs & 2) != 0;
+    return slot == TPT_K_THOMAS;
+}
+
+// Steps 2.1-2.5 on nf stacked fields (nf <= work_fields).  Buffers: the transforms are out of place and alternate
+// between the plan workspace W and `out`, starting with W (rhs may alias out); the sweep works in place on whichever
+// holds the data — or straight from rhs to out when no transform is active (the "z" choice of PAPER.md:209) — so the
+// result always lands in `out`:  xyz: rhs->W->out->[T]->W->out   yz: rhs->W->[T]->out   z: rhs->[T]->out.
+int run_pipeline(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream_t st, cudaEvent_t *ev, int *launches) {
+    const double *cur = rhs;
+    double *W = p->d_work;
+    const size_t pts = p->points();
+    const int nk = p->nz * nf;
+    if (ev && cudaEventRecord(ev[0], st) != cudaSuccess) return TPT_ECUDA;
+    for (int s = 0; s < TPT_K_COUNT; ++s) {
+        int rc = TPT_OK;
+        if (s == TPT_K_THOMAS) {
+            double *dst = (cur == rhs) ? out : const_cast<double *>(cur);
+            double *scratch = (dst == W) ? out : W;
+            for (int f = 0; f < nf && rc == TPT_OK; ++f)
+                rc = run_thomas(p, cur + f * pts, dst + f * pts, scratch + f * pts, st, launches);
+            cur = dst;
+        } else if (slot_active(p, s)) {
+            double *dst = (cur == W) ? out : W;
+            rc = run_slot(p, s, cur, dst, st, launches, nk);
+            cur = dst;
+        }
+        if (rc != TPT_OK) return rc;
+        if (ev && cudaEventRecord(ev[s + 1], st) != cudaSuccess) return TPT_ECUDA;
+    }
+    return cur == out ? TPT_OK : TPT_ECUDA;
 }
 
 bool aligned16(const void *q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; }
@@ -142,7 +185,14 @@ extern "C" {
 
 int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
                     const double *zf, const int bc[3], double helmholtz_alpha) {
+    return tpt_plan_create_dirs(plan_out, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha, TPT_DIRS_XYZ);
+}
+
+int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
+                         const double *zf, const int bc[3], double helmholtz_alpha, int implicit_dirs) {
     if (!plan_out || !bc) return TPT_EINVAL;
+    if (implicit_dirs != TPT_DIRS_XYZ && implicit_dirs != TPT_DIRS_YZ && implicit_dirs != TPT_DIRS_Z) return TPT_EINVAL;
+    if (implicit_dirs != TPT_DIRS_XYZ && !(helmholtz_alpha > 0.0)) return TPT_EINVAL;   // Eq. 2c carries the full L
     if (!tpt::faces_valid(nx, xf) || !tpt::faces_valid(ny, yf) || !tpt::faces_valid(nz, zf)) return TPT_EINVAL;
     if (!bc_valid(bc[0]) || !bc_valid(bc[1]) || !bc_valid(bc[2])) return TPT_EINVAL;
     if (!(helmholtz_alpha >= 0.0) || !std::isfinite(helmholtz_alpha)) return TPT_EINVAL;
@@ -167,14 +217,19 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
     p->nx = nx; p->ny = ny; p->nz = nz;
     p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
     p->alpha = helmholtz_alpha;
+    p->dirs = implicit_dirs;
     p->device = dev;
     p->sms = sm_count;
     p->singular = (helmholtz_alpha == 0.0 && bc[0] == TPT_BC_NEUMANN && bc[1] == TPT_BC_NEUMANN &&
                    bc[2] == TPT_BC_NEUMANN) ? 1 : 0;
     // Helmholtz (I - alpha T) u = f  <=>  (T - I/alpha) u = -f/alpha: same z kernel with a constant
-    // extra shift, the -1/alpha scale folded into the forward-x matrix ("constant shift").
+    // extra shift, the -1/alpha scale folded into the first forward matrix ("constant shift").
+    // With no transform at all (the "z" choice) the sweep solves (I - alpha T_z) u = f on scaled coefficients.
+    const bool use_x = (implicit_dirs & 1) != 0, use_y = (implicit_dirs & 2) != 0;
+    const bool z_only = !use_x && !use_y;
     const double rhs_scale = helmholtz_alpha > 0.0 ? -1.0 / helmholtz_alpha : 1.0;
-    p->shift0 = helmholtz_alpha > 0.0 ? -1.0 / helmholtz_alpha : 0.0;
+    const double x_scale = use_x ? rhs_scale : 1.0, y_scale = use_x ? 1.0 : rhs_scale;
+    p->shift0 = (helmholtz_alpha > 0.0 && !z_only) ? -1.0 / helmholtz_alpha : 0.0;
 
     int rc = TPT_OK;
     try {
@@ -182,16 +237,26 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
         tpt::build_operator(nx, xf, bc[0], ox);
         tpt::build_operator(ny, yf, bc[1], oy);
         tpt::build_operator(nz, zf, bc[2], oz);
-        if (tpt::eigen_decompose(ox, p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
-        if (rc == TPT_OK) {
-            bool same = (nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
+        if (z_only) {   // (I - alpha T_z): sub/diag/super = -alpha a, 1 - alpha b, -alpha c
+            for (int k = 0; k < nz; ++k) {
+                oz.a[k] *= -helmholtz_alpha;
+                oz.b[k] = 1.0 - helmholtz_alpha * oz.b[k];
+                oz.c[k] *= -helmholtz_alpha;
+            }
+        }
+        // a direction that is not diagonalised contributes no modal shift (Eq. 9 restricted)
+        p->lamx.assign(nx, 0.0);
+        p->lamy.assign(ny, 0.0);
+        if (use_x && tpt::eigen_decompose(ox, p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
+        if (rc == TPT_OK && use_y) {
+            bool same = (use_x && nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
             if (same) { p->lamy = p->lamx; p->qy = p->qx; }
             else if (tpt::eigen_decompose(oy, p->lamy, p->qy) != 0) rc = TPT_ENUMERIC;
         }
-        if (rc == TPT_OK) {
+        if (rc == TPT_OK && use_x) {
             std::vector<double> m((size_t)nx * nx);
             for (int i = 0; i < nx; ++i) {
-                const double s = rhs_scale * std::sqrt(ox.w[i]);
+                const double s = x_scale * std::sqrt(ox.w[i]);
                 for (int k = 0; k < nx; ++k) m[(size_t)i * nx + k] = s * p->qx[(size_t)i * nx + k];
             }
             rc = upload(&p->d_xfwd, m);
@@ -202,10 +267,12 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
                 }
                 rc = upload(&p->d_xinv, m);
             }
-            m.assign((size_t)ny * ny, 0.0);
+        }
+        if (rc == TPT_OK && use_y) {
+            std::vector<double> m((size_t)ny * ny, 0.0);
             if (rc == TPT_OK) {
                 for (int j = 0; j < ny; ++j) {
-                    const double s = std::sqrt(oy.w[j]);
+                    const double s = y_scale * std::sqrt(oy.w[j]);
                     for (int k = 0; k < ny; ++k) m[(size_t)k * ny + j] = s * p->qy[(size_t)j * ny + k];
                 }
                 rc = upload(&p->d_yfwd, m);
@@ -274,17 +341,37 @@ int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_st
         ev = p->ev_pool.data() + p->ev_used;
         p->ev_used = need;
     }
-    // rhs -> W -> out -> [Thomas in place on out, c' in W] -> W -> out
-    const double *ins[TPT_K_COUNT] = {rhs_dev, p->d_work, out_dev, out_dev, p->d_work};
-    double *outs[TPT_K_COUNT] = {p->d_work, out_dev, out_dev, p->d_work, out_dev};
-    if (prof && cudaEventRecord(ev[0], st) != cudaSuccess) return TPT_ECUDA;
-    for (int s = 0; s < TPT_K_COUNT; ++s) {
-        int rc = run_slot(p, s, ins[s], outs[s], st, &launches);
-        if (rc != TPT_OK) return rc;
-        if (prof && cudaEventRecord(ev[s + 1], st) != cudaSuccess) return TPT_ECUDA;
-    }
+    int rc = run_pipeline(p, rhs_dev, out_dev, 1, st, ev, &launches);
+    if (rc != TPT_OK) return rc;
     p->launches_last = launches;
     if (prof) p->launches_accum += launches;
+    return TPT_OK;
+}
+
+int tpt_plan_reserve_batch(tpt_plan *p, int nrhs) {
+    if (!p || nrhs < 1 || (double)nrhs * (double)p->points() > 8.0e9) return TPT_EINVAL;
+    if (nrhs <= p->work_fields) return TPT_OK;
+    if (cudaDeviceSynchronize() != cudaSuccess) return TPT_ECUDA;
+    double *w = nullptr;
+    cudaError_t e = cudaMalloc(&w, (size_t)nrhs * p->points() * sizeof(double));
+    if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
+    cudaFree(p->d_work);
+    p->d_work = w;
+    p->work_fields = nrhs;
+    return TPT_OK;
+}
+
+int tpt_solve_batch(tpt_plan *p, const double *rhs_dev, double *out_dev, int nrhs, void *cuda_stream) {
+    if (!p || !rhs_dev || !out_dev || nrhs < 1 || !aligned16(rhs_dev) || !aligned16(out_dev)) return TPT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0;
+    const size_t pts = p->points();
+    for (int f0 = 0; f0 < nrhs; f0 += p->work_fields) {
+        const int nf = nrhs - f0 < p->work_fields ? nrhs - f0 : p->work_fields;
+        int rc = run_pipeline(p, rhs_dev + (size_t)f0 * pts, out_dev + (size_t)f0 * pts, nf, st, nullptr, &launches);
+        if (rc != TPT_OK) return rc;
+    }
+    p->launches_last = launches;
     return TPT_OK;
 }
 
@@ -326,28 +413,43 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
     int launches = 0;
     if (cudaEventRecord(p->ev_start, st) != cudaSuccess) return TPT_ECUDA;          // order after earlier work on st
     if (cudaStreamWaitEvent(p->st_h2d, p->ev_start, 0) != cudaSuccess) return TPT_ECUDA;
+    // buffers alternate between the staging field and the workspace, as in run_pipeline
+    double *const S = p->d_stage, *const W = p->d_work;
+    const int fwd[2] = {TPT_K_FWD_X, TPT_K_FWD_Y}, inv[2] = {TPT_K_INV_Y, TPT_K_INV_X};
+    double *cur = S;
     for (int s = 0; s < ns; ++s) {
         const int k0 = k_lo(s), nk = k_lo(s + 1) - k0;
         const size_t off = plane * k0, cnt = plane * nk;
-        if (cudaMemcpyAsync(p->d_stage + off, rhs_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, p->st_h2d) != cudaSuccess ||
+        if (cudaMemcpyAsync(S + off, rhs_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, p->st_h2d) != cudaSuccess ||
             cudaEventRecord(p->ev_slab[2 * s], p->st_h2d) != cudaSuccess ||
             cudaStreamWaitEvent(st, p->ev_slab[2 * s], 0) != cudaSuccess)
             return TPT_ECUDA;
-        int rc = run_slot(p, TPT_K_FWD_X, p->d_stage + off, p->d_work + off, st, &launches, nk);
-        if (rc == TPT_OK) rc = run_slot(p, TPT_K_FWD_Y, p->d_work + off, p->d_stage + off, st, &launches, nk);
-        if (rc != TPT_OK) return rc;
+        cur = S;
+        for (int q = 0; q < 2; ++q) {
+            if (!slot_active(p, fwd[q])) continue;
+            double *dst = cur == S ? W : S;
+            int rc = run_slot(p, fwd[q], cur + off, dst + off, st, &launches, nk);
+            if (rc != TPT_OK) return rc;
+            cur = dst;
+        }
     }
-    int rc = run_slot(p, TPT_K_THOMAS, p->d_stage, p->d_stage, st, &launches);
+    int rc = run_thomas(p, cur, cur, cur == S ? W : S, st, &launches);
     if (rc != TPT_OK) return rc;
+    double *const mid = cur;
     for (int s = 0; s < ns; ++s) {
         const int k0 = k_lo(s), nk = k_lo(s + 1) - k0;
         const size_t off = plane * k0, cnt = plane * nk;
-        rc = run_slot(p, TPT_K_INV_Y, p->d_stage + off, p->d_work + off, st, &launches, nk);
-        if (rc == TPT_OK) rc = run_slot(p, TPT_K_INV_X, p->d_work + off, p->d_stage + off, st, &launches, nk);
-        if (rc != TPT_OK) return rc;
+        cur = mid;
+        for (int q = 0; q < 2; ++q) {
+            if (!slot_active(p, inv[q])) continue;
+            double *dst = cur == S ? W : S;
+            rc = run_slot(p, inv[q], cur + off, dst + off, st, &launches, nk);
+            if (rc != TPT_OK) return rc;
+            cur = dst;
+        }
         if (cudaEventRecord(p->ev_slab[2 * s + 1], st) != cudaSuccess ||
             cudaStreamWaitEvent(p->st_d2h, p->ev_slab[2 * s + 1], 0) != cudaSuccess ||
-            cudaMemcpyAsync(out_host + off, p->d_stage + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, p->st_d2h) != cudaSuccess)
+            cudaMemcpyAsync(out_host + off, cur + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, p->st_d2h) != cudaSuccess)
             return TPT_ECUDA;
     }
     if (cudaEventRecord(p->ev_done, p->st_d2h) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_done, 0) != cudaSuccess)
@@ -367,6 +469,7 @@ int tpt_plan_get_eigen(const tpt_plan *p, int dir, double *lambda_host, double *
     if (!p || (dir != 0 && dir != 1)) return TPT_EINVAL;
     const std::vector<double> &l = dir == 0 ? p->lamx : p->lamy;
     const std::vector<double> &q = dir == 0 ? p->qx : p->qy;
+    if (q.empty()) return TPT_EINVAL;   // this plan does not diagonalise that direction
     if (lambda_host) std::memcpy(lambda_host, l.data(), l.size() * sizeof(double));
     if (qtilde_host) std::memcpy(qtilde_host, q.data(), q.size() * sizeof(double));
     return TPT_OK;
@@ -378,7 +481,7 @@ int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
     if (!p || !bytes_out) return TPT_EINVAL;
     size_t b = 2 * ((size_t)p->nx * p->nx + (size_t)p->ny * p->ny) * sizeof(double);
     b += ((size_t)p->nx + p->ny + 4 * (size_t)p->nz + 8) * sizeof(double);
-    b += p->points() * sizeof(double) * (p->d_stage ? 2 : 1);
+    b += p->points() * sizeof(double) * ((size_t)p->work_fields + (p->d_stage ? 1 : 0));
     *bytes_out = b;
     return TPT_OK;
 }
@@ -388,13 +491,9 @@ int tpt_stage(tpt_plan *p, int slot, const double *in_dev, double *out_dev, void
     if (!aligned16(in_dev) || !aligned16(out_dev)) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int launches = 0;
-    if (slot == TPT_K_THOMAS) {
-        if (in_dev != out_dev &&
-            cudaMemcpyAsync(out_dev, in_dev, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
-            return TPT_ECUDA;
-    } else if (in_dev == out_dev) {
-        return TPT_EINVAL;   // the transforms are out of place
-    }
+    if (!slot_active(p, slot)) return TPT_EINVAL;   // this plan does not diagonalise that direction
+    if (slot == TPT_K_THOMAS) return run_thomas(p, in_dev, out_dev, p->d_work, st, &launches);
+    if (in_dev == out_dev) return TPT_EINVAL;   // the transforms are out of place
     return run_slot(p, slot, in_dev, out_dev, st, &launches);
 }
 

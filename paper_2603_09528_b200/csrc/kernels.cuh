@@ -40,12 +40,13 @@ cudaError_t launch_thomas(double *x, double *cprime, const double *az, const dou
                           int singular, cudaStream_t stream);
 
 // Same solve with the z-columns resident on chip (thomas_onchip.cu): 16 B/pt of HBM traffic, no scratch field.
+// Reads the right-hand sides from `in` and writes the solution to `x` (in == x: in place).
 // tab: device copy of the two tables thomas_onchip_tables() builds (8 * (nz + THOMAS_TABLE_PAD) doubles).
 // sms = SM count.
 constexpr int THOMAS_TABLE_PAD = 64;
 bool thomas_onchip_supported(int nx, int ny, int nz);
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out);
-cudaError_t launch_thomas_onchip(double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
+cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
                                  int nz, double shift0, int singular, int sms, cudaStream_t stream);
 
 // Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean).

@@ -34,7 +34,8 @@ constexpr int ROW_BYTES = TCOLS * (int)sizeof(double);
 
 template <int M, int MAXT>
 __global__ void __launch_bounds__(MAXT)
-thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__restrict__ tab_reg,
+thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_out,
+                     const double *__restrict__ tab_reg,
                      const double *__restrict__ tab_null, const double *__restrict__ lamx,
                      const double *__restrict__ lamy, int nx, int nz, int S, int nbuf, int box_rows, int nbox,
                      int buf_rows, double shift0, int singular, int ntiles) {
@@ -50,6 +51,7 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__r
 
     if (tid == 0) {
         ptx::tma_prefetch_desc(&tmap);
+        ptx::tma_prefetch_desc(&tmap_out);
         for (int b = 0; b < nbuf; ++b) ptx::mbar_init(&full[b], 1);
         ptx::fence_mbar_init();
     }
@@ -184,7 +186,7 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const double *__r
         if (tid == 0) {                        // rows past nz are clipped by the tensor map
             const double *src = bufs + (size_t)b * tile_elems;
             for (int q = 0; q < nbox; ++q)
-                ptx::tma_store_2d(&tmap, tile * TCOLS, q * box_rows, src + (size_t)q * box_rows * TCOLS);
+                ptx::tma_store_2d(&tmap_out, tile * TCOLS, q * box_rows, src + (size_t)q * box_rows * TCOLS);
             ptx::bulk_commit();
         }
         if (++b == nbuf) {
@@ -213,20 +215,20 @@ EncodeTiledFn encode_tiled_fn() {
 }
 
 // field viewed as a 2-D tensor: dim0 = nx*ny contiguous columns, dim1 = nz rows of stride nx*ny
-bool make_field_map(CUtensorMap *map, double *x, size_t plane, int nz, int box_rows) {
+bool make_field_map(CUtensorMap *map, const double *x, size_t plane, int nz, int box_rows) {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)plane, (cuuint64_t)nz};
     const cuuint64_t strides[1] = {(cuuint64_t)plane * sizeof(double)};
     const cuuint32_t box[2] = {(cuuint32_t)TCOLS, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
-    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, x, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(x), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <int M, int MAXT>
-cudaError_t launch_m(double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny, int nz,
+cudaError_t launch_m(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny, int nz,
                      double shift0, int singular, int sms, cudaStream_t stream) {
     int S = (nz + M - 1) / M;
     if (S & 1) ++S;                                          // whole warps: 2 segments x 16 columns
@@ -259,13 +261,14 @@ cudaError_t launch_m(double *x, const double *tab, const double *lamx, const dou
         per_sm_cache[0] = key;
         per_sm_cache[1] = per_sm;
     }
-    CUtensorMap tmap;
-    if (!make_field_map(&tmap, x, (size_t)nx * ny, nz, box_rows)) return cudaErrorUnknown;
+    CUtensorMap tmap, tmap_out;
+    if (!make_field_map(&tmap, in, (size_t)nx * ny, nz, box_rows)) return cudaErrorUnknown;
+    if (!make_field_map(&tmap_out, x, (size_t)nx * ny, nz, box_rows)) return cudaErrorUnknown;
     const int ntiles = (int)(((size_t)nx * ny) / TCOLS);
     int grid = sms * per_sm_cache[1];
     if (grid > ntiles) grid = ntiles;
     thomas_onchip_kernel<M, MAXT><<<grid, threads, smem, stream>>>(
-        tmap, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf, box_rows, nbox, buf_rows, shift0,
+        tmap, tmap_out, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf, box_rows, nbox, buf_rows, shift0,
         singular, ntiles);
     return cudaGetLastError();
 }
@@ -276,12 +279,12 @@ bool thomas_onchip_supported(int nx, int ny, int nz) {
     return ((size_t)nx * ny) % TCOLS == 0 && nz >= 2 && nz <= 768;
 }
 
-cudaError_t launch_thomas_onchip(double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
+cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
                                  int nz, double shift0, int singular, int sms, cudaStream_t stream) {
     if (!thomas_onchip_supported(nx, ny, nz)) return cudaErrorInvalidValue;
-    if (nz <= 128) return launch_m<8, 256>(x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    if (nz <= 512) return launch_m<16, 512>(x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    return launch_m<32, 384>(x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+    if (nz <= 128) return launch_m<8, 256>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+    if (nz <= 512) return launch_m<16, 512>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+    return launch_m<32, 384>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
 }
 
 // Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows

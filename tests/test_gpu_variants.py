@@ -1,0 +1,191 @@
+"""GPU parity tests of the widened rows: partial implicit-diffusion variants,
+batched multi-RHS solves, and the slab-pipelined host path — each against the CPU oracle or, where the claim is
+"same arithmetic, different schedule", bit-for-bit against the plain device solve."""
+import numpy as np
+import pytest
+
+from paper_2603_09528_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+PARITY_TOL = 1e-10
+RESID_TOL = 1e-11
+N_, D_ = I.NEUMANN, I.DIRICHLET
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def tpt(torch):
+    from paper_2603_09528_b200 import api
+
+    api.lib()
+    return api
+
+
+def _rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def _solve(torch, plan, f, inplace=False):
+    d_f = torch.from_numpy(np.ascontiguousarray(f)).cuda()
+    d_o = d_f if inplace else torch.empty_like(d_f)
+    plan.solve(d_f, d_o)
+    torch.cuda.synchronize()
+    return d_o.cpu().numpy()
+
+
+DIRS_CASES = [
+    # name, n, L, beta, bc, alpha
+    ("ragged", (40, 36, 33), (1.0, 1.0, 2.0), (2.0, 1.5, 2.5), (N_, N_, D_), 1e-3),      # generic GEMM, streaming-capable
+    ("odd", (5, 7, 6), (1.0, 2.0, 1.5), (1.2, 2.0, 1.0), (N_, D_, D_), 0.4),             # nx*ny % 16 != 0: streaming sweep
+    ("t128", (256, 128, 48), (2.0, 1.0, 1.0), (2.5, 2.0, 3.0), (N_, N_, D_), 5e-4),      # TMA GEMM + on-chip sweep
+    ("t128-nnn", (128, 128, 40), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 2e-2),  # all-Neumann Helmholtz: regular
+]
+
+
+@pytest.mark.parametrize("case", DIRS_CASES, ids=[c[0] for c in DIRS_CASES])
+@pytest.mark.parametrize("dirs_name", ["z", "yz", "xyz"])
+@pytest.mark.parametrize("thomas_variant", [1, 0])
+def test_partial_dirs_parity(tpt, torch, orc, case, dirs_name, thomas_variant):
+    name, n, L, beta, bc, alpha = case
+    dirs = {"z": tpt.DIRS_Z, "yz": tpt.DIRS_YZ, "xyz": tpt.DIRS_XYZ}[dirs_name]
+    P = I.Problem(name, n, L, beta, bc, alpha, seed=31 + n[0])
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, bc, alpha, dirs=dirs)
+    plan.set_thomas_variant(thomas_variant)
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha, dirs=dirs).solve(f)
+    for inplace in (False, True):
+        u = _solve(torch, plan, f, inplace)
+        assert _rel(u, ref) <= PARITY_TOL
+        r = orc.residual_norms(xf, yf, zf, bc, alpha, f, u, dirs=dirs)
+        assert r["rel2"] <= RESID_TOL and r["relL2vol"] <= RESID_TOL
+    assert not plan.singular
+    plan.destroy()
+
+
+def test_partial_dirs_argument_checks_and_skipped_slots(tpt, torch):
+    P = I.Problem("chk", (32, 16, 16), (1.0, 1.0, 1.0), (1.0, 1.0, 1.0), (N_, N_, D_), 1e-2, 3)
+    xf, yf, zf = P.faces()
+    with pytest.raises(tpt.TptError):
+        tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0, dirs=tpt.DIRS_YZ)      # Poisson carries the full Laplacian (Eq. 2c)
+    with pytest.raises(tpt.TptError):
+        tpt.plan_create(*P.n, xf, yf, zf, P.bc, 1e-2, dirs=5)
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 1e-2, dirs=tpt.DIRS_YZ)
+    with pytest.raises(tpt.TptError):
+        plan.eigen(0)                                                        # x is not diagonalised
+    lamy, qy = plan.eigen(1)
+    assert np.abs(qy.T @ qy - np.eye(16)).max() < 1e-13
+    d = torch.from_numpy(P.rhs()).cuda()
+    o = torch.empty_like(d)
+    with pytest.raises(tpt.TptError):
+        plan.stage(tpt.K_FWD_X, d, o)
+    plan.set_profiling(True)
+    plan.solve(d, o)
+    ms, launches, solves = plan.kernel_times()
+    assert launches == 3 and solves == 1                                     # fwd y, sweep, inv y
+    plan.destroy()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 1e-2, dirs=tpt.DIRS_Z)
+    plan.set_profiling(True)
+    plan.solve(d, o)
+    assert plan.kernel_times()[1] == 1                                       # "only the tridiagonal solve"
+    plan.destroy()
+
+
+@pytest.mark.parametrize("dirs_name", ["z", "yz"])
+def test_partial_dirs_c5_helmholtz_thin_z(tpt, torch, orc, dirs_name):
+    # BASELINE configs[4]'s Helmholtz plan (768 x 768, beta = 3, alpha = 5e-4) on a 16-cell z slab
+    dirs = {"z": tpt.DIRS_Z, "yz": tpt.DIRS_YZ}[dirs_name]
+    P = I.CONFIGS["c5"][0].thin_z(16)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, dirs=dirs)
+    u = _solve(torch, plan, f)
+    ref = orc.OraclePlan(xf, yf, zf, P.bc, P.alpha, dirs=dirs).solve(f)
+    assert _rel(u, ref) <= PARITY_TOL
+    plan.destroy()
+
+
+@pytest.mark.parametrize("dirs_name", ["z", "yz", "xyz"])
+@pytest.mark.parametrize("reserve", [1, 2, 3])
+def test_batched_solve_equals_single_solves(tpt, torch, orc, dirs_name, reserve):
+    # three right-hand sides of one Helmholtz plan (the velocity components of Eq. 2b): same bits as three solves
+    dirs = {"z": tpt.DIRS_Z, "yz": tpt.DIRS_YZ, "xyz": tpt.DIRS_XYZ}[dirs_name]
+    P = I.Problem("batch", (128, 128, 24), (1.0, 1.0, 1.0), (2.0, 2.0, 2.5), (N_, N_, D_), 1e-3, 8)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, dirs=dirs)
+    fs = np.stack([I.uniform_pm1(100 + r, P.points).reshape(P.n[::-1]) for r in range(3)])
+    singles = np.stack([_solve(torch, plan, fs[r]) for r in range(3)])
+    plan.reserve_batch(reserve)
+    d = torch.from_numpy(fs).cuda()
+    o = torch.empty_like(d)
+    plan.solve_batch(d, o)
+    torch.cuda.synchronize()
+    assert np.array_equal(o.cpu().numpy(), singles)
+    plan.solve_batch(d, d)                                                   # in place
+    torch.cuda.synchronize()
+    assert np.array_equal(d.cpu().numpy(), singles)
+    ref = orc.OraclePlan(xf, yf, zf, P.bc, P.alpha, dirs=dirs).solve(fs[2])
+    assert _rel(singles[2], ref) <= PARITY_TOL
+    assert plan.device_bytes() >= reserve * P.points * 8
+    plan.destroy()
+
+
+def test_batched_solve_singular_plan_gauges_every_field(tpt, torch):
+    P = I.Problem("batch-sing", (64, 64, 32), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, 9)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0)
+    plan.reserve_batch(2)
+    fs = np.stack([I.remove_weighted_mean(I.uniform_pm1(7 + r, P.points).reshape(P.n[::-1]), xf, yf, zf) for r in range(2)])
+    d = torch.from_numpy(fs).cuda()
+    o = torch.empty_like(d)
+    plan.solve_batch(d, o)
+    torch.cuda.synchronize()
+    out = o.cpu().numpy()
+    V = np.diff(zf)[:, None, None] * np.diff(yf)[None, :, None] * np.diff(xf)[None, None, :]
+    for r in range(2):
+        assert np.array_equal(out[r], _solve(torch, plan, fs[r]))
+        assert abs((V * out[r]).sum()) < 1e-13 * np.abs(out[r]).max() * V.sum()
+    plan.destroy()
+
+
+@pytest.mark.parametrize("dirs_name,nz", [("xyz", 161), ("yz", 160), ("z", 160)])
+def test_host_path_slab_pipeline_equals_device_solve(tpt, torch, dirs_name, nz):
+    # 80 MiB field -> the host solve crosses the bus in 2 z-slabs (uneven for nz = 161); the transforms act plane
+    # by plane, so the result must equal the one-shot device solve bit for bit.
+    dirs = {"z": tpt.DIRS_Z, "yz": tpt.DIRS_YZ, "xyz": tpt.DIRS_XYZ}[dirs_name]
+    P = I.Problem("host", (256, 256, nz), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, D_), 1e-3, 12)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, dirs=dirs)
+    dev = _solve(torch, plan, f)
+    h_in = torch.from_numpy(f).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    for _ in range(2):
+        h_out.zero_()
+        plan.solve_host(h_in, h_out)
+        assert np.array_equal(h_out.numpy(), dev)
+    plan.solve_host(h_in, h_in)                                              # aliasing host buffers
+    assert np.array_equal(h_in.numpy(), dev)
+    plan.destroy()
+
+
+def test_host_path_poisson_singular_multi_slab(tpt, torch, orc):
+    P = I.Problem("host-sing", (256, 128, 320), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, 13)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0)
+    dev = _solve(torch, plan, f)
+    out = np.empty_like(f)
+    plan.solve_host(f, out)                                                  # pageable buffers, 2 slabs
+    assert np.array_equal(out, dev)
+    r = orc.residual_norms(xf, yf, zf, P.bc, 0.0, f, out)
+    assert r["rel2"] <= RESID_TOL
+    plan.destroy()
