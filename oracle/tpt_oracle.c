@@ -24,7 +24,7 @@ int orc_num_threads(void) {
 #endif
 }
 
-static int bc_ok(int bc) { return bc == ORC_BC_NEUMANN || bc == ORC_BC_DIRICHLET; }
+static int bc_ok(int bc) { return bc == ORC_BC_NEUMANN || bc == ORC_BC_DIRICHLET || bc == ORC_BC_PERIODIC; }
 
 static int faces_ok(int n, const double *xf) {
     if (n < 2 || !xf) return 0;
@@ -34,8 +34,10 @@ static int faces_ok(int n, const double *xf) {
 }
 
 /* Centre spacings delta[0..n] [A2,A3]: delta_i = x_c,i - x_c,i-1 for interior faces (the paper's
- * Delta x_{i-1/2}); boundary faces use the mirror ghost cell, delta_0 = w_0, delta_n = w_{n-1}. */
-static void centre_spacings(int n, const double *xf, double *delta) {
+ * Delta x_{i-1/2}); boundary faces use the mirror ghost cell, delta_0 = w_0, delta_n = w_{n-1}.
+ * Periodic [A17]: face 0 and face n are the same face, between cell n-1 (one period back) and cell 0:
+ * delta_0 = delta_n = (w_0 + w_{n-1})/2. */
+static void centre_spacings(int n, const double *xf, int bc, double *delta) {
     for (int i = 1; i < n; ++i) {
         double xc_i = 0.5 * (xf[i] + xf[i + 1]);
         double xc_im = 0.5 * (xf[i - 1] + xf[i]);
@@ -43,6 +45,7 @@ static void centre_spacings(int n, const double *xf, double *delta) {
     }
     delta[0] = xf[1] - xf[0];
     delta[n] = xf[n] - xf[n - 1];
+    if (bc == ORC_BC_PERIODIC) delta[0] = delta[n] = 0.5 * ((xf[1] - xf[0]) + (xf[n] - xf[n - 1]));
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -50,17 +53,25 @@ static void centre_spacings(int n, const double *xf, double *delta) {
  * b_i = -(a_i + c_i) follow from Eq. 3 [A1].  Boundary rows [A3]: homogeneous Neumann mirrors
  * phi_{-1} = phi_0 (b_0 += a_0); homogeneous Dirichlet at the boundary FACE mirrors
  * phi_{-1} = -phi_0 (b_0 -= a_0); likewise at the far end.  a_0 and c_{n-1} are then zeroed.
+ * Periodic ("periodic couplings add the cyclic corner entries") [A17]: phi_{-1} = phi_{n-1},
+ * phi_n = phi_0; rows 0 and n-1 are ordinary rows and a_0 (coupling to cell n-1), c_{n-1} (coupling
+ * to cell 0) are KEPT as the corner entries.  Needs n >= 3 (with n = 2 the two couplings coincide).
  * ------------------------------------------------------------------------------------------ */
 int orc_operator_1d(int n, const double *xf, int bc, double *w, double *a, double *b, double *c) {
     if (!faces_ok(n, xf) || !bc_ok(bc) || !w || !a || !b || !c) return ORC_EINVAL;
+    if (bc == ORC_BC_PERIODIC && n < 3) return ORC_EINVAL;
     double *delta = (double *)malloc((size_t)(n + 1) * sizeof(double));
     if (!delta) return ORC_ENOMEM;
-    centre_spacings(n, xf, delta);
+    centre_spacings(n, xf, bc, delta);
     for (int i = 0; i < n; ++i) {
         w[i] = xf[i + 1] - xf[i];
         a[i] = 1.0 / (w[i] * delta[i]);
         c[i] = 1.0 / (w[i] * delta[i + 1]);
         b[i] = -(a[i] + c[i]);
+    }
+    if (bc == ORC_BC_PERIODIC) {
+        free(delta);
+        return ORC_OK;
     }
     if (bc == ORC_BC_NEUMANN) {
         b[0] += a[0];
@@ -145,11 +156,18 @@ static int jacobi_eig(int n, double *A, double *Vt) {
 /* ------------------------------------------------------------------------------------------
  * Factored form  -T~ = B^T B  [A9; DESIGN.md §Accuracy rule].  Rows of B, one per face carrying a
  * flux: interior face f (between cells f-1 and f): (B q)_f = (q_f/sqrt(w_f) - q_{f-1}/sqrt(w_{f-1}))/sqrt(delta_f);
- * Dirichlet boundary face: sqrt(2) q_0 / w_0 (resp. q_{n-1}/w_{n-1}); Neumann boundary face: no row.
+ * Dirichlet boundary face: sqrt(2) q_0 / w_0 (resp. q_{n-1}/w_{n-1}); Neumann boundary face: no row;
+ * periodic: one more interior row for the wrap-around face.
  * BX has nrows_B rows and n columns; X is n x n row-major, column m = vector m.
  * ------------------------------------------------------------------------------------------ */
 static int apply_B(int n, const double *w, const double *delta, int bc, const double *X, double *BX) {
     int row = 0;
+    if (bc == ORC_BC_PERIODIC) {   /* the wrap-around face between cell n-1 and cell 0 is an interior face */
+        double sf = 1.0 / sqrt(w[0]), sm = 1.0 / sqrt(w[n - 1]), sd = 1.0 / sqrt(delta[0]);
+        const double *Xm = X + (size_t)(n - 1) * n;
+        for (int m = 0; m < n; ++m) BX[m] = (X[m] * sf - Xm[m] * sm) * sd;
+        ++row;
+    }
     if (bc == ORC_BC_DIRICHLET) {
         double s = sqrt(2.0) / w[0];
         for (int m = 0; m < n; ++m) BX[(size_t)row * n + m] = s * X[m];
@@ -261,7 +279,7 @@ int orc_eig_1d(int n, const double *xf, int bc, int refine_steps, double *lambda
 
     orc_operator_1d(n, xf, bc, w, a, b, c);
     orc_symmetrize_1d(n, w, a, b, c, dg, of);
-    centre_spacings(n, xf, delta);
+    centre_spacings(n, xf, bc, delta);
 
     /* 1.2: T~ = Q~ Lambda Q~^T — base solver: cyclic Jacobi on the dense form of T~. */
     memset(A, 0, sizeof(double) * nn);
@@ -269,6 +287,11 @@ int orc_eig_1d(int n, const double *xf, int bc, int refine_steps, double *lambda
     for (int i = 0; i + 1 < n; ++i) {
         A[(size_t)i * n + i + 1] = of[i];
         A[(size_t)(i + 1) * n + i] = of[i];
+    }
+    if (bc == ORC_BC_PERIODIC) {   /* cyclic corners ("symmetric cyclic operator, stored as a dense matrix") */
+        double corner = sqrt(w[n - 1] / w[0]) * c[n - 1];      /* = sqrt(c_{n-1} a_0) */
+        A[(size_t)(n - 1) * n] = corner;
+        A[n - 1] = corner;
     }
     jacobi_eig(n, A, Vt);
     for (int i = 0; i < n; ++i)
@@ -311,7 +334,7 @@ int orc_eig_1d(int n, const double *xf, int bc, int refine_steps, double *lambda
     }
     /* Neumann–Neumann: the null pair is known exactly: lambda = 0, q~_i = sqrt(w_i/L)
      * (T 1 = 0  =>  T~ D^{1/2} 1 = 0). */
-    if (bc == ORC_BC_NEUMANN) {
+    if (bc == ORC_BC_NEUMANN || bc == ORC_BC_PERIODIC) {
         double L = 0.0;
         for (int i = 0; i < n; ++i) L += w[i];
         lambda[0] = 0.0;
@@ -372,6 +395,8 @@ int orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
                              const double *lamx, const double *qx, const double *lamy, const double *qy) {
     if (!out || !bc || !faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf)) return ORC_EINVAL;
     if (!bc_ok(bc[0]) || !bc_ok(bc[1]) || !bc_ok(bc[2]) || !(alpha >= 0.0) || !isfinite(alpha)) return ORC_EINVAL;
+    /* periodic directions are diagonalised (x, y); the z sweep is the plain Thomas algorithm */
+    if (bc[2] == ORC_BC_PERIODIC || (bc[0] == ORC_BC_PERIODIC && nx < 3) || (bc[1] == ORC_BC_PERIODIC && ny < 3)) return ORC_EINVAL;
     if (!lamx || !qx || !lamy || !qy) return ORC_EINVAL;
     orc_plan *p = (orc_plan *)calloc(1, sizeof(orc_plan));
     if (!p) return ORC_ENOMEM;
@@ -379,7 +404,7 @@ int orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
     p->dirs = ORC_DIRS_XYZ;
     p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
     /* [A7] structural detection of the null mode: all-Neumann and Poisson. */
-    p->singular = (alpha == 0.0 && bc[0] == ORC_BC_NEUMANN && bc[1] == ORC_BC_NEUMANN && bc[2] == ORC_BC_NEUMANN);
+    p->singular = (alpha == 0.0 && bc[0] != ORC_BC_DIRICHLET && bc[1] != ORC_BC_DIRICHLET && bc[2] == ORC_BC_NEUMANN);
     p->wx = dup_array(NULL, nx); p->wy = dup_array(NULL, ny); p->wz = dup_array(NULL, nz);
     p->az = dup_array(NULL, nz); p->bz = dup_array(NULL, nz); p->cz = dup_array(NULL, nz);
     p->lamx = dup_array(lamx, nx); p->lamy = dup_array(lamy, ny);
@@ -402,7 +427,7 @@ int orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
 int orc_plan_create(orc_plan **out, int nx, int ny, int nz,
                     const double *xf, const double *yf, const double *zf, const int bc[3], double alpha) {
     if (!out || !bc || !faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf)) return ORC_EINVAL;
-    if (!bc_ok(bc[0]) || !bc_ok(bc[1]) || !bc_ok(bc[2])) return ORC_EINVAL;
+    if (!bc_ok(bc[0]) || !bc_ok(bc[1]) || !bc_ok(bc[2]) || bc[2] == ORC_BC_PERIODIC) return ORC_EINVAL;
     double *lamx = dup_array(NULL, nx), *lamy = dup_array(NULL, ny);
     double *qx = dup_array(NULL, (size_t)nx * nx), *qy = dup_array(NULL, (size_t)ny * ny);
     int rc = ORC_ENOMEM;
@@ -606,9 +631,15 @@ int orc_solve(const orc_plan *p, const double *f, double *phi, double *work) {
  * Ghost values [A3]: Neumann phi_ghost = phi_boundary-cell (zero flux); Dirichlet phi_ghost = -phi.
  * ------------------------------------------------------------------------------------------ */
 static double lap1d_flux(const double *xf, int n, int bc, int i, double um, double u0, double up) {
-    /* um/up are neighbours or ignored at the boundary */
+    /* um/up are neighbours (periodic: the wrapped ones) or ignored at a Neumann/Dirichlet boundary */
     double w = xf[i + 1] - xf[i];
     double fl, fr;
+    if (bc == ORC_BC_PERIODIC && (i == 0 || i == n - 1)) {
+        double dwrap = 0.5 * ((xf[1] - xf[0]) + (xf[n] - xf[n - 1]));
+        double dl = i == 0 ? dwrap : 0.5 * (xf[i] + xf[i + 1]) - 0.5 * (xf[i - 1] + xf[i]);
+        double dr = i == n - 1 ? dwrap : 0.5 * (xf[i + 1] + xf[i + 2]) - 0.5 * (xf[i] + xf[i + 1]);
+        return ((up - u0) / dr - (u0 - um) / dl) / w;
+    }
     if (i > 0) {
         double dl = 0.5 * (xf[i] + xf[i + 1]) - 0.5 * (xf[i - 1] + xf[i]);
         fl = (u0 - um) / dl;
@@ -642,9 +673,13 @@ int orc_apply_operator_flux_dirs(int nx, int ny, int nz, const double *xf, const
             for (int i = 0; i < nx; ++i) {
                 size_t id = i + (size_t)nx * j + plane * k;
                 double u0 = phi[id];
-                double lx = lap1d_flux(xf, nx, bc[0], i, i > 0 ? phi[id - 1] : 0.0, u0, i < nx - 1 ? phi[id + 1] : 0.0);
-                double ly = lap1d_flux(yf, ny, bc[1], j, j > 0 ? phi[id - nx] : 0.0, u0, j < ny - 1 ? phi[id + nx] : 0.0);
-                double lz = lap1d_flux(zf, nz, bc[2], k, k > 0 ? phi[id - plane] : 0.0, u0, k < nz - 1 ? phi[id + plane] : 0.0);
+                const int px = bc[0] == ORC_BC_PERIODIC, py = bc[1] == ORC_BC_PERIODIC, pz = bc[2] == ORC_BC_PERIODIC;
+                double lx = lap1d_flux(xf, nx, bc[0], i, i > 0 ? phi[id - 1] : (px ? phi[id + (nx - 1)] : 0.0), u0,
+                                       i < nx - 1 ? phi[id + 1] : (px ? phi[id - (nx - 1)] : 0.0));
+                double ly = lap1d_flux(yf, ny, bc[1], j, j > 0 ? phi[id - nx] : (py ? phi[id + (size_t)nx * (ny - 1)] : 0.0), u0,
+                                       j < ny - 1 ? phi[id + nx] : (py ? phi[id - (size_t)nx * (ny - 1)] : 0.0));
+                double lz = lap1d_flux(zf, nz, bc[2], k, k > 0 ? phi[id - plane] : (pz ? phi[id + plane * (nz - 1)] : 0.0), u0,
+                                       k < nz - 1 ? phi[id + plane] : (pz ? phi[id - plane * (nz - 1)] : 0.0));
                 double lap = ((dirs & 1) ? lx : 0.0) + ((dirs & 2) ? ly : 0.0) + lz;
                 out[id] = (alpha == 0.0) ? lap : u0 - alpha * lap;
             }
@@ -719,7 +754,7 @@ int orc_dense_solve_3d_dirs(int nx, int ny, int nz, const double *xf, const doub
     if (!faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf) || !bc || !f || !phi) return ORC_EINVAL;
     long n = (long)nx * ny * nz;
     if (n > 4096) return ORC_EINVAL;
-    int singular = (alpha == 0.0 && bc[0] == ORC_BC_NEUMANN && bc[1] == ORC_BC_NEUMANN && bc[2] == ORC_BC_NEUMANN);
+    int singular = (alpha == 0.0 && bc[0] != ORC_BC_DIRICHLET && bc[1] != ORC_BC_DIRICHLET && bc[2] != ORC_BC_DIRICHLET);
     long N = n + (singular ? 1 : 0);
     double *M = (double *)calloc((size_t)N * (N + 1), sizeof(double));   /* augmented [M | rhs] */
     double *co[3][4];
@@ -740,7 +775,9 @@ int orc_dense_solve_3d_dirs(int nx, int ny, int nz, const double *xf, const doub
                     int q = id[d];
                     row[r] += co[d][2][q];
                     if (q > 0) row[r - st[d]] += co[d][1][q];
+                    else if (bc[d] == ORC_BC_PERIODIC) row[r + st[d] * (nn[d] - 1)] += co[d][1][q];   /* cyclic corner */
                     if (q < nn[d] - 1) row[r + st[d]] += co[d][3][q];
+                    else if (bc[d] == ORC_BC_PERIODIC) row[r - st[d] * (nn[d] - 1)] += co[d][3][q];
                 }
                 if (alpha != 0.0) {
                     for (long cidx = 0; cidx < n; ++cidx) row[cidx] *= -alpha;

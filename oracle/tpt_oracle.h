@@ -33,7 +33,8 @@
 extern "C" {
 #endif
 
-enum { ORC_BC_NEUMANN = 0, ORC_BC_DIRICHLET = 1 };
+/* PERIODIC (P:102 cyclic corners, P:211 dense cyclic operator): x and y only — the z sweep is the plain Thomas algorithm. */
+enum { ORC_BC_NEUMANN = 0, ORC_BC_DIRICHLET = 1, ORC_BC_PERIODIC = 2 };
 /* Implicitly treated directions L_I of the Helmholtz problem, Eq. 2b: bit 0 = x, 1 = y, 2 = z. */
 enum { ORC_DIRS_Z = 4, ORC_DIRS_YZ = 6, ORC_DIRS_XYZ = 7 };
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ENUMERIC = -4 };

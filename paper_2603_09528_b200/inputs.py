@@ -24,6 +24,7 @@ import numpy as np
 
 NEUMANN = 0
 DIRICHLET = 1
+PERIODIC = 2      # x and y only; the paper's benchmark BCs are periodic x, Neumann y, z
 
 _M1 = np.uint64(0xBF58476D1CE4E5B9)
 _M2 = np.uint64(0x94D049BB133111EB)
@@ -78,13 +79,13 @@ class Problem:
     n: tuple            # (nx, ny, nz)
     length: tuple       # (Lx, Ly, Lz)
     beta: tuple         # tanh beta per direction (0 = uniform)
-    bc: tuple           # (bc_x, bc_y, bc_z) in {NEUMANN, DIRICHLET}
+    bc: tuple           # (bc_x, bc_y, bc_z) in {NEUMANN, DIRICHLET, PERIODIC}
     alpha: float        # 0 -> Poisson  L phi = f ; > 0 -> (I - alpha L) u = f
     seed: int
 
     @property
     def singular(self) -> bool:
-        return self.alpha == 0.0 and all(b == NEUMANN for b in self.bc)
+        return self.alpha == 0.0 and all(b != DIRICHLET for b in self.bc)
 
     @property
     def points(self) -> int:
