@@ -30,7 +30,10 @@ extern "C" {
 
 typedef struct tpt_plan tpt_plan; /* opaque */
 
-enum { TPT_BC_NEUMANN = 0, TPT_BC_DIRICHLET = 1 }; /* homogeneous, same at both ends of a direction */
+/* Homogeneous, the same at both ends of a direction.  PERIODIC (PAPER.md:102 "cyclic corners", :211 dense cyclic
+ * operator; the paper's benchmark BCs are periodic x, Neumann y and z) is accepted for x and y,
+ * the diagonalised directions; the z sweep is the plain Thomas algorithm, so periodic z is TPT_EINVAL. */
+enum { TPT_BC_NEUMANN = 0, TPT_BC_DIRICHLET = 1, TPT_BC_PERIODIC = 2 };
 
 /* Implicitly treated directions L_I of the Helmholtz problem, Eq. 2b: bit 0 = x, 1 = y, 2 = z. */
 enum { TPT_DIRS_Z = 4, TPT_DIRS_YZ = 6, TPT_DIRS_XYZ = 7 };
@@ -62,7 +65,7 @@ enum {
  *   nx, ny, nz >= 2 cells.  xf, yf, zf: HOST, face coordinates, lengths nx+1, ny+1, nz+1, finite and
  *   strictly increasing.  bc: HOST, {bc_x, bc_y, bc_z}.  helmholtz_alpha: 0 selects Poisson, > 0
  *   Helmholtz; negative / non-finite is TPT_EINVAL.
- *   All three bc Neumann with alpha == 0 gives a SINGULAR plan: tpt_solve then returns the solution
+ *   No Dirichlet direction (every bc Neumann or periodic) with alpha == 0 gives a SINGULAR plan: tpt_solve then returns the solution
  *   with zero cell-volume-weighted mean; following PAPER.md:219 the last z-equation of mode (0,0)
  *   is replaced by "unknown = 0", so an incompatible rhs is not projected.
  *   Ownership: the plan owns its device matrices, coefficient vectors and ONE field-sized

@@ -17,7 +17,7 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libtpt.so")
 
-NEUMANN, DIRICHLET = 0, 1
+NEUMANN, DIRICHLET, PERIODIC = 0, 1, 2
 DIRS_Z, DIRS_YZ, DIRS_XYZ = 4, 6, 7   # implicitly treated directions of Eq. 2b: bit 0 = x, 1 = y, 2 = z
 K_FWD_X, K_FWD_Y, K_THOMAS, K_INV_Y, K_INV_X, K_COUNT = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")

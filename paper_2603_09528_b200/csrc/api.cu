@@ -50,7 +50,7 @@ struct tpt_plan {
 
 namespace {
 
-bool bc_valid(int b) { return b == TPT_BC_NEUMANN || b == TPT_BC_DIRICHLET; }
+bool bc_valid(int b) { return b == TPT_BC_NEUMANN || b == TPT_BC_DIRICHLET || b == TPT_BC_PERIODIC; }
 
 void free_plan(tpt_plan *p) {
     if (!p) return;
@@ -195,6 +195,8 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
     if (implicit_dirs != TPT_DIRS_XYZ && !(helmholtz_alpha > 0.0)) return TPT_EINVAL;   // Eq. 2c carries the full L
     if (!tpt::faces_valid(nx, xf) || !tpt::faces_valid(ny, yf) || !tpt::faces_valid(nz, zf)) return TPT_EINVAL;
     if (!bc_valid(bc[0]) || !bc_valid(bc[1]) || !bc_valid(bc[2])) return TPT_EINVAL;
+    // periodic directions are diagonalised (x, y); the z sweep is the plain Thomas algorithm
+    if (bc[2] == TPT_BC_PERIODIC || (bc[0] == TPT_BC_PERIODIC && nx < 3) || (bc[1] == TPT_BC_PERIODIC && ny < 3)) return TPT_EINVAL;
     if (!(helmholtz_alpha >= 0.0) || !std::isfinite(helmholtz_alpha)) return TPT_EINVAL;
     if ((double)nx * ny * nz > 4.0e9) return TPT_EINVAL;
 
@@ -220,7 +222,7 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
     p->dirs = implicit_dirs;
     p->device = dev;
     p->sms = sm_count;
-    p->singular = (helmholtz_alpha == 0.0 && bc[0] == TPT_BC_NEUMANN && bc[1] == TPT_BC_NEUMANN &&
+    p->singular = (helmholtz_alpha == 0.0 && bc[0] != TPT_BC_DIRICHLET && bc[1] != TPT_BC_DIRICHLET &&
                    bc[2] == TPT_BC_NEUMANN) ? 1 : 0;
     // Helmholtz (I - alpha T) u = f  <=>  (T - I/alpha) u = -f/alpha: same z kernel with a constant
     // extra shift, the -1/alpha scale folded into the first forward matrix ("constant shift").

@@ -35,13 +35,16 @@ void build_operator(int n, const double *xf, int bc, Operator1D &op) {
     for (int i = 1; i < n; ++i) op.delta[i] = 0.5 * (xf[i + 1] - xf[i - 1]);
     op.delta[0] = op.w[0];
     op.delta[n] = op.w[n - 1];
+    // Periodic ("cyclic corners", A17): faces 0 and n are one face, between the last cell
+    // (one period back) and the first; a[0] then couples to cell n-1 and c[n-1] to cell 0.
+    if (bc == 2) op.delta[0] = op.delta[n] = 0.5 * (op.w[0] + op.w[n - 1]);
     for (int i = 0; i < n; ++i) {
         const double lo = 1.0 / (op.w[i] * op.delta[i]);      // coupling through the lower face
         const double hi = 1.0 / (op.w[i] * op.delta[i + 1]);  // coupling through the upper face
         double diag = 0.0;
-        if (i > 0) { op.a[i] = lo; diag -= lo; }
+        if (i > 0 || bc == 2) { op.a[i] = lo; diag -= lo; }
         else if (bc == 1) diag -= 2.0 * lo;                   // Dirichlet ghost
-        if (i < n - 1) { op.c[i] = hi; diag -= hi; }
+        if (i < n - 1 || bc == 2) { op.c[i] = hi; diag -= hi; }
         else if (bc == 1) diag -= 2.0 * hi;
         op.b[i] = diag;
     }
@@ -106,6 +109,69 @@ int ql_implicit(int n, std::vector<double> &d, std::vector<double> &e, std::vect
     return 0;
 }
 
+// Householder reduction of a dense symmetric matrix A (n x n, row-major, destroyed) to tridiagonal form
+// Q^T A Q = tridiag(d, e), for the cyclic operator of a periodic direction ("stored as a dense matrix").
+// On return qt holds Q^T (row k = k-th basis vector), ready to be rotated by ql_implicit.
+void householder_tridiagonalise(int n, std::vector<double> &A, std::vector<double> &d, std::vector<double> &e,
+                                std::vector<double> &qt) {
+    std::vector<double> v(n), pv(n);
+    std::vector<std::vector<double>> refl;      // unit reflector vectors, v_k acts on indices k+1..n-1
+    refl.reserve(n);
+    for (int k = 0; k + 2 < n; ++k) {
+        double norm2 = 0.0;
+        for (int i = k + 1; i < n; ++i) norm2 += A[(size_t)i * n + k] * A[(size_t)i * n + k];
+        const double x0 = A[(size_t)(k + 1) * n + k];
+        const double tail2 = norm2 - x0 * x0;
+        std::fill(v.begin(), v.end(), 0.0);
+        if (tail2 <= 0.0) { refl.emplace_back(); continue; }   // column already tridiagonal
+        const double alpha = -std::copysign(std::sqrt(norm2), x0);
+        for (int i = k + 1; i < n; ++i) v[i] = A[(size_t)i * n + k];
+        v[k + 1] -= alpha;
+        double vn = 0.0;
+        for (int i = k + 1; i < n; ++i) vn += v[i] * v[i];
+        vn = 1.0 / std::sqrt(vn);
+        for (int i = k + 1; i < n; ++i) v[i] *= vn;
+        // trailing block A' (indices > k):  A' <- H A' H,  H = I - 2 v v^T
+        double K = 0.0;
+        for (int i = k + 1; i < n; ++i) {
+            double t = 0.0;
+            for (int j = k + 1; j < n; ++j) t += A[(size_t)i * n + j] * v[j];
+            pv[i] = t;
+            K += v[i] * t;
+        }
+        for (int i = k + 1; i < n; ++i) pv[i] -= K * v[i];
+        for (int i = k + 1; i < n; ++i)
+            for (int j = k + 1; j < n; ++j) A[(size_t)i * n + j] -= 2.0 * (v[i] * pv[j] + pv[i] * v[j]);
+        A[(size_t)(k + 1) * n + k] = A[(size_t)k * n + k + 1] = alpha;
+        for (int i = k + 2; i < n; ++i) A[(size_t)i * n + k] = A[(size_t)k * n + i] = 0.0;
+        refl.emplace_back(v.begin(), v.end());
+    }
+    d.resize(n);
+    e.assign(n, 0.0);
+    for (int i = 0; i < n; ++i) d[i] = A[(size_t)i * n + i];
+    for (int i = 0; i + 1 < n; ++i) e[i] = A[(size_t)(i + 1) * n + i];
+    // Q = H_0 H_1 ... H_m (each H symmetric), so Q^T = H_m ... H_1 H_0: apply the reflectors to the identity in
+    // ascending order, qt <- H_k qt (rows k+1.. of qt are combined).
+    qt.assign((size_t)n * n, 0.0);
+    for (int i = 0; i < n; ++i) qt[(size_t)i * n + i] = 1.0;
+    std::vector<double> t(n);
+    for (size_t k = 0; k < refl.size(); ++k) {
+        const std::vector<double> &u = refl[k];
+        if (u.empty()) continue;
+        std::fill(t.begin(), t.end(), 0.0);
+        for (int i = (int)k + 1; i < n; ++i) {
+            const double ui = u[i];
+            const double *row = &qt[(size_t)i * n];
+            for (int c = 0; c < n; ++c) t[c] += ui * row[c];
+        }
+        for (int i = (int)k + 1; i < n; ++i) {
+            const double ui = 2.0 * u[i];
+            double *row = &qt[(size_t)i * n];
+            for (int c = 0; c < n; ++c) row[c] -= ui * t[c];
+        }
+    }
+}
+
 // Y = B X where -T~ = B^T B is the flux factorisation: one row per face that carries a flux.
 // X, Y row-major with n columns.  Returns the number of rows of Y.
 int apply_flux_factor(const Operator1D &op, const std::vector<double> &X, std::vector<double> &Y) {
@@ -119,6 +185,14 @@ int apply_flux_factor(const Operator1D &op, const std::vector<double> &X, std::v
         ++rows;
     };
     if (op.bc == 1) boundary_row(0);
+    if (op.bc == 2) {   // the wrap-around face between cell n-1 and cell 0 carries a flux like any interior face
+        const double isd = 1.0 / std::sqrt(op.delta[0]);
+        const double up = isw[0] * isd, dn = isw[n - 1] * isd;
+        const double *xu = &X[0], *xd = &X[(size_t)(n - 1) * n];
+        double *y = &Y[(size_t)rows * n];
+        for (int m = 0; m < n; ++m) y[m] = xu[m] * up - xd[m] * dn;
+        ++rows;
+    }
     for (int f = 1; f < n; ++f) {
         const double isd = 1.0 / std::sqrt(op.delta[f]);
         const double up = isw[f] * isd, dn = isw[f - 1] * isd;
@@ -203,8 +277,20 @@ int eigen_decompose(const Operator1D &op, std::vector<double> &lambda, std::vect
     std::vector<double> d(op.b), e(n, 0.0);
     for (int i = 0; i + 1 < n; ++i) e[i] = std::sqrt(op.c[i] * op.a[i + 1]);
     // Step 1.2: base solver.
-    std::vector<double> zt(nn, 0.0);
-    for (int i = 0; i < n; ++i) zt[(size_t)i * n + i] = 1.0;
+    std::vector<double> zt;
+    if (op.bc == 2) {
+        // cyclic operator: dense T~ with the corner sqrt(c_{n-1} a_0), Householder reduction, then the same QL
+        std::vector<double> A(nn, 0.0);
+        for (int i = 0; i < n; ++i) A[(size_t)i * n + i] = op.b[i];
+        for (int i = 0; i + 1 < n; ++i) A[(size_t)i * n + i + 1] = A[(size_t)(i + 1) * n + i] = e[i];
+        const double corner = std::sqrt(op.c[n - 1] * op.a[0]);
+        A[(size_t)(n - 1) * n] += corner;
+        A[n - 1] += corner;
+        householder_tridiagonalise(n, A, d, e, zt);
+    } else {
+        zt.assign(nn, 0.0);
+        for (int i = 0; i < n; ++i) zt[(size_t)i * n + i] = 1.0;
+    }
     if (ql_implicit(n, d, e, zt) != 0) return -1;
     std::vector<double> X(nn), Xprev, Y((size_t)(n + 1) * n), S(nn), E(nn), lam(n), lamprev(n);
     for (int m = 0; m < n; ++m)
@@ -248,7 +334,7 @@ int eigen_decompose(const Operator1D &op, std::vector<double> &lambda, std::vect
         for (int i = 0; i < n; ++i) q[(size_t)i * n + m] = X[(size_t)i * n + src] * nrm;
     }
     const double L = std::accumulate(op.w.begin(), op.w.end(), 0.0);
-    if (op.bc == 0) {   // Neumann–Neumann: exact null pair (T 1 = 0 => T~ D^{1/2} 1 = 0)
+    if (op.bc == 0 || op.bc == 2) {   // Neumann–Neumann or periodic: exact null pair (T 1 = 0 => T~ D^{1/2} 1 = 0)
         lambda[0] = 0.0;
         for (int i = 0; i < n; ++i) q[(size_t)i * n] = std::sqrt(op.w[i] / L);
     }

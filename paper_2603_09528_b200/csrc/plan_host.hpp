@@ -1,5 +1,6 @@
 // plan_host.hpp — plan-time host code of the CUDA library (steps 1.1–1.3).
-// Independent of oracle/: different base eigen-solver (implicit-shift QL on the tridiagonal),
+// Independent of oracle/: different base eigen-solver (implicit-shift QL on the tridiagonal; Householder
+// reduction first for the dense cyclic operator of a periodic direction),
 // own operator assembly and own refinement code.
 #pragma once
 
@@ -18,7 +19,8 @@ struct Operator1D {
 // true iff n >= 2 and faces are finite and strictly increasing
 bool faces_valid(int n, const double *xf);
 
-// Eq. 3–4 with mirror-ghost boundary rows (readings A1–A3).
+// Eq. 3–4 with mirror-ghost boundary rows (readings A1–A3); bc: 0 Neumann,
+// 1 Dirichlet, 2 periodic (cyclic corners kept in a[0], c[n-1], reading A17; needs n >= 3).
 void build_operator(int n, const double *xf, int bc, Operator1D &op);
 
 // Eigen-decomposition of T~ = D^{1/2} T D^{-1/2} (Eq. 5): lambda[n] descending (mode 0 smoothest),

@@ -111,6 +111,12 @@ class Problem:
 N_, D_ = NEUMANN, DIRICHLET
 _PI = math.pi
 
+# The paper's own single-GPU benchmark case: 1024^3, periodic x, Neumann y and z, GEMM transforms
+# in x and y ("GG").  x uniform (the paper's FFT-vs-GEMM comparison needs it), y and z tanh-stretched here (the cost of
+# the direct method does not depend on the grading).  Not a BASELINE.json config: context for BASELINE.md.
+PAPER_GG = Problem("paper-gg-1024-periodic-x", (1024, 1024, 1024), (1.0, 1.0, 1.0), (0.0, 2.0, 2.0),
+                   (PERIODIC, NEUMANN, NEUMANN), 0.0, 8)
+
 # BASELINE.json `configs`, in order.  Config 5 is a step of four solves (3 Helmholtz + 1 Poisson).
 CONFIGS = {
     "c1": [Problem("c1-poisson-16", (16, 16, 16), (1.0, 1.0, 1.0), (1.2, 1.2, 1.5), (N_, N_, D_), 0.0, 0)],
@@ -120,4 +126,5 @@ CONFIGS = {
     "c5": [Problem(f"c5-helmholtz-768-{s}", (768, 768, 768), (1.0, 1.0, 1.0), (3.0, 3.0, 3.0), (N_, N_, D_), 5e-4, s)
            for s in (4, 5, 6)]
           + [Problem("c5-poisson-768-neumann", (768, 768, 768), (1.0, 1.0, 1.0), (3.0, 3.0, 3.0), (N_, N_, N_), 0.0, 7)],
+    "p1024": [PAPER_GG],
 }

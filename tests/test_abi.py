@@ -48,7 +48,10 @@ def test_argument_validation_needs_no_gpu(tpt):
         tpt.plan_create(8, 8, 8, bad, good, good, (0, 0, 1), 0.0)
     assert e.value.status == -1
     with pytest.raises(tpt.TptError) as e:
-        tpt.plan_create(8, 8, 8, good, good, good, (0, 2, 1), 0.0)
+        tpt.plan_create(8, 8, 8, good, good, good, (0, 3, 1), 0.0)
+    assert e.value.status == -1
+    with pytest.raises(tpt.TptError) as e:
+        tpt.plan_create(8, 8, 8, good, good, good, (0, 0, 2), 0.0)      # periodic z: the sweep is the plain Thomas algorithm
     assert e.value.status == -1
     with pytest.raises(tpt.TptError) as e:
         tpt.plan_create(8, 8, 8, good, good, good, (0, 0, 1), -1.0)

@@ -189,3 +189,77 @@ def test_host_path_poisson_singular_multi_slab(tpt, torch, orc):
     r = orc.residual_norms(xf, yf, zf, P.bc, 0.0, f, out)
     assert r["rel2"] <= RESID_TOL
     plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# Periodic directions; the paper's benchmark BCs are periodic x, Neumann y and z
+# ------------------------------------------------------------------------------------------------------------
+P_ = I.PERIODIC
+
+PERIODIC_CASES = [
+    # name, n, L, beta, bc, alpha
+    ("duct-ragged", (40, 36, 33), (6.0, 1.0, 1.0), (0.0, 2.0, 2.0), (P_, N_, N_), 0.0),      # singular, generic GEMM
+    ("odd", (5, 7, 6), (1.0, 2.0, 1.5), (1.2, 0.0, 1.0), (P_, P_, D_), 0.0),                   # stretched periodic x
+    ("t128-duct", (256, 128, 48), (6.0, 1.0, 1.0), (0.0, 2.0, 2.5), (P_, N_, N_), 0.0),      # singular, TMA GEMM
+    ("t128-pp", (128, 128, 40), (1.0, 1.0, 1.0), (1.5, 0.0, 2.0), (P_, P_, D_), 0.0),          # both periodic
+    ("t128-helm", (128, 256, 24), (1.0, 2.0, 1.0), (0.0, 1.0, 2.0), (N_, P_, N_), 1e-3),       # Helmholtz, periodic y
+]
+
+
+@pytest.mark.parametrize("case", PERIODIC_CASES, ids=[c[0] for c in PERIODIC_CASES])
+def test_periodic_parity(tpt, torch, orc, case):
+    name, n, L, beta, bc, alpha = case
+    P = I.Problem(name, n, L, beta, bc, alpha, seed=51 + n[0])
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, bc, alpha)
+    assert plan.singular == P.singular
+    u = _solve(torch, plan, f)
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha).solve(f)
+    assert _rel(u, ref) <= PARITY_TOL
+    r = orc.residual_norms(xf, yf, zf, bc, alpha, f, u)
+    assert r["rel2"] <= RESID_TOL and r["relL2vol"] <= RESID_TOL
+    if P.singular:
+        V = np.diff(zf)[:, None, None] * np.diff(yf)[None, :, None] * np.diff(xf)[None, None, :]
+        assert abs((V * u).sum()) < 1e-13 * np.abs(u).max() * V.sum()
+    plan.destroy()
+
+
+def test_periodic_uniform_plan_eigenpairs_are_fourier(tpt, torch):
+    n, L = 256, 6.0
+    xf = I.tanh_faces(n, L, 0.0)
+    yf = I.tanh_faces(16, 1.0, 1.0)
+    plan = tpt.plan_create(n, 16, 16, xf, yf, yf, (P_, N_, D_), 0.0)
+    lam, q = plan.eigen(0)
+    dx = L / n
+    cf = np.sort(-(4 / dx ** 2) * np.sin(np.pi * np.arange(n) / n) ** 2)[::-1]
+    assert np.abs(lam - cf).max() <= 1e-13 * np.abs(cf).max()
+    assert np.abs(q.T @ q - np.eye(n)).max() < 1e-13
+    F = np.fft.fft(q, axis=0)
+    for m in range(n):
+        kk = int(round(np.arcsin(np.sqrt(min(1.0, -lam[m] * dx * dx / 4))) * n / np.pi))
+        mask = np.ones(n, bool)
+        mask[[kk % n, (n - kk) % n]] = False
+        assert np.abs(F[mask, m]).max() < 1e-10
+    plan.destroy()
+
+
+def test_periodic_z_and_tiny_periodic_are_rejected(tpt, torch):
+    xf = I.tanh_faces(16, 1.0, 0.0)
+    with pytest.raises(tpt.TptError):
+        tpt.plan_create(16, 16, 16, xf, xf, xf, (N_, N_, P_), 0.0)
+    x2 = I.tanh_faces(2, 1.0, 0.0)
+    with pytest.raises(tpt.TptError):
+        tpt.plan_create(2, 16, 16, x2, xf, xf, (P_, N_, N_), 0.0)
+
+
+def test_paper_benchmark_case_thin_z_parity(tpt, torch, orc):
+    # 1024 x 1024 in x, y (periodic x, Neumann y), 16 cells in z for the oracle's sake
+    P = I.PAPER_GG.thin_z(16)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
+    u = _solve(torch, plan, f)
+    ref = orc.OraclePlan(xf, yf, zf, P.bc, P.alpha).solve(f)
+    assert _rel(u, ref) <= PARITY_TOL
+    plan.destroy()
