@@ -79,11 +79,12 @@ int upload(double **dst, const std::vector<double> &src) {
 }
 
 // The transforms act plane by plane in z, so a solve may be issued on z-slabs [k0, k0 + nk) (tpt_solve_host
-// overlaps the slabs' copies with their transforms); in / out point at plane k0.
-tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *mat, int nk) {
+// overlaps the slabs' copies with their transforms); in / out point at the FIELD, the builders add the slab offset.
+tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *mat, int k0, int nk) {
     // steps 2.1 / 2.5: all N_y*nk lines at once, out[r][:] = in[r][:] * mat
+    const size_t off = (size_t)p->nx * p->ny * k0;
     tpt::GemmArgs g{};
-    g.A = in; g.B = mat; g.C = out;
+    g.A = in + off; g.B = mat; g.C = out + off;
     g.M = p->ny * nk; g.N = p->nx; g.K = p->nx;
     g.lda = p->nx; g.ldb = p->nx; g.ldc = p->nx;
     g.strideA = g.strideB = g.strideC = 0;
@@ -91,30 +92,47 @@ tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const dou
     return g;
 }
 
-tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat, int nk) {
-    // steps 2.2 / 2.4: per z-plane, out_k = mat * in_k  (strided-batched, no transposes)
+// steps 2.2 / 2.4: per z-plane, out_k = mat * in_k  (strided-batched, no transposes).  in_blocked / out_blocked: that
+// side is the mode-space field in the tile-blocked layout (kernels.cuh), whose z index has stride 16.
+tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat, int k0, int nk,
+                     bool in_blocked, bool out_blocked) {
+    const int64_t plane = (int64_t)p->nx * p->ny;
     tpt::GemmArgs g{};
-    g.A = mat; g.B = in; g.C = out;
+    g.A = mat;
     g.M = p->ny; g.N = p->nx; g.K = p->ny;
-    g.lda = p->ny; g.ldb = p->nx; g.ldc = p->nx;
-    g.strideA = 0; g.strideB = (int64_t)p->nx * p->ny; g.strideC = (int64_t)p->nx * p->ny;
+    g.lda = p->ny; g.strideA = 0;
     g.batch = nk;
+    if (in_blocked) { g.B = in + (size_t)16 * k0; g.ldb = (int64_t)p->nx * p->nz; g.strideB = 16; g.ldgB = (int64_t)16 * p->nz; }
+    else { g.B = in + (size_t)plane * k0; g.ldb = p->nx; g.strideB = plane; }
+    if (out_blocked) { g.C = out + (size_t)16 * k0; g.ldc = (int64_t)p->nx * p->nz; g.strideC = 16; g.ldgC = (int64_t)16 * p->nz; }
+    else { g.C = out + (size_t)plane * k0; g.ldc = p->nx; g.strideC = plane; }
     return g;
 }
 
 // variant 2 = persistent TMA/mbarrier DMMA kernel where the shape allows, else the variant-1 / generic kernels
 cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st) {
     if (p->gemm_variant == 2 && tpt::gemm_tma_supported(g)) return tpt::launch_gemm_tma(g, p->sms, st);
+    if (g.ldgB > 16 || g.ldgC > 16) return cudaErrorInvalidValue;   // only the TMA kernel knows the blocked layout
     return tpt::launch_gemm(g, p->gemm_variant >= 1 ? 1 : 0, st);
 }
 
+// The mode-space field (between steps 2.2 and 2.4) is kept tile-blocked when the kernels on both sides of it can:
+// the TMA GEMM for the y transforms and the on-chip sweep.  tpt_stage always uses the natural layout.
+bool use_blocked(const tpt_plan *p) {
+    if (p->gemm_variant != 2 || p->thomas_variant != 1 || !(p->dirs & 2)) return false;
+    if (!tpt::blocked_layout_supported(p->nx, p->ny, p->nz) || !tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) return false;
+    return p->ny % 128 == 0 && p->nx % 128 == 0;   // the TMA GEMM's tile shape (M = K = ny, N = nx)
+}
+
 // Step 2.3 on one field: in -> out (in == out allowed); `scratch` is a free field (used by the streaming kernel only).
-int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches) {
+int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches, bool blocked = false,
+               bool blocked_shape = false) {
     cudaError_t e;
     if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) {
         e = tpt::launch_thomas_onchip(in, out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
-                                      p->singular, p->sms, st);
+                                      p->singular, blocked, blocked_shape, p->sms, st);
     } else {   // streaming kernel: in place on `out`, c' spilled to `scratch`
+        if (blocked) return TPT_ECUDA;
         if (in != out && cudaMemcpyAsync(out, in, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
             return TPT_ECUDA;
         e = tpt::launch_thomas(out, scratch, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
@@ -122,21 +140,22 @@ int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cuda
     }
     ++*launches;
     if (e == cudaSuccess && p->singular) {
-        e = tpt::launch_gauge(out, p->d_wz, p->nx, p->ny, p->nz, st);
+        e = tpt::launch_gauge(out, p->d_wz, blocked ? (size_t)16 : (size_t)p->nx * p->ny, p->nz, st);
         ++*launches;
     }
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
 }
 
-// Runs one transform slot on nk z-planes starting at in / out; *launches incremented by the kernels enqueued.
-int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int nk = -1) {
+// Runs one transform slot on z-planes [k0, k0 + nk) of the fields at in / out; *launches incremented by the kernels
+// enqueued.  `blocked`: the mode-space side of a y transform (output of 2.2, input of 2.4) is tile-blocked.
+int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int k0, int nk,
+             bool blocked = false) {
     cudaError_t e = cudaSuccess;
-    if (nk < 0) nk = p->nz;
     switch (slot) {
-        case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd, nk), st); ++*launches; break;
-        case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv, nk), st); ++*launches; break;
-        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd, nk), st); ++*launches; break;
-        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv, nk), st); ++*launches; break;
+        case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd, k0, nk), st); ++*launches; break;
+        case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv, k0, nk), st); ++*launches; break;
+        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd, k0, nk, false, blocked), st); ++*launches; break;
+        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv, k0, nk, blocked, false), st); ++*launches; break;
         default: return TPT_EINVAL;
     }
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
@@ -157,6 +176,7 @@ int run_pipeline(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream
     double *W = p->d_work;
     const size_t pts = p->points();
     const int nk = p->nz * nf;
+    const bool blk = use_blocked(p);
     if (ev && cudaEventRecord(ev[0], st) != cudaSuccess) return TPT_ECUDA;
     for (int s = 0; s < TPT_K_COUNT; ++s) {
         int rc = TPT_OK;
@@ -164,11 +184,16 @@ int run_pipeline(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream
             double *dst = (cur == rhs) ? out : const_cast<double *>(cur);
             double *scratch = (dst == W) ? out : W;
             for (int f = 0; f < nf && rc == TPT_OK; ++f)
-                rc = run_thomas(p, cur + f * pts, dst + f * pts, scratch + f * pts, st, launches);
+                rc = run_thomas(p, cur + f * pts, dst + f * pts, scratch + f * pts, st, launches, blk);
             cur = dst;
         } else if (slot_active(p, s)) {
             double *dst = (cur == W) ? out : W;
-            rc = run_slot(p, s, cur, dst, st, launches, nk);
+            if (blk && (s == TPT_K_FWD_Y || s == TPT_K_INV_Y)) {   // the blocked layout is per field: one launch each
+                for (int f = 0; f < nf && rc == TPT_OK; ++f)
+                    rc = run_slot(p, s, cur + f * pts, dst + f * pts, st, launches, 0, p->nz, true);
+            } else {
+                rc = run_slot(p, s, cur, dst, st, launches, 0, nk);   // the stack is just a longer z axis
+            }
             cur = dst;
         }
         if (rc != TPT_OK) return rc;
@@ -419,6 +444,9 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
     double *const S = p->d_stage, *const W = p->d_work;
     const int fwd[2] = {TPT_K_FWD_X, TPT_K_FWD_Y}, inv[2] = {TPT_K_INV_Y, TPT_K_INV_X};
     double *cur = S;
+    // natural layout throughout: the tile-blocked mode-space layout scatters a slab's output over the whole field,
+    // which here would overwrite later slabs still waiting in the same buffers (and the path is PCIe-bound anyway)
+    const bool blk = false;
     for (int s = 0; s < ns; ++s) {
         const int k0 = k_lo(s), nk = k_lo(s + 1) - k0;
         const size_t off = plane * k0, cnt = plane * nk;
@@ -430,12 +458,12 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
         for (int q = 0; q < 2; ++q) {
             if (!slot_active(p, fwd[q])) continue;
             double *dst = cur == S ? W : S;
-            int rc = run_slot(p, fwd[q], cur + off, dst + off, st, &launches, nk);
+            int rc = run_slot(p, fwd[q], cur, dst, st, &launches, k0, nk, blk);
             if (rc != TPT_OK) return rc;
             cur = dst;
         }
     }
-    int rc = run_thomas(p, cur, cur, cur == S ? W : S, st, &launches);
+    int rc = run_thomas(p, cur, cur, cur == S ? W : S, st, &launches, blk, use_blocked(p));   // same partition as tpt_solve
     if (rc != TPT_OK) return rc;
     double *const mid = cur;
     for (int s = 0; s < ns; ++s) {
@@ -445,7 +473,7 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
         for (int q = 0; q < 2; ++q) {
             if (!slot_active(p, inv[q])) continue;
             double *dst = cur == S ? W : S;
-            rc = run_slot(p, inv[q], cur + off, dst + off, st, &launches, nk);
+            rc = run_slot(p, inv[q], cur, dst, st, &launches, k0, nk, blk);
             if (rc != TPT_OK) return rc;
             cur = dst;
         }
@@ -496,7 +524,7 @@ int tpt_stage(tpt_plan *p, int slot, const double *in_dev, double *out_dev, void
     if (!slot_active(p, slot)) return TPT_EINVAL;   // this plan does not diagonalise that direction
     if (slot == TPT_K_THOMAS) return run_thomas(p, in_dev, out_dev, p->d_work, st, &launches);
     if (in_dev == out_dev) return TPT_EINVAL;   // the transforms are out of place
-    return run_slot(p, slot, in_dev, out_dev, st, &launches);
+    return run_slot(p, slot, in_dev, out_dev, st, &launches, 0, p->nz);
 }
 
 int tpt_plan_set_profiling(tpt_plan *p, int enabled) {

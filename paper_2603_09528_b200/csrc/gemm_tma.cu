@@ -33,6 +33,7 @@ constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 /*alignment sl
 struct TmaGemmParams {
     double *C;
     int64_t ldc, strideC;
+    int64_t ldg;         // stride between 16-column groups of C (16 = plain row-major)
     int KT;              // K / 16
     int tiles_n;         // N / 128
     int tiles_mn;        // (M / 128) * (N / 128)
@@ -74,13 +75,13 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 const int mn = tile - b * p.tiles_mn;
                 const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
                 const int a_row = b * p.a_batch_rows + mt * BM;
-                const int b_row = b * p.b_batch_rows;
+                const int b_sel = p.b_batch_rows ? b : 0;
                 for (int kt = 0; kt < KT; ++kt) {
                     ptx::mbar_wait(&empty[slot], phase ^ 1);
                     unsigned char *st = smem + (size_t)slot * STAGE_BYTES;
                     ptx::mbar_arrive_expect_tx(&full[slot], STAGE_BYTES);
                     ptx::tma_load_2d(st, &mapA, kt * BK, a_row, &full[slot]);
-                    ptx::tma_load_3d(st + A_BYTES, &mapB, 0, b_row + kt * BK, nt * (BN / 16), &full[slot]);
+                    ptx::tma_load_4d(st + A_BYTES, &mapB, 0, kt * BK, nt * (BN / 16), b_sel, &full[slot]);
                     if (++slot == STAGES) { slot = 0; phase ^= 1; }
                 }
             }
@@ -155,13 +156,13 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         const int b = tile / p.tiles_mn;
         const int mn = tile - b * p.tiles_mn;
         const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
-        double *Cw = p.C + (int64_t)b * p.strideC + ((int64_t)mt * BM + wm0 + rho) * p.ldc + (int64_t)nt * BN + wn0 +
-                     ((t >> 1) << 1) + ((t & 1) << 3);
+        double *Cw = p.C + (int64_t)b * p.strideC + ((int64_t)mt * BM + wm0 + rho) * p.ldc +
+                     (int64_t)(nt * (BN / 16) + wn0 / 16) * p.ldg + ((t >> 1) << 1) + ((t & 1) << 3);
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                *reinterpret_cast<double2 *>(Cw + (int64_t)(8 * i) * p.ldc + (j >> 1) * 16 + (j & 1) * 4) =
+                *reinterpret_cast<double2 *>(Cw + (int64_t)(8 * i) * p.ldc + (int64_t)(j >> 1) * p.ldg + (j & 1) * 4) =
                     make_double2(acc[i][j][0], acc[i][j][1]);
     }
 }
@@ -177,8 +178,9 @@ bool gemm_tma_supported(const GemmArgs &g) {
     // batches are folded into the row dimension of the operand tensors: a batched operand must be densely stacked
     if (g.batch > 1) {
         if (g.strideA != 0 && g.strideA != (int64_t)g.M * g.lda) return false;
-        if (g.strideB != 0 && g.strideB != (int64_t)g.K * g.ldb) return false;
+        if (g.strideB != 0 && g.strideB % 2) return false;
     }
+    if (g.ldgB % 2 || g.ldgC % 2) return false;
     const int64_t tiles = (int64_t)(g.M / BM) * (g.N / BN) * g.batch;
     return tiles < (int64_t)1 << 30;
 }
@@ -199,16 +201,18 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
         if (!make_f64_map(&mapA, g.A, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) return cudaErrorUnknown;
     }
     {
-        // B viewed as [N/16 groups][K rows][16 columns]: one box = 8 sub-tiles of 16 k x 16 n (128-byte rows)
-        const uint64_t dims[3] = {16, (uint64_t)g.K * (b_batched ? g.batch : 1), (uint64_t)g.N / 16};
-        const uint64_t strides[2] = {(uint64_t)g.ldb * 8, 128};
-        const uint32_t box[3] = {16, BK, BN / 16};
-        if (!make_f64_map(&mapB, g.B, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) return cudaErrorUnknown;
+        // B viewed as [batch][N/16 groups][K rows][16 columns]: one box = 8 sub-tiles of 16 k x 16 n (128-byte rows)
+        const uint64_t ldg = g.ldgB ? (uint64_t)g.ldgB : 16;
+        const uint64_t dims[4] = {16, (uint64_t)g.K, (uint64_t)g.N / 16, (uint64_t)(b_batched ? g.batch : 1)};
+        const uint64_t strides[3] = {(uint64_t)g.ldb * 8, ldg * 8, (uint64_t)(b_batched ? g.strideB : (int64_t)g.K * g.ldb) * 8};
+        const uint32_t box[4] = {16, BK, BN / 16, 1};
+        if (!make_f64_map(&mapB, g.B, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) return cudaErrorUnknown;
     }
     TmaGemmParams p;
     p.C = g.C;
     p.ldc = g.ldc;
     p.strideC = g.strideC;
+    p.ldg = g.ldgC ? g.ldgC : 16;
     p.KT = g.K / BK;
     p.tiles_n = g.N / BN;
     p.tiles_mn = (g.M / BM) * (g.N / BN);

@@ -353,8 +353,8 @@ __global__ void __launch_bounds__(256) gauge_kernel(double *x, const double *__r
     for (int k = threadIdx.x; k < nz; k += 256) x[(size_t)k * plane] -= mean;
 }
 
-cudaError_t launch_gauge(double *x, const double *wz, int nx, int ny, int nz, cudaStream_t stream) {
-    gauge_kernel<<<1, 256, 0, stream>>>(x, wz, (size_t)nx * ny, nz);
+cudaError_t launch_gauge(double *x, const double *wz, size_t stride, int nz, cudaStream_t stream) {
+    gauge_kernel<<<1, 256, 0, stream>>>(x, wz, stride, nz);
     return cudaGetLastError();
 }
 

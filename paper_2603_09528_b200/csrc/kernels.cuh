@@ -18,7 +18,18 @@ struct GemmArgs {
     int64_t lda, ldb, ldc;
     int64_t strideA, strideB, strideC;
     int batch;
+    // Column-group strides (elements) of B and C: column n lives at (n / 16) * ldg + n % 16 within its row.
+    // 0 or 16 = plain row-major.  Anything else is the tile-blocked mode-space layout of the y transforms (below);
+    // only the TMA kernel (variant 2) takes it.
+    int64_t ldgB = 0, ldgC = 0;
 };
+
+// Tile-blocked layout of the mode-space field between steps 2.2 and 2.4 (the z sweep's input and output):
+//   element (i, m, k) at  ((m * (nx/16) + i/16) * nz + k) * 16 + i % 16
+// i.e. the nz rows of every 16-column Thomas tile are contiguous (nz * 128 bytes), so the sweep reads and writes whole
+// DRAM pages instead of one 128-byte line per page (natural layout: rows nx*ny*8 bytes apart; measured 4.6 vs 6.1 TB/s
+// for the bare tile traffic).  Written by the forward-y GEMM epilogue, read back by the inverse-y GEMM's B tensor map.
+inline bool blocked_layout_supported(int nx, int ny, int nz) { return nx % 16 == 0 && ny >= 1 && nz >= 1; }
 
 // variant 0: generic FP64-FMA tile kernel, any shape.  variant 1: DMMA pipelined kernel when the
 // shape allows (falls back to the generic kernel otherwise).  Returns the launch's cudaError_t.
@@ -43,14 +54,15 @@ cudaError_t launch_thomas(double *x, double *cprime, const double *az, const dou
 // Reads the right-hand sides from `in` and writes the solution to `x` (in == x: in place).
 // tab: device copy of the two tables thomas_onchip_tables() builds (8 * (nz + THOMAS_TABLE_PAD) doubles).
 // sms = SM count.
-constexpr int THOMAS_TABLE_PAD = 64;
+constexpr int THOMAS_TABLE_PAD = 128;   // >= the rows by which S*M can exceed nz in any launch shape
 bool thomas_onchip_supported(int nx, int ny, int nz);
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out);
 cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
-                                 int nz, double shift0, int singular, int sms, cudaStream_t stream);
+                                 int nz, double shift0, int singular, bool blocked, bool blocked_shape, int sms, cudaStream_t stream);
 
-// Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean).
-cudaError_t launch_gauge(double *x, const double *wz, int nx, int ny, int nz, cudaStream_t stream);
+// Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean); `stride` = distance
+// between consecutive z levels of that column (nx*ny in the natural layout, 16 in the tile-blocked one).
+cudaError_t launch_gauge(double *x, const double *wz, size_t stride, int nz, cudaStream_t stream);
 
 // FP64 pipe microbenchmarks (kind 0: DFMA, 1: DMMA).  Returns TFLOP/s.
 cudaError_t run_fp64_peak(int kind, double *tflops);

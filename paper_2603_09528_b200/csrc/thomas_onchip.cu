@@ -24,16 +24,15 @@
 
 #include "kernels.cuh"
 #include "ptx.cuh"
+#include "tmap.hpp"
 
 namespace tpt {
 
 namespace {
 
-constexpr int TCOLS = 16;                       // columns per tile: one 128-byte row per z level
-constexpr int ROW_BYTES = TCOLS * (int)sizeof(double);
 
-template <int M, int MAXT>
-__global__ void __launch_bounds__(MAXT)
+template <int M, int TCOLS, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB)
 thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_out,
                      const double *__restrict__ tab_reg,
                      const double *__restrict__ tab_null, const double *__restrict__ lamx,
@@ -46,8 +45,10 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     uint64_t *full = reinterpret_cast<uint64_t *>(scratch + 6 * S * TCOLS);
 
     const int tid = threadIdx.x;
+    constexpr int ROW_BYTES = TCOLS * (int)sizeof(double);
+    constexpr int SUB = 16 / TCOLS;              // tiles per 16-column group
     const int col = tid & (TCOLS - 1);
-    const int seg = tid >> 4;
+    const int seg = tid / TCOLS;
 
     if (tid == 0) {
         ptx::tma_prefetch_desc(&tmap);
@@ -66,7 +67,7 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         ptx::mbar_arrive_expect_tx(&full[b], (uint32_t)((size_t)nbox * box_rows * ROW_BYTES));
         double *dst = bufs + (size_t)b * tile_elems;
         for (int q = 0; q < nbox; ++q)
-            ptx::tma_load_2d(dst + (size_t)q * box_rows * TCOLS, &tmap, tile * TCOLS, q * box_rows, &full[b]);
+            ptx::tma_load_4d(dst + (size_t)q * box_rows * TCOLS, &tmap, 0, q * box_rows, tile % SUB, tile / SUB, &full[b]);
     };
 
     const int first = blockIdx.x;
@@ -79,11 +80,18 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     double *const set0 = scratch, *const set1 = scratch + 3 * STR;
     int b = 0;
     uint32_t parity = 0;
+    // the spectral shift of my column in the next tile is fetched one tile ahead (its latency hides under the sweep)
+    auto shift_of = [&](int tile) {
+        const int gc = tile * TCOLS + col;
+        return __ldg(lamx + gc % nx) + __ldg(lamy + gc / nx) + shift0;
+    };
+    double s_next = n_my > 0 ? shift_of(first) : 0.0;
     for (int it = 0; it < n_my; ++it) {
         const int tile = first + it * (int)gridDim.x;
         double *buf = bufs + (size_t)b * tile_elems + (size_t)k0 * TCOLS + col;   // my segment, my column
         const int gcol = tile * TCOLS + col;
-        const double s = __ldg(lamx + gcol % nx) + __ldg(lamy + gcol / nx) + shift0;
+        const double s = s_next;
+        if (it + 1 < n_my) s_next = shift_of(tile + (int)gridDim.x);
         // the null column of a singular plan reads a table whose last row is "-x = p", and zeroes p
         const bool null_col = singular && gcol == 0;
         const double2 *tab = reinterpret_cast<const double2 *>(null_col ? tab_null : tab_reg) + 2 * k0;
@@ -102,7 +110,7 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             const double p = buf[t * TCOLS];
             const double bb = t0.y + s;
             const double den = t == 0 ? bb : fma(-t0.x, rprev, bb);
-            const double r = ptx::fast_rcp(den);
+            const double r = ptx::fast_rcp3(den);
             cp[t] = t1.y * r;
             const double d = (t == 0 ? p : fma(-t1.x, dprev, p)) * r;
             g[t] = (t == 0 ? t1.x : -t1.x * g[t - 1]) * r;
@@ -148,7 +156,9 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             wr[me] = A;
             wr[STR + me] = C;
             wr[2 * STR + me] = D;
-            __syncthreads();
+            // Early exit: once every coupling of the tile is below 1e-30 the remaining rounds would change D by less
+            // than 1e-30 |D_neighbour| — nothing in FP64.  (High modes decouple after one or two rounds: |c'| << 1.)
+            if (!__syncthreads_or(fmax(fabs(A), fabs(C)) > 1e-30)) break;
             double Al = 0.0, Cl = 0.0, Dl = 0.0, Ah = 0.0, Ch = 0.0, Dh = 0.0;
             if (seg - dlt >= 0) {
                 const int o = me - dlt * TCOLS;
@@ -186,7 +196,7 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         if (tid == 0) {                        // rows past nz are clipped by the tensor map
             const double *src = bufs + (size_t)b * tile_elems;
             for (int q = 0; q < nbox; ++q)
-                ptx::tma_store_2d(&tmap_out, tile * TCOLS, q * box_rows, src + (size_t)q * box_rows * TCOLS);
+                ptx::tma_store_4d(&tmap_out, 0, q * box_rows, tile % SUB, tile / SUB, src + (size_t)q * box_rows * TCOLS);
             ptx::bulk_commit();
         }
         if (++b == nbuf) {
@@ -197,94 +207,91 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     ptx::bulk_wait<0>();
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked directly).
-using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_tiled_fn() {
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void *ptr = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(ptr);
-    }
-    return fn;
+// The field as a 4-D tensor [16-column group][tile of the group][z][columns of the tile] (TC = 16: one tile per group).
+// Natural layout (x contiguous, z slowest): a group is 16 consecutive elements of a plane, rows nx*ny apart.
+// Tile-blocked layout (`blocked`, see kernels.cuh): the nz rows of a group are contiguous (128 bytes each), so a
+// group is one dense block of nz*128 bytes — DRAM pages are read and written whole.
+bool make_field_map(CUtensorMap *map, const double *x, size_t plane, int nz, int tc, int box_rows, bool blocked) {
+    const uint64_t dims[4] = {(uint64_t)tc, (uint64_t)nz, (uint64_t)(16 / tc), (uint64_t)(plane / 16)};
+    const uint64_t strides[3] = {blocked ? (uint64_t)128 : (uint64_t)plane * sizeof(double), (uint64_t)tc * sizeof(double),
+                                 blocked ? (uint64_t)nz * 128 : (uint64_t)128};
+    const uint32_t box[4] = {(uint32_t)tc, (uint32_t)box_rows, 1, 1};
+    return make_f64_map(map, x, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE);
 }
 
-// field viewed as a 2-D tensor: dim0 = nx*ny contiguous columns, dim1 = nz rows of stride nx*ny
-bool make_field_map(CUtensorMap *map, const double *x, size_t plane, int nz, int box_rows) {
-    EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn) return false;
-    const cuuint64_t dims[2] = {(cuuint64_t)plane, (cuuint64_t)nz};
-    const cuuint64_t strides[1] = {(cuuint64_t)plane * sizeof(double)};
-    const cuuint32_t box[2] = {(cuuint32_t)TCOLS, (cuuint32_t)box_rows};
-    const cuuint32_t estr[2] = {1, 1};
-    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(x), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
+constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_CTA_RESERVED = 1024, SMEM_CTA_MAX = 227 * 1024;
 
-template <int M, int MAXT>
+// M rows per segment, TC columns per tile, CTAS co-resident CTAs per SM (their barrier phases interleave).
+template <int M, int TC, int MAXT, int CTAS>
 cudaError_t launch_m(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny, int nz,
-                     double shift0, int singular, int sms, cudaStream_t stream) {
+                     double shift0, int singular, bool blocked, int sms, cudaStream_t stream) {
+    constexpr int ROW_BYTES = TC * (int)sizeof(double);
     int S = (nz + M - 1) / M;
-    if (S & 1) ++S;                                          // whole warps: 2 segments x 16 columns
+    while ((S * TC) % 32) ++S;                               // whole warps
     const int nbox = (nz + 255) / 256;                       // TMA boxes are at most 256 rows tall
-    const int box_rows = (nz + nbox - 1) / nbox;
+    int box_rows = (nz + nbox - 1) / nbox;
+    if ((box_rows * ROW_BYTES) % 128) ++box_rows;            // TMA wants 128-byte aligned shared-memory boxes
     const int buf_rows = S * M > nbox * box_rows ? S * M : nbox * box_rows;
     const size_t tile_bytes = (size_t)buf_rows * ROW_BYTES;
-    const size_t fixed = (size_t)6 * S * TCOLS * sizeof(double) + 64;
-    int nbuf = (int)((220 * 1024 - fixed) / tile_bytes);
+    const size_t fixed = (size_t)6 * S * TC * sizeof(double) + 64;
+    size_t budget = SMEM_PER_SM / CTAS - SMEM_CTA_RESERVED;
+    if (budget > SMEM_CTA_MAX) budget = SMEM_CTA_MAX;
+    int nbuf = (int)((budget - fixed) / tile_bytes);
     if (nbuf > 3) nbuf = 3;
     if (nbuf < 2) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)nbuf * tile_bytes + fixed;
+    auto kern = thomas_onchip_kernel<M, TC, MAXT, CTAS>;
     static bool configured = false;
     static int per_sm_cache[2] = {0, 0};                     // {threads*2^20 + smem key, blocks per SM}
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(thomas_onchip_kernel<M, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             220 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CTA_MAX);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const int threads = TCOLS * S;
+    const int threads = TC * S;
     if (threads > MAXT) return cudaErrorInvalidConfiguration;
     const int key = threads * 4096 + (int)(smem / 64);
     if (per_sm_cache[0] != key) {
         int per_sm = 0;
-        cudaError_t e =
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, thomas_onchip_kernel<M, MAXT>, threads, smem);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem);
         if (e != cudaSuccess) return e;
         if (per_sm < 1) return cudaErrorInvalidConfiguration;
         per_sm_cache[0] = key;
         per_sm_cache[1] = per_sm;
     }
     CUtensorMap tmap, tmap_out;
-    if (!make_field_map(&tmap, in, (size_t)nx * ny, nz, box_rows)) return cudaErrorUnknown;
-    if (!make_field_map(&tmap_out, x, (size_t)nx * ny, nz, box_rows)) return cudaErrorUnknown;
-    const int ntiles = (int)(((size_t)nx * ny) / TCOLS);
+    if (!make_field_map(&tmap, in, (size_t)nx * ny, nz, TC, box_rows, blocked)) return cudaErrorUnknown;
+    if (!make_field_map(&tmap_out, x, (size_t)nx * ny, nz, TC, box_rows, blocked)) return cudaErrorUnknown;
+    const int ntiles = (int)(((size_t)nx * ny) / TC);
     int grid = sms * per_sm_cache[1];
     if (grid > ntiles) grid = ntiles;
-    thomas_onchip_kernel<M, MAXT><<<grid, threads, smem, stream>>>(
-        tmap, tmap_out, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf, box_rows, nbox, buf_rows, shift0,
-        singular, ntiles);
+    kern<<<grid, threads, smem, stream>>>(tmap, tmap_out, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf,
+                                          box_rows, nbox, buf_rows, shift0, singular, ntiles);
     return cudaGetLastError();
 }
 
 }  // namespace
 
 bool thomas_onchip_supported(int nx, int ny, int nz) {
-    return ((size_t)nx * ny) % TCOLS == 0 && nz >= 2 && nz <= 768;
+    return ((size_t)nx * ny) % 16 == 0 && nz >= 2 && nz <= 768;
 }
 
 cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
-                                 int nz, double shift0, int singular, int sms, cudaStream_t stream) {
+                                 int nz, double shift0, int singular, bool blocked, bool blocked_shape, int sms, cudaStream_t stream) {
     if (!thomas_onchip_supported(nx, ny, nz)) return cudaErrorInvalidValue;
-    if (nz <= 128) return launch_m<8, 256>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    if (nz <= 512) return launch_m<16, 512>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
-    return launch_m<32, 384>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, sms, stream);
+#define TPT_GO(M, TC, MAXT, CTAS) launch_m<M, TC, MAXT, CTAS>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, blocked, sms, stream)
+    // Measured on the box (profiles/r1c_*.md): the sweep is bound by the FP64 + shared-memory pipes of the 16 warps the
+    // register file admits per SM, so the shapes differ only in how well the phases of co-resident CTAs interleave.
+    if (nz <= 128) return TPT_GO(8, 16, 256, 2);
+    if (nz <= 256) return TPT_GO(16, 16, 256, 2);
+    // 8-column tiles, odd segment length (rows of the two segments of a half-warp then fall into opposite 64-byte
+    // halves of the banks: conflict-free), two CTAs per SM.  Meant for the blocked layout (in the natural one an
+    // 8-column row is a 64-byte piece of a DRAM page); `blocked_shape` asks for the same partition — hence the same
+    // rounding — on a natural-layout field (tpt_solve_host, whose results equal tpt_solve's bit for bit).
+    if ((blocked || blocked_shape) && nz <= 544) return TPT_GO(17, 8, 256, 2);
+    if (nz <= 512) return TPT_GO(16, 16, 512, 1);
+    return TPT_GO(32, 16, 384, 1);
+#undef TPT_GO
 }
 
 // Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows

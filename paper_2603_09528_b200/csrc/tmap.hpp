@@ -27,14 +27,14 @@ inline EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-// FP64 tensor of rank 2 or 3.  dims[] in elements (dim 0 contiguous), strides_bytes[] for dims 1.. (multiples of 16),
+// FP64 tensor of rank 2 to 4.  dims[] in elements (dim 0 contiguous), strides_bytes[] for dims 1.. (multiples of 16),
 // box[] in elements.  Returns false if the driver entry point is missing or the encoding is rejected.
 inline bool make_f64_map(CUtensorMap *map, const void *base, int rank, const uint64_t *dims,
                          const uint64_t *strides_bytes, const uint32_t *box, CUtensorMapSwizzle swizzle) {
     EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn || rank < 2 || rank > 3) return false;
-    cuuint64_t d[3], s[2];
-    cuuint32_t b[3], e[3] = {1, 1, 1};
+    if (!fn || rank < 2 || rank > 4) return false;
+    cuuint64_t d[4], s[3];
+    cuuint32_t b[4], e[4] = {1, 1, 1, 1};
     for (int q = 0; q < rank; ++q) { d[q] = dims[q]; b[q] = box[q]; }
     for (int q = 0; q + 1 < rank; ++q) s[q] = strides_bytes[q];
     return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, const_cast<void *>(base), d, s, b, e,
