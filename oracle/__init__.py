@@ -9,6 +9,10 @@ from .binding import (  # noqa: F401
     OraclePlan,
     apply_operator_flux,
     dense_solve_3d,
+    divergence,
+    face_shapes,
+    gradient,
+    project,
     eig_1d,
     num_threads,
     operator_1d,

@@ -52,6 +52,9 @@ def lib():
                                               _dp, _dp]
         L.orc_dense_solve_3d_dirs.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, C.c_double, C.c_int, _dp,
                                               _dp]
+        L.orc_divergence.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, _dp, _dp, _dp, C.c_double, _dp]
+        L.orc_gradient.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _ip, _dp, _dp, _dp, _dp]
+        L.orc_project.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_double, _dp, _dp, _dp, _dp, _dp, C.c_double, C.c_int]
         L.orc_num_threads.argtypes = []
         _lib = L
     return _lib
@@ -201,3 +204,45 @@ def dense_solve_3d(xf, yf, zf, bc, alpha, f, dirs: int = DIRS_XYZ):
     _check(lib().orc_dense_solve_3d_dirs(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), float(alpha), int(dirs),
                                          _ptr(f), _ptr(phi)), "dense_solve_3d")
     return phi
+
+
+def face_shapes(nx, ny, nz):
+    """Shapes of the staggered velocity arrays (reading A18): u on x-faces, v on y-faces, w on z-faces."""
+    return (nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)
+
+
+def divergence(xf, yf, zf, bc, u, v, w, scale: float = 1.0):
+    xf, yf, zf = _faces(xf), _faces(yf), _faces(zf)
+    nx, ny, nz = xf.size - 1, yf.size - 1, zf.size - 1
+    su, sv, sw = face_shapes(nx, ny, nz)
+    u = np.ascontiguousarray(u, dtype=np.float64).reshape(su)
+    v = np.ascontiguousarray(v, dtype=np.float64).reshape(sv)
+    w = np.ascontiguousarray(w, dtype=np.float64).reshape(sw)
+    out = np.empty((nz, ny, nx))
+    _check(lib().orc_divergence(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), _ptr(u), _ptr(v), _ptr(w),
+                                float(scale), _ptr(out)), "divergence")
+    return out
+
+
+def gradient(xf, yf, zf, bc, phi):
+    xf, yf, zf = _faces(xf), _faces(yf), _faces(zf)
+    nx, ny, nz = xf.size - 1, yf.size - 1, zf.size - 1
+    su, sv, sw = face_shapes(nx, ny, nz)
+    phi = np.ascontiguousarray(phi, dtype=np.float64).reshape(nz, ny, nx)
+    gu, gv, gw = np.empty(su), np.empty(sv), np.empty(sw)
+    _check(lib().orc_gradient(nx, ny, nz, _ptr(xf), _ptr(yf), _ptr(zf), _bc(bc), _ptr(phi), _ptr(gu), _ptr(gv),
+                              _ptr(gw)), "gradient")
+    return gu, gv, gw
+
+
+def project(plan: "OraclePlan", c: float, u, v, w, p=None, alpha_p: float = 0.0, dirs: int = DIRS_XYZ):
+    """Eq. 2c-2e with the Poisson plan `plan`: returns (u, v, w, phi, p) as new arrays."""
+    su, sv, sw = face_shapes(plan.nx, plan.ny, plan.nz)
+    u = np.array(u, dtype=np.float64, order="C").reshape(su)
+    v = np.array(v, dtype=np.float64, order="C").reshape(sv)
+    w = np.array(w, dtype=np.float64, order="C").reshape(sw)
+    phi = np.empty(plan.shape)
+    pp = None if p is None else np.array(p, dtype=np.float64, order="C").reshape(plan.shape)
+    _check(lib().orc_project(plan._h, _ptr(plan.xf), _ptr(plan.yf), _ptr(plan.zf), float(c), _ptr(u), _ptr(v), _ptr(w),
+                             _ptr(phi), None if pp is None else _ptr(pp), float(alpha_p), int(dirs)), "project")
+    return u, v, w, phi, pp

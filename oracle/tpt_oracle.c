@@ -816,3 +816,122 @@ int orc_dense_solve_3d_dirs(int nx, int ny, int nz, const double *xf, const doub
     free(M);
     return rc;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Pressure projection on the staggered grid, Eq. 2c-2e (staggered arrangement P:57).
+ *
+ * [A18] Layout and boundary closure (the paper gives neither; both follow from L = D G having to be the
+ * operator of Eq. 3 with the boundary rows of [A3] and the cyclic corners of P:102):
+ *   velocities live on faces: u[k][j][f] on x-faces f = 0..nx (row length nx+1), v[k][g][i] on y-faces
+ *   g = 0..ny, w[h][j][i] on z-faces h = 0..nz; face f lies between cells f-1 and f.
+ *   divergence (cells):  (D u)_i = (u_{i+1} - u_i)/w_i  + the same in y and z.
+ *   gradient (faces):    interior (G phi)_f = (phi_f - phi_{f-1}) / delta_f,  delta_f = x_c,f - x_c,f-1;
+ *                        Neumann boundary face: 0 (mirror ghost phi_-1 = phi_0: a wall, the normal velocity there
+ *                        is prescribed and not corrected); Dirichlet boundary face: ghost phi_-1 = -phi_0 at
+ *                        distance w_0: (G phi)_0 = 2 phi_0 / w_0, (G phi)_n = -2 phi_{n-1} / w_{n-1};
+ *                        periodic: faces 0 and n are the same face, (phi_0 - phi_{n-1}) / ((w_0 + w_{n-1})/2) [A17];
+ *                        on input the entry of face n is ignored (D takes face 0 as the high face of cell n-1), on
+ *                        output it is written as a copy of face 0.
+ * ------------------------------------------------------------------------------------------ */
+static double grad_face(const double *xf, int n, int bc, int f, const double *phi, size_t stride) {
+    /* phi points at cell 0 of the line, cells `stride` apart */
+    if (f > 0 && f < n) {
+        double delta = 0.5 * (xf[f] + xf[f + 1]) - 0.5 * (xf[f - 1] + xf[f]);
+        return (phi[(size_t)f * stride] - phi[(size_t)(f - 1) * stride]) / delta;
+    }
+    if (bc == ORC_BC_NEUMANN) return 0.0;
+    if (bc == ORC_BC_PERIODIC) {
+        double delta = 0.5 * ((xf[1] - xf[0]) + (xf[n] - xf[n - 1]));
+        return (phi[0] - phi[(size_t)(n - 1) * stride]) / delta;
+    }
+    if (f == 0) return (phi[0] - (-phi[0])) / (xf[1] - xf[0]);
+    return ((-phi[(size_t)(n - 1) * stride]) - phi[(size_t)(n - 1) * stride]) / (xf[n] - xf[n - 1]);
+}
+
+/* out = scale * D(u, v, w)   (Eq. 2c's right-hand side with scale = 1/(gamma_k dt)) */
+int orc_divergence(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf, const int bc[3],
+                   const double *u, const double *v, const double *w, double scale, double *out) {
+    if (!faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf) || !bc || !u || !v || !w || !out) return ORC_EINVAL;
+    const size_t plane = (size_t)nx * ny;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                /* high faces: in a periodic direction face n is face 0 */
+                int ih = (bc[0] == ORC_BC_PERIODIC && i == nx - 1) ? 0 : i + 1;
+                int jh = (bc[1] == ORC_BC_PERIODIC && j == ny - 1) ? 0 : j + 1;
+                int kh = (bc[2] == ORC_BC_PERIODIC && k == nz - 1) ? 0 : k + 1;
+                double du = (u[ih + (size_t)(nx + 1) * (j + (size_t)ny * k)] - u[i + (size_t)(nx + 1) * (j + (size_t)ny * k)]) / (xf[i + 1] - xf[i]);
+                double dv = (v[i + (size_t)nx * (jh + (size_t)(ny + 1) * k)] - v[i + (size_t)nx * (j + (size_t)(ny + 1) * k)]) / (yf[j + 1] - yf[j]);
+                double dw = (w[i + (size_t)nx * j + plane * kh] - w[i + (size_t)nx * j + plane * k]) / (zf[k + 1] - zf[k]);
+                out[i + (size_t)nx * j + plane * k] = scale * (du + dv + dw);
+            }
+    return ORC_OK;
+}
+
+/* (gu, gv, gw) = G phi on every face (boundary faces by the closure above). */
+int orc_gradient(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf, const int bc[3],
+                 const double *phi, double *gu, double *gv, double *gw) {
+    if (!faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf) || !bc || !phi || !gu || !gv || !gw) return ORC_EINVAL;
+    const size_t plane = (size_t)nx * ny;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int f = 0; f <= nx; ++f)
+                gu[f + (size_t)(nx + 1) * (j + (size_t)ny * k)] = grad_face(xf, nx, bc[0], f, phi + (size_t)nx * j + plane * k, 1);
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int g = 0; g <= ny; ++g)
+            for (int i = 0; i < nx; ++i)
+                gv[i + (size_t)nx * (g + (size_t)(ny + 1) * k)] = grad_face(yf, ny, bc[1], g, phi + i + plane * k, (size_t)nx);
+#pragma omp parallel for schedule(static)
+    for (int h = 0; h <= nz; ++h)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i)
+                gw[i + (size_t)nx * j + plane * h] = grad_face(zf, nz, bc[2], h, phi + i + (size_t)nx * j, plane);
+    return ORC_OK;
+}
+
+/* One projection, in the paper's order:
+ *   Eq. 2c   L Phi = D u* / c          (c = gamma_k dt; `poisson` is a plan of the full operator, alpha = 0)
+ *   Eq. 2d   u <- u* - c G Phi
+ *   Eq. 2e   P <- P + Phi - alpha_p L_I Phi   (skipped if p == NULL; alpha_p = gamma_k nu dt / 2; L_I by `dirs`,
+ *            evaluated in flux form; alpha_p == 0 is the fully explicit choice L_I = 0)
+ * u, v, w are updated in place; phi receives Phi. */
+int orc_project(const orc_plan *poisson, const double *xf, const double *yf, const double *zf, double c,
+                double *u, double *v, double *w, double *phi, double *p, double alpha_p, int dirs) {
+    if (!poisson || poisson->alpha != 0.0 || poisson->dirs != ORC_DIRS_XYZ || !(c > 0.0) || !u || !v || !w || !phi) return ORC_EINVAL;
+    if (p && alpha_p != 0.0 && dirs != ORC_DIRS_XYZ && dirs != ORC_DIRS_YZ && dirs != ORC_DIRS_Z) return ORC_EINVAL;
+    const int nx = poisson->nx, ny = poisson->ny, nz = poisson->nz;
+    const int *bc = poisson->bc;
+    const size_t n = (size_t)nx * ny * nz;
+    const size_t nu = (size_t)(nx + 1) * ny * nz, nv = (size_t)nx * (ny + 1) * nz, nw = (size_t)nx * ny * (nz + 1);
+    double *rhs = (double *)malloc(sizeof(double) * n), *work = (double *)malloc(sizeof(double) * n);
+    double *gu = (double *)malloc(sizeof(double) * nu), *gv = (double *)malloc(sizeof(double) * nv), *gw = (double *)malloc(sizeof(double) * nw);
+    int rc = (rhs && work && gu && gv && gw) ? ORC_OK : ORC_ENOMEM;
+    if (rc == ORC_OK) rc = orc_divergence(nx, ny, nz, xf, yf, zf, bc, u, v, w, 1.0 / c, rhs);     /* 2c, rhs */
+    if (rc == ORC_OK) rc = orc_solve(poisson, rhs, phi, work);                                    /* 2c */
+    if (rc == ORC_OK) rc = orc_gradient(nx, ny, nz, xf, yf, zf, bc, phi, gu, gv, gw);
+    if (rc == ORC_OK) {                                                                           /* 2d */
+        for (size_t q = 0; q < nu; ++q) u[q] -= c * gu[q];
+        for (size_t q = 0; q < nv; ++q) v[q] -= c * gv[q];
+        for (size_t q = 0; q < nw; ++q) w[q] -= c * gw[q];
+        /* periodic: face n is written as a copy of face 0 */
+        if (bc[0] == ORC_BC_PERIODIC)
+            for (size_t r = 0; r < (size_t)ny * nz; ++r) u[r * (nx + 1) + nx] = u[r * (nx + 1)];
+        if (bc[1] == ORC_BC_PERIODIC)
+            for (int k = 0; k < nz; ++k)
+                for (int i = 0; i < nx; ++i) v[i + (size_t)nx * (ny + (size_t)(ny + 1) * k)] = v[i + (size_t)nx * (0 + (size_t)(ny + 1) * k)];
+    }
+    if (rc == ORC_OK && p) {                                                                      /* 2e */
+        if (alpha_p == 0.0) {
+            for (size_t q = 0; q < n; ++q) p[q] += phi[q];
+        } else {
+            rc = orc_apply_operator_flux_dirs(nx, ny, nz, xf, yf, zf, bc, alpha_p, dirs, phi, work);   /* (I - alpha L_I) Phi */
+            if (rc == ORC_OK)
+                for (size_t q = 0; q < n; ++q) p[q] += work[q];
+        }
+    }
+    free(rhs); free(work); free(gu); free(gv); free(gw);
+    return rc;
+}

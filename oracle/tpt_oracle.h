@@ -23,8 +23,9 @@
  * Parity pins (tests/, -m "not gpu"): brute-force dense LU of the assembled operator on <= 8^3
  * grids; closed-form eigenvalues / DCT-II eigenvectors on uniform grids; Q^T Q = I; flux-form
  * residual at round-off; discrete eigenfunction rhs; manufactured smooth solutions; lambda_1
- * -> -pi^2; gauge invariance; footnote-4 grading ratios (inputs).  No function here is
- * "parity unpinned".
+ * -> -pi^2; gauge invariance; footnote-4 grading ratios (inputs); for the projection (Eq. 2c-2e): D G = the
+ * flux-form Laplacian, closed forms of D and G on polynomial fields, summation by parts (D = -G^T in the cell /
+ * face volume inner products), discretely divergence-free result.  No function here is "parity unpinned".
  */
 #ifndef TPT_ORACLE_H
 #define TPT_ORACLE_H
@@ -120,6 +121,16 @@ int  orc_dense_solve_3d(int nx, int ny, int nz,
 int  orc_dense_solve_3d_dirs(int nx, int ny, int nz,
                              const double *xf, const double *yf, const double *zf,
                              const int bc[3], double alpha, int dirs, const double *f, double *phi);
+
+/* ---- pressure projection on the staggered grid, Eq. 2c-2e ------------------------------ */
+/* Face arrays: u (nz, ny, nx+1), v (nz, ny+1, nx), w (nz+1, ny, nx); closure of the boundary faces: reading [A18]. */
+int  orc_divergence(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf, const int bc[3],
+                    const double *u, const double *v, const double *w, double scale, double *out);
+int  orc_gradient(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf, const int bc[3],
+                  const double *phi, double *gu, double *gv, double *gw);
+/* L Phi = D u / c;  u -= c G Phi;  p += Phi - alpha_p L_I Phi  (p may be NULL).  `poisson`: alpha = 0 plan. */
+int  orc_project(const orc_plan *poisson, const double *xf, const double *yf, const double *zf, double c,
+                 double *u, double *v, double *w, double *phi, double *p, double alpha_p, int dirs);
 
 int  orc_num_threads(void);
 
