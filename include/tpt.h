@@ -121,6 +121,35 @@ int tpt_plan_reserve_batch(tpt_plan *plan, int nrhs);
  */
 int tpt_solve_host(tpt_plan *plan, const double *rhs_host, double *out_host, void *cuda_stream);
 
+/*
+ * Pressure projection of the fractional-step method on the staggered grid, Eq. 2c–2e (staggered
+ * arrangement PAPER.md:57; "applying the pressure-projection step to a white-noise velocity field produces a
+ * discretely divergence-free field to machine precision").
+ *   Velocity components live on cell faces: u_dev (nz, ny, nx+1) on x-faces, v_dev (nz, ny+1, nx) on y-faces,
+ *   w_dev (nz+1, ny, nx) on z-faces, each dense with x contiguous; face f of a direction lies between cells f-1 and f.
+ *   Divergence D (cells) and gradient G (faces) are the second-order differences whose product D G is the Laplacian
+ *   of Eq. 3 with the plan's boundary rows.  Boundary faces follow the pressure BC of their direction: NEUMANN = wall
+ *   (G Phi = 0 there; the face keeps its prescribed normal velocity), DIRICHLET = ghost value -Phi one cell width
+ *   away, PERIODIC = faces 0 and n are one face (entry n is ignored on input and written as a copy of entry 0).
+ *
+ * tpt_divergence      out = scale * D(u, v, w)                    (right-hand side of Eq. 2c with scale = 1/(gamma_k dt))
+ * tpt_gradient_correct u -= c G phi  (Eq. 2d);  if p_dev != NULL:  p += phi - alpha_p L_I phi  (Eq. 2e), L_I the 1-D
+ *                     Laplacians of the directions in implicit_dirs (TPT_DIRS_*; alpha_p = gamma_k nu dt / 2;
+ *                     alpha_p == 0 is the fully explicit choice L_I = 0), evaluated in flux form.
+ * tpt_project         Eq. 2c, 2d, 2e in order: phi_dev = L^{-1} (D u / gamma_dt) through tpt_solve, then the correction.
+ *                     The plan must be a Poisson plan of the full operator (helmholtz_alpha == 0, TPT_DIRS_XYZ):
+ *                     TPT_EINVAL otherwise.  On a singular plan the velocity field must be compatible (zero net flux
+ *                     through the walls), as in the paper's solver; Phi then has zero volume-weighted mean.
+ * All DEVICE pointers, 16-byte aligned, no aliasing between arguments; phi_dev / out_dev: nx*ny*nz doubles.
+ * Asynchronous on cuda_stream, no allocation, no host synchronisation.  gamma_dt, c > 0; alpha_p >= 0.
+ */
+int tpt_divergence(tpt_plan *plan, const double *u_dev, const double *v_dev, const double *w_dev, double scale,
+                   double *out_dev, void *cuda_stream);
+int tpt_gradient_correct(tpt_plan *plan, const double *phi_dev, double c, double *u_dev, double *v_dev, double *w_dev,
+                         double *p_dev, double alpha_p, int implicit_dirs, void *cuda_stream);
+int tpt_project(tpt_plan *plan, double *u_dev, double *v_dev, double *w_dev, double gamma_dt, double *phi_dev,
+                double *p_dev, double alpha_p, int implicit_dirs, void *cuda_stream);
+
 /* tpt_plan_destroy — frees everything the plan owns (synchronises the device). NULL is a no-op. */
 int tpt_plan_destroy(tpt_plan *plan);
 

@@ -27,6 +27,7 @@ SYMBOLS = (
     "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
+    "tpt_divergence", "tpt_gradient_correct", "tpt_project",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -55,6 +56,9 @@ def lib():
         L.tpt_solve_batch.argtypes = [vp, vp, vp, i, vp]
         L.tpt_plan_reserve_batch.argtypes = [vp, i]
         L.tpt_solve_host.argtypes = [vp, vp, vp, vp]
+        L.tpt_divergence.argtypes = [vp, vp, vp, vp, d, vp, vp]
+        L.tpt_gradient_correct.argtypes = [vp, vp, d, vp, vp, vp, vp, d, i, vp]
+        L.tpt_project.argtypes = [vp, vp, vp, vp, d, vp, vp, d, i, vp]
         L.tpt_plan_destroy.argtypes = [vp]
         L.tpt_plan_get_eigen.argtypes = [vp, i, _dp, _dp]
         L.tpt_plan_is_singular.argtypes = [vp]
@@ -241,6 +245,37 @@ def solve_host(plan: Plan, rhs_host, out_host, stream=None):
     _check(lib().tpt_solve_host(plan._h, hp(rhs_host, "rhs"), hp(out_host, "out"), _stream_handle(stream)),
            "tpt_solve_host")
     return out_host
+
+
+def face_counts(plan: Plan):
+    """Element counts of the staggered velocity arrays u (nz, ny, nx+1), v (nz, ny+1, nx), w (nz+1, ny, nx)."""
+    return ((plan.nx + 1) * plan.ny * plan.nz, plan.nx * (plan.ny + 1) * plan.nz, plan.nx * plan.ny * (plan.nz + 1))
+
+
+def divergence(plan: Plan, u, v, w, out, scale: float = 1.0, stream=None):
+    """out = scale * D(u, v, w) on the staggered grid (right-hand side of Eq. 2c).  Asynchronous."""
+    cu, cv, cw = face_counts(plan)
+    _check(lib().tpt_divergence(plan._h, _dev_ptr(u, cu, "u"), _dev_ptr(v, cv, "v"), _dev_ptr(w, cw, "w"), float(scale),
+                                _dev_ptr(out, plan.points, "out"), _stream_handle(stream)), "tpt_divergence")
+    return out
+
+
+def gradient_correct(plan: Plan, phi, c: float, u, v, w, p=None, alpha_p: float = 0.0, dirs: int = DIRS_XYZ, stream=None):
+    """u -= c G phi (Eq. 2d) and, if p is given, p += phi - alpha_p L_I phi (Eq. 2e).  In place, asynchronous."""
+    cu, cv, cw = face_counts(plan)
+    _check(lib().tpt_gradient_correct(plan._h, _dev_ptr(phi, plan.points, "phi"), float(c), _dev_ptr(u, cu, "u"),
+                                      _dev_ptr(v, cv, "v"), _dev_ptr(w, cw, "w"),
+                                      None if p is None else _dev_ptr(p, plan.points, "p"), float(alpha_p), int(dirs),
+                                      _stream_handle(stream)), "tpt_gradient_correct")
+
+
+def project(plan: Plan, u, v, w, gamma_dt: float, phi, p=None, alpha_p: float = 0.0, dirs: int = DIRS_XYZ, stream=None):
+    """One pressure projection (Eq. 2c-2e) with a Poisson plan: u, v, w (and p) updated in place, phi = Phi."""
+    cu, cv, cw = face_counts(plan)
+    _check(lib().tpt_project(plan._h, _dev_ptr(u, cu, "u"), _dev_ptr(v, cv, "v"), _dev_ptr(w, cw, "w"), float(gamma_dt),
+                             _dev_ptr(phi, plan.points, "phi"), None if p is None else _dev_ptr(p, plan.points, "p"),
+                             float(alpha_p), int(dirs), _stream_handle(stream)), "tpt_project")
+    return phi
 
 
 def plan_destroy(plan: Plan):

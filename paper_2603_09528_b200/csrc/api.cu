@@ -33,6 +33,8 @@ struct tpt_plan {
     double *d_yfwd = nullptr;   // [m][j]  = sqrt(wy_j) Q~y[j][m]           A-operand of step 2.2
     double *d_yinv = nullptr;   // [j][m]  = Q~y[j][m] / sqrt(wy_j)         A-operand of step 2.4
     double *d_vec = nullptr;    // lamx | lamy | az | bz | cz | wz
+    double *d_geo = nullptr;    // rwx | gfx | rwy | gfy | rwz | gfz: 1/width per cell, 1/centre spacing per face (projection.cu)
+    tpt::ProjGeom geo{};
     double *d_abc = nullptr;    // coefficient tables of the on-chip Thomas kernel (thomas_onchip_tables)
     double *d_lamx = nullptr, *d_lamy = nullptr, *d_az = nullptr, *d_bz = nullptr, *d_cz = nullptr, *d_wz = nullptr;
     double *d_work = nullptr;   // one field
@@ -60,6 +62,7 @@ void free_plan(tpt_plan *p) {
     cudaFree(p->d_yinv);
     cudaFree(p->d_vec);
     cudaFree(p->d_abc);
+    cudaFree(p->d_geo);
     cudaFree(p->d_work);
     cudaFree(p->d_stage);
     for (auto &e : p->ev_pool) cudaEventDestroy(e);
@@ -326,6 +329,25 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
             p->d_lamx = p->d_vec + o_lamx; p->d_lamy = p->d_vec + o_lamy;
             p->d_az = p->d_vec + o_az; p->d_bz = p->d_vec + o_bz; p->d_cz = p->d_vec + o_cz; p->d_wz = p->d_vec + o_wz;
         }
+        if (rc == TPT_OK) {   // geometry of the staggered divergence / gradient (Eq. 2c-2e)
+            std::vector<double> v;
+            size_t off[6];
+            const tpt::Operator1D *ops[3] = {&ox, &oy, &oz};
+            for (int d = 0; d < 3; ++d) {
+                off[2 * d] = v.size();
+                for (double wd : ops[d]->w) v.push_back(1.0 / wd);
+                if (v.size() & 1) v.push_back(0.0);
+                off[2 * d + 1] = v.size();
+                for (double dl : ops[d]->delta) v.push_back(1.0 / dl);
+                if (v.size() & 1) v.push_back(0.0);
+            }
+            rc = upload(&p->d_geo, v);
+            p->geo.nx = nx; p->geo.ny = ny; p->geo.nz = nz;
+            for (int d = 0; d < 3; ++d) p->geo.bc[d] = bc[d];
+            p->geo.rwx = p->d_geo + off[0]; p->geo.gfx = p->d_geo + off[1];
+            p->geo.rwy = p->d_geo + off[2]; p->geo.gfy = p->d_geo + off[3];
+            p->geo.rwz = p->d_geo + off[4]; p->geo.gfz = p->d_geo + off[5];
+        }
         if (rc == TPT_OK) {
             std::vector<double> t;
             tpt::thomas_onchip_tables(nz, oz.a.data(), oz.b.data(), oz.c.data(), t);
@@ -486,6 +508,43 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
         return TPT_ECUDA;
     p->launches_last = launches;
     return cudaStreamSynchronize(st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+int tpt_divergence(tpt_plan *p, const double *u_dev, const double *v_dev, const double *w_dev, double scale, double *out_dev,
+                   void *cuda_stream) {
+    if (!p || !u_dev || !v_dev || !w_dev || !out_dev || !std::isfinite(scale)) return TPT_EINVAL;
+    cudaError_t e = tpt::launch_divergence(u_dev, v_dev, w_dev, p->geo, scale, out_dev, static_cast<cudaStream_t>(cuda_stream));
+    p->launches_last = 1;
+    return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+static bool dirs_valid(int d) { return d == TPT_DIRS_XYZ || d == TPT_DIRS_YZ || d == TPT_DIRS_Z; }
+
+int tpt_gradient_correct(tpt_plan *p, const double *phi_dev, double c, double *u_dev, double *v_dev, double *w_dev, double *p_dev,
+                         double alpha_p, int implicit_dirs, void *cuda_stream) {
+    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c)) return TPT_EINVAL;
+    if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
+    cudaError_t e = tpt::launch_correct(phi_dev, u_dev, v_dev, w_dev, p_dev, p->geo, c, alpha_p, implicit_dirs,
+                                        static_cast<cudaStream_t>(cuda_stream));
+    p->launches_last = 1;
+    return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+int tpt_project(tpt_plan *p, double *u_dev, double *v_dev, double *w_dev, double gamma_dt, double *phi_dev, double *p_dev,
+                double alpha_p, int implicit_dirs, void *cuda_stream) {
+    if (!p || !u_dev || !v_dev || !w_dev || !phi_dev || !aligned16(phi_dev)) return TPT_EINVAL;
+    if (p->alpha != 0.0 || p->dirs != TPT_DIRS_XYZ) return TPT_EINVAL;       // Eq. 2c carries the full Laplacian
+    if (!(gamma_dt > 0.0) || !std::isfinite(gamma_dt)) return TPT_EINVAL;
+    if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (tpt::launch_divergence(u_dev, v_dev, w_dev, p->geo, 1.0 / gamma_dt, phi_dev, st) != cudaSuccess) return TPT_ECUDA;
+    int rc = tpt_solve(p, phi_dev, phi_dev, cuda_stream);                      // in place: rhs -> Phi
+    if (rc != TPT_OK) return rc;
+    const int solve_launches = p->launches_last;
+    if (tpt::launch_correct(phi_dev, u_dev, v_dev, w_dev, p_dev, p->geo, gamma_dt, alpha_p, implicit_dirs, st) != cudaSuccess)
+        return TPT_ECUDA;
+    p->launches_last = solve_launches + 2;
+    return TPT_OK;
 }
 
 int tpt_plan_destroy(tpt_plan *p) {

@@ -64,6 +64,21 @@ cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab,
 // between consecutive z levels of that column (nx*ny in the natural layout, 16 in the tile-blocked one).
 cudaError_t launch_gauge(double *x, const double *wz, size_t stride, int nz, cudaStream_t stream);
 
+// Staggered-grid operators of the pressure projection, Eq. 2c-2e (projection.cu).  Device vectors of the plan:
+// rw* = 1 / cell width (n entries), gf* = 1 / centre spacing at every face (n + 1 entries; boundary faces: one cell
+// width, periodic: the wrap spacing).  bc as in tpt.h.
+struct ProjGeom {
+    int nx, ny, nz;
+    int bc[3];
+    const double *rwx, *rwy, *rwz, *gfx, *gfy, *gfz;
+};
+// out = scale * D(u, v, w)
+cudaError_t launch_divergence(const double *u, const double *v, const double *w, const ProjGeom &g, double scale,
+                              double *out, cudaStream_t stream);
+// u -= c G phi (all three face arrays); if p: p += phi - alpha L_I phi, L_I = the directions in `dirs` (z always)
+cudaError_t launch_correct(const double *phi, double *u, double *v, double *w, double *p, const ProjGeom &g, double c,
+                           double alpha, int dirs, cudaStream_t stream);
+
 // FP64 pipe microbenchmarks (kind 0: DFMA, 1: DMMA).  Returns TFLOP/s.
 cudaError_t run_fp64_peak(int kind, double *tflops);
 

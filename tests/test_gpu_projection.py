@@ -1,0 +1,158 @@
+"""GPU parity of the pressure projection (Eq. 2c-2e) against the CPU oracle: divergence, gradient
+correction with every boundary closure, the fused pressure update, the whole projection, and the property the paper
+states for it (discretely divergence-free white noise) at a size that spans many thread blocks."""
+import numpy as np
+import pytest
+
+from paper_2603_09528_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+N_, D_, P_ = I.NEUMANN, I.DIRICHLET, I.PERIODIC
+# D and G are a handful of flops per output, but the centre spacing delta is a difference of face coordinates: the
+# library's 0.5 (x_{f+1} - x_{f-1}) and the oracle's x_c,f - x_c,f-1 are two roundings of it that differ by
+# eps |x| / delta ~ 1.1e-16 / 2e-4 ~ 5e-13 relative on these grids (the same input rounding the solver's parity budget has)
+STENCIL_TOL = 3e-12
+PARITY_TOL = 1e-10       # through the solve (BASELINE.json north_star)
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def tpt(torch):
+    from paper_2603_09528_b200 import api
+
+    api.lib()
+    return api
+
+
+def _rel(a, b):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def _velocity(orc, n, bc, seed):
+    su, sv, sw = orc.face_shapes(*n)
+    u = I.uniform_pm1(seed, int(np.prod(su))).reshape(su)
+    v = I.uniform_pm1(seed + 1, int(np.prod(sv))).reshape(sv)
+    w = I.uniform_pm1(seed + 2, int(np.prod(sw))).reshape(sw)
+    if bc[0] == N_:
+        u[:, :, 0] = u[:, :, -1] = 0.0
+    if bc[1] == N_:
+        v[:, 0, :] = v[:, -1, :] = 0.0
+    if bc[2] == N_:
+        w[0] = w[-1] = 0.0
+    return u, v, w
+
+
+CASES = [
+    # name, n, beta, bc
+    ("ragged-nnd", (37, 21, 19), (2.0, 1.5, 2.5), (N_, N_, D_)),
+    ("ragged-pdn", (33, 18, 35), (0.0, 2.0, 2.0), (P_, D_, N_)),
+    ("ragged-dpd", (130, 9, 17), (1.5, 0.0, 1.0), (D_, P_, D_)),
+    ("wide-nnn", (300, 12, 40), (2.0, 2.0, 2.0), (N_, N_, N_)),     # several x blocks and z chunks
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=[c[0] for c in CASES])
+def test_divergence_and_correction_match_the_oracle(tpt, torch, orc, case):
+    name, n, beta, bc = case
+    P = I.Problem(name, n, (1.0, 2.0, 1.5), beta, bc, 0.0, 5)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, 1e-3 if bc == (N_, N_, N_) else 0.0)   # any plan carries the geometry
+    u, v, w = _velocity(orc, n, bc, 40)
+    du, dv, dw = (torch.from_numpy(a).cuda() for a in (u, v, w))
+    out = torch.empty(n[::-1], dtype=torch.float64, device="cuda")
+    tpt.divergence(plan, du, dv, dw, out, scale=2.5)
+    torch.cuda.synchronize()
+    ref = orc.divergence(xf, yf, zf, bc, u, v, w, scale=2.5)
+    assert _rel(out.cpu().numpy(), ref) <= STENCIL_TOL
+
+    phi = I.uniform_pm1(50, P.points).reshape(n[::-1])
+    p0 = I.uniform_pm1(51, P.points).reshape(n[::-1])
+    gu, gv, gw = orc.gradient(xf, yf, zf, bc, phi)
+    c, alpha_p = 0.7, 2e-3
+    for dirs in (tpt.DIRS_XYZ, tpt.DIRS_YZ, tpt.DIRS_Z, None):
+        du, dv, dw = (torch.from_numpy(a).cuda() for a in (u, v, w))
+        dp = None if dirs is None else torch.from_numpy(p0).cuda()
+        tpt.gradient_correct(plan, torch.from_numpy(phi).cuda(), c, du, dv, dw, p=dp, alpha_p=alpha_p,
+                             dirs=tpt.DIRS_XYZ if dirs is None else dirs)
+        torch.cuda.synchronize()
+        eu, ev, ew = u - c * gu, v - c * gv, w - c * gw
+        if bc[0] == P_:
+            eu[:, :, -1] = eu[:, :, 0]
+        if bc[1] == P_:
+            ev[:, -1, :] = ev[:, 0, :]
+        scale = max(np.abs(c * gu).max(), np.abs(c * gv).max(), np.abs(c * gw).max())
+        for got, exp in ((du, eu), (dv, ev), (dw, ew)):
+            assert np.abs(got.cpu().numpy() - exp).max() <= STENCIL_TOL * scale
+        if dirs is not None:
+            odirs = {tpt.DIRS_XYZ: orc.DIRS_XYZ, tpt.DIRS_YZ: orc.DIRS_YZ, tpt.DIRS_Z: orc.DIRS_Z}[dirs]
+            ep = p0 + orc.apply_operator_flux(xf, yf, zf, bc, alpha_p, phi, dirs=odirs)
+            assert _rel(dp.cpu().numpy(), ep) <= 1e-12
+    # wall faces are left exactly as they were
+    if bc[0] == N_:
+        assert np.array_equal(du.cpu().numpy()[:, :, 0], u[:, :, 0]) and np.array_equal(du.cpu().numpy()[:, :, -1], u[:, :, -1])
+    plan.destroy()
+
+
+PROJECT_CASES = [
+    ("ragged", (40, 36, 33), (2.0, 1.5, 2.5), (N_, N_, D_)),
+    ("singular", (128, 128, 40), (2.0, 2.0, 2.0), (N_, N_, N_)),
+    ("duct", (128, 128, 48), (0.0, 2.0, 2.5), (P_, N_, N_)),
+]
+
+
+@pytest.mark.parametrize("case", PROJECT_CASES, ids=[c[0] for c in PROJECT_CASES])
+def test_projection_parity_and_divergence_free(tpt, torch, orc, case):
+    name, n, beta, bc = case
+    P = I.Problem(name, n, (1.0, 1.0, 1.0), beta, bc, 0.0, 6)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, 0.0)
+    u, v, w = _velocity(orc, n, bc, 60)
+    p0 = I.uniform_pm1(70, P.points).reshape(n[::-1])
+    c, alpha_p = 0.31, 1e-3
+    du, dv, dw, dp = (torch.from_numpy(a).cuda() for a in (u, v, w, p0))
+    phi = torch.empty(n[::-1], dtype=torch.float64, device="cuda")
+    tpt.project(plan, du, dv, dw, c, phi, p=dp, alpha_p=alpha_p, dirs=tpt.DIRS_YZ)
+    torch.cuda.synchronize()
+    ru, rv, rw, rphi, rp = orc.project(orc.OraclePlan(xf, yf, zf, bc, 0.0), c, u, v, w, p=p0, alpha_p=alpha_p, dirs=orc.DIRS_YZ)
+    assert _rel(phi.cpu().numpy(), rphi) <= PARITY_TOL
+    assert _rel(dp.cpu().numpy(), rp) <= PARITY_TOL
+    corr = max(np.abs(ru - u).max(), np.abs(rv - v).max(), np.abs(rw - w).max())
+    for got, exp in ((du, ru), (dv, rv), (dw, rw)):
+        assert np.abs(got.cpu().numpy() - exp).max() <= PARITY_TOL * corr
+    # divergence-free to machine precision (checked with the oracle's divergence, not the library's own)
+    d0 = orc.divergence(xf, yf, zf, bc, u, v, w)
+    d1 = orc.divergence(xf, yf, zf, bc, du.cpu().numpy(), dv.cpu().numpy(), dw.cpu().numpy())
+    assert np.abs(d1).max() <= 1e-11 * np.abs(d0).max()
+    plan.destroy()
+
+
+def test_project_argument_checks(tpt, torch):
+    n = (16, 16, 16)
+    P = I.Problem("chk", n, (1.0, 1.0, 1.0), (1.0, 1.0, 1.0), (N_, N_, D_), 1e-3, 1)
+    xf, yf, zf = P.faces()
+    helm = tpt.plan_create(*n, xf, yf, zf, P.bc, 1e-3)
+    cu, cv, cw = tpt.face_counts(helm)
+    z = lambda m: torch.zeros(m, dtype=torch.float64, device="cuda")
+    u, v, w, phi = z(cu), z(cv), z(cw), z(helm.points)
+    with pytest.raises(tpt.TptError):          # Eq. 2c needs the Poisson plan of the full operator
+        tpt.project(helm, u, v, w, 0.1, phi)
+    helm.destroy()
+    pois = tpt.plan_create(*n, xf, yf, zf, P.bc, 0.0)
+    with pytest.raises(tpt.TptError):
+        tpt.project(pois, u, v, w, 0.0, phi)   # gamma dt must be positive
+    with pytest.raises(tpt.TptError):
+        tpt.project(pois, u, v, w, 0.1, phi, p=z(pois.points), alpha_p=-1.0)
+    with pytest.raises(ValueError):
+        tpt.project(pois, z(cu - 1), v, w, 0.1, phi)
+    tpt.project(pois, u, v, w, 0.1, phi)       # zero velocity: Phi = 0, nothing changes
+    torch.cuda.synchronize()
+    assert float(phi.abs().max()) == 0.0 and float(u.abs().max()) == 0.0
+    pois.destroy()
