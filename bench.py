@@ -38,8 +38,8 @@ UNIT = "Gpts/s"
 SM_COUNT, FP64_FMA_PER_CLK_SM = 148, 64
 ORACLE_SAMPLE_NZ = 64
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (gemm_tma_kernel), from the one
-# `ncu --set full` capture summarised in profiles/r1b_tma_gemm_onchip_thomas.md (config c3; bytes).  Other configs: null.
-NCU_TRAFFIC_BYTES = {"c3": 1.076042e9 + 1.030894e9}
+# `ncu --set full` capture summarised in profiles/r1c_blocked_layout_projection.md (config c3; bytes).  Other configs: null.
+NCU_TRAFFIC_BYTES = {"c3": 1.077565e9 + 1.031300e9}
 
 
 def _peaks():
@@ -282,6 +282,43 @@ def run_gpu(args):
     e2e_val = whole_job_value(world, pts_step, e2e_steps, e2e_s)
     e2e_ok = all(np.array_equal(b.numpy(), o.cpu().numpy()) for b, o in zip(pin_out, d_out))
 
+    # ---- widened row: one pressure projection (Eq. 2c-2e) = divergence + this solve + correction,
+    # timed on the device on the workload's Poisson plan (outside the headline timed region; rank 0 only)
+    projection = None
+    pois = [(pl, P) for pl, P in zip(plans, probs) if P.alpha == 0.0]
+    if rank == 0 and pois and not args.no_projection:
+        pl, P = pois[0]
+        cu, cv, cw = api.face_counts(pl)
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(1234)
+        fu, fv, fw = (torch.rand(m, dtype=torch.float64, device="cuda", generator=gen) * 2 - 1 for m in (cu, cv, cw))
+        phi, pr = torch.empty(pl.points, dtype=torch.float64, device="cuda"), torch.zeros(pl.points, dtype=torch.float64, device="cuda")
+
+        def timed(fn, reps=10):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+            e[0].record(stream)
+            for q in range(reps):
+                fn()
+                e[q + 1].record(stream)
+            torch.cuda.synchronize()
+            return e[0].elapsed_time(e[-1]) / reps
+
+        t_div = timed(lambda: api.divergence(pl, fu, fv, fw, phi, 1.0, stream))
+        t_cor = timed(lambda: api.gradient_correct(pl, phi, 1e-9, fu, fv, fw, p=pr, alpha_p=1e-9, dirs=api.DIRS_XYZ, stream=stream))
+        t_all = timed(lambda: api.project(pl, fu, fv, fw, 1.0, phi, p=pr, alpha_p=1e-9, dirs=api.DIRS_XYZ, stream=stream))
+        hbm = _peaks()[0]["hbm_gbs"]
+        projection = {
+            "workload": f"tpt_project on {P.name}: white-noise face velocities, pressure update fused (Eq. 2e, L_I = L)",
+            "ms_per_projection": t_all, "gpts_per_s": P.points / t_all / 1e6,
+            "divergence": {"ms": t_div, "algorithmic_B_per_pt": 32, "frac_of_hbm_peak": 32.0 * P.points / t_div / 1e6 / hbm},
+            "correction_with_pressure_update": {"ms": t_cor, "algorithmic_B_per_pt": 72,
+                                                "frac_of_hbm_peak": 72.0 * P.points / t_cor / 1e6 / hbm},
+        }
+        del fu, fv, fw, phi, pr
+
     if rank == 0:
         peaks, peak_kind = _peaks()
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
@@ -314,7 +351,7 @@ def run_gpu(args):
             "peak_measured_dmma_loop": dmma_meas, "peak_measured_dfma_loop": dfma_meas,
             "frac_of_measured_dmma_loop": kernels[dom]["achieved_tflops"] / dmma_meas,
             "algorithmic_flops_per_launch": flops[dom], "algorithmic_dram_bytes_per_launch": 16.0 * pts,
-            "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1b_*.md)",
+            "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1c_*.md)",
         }
         cpu = _oracle_sample(probs, 1, 1)
         n20 = per_step[: min(20, len(per_step))]
@@ -324,6 +361,7 @@ def run_gpu(args):
             "dtype": "f64", "data": "synthetic",
             "config": _config_json(args.config, probs, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
             "clocks": clocks,
+            "projection": projection,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * pts_step, "d2h_bytes_per_step": 8 * pts_step,
                     "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3, "matches_device_result": bool(e2e_ok)},
             "gpu_launches": launches,
@@ -348,6 +386,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c3", choices=sorted(I.CONFIGS))
+    ap.add_argument("--no-projection", dest="no_projection", action="store_true",
+                    help="skip the (untimed-region) pressure-projection measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
