@@ -89,6 +89,24 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz,
                          const int bc[3], double helmholtz_alpha, int implicit_dirs);
 
 /*
+ * tpt_plan_create_ex — the same with the transform type chosen per diagonalised direction ("the transform
+ * type is selected independently in each diagonalized direction.  A uniform direction may use either FFT-based
+ * transforms or numerical eigenbasis transforms evaluated with GEMM, whereas a non-uniform direction uses the latter";
+ * "for a uniform direction, the analytical eigenvalues are stored"; O(N log N) per line).
+ *   transform: HOST, {transform_x, transform_y}.  TPT_TRANSFORM_FFT needs a direction that is diagonalised, has
+ *   2^m cells with 16 <= n <= 2048 and is uniform (every width within rounding of (x_n - x_0)/n; the plan then solves
+ *   the exactly uniform operator of that spacing); for y also nx % 16 == 0.  TPT_EINVAL otherwise.  All three boundary
+ *   types are taken: cosine transforms (Neumann), sine transforms (Dirichlet), the real DFT (periodic), each as one
+ *   complex FFT per pair of lines in shared memory.  tpt_plan_get_eigen returns the analytical eigenvalues of such a
+ *   direction; its basis is not stored (qtilde_host must be NULL).
+ * Combinations: GEMM/GEMM = the paper's GG variant, FFT/GEMM = FG, GEMM/FFT = GF, FFT/FFT = FF.
+ */
+enum { TPT_TRANSFORM_GEMM = 0, TPT_TRANSFORM_FFT = 1 };
+int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz,
+                       const double *xf, const double *yf, const double *zf,
+                       const int bc[3], double helmholtz_alpha, int implicit_dirs, const int transform[2]);
+
+/*
  * tpt_solve — steps 2.1–2.5: five kernels (+ one tiny gauge kernel on a singular
  * plan) enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
  * Asynchronous: returns after enqueueing; no host synchronisation, no allocation.

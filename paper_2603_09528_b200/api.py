@@ -23,11 +23,13 @@ K_FWD_X, K_FWD_Y, K_THOMAS, K_INV_Y, K_INV_X, K_COUNT = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")
 
 # every symbol include/tpt.h declares (tests check the library exports exactly these)
+TRANSFORM_GEMM, TRANSFORM_FFT = 0, 1   # per diagonalised direction: eigenbasis GEMM / fast transform
+
 SYMBOLS = (
     "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
-    "tpt_divergence", "tpt_gradient_correct", "tpt_project",
+    "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -52,6 +54,7 @@ def lib():
         vp, i, d = C.c_void_p, C.c_int, C.c_double
         L.tpt_plan_create.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d]
         L.tpt_plan_create_dirs.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i]
+        L.tpt_plan_create_ex.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i, C.POINTER(i)]
         L.tpt_solve.argtypes = [vp, vp, vp, vp]
         L.tpt_solve_batch.argtypes = [vp, vp, vp, i, vp]
         L.tpt_plan_reserve_batch.argtypes = [vp, i]
@@ -141,6 +144,12 @@ class Plan:
                "tpt_plan_get_eigen")
         return lam, q
 
+    def eigenvalues(self, direction: int):
+        """lambda only (also available for a fast-transform direction, whose basis is not stored)."""
+        lam = np.empty(self.nx if direction == 0 else self.ny)
+        _check(lib().tpt_plan_get_eigen(self._h, direction, lam.ctypes.data_as(_dp), None), "tpt_plan_get_eigen")
+        return lam
+
     def device_bytes(self) -> int:
         b = C.c_size_t()
         _check(lib().tpt_plan_device_bytes(self._h, C.byref(b)), "tpt_plan_device_bytes")
@@ -198,7 +207,8 @@ class Plan:
             pass
 
 
-def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0, dirs: int = DIRS_XYZ) -> Plan:
+def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0, dirs: int = DIRS_XYZ,
+                transform=(TRANSFORM_GEMM, TRANSFORM_GEMM)) -> Plan:
     xa, xp = _faces(xf)
     ya, yp = _faces(yf)
     za, zp = _faces(zf)
@@ -206,8 +216,9 @@ def plan_create(nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0, dirs: 
         raise ValueError("face arrays must have n+1 entries per direction")
     bca = (C.c_int * 3)(*[int(b) for b in bc])
     h = C.c_void_p()
-    _check(lib().tpt_plan_create_dirs(C.byref(h), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha), int(dirs)),
-           "tpt_plan_create_dirs")
+    tra = (C.c_int * 2)(*[int(t) for t in transform])
+    _check(lib().tpt_plan_create_ex(C.byref(h), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha), int(dirs), tra),
+           "tpt_plan_create_ex")
     return Plan(h, nx, ny, nz)
 
 

@@ -15,7 +15,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libtpt.so")
-SOURCES = ["api.cu", "kernels.cu", "gemm_tma.cu", "thomas_onchip.cu", "projection.cu", "plan_host.cpp"]
+SOURCES = ["api.cu", "kernels.cu", "gemm_tma.cu", "thomas_onchip.cu", "projection.cu", "fft.cu", "plan_host.cpp"]
 HEADERS = [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "tmap.hpp"), os.path.join(CSRC, "plan_host.hpp"), os.path.join(ROOT, "include", "tpt.h")]
 
 NVCC_FLAGS = [

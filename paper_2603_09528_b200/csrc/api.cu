@@ -21,6 +21,9 @@ struct tpt_plan {
     int work_fields = 1;          // fields the workspace holds (tpt_plan_reserve_batch)
     int device = 0;
     double shift0 = 0.0;          // 0 (Poisson) or -1/alpha (Helmholtz, A5)
+    int transform[2] = {0, 0};    // per diagonalised direction: TPT_TRANSFORM_GEMM / TPT_TRANSFORM_FFT (uniform directions)
+    double fft_s[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};   // [dir]: forward s0, s1, inverse s0, s1 (fft.cu)
+    double *d_fft[2] = {nullptr, nullptr};   // twiddle tables
     int gemm_variant = 2;
     int thomas_variant = 1;       // 1 = on-chip partitioned kernel where supported, 0 = streaming kernel
     int sms = 0;
@@ -63,6 +66,8 @@ void free_plan(tpt_plan *p) {
     cudaFree(p->d_vec);
     cudaFree(p->d_abc);
     cudaFree(p->d_geo);
+    cudaFree(p->d_fft[0]);
+    cudaFree(p->d_fft[1]);
     cudaFree(p->d_work);
     cudaFree(p->d_stage);
     for (auto &e : p->ev_pool) cudaEventDestroy(e);
@@ -122,7 +127,7 @@ cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st)
 // The mode-space field (between steps 2.2 and 2.4) is kept tile-blocked when the kernels on both sides of it can:
 // the TMA GEMM for the y transforms and the on-chip sweep.  tpt_stage always uses the natural layout.
 bool use_blocked(const tpt_plan *p) {
-    if (p->gemm_variant != 2 || p->thomas_variant != 1 || !(p->dirs & 2)) return false;
+    if (p->gemm_variant != 2 || p->thomas_variant != 1 || !(p->dirs & 2) || p->transform[1] != TPT_TRANSFORM_GEMM) return false;
     if (!tpt::blocked_layout_supported(p->nx, p->ny, p->nz) || !tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) return false;
     return p->ny % 128 == 0 && p->nx % 128 == 0;   // the TMA GEMM's tile shape (M = K = ny, N = nx)
 }
@@ -154,6 +159,15 @@ int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cuda
 int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int k0, int nk,
              bool blocked = false) {
     cudaError_t e = cudaSuccess;
+    const int d = (slot == TPT_K_FWD_X || slot == TPT_K_INV_X) ? 0 : 1;
+    if (p->transform[d] == TPT_TRANSFORM_FFT) {   // uniform direction: fast transform in the natural layout
+        const bool inv = slot == TPT_K_INV_X || slot == TPT_K_INV_Y;
+        const size_t off = (size_t)p->nx * p->ny * k0;
+        tpt::FftArgs a{in + off, out + off, p->d_fft[d], d, inv ? 1 : 0, p->bc[d], p->nx, p->ny, nk,
+                       p->fft_s[d][inv ? 2 : 0], p->fft_s[d][inv ? 3 : 1]};
+        ++*launches;
+        return tpt::launch_fft(a, st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+    }
     switch (slot) {
         case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd, k0, nk), st); ++*launches; break;
         case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv, k0, nk), st); ++*launches; break;
@@ -218,7 +232,24 @@ int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *x
 
 int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
                          const double *zf, const int bc[3], double helmholtz_alpha, int implicit_dirs) {
-    if (!plan_out || !bc) return TPT_EINVAL;
+    const int gemm[2] = {TPT_TRANSFORM_GEMM, TPT_TRANSFORM_GEMM};
+    return tpt_plan_create_ex(plan_out, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha, implicit_dirs, gemm);
+}
+
+// uniform to rounding: every width within a few ulps of the coordinate scale of (x_n - x_0) / n
+static bool direction_uniform(int n, const double *f) {
+    const double d = (f[n] - f[0]) / n;
+    const double tol = 16.0 * 2.220446049250313e-16 * std::fmax(std::fabs(f[0]), std::fabs(f[n]));
+    for (int i = 0; i < n; ++i)
+        if (std::fabs((f[i + 1] - f[i]) - d) > tol) return false;
+    return true;
+}
+
+int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
+                       const double *zf, const int bc[3], double helmholtz_alpha, int implicit_dirs, const int transform[2]) {
+    if (!plan_out || !bc || !transform) return TPT_EINVAL;
+    for (int d = 0; d < 2; ++d)
+        if (transform[d] != TPT_TRANSFORM_GEMM && transform[d] != TPT_TRANSFORM_FFT) return TPT_EINVAL;
     if (implicit_dirs != TPT_DIRS_XYZ && implicit_dirs != TPT_DIRS_YZ && implicit_dirs != TPT_DIRS_Z) return TPT_EINVAL;
     if (implicit_dirs != TPT_DIRS_XYZ && !(helmholtz_alpha > 0.0)) return TPT_EINVAL;   // Eq. 2c carries the full L
     if (!tpt::faces_valid(nx, xf) || !tpt::faces_valid(ny, yf) || !tpt::faces_valid(nz, zf)) return TPT_EINVAL;
@@ -227,6 +258,11 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
     if (bc[2] == TPT_BC_PERIODIC || (bc[0] == TPT_BC_PERIODIC && nx < 3) || (bc[1] == TPT_BC_PERIODIC && ny < 3)) return TPT_EINVAL;
     if (!(helmholtz_alpha >= 0.0) || !std::isfinite(helmholtz_alpha)) return TPT_EINVAL;
     if ((double)nx * ny * nz > 4.0e9) return TPT_EINVAL;
+    // fast transforms: diagonalised, uniform, power-of-two directions only; y tiles need nx % 16 == 0
+    if (transform[0] == TPT_TRANSFORM_FFT &&
+        (!(implicit_dirs & 1) || !tpt::fft_supported(nx) || !direction_uniform(nx, xf))) return TPT_EINVAL;
+    if (transform[1] == TPT_TRANSFORM_FFT &&
+        (!(implicit_dirs & 2) || !tpt::fft_supported(ny) || !direction_uniform(ny, yf) || nx % 16)) return TPT_EINVAL;
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
@@ -248,6 +284,7 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
     p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
     p->alpha = helmholtz_alpha;
     p->dirs = implicit_dirs;
+    p->transform[0] = transform[0]; p->transform[1] = transform[1];
     p->device = dev;
     p->sms = sm_count;
     p->singular = (helmholtz_alpha == 0.0 && bc[0] != TPT_BC_DIRICHLET && bc[1] != TPT_BC_DIRICHLET &&
@@ -277,13 +314,35 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
         // a direction that is not diagonalised contributes no modal shift (Eq. 9 restricted)
         p->lamx.assign(nx, 0.0);
         p->lamy.assign(ny, 0.0);
-        if (use_x && tpt::eigen_decompose(ox, p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
-        if (rc == TPT_OK && use_y) {
-            bool same = (use_x && nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
+        const bool fx = use_x && transform[0] == TPT_TRANSFORM_FFT, fy = use_y && transform[1] == TPT_TRANSFORM_FFT;
+        // uniform direction with a fast transform: analytical eigenvalues, closed-form basis of fft.cu;
+        // the operator is the exactly uniform one with spacing (x_n - x_0) / n
+        auto setup_fft = [&](int d, int n, const double *f, int b, double scale, std::vector<double> &lam) {
+            const long double pi = 3.14159265358979323846264338327950288L;
+            const double dl = (f[n] - f[0]) / n;
+            for (int slot = 0; slot < n; ++slot) {
+                const long double arg = b == TPT_BC_NEUMANN ? pi * slot / (2.0L * n)
+                                      : b == TPT_BC_DIRICHLET ? pi * (slot + 1) / (2.0L * n) : pi * ((slot + 1) / 2) / (long double)n;
+                const long double sn = sinl(arg);
+                lam[slot] = (double)(-4.0L * sn * sn / ((long double)dl * dl));
+            }
+            p->fft_s[d][0] = scale * std::sqrt(dl) * std::sqrt(1.0 / n);
+            p->fft_s[d][1] = scale * std::sqrt(dl) * std::sqrt(2.0 / n);
+            p->fft_s[d][2] = std::sqrt(1.0 / n) / std::sqrt(dl);
+            p->fft_s[d][3] = std::sqrt(2.0 / n) / std::sqrt(dl);
+            std::vector<double> t;
+            tpt::fft_tables(n, t);
+            return upload(&p->d_fft[d], t);
+        };
+        if (fx) rc = setup_fft(0, nx, xf, bc[0], x_scale, p->lamx);
+        if (rc == TPT_OK && fy) rc = setup_fft(1, ny, yf, bc[1], y_scale, p->lamy);
+        if (rc == TPT_OK && use_x && !fx && tpt::eigen_decompose(ox, p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
+        if (rc == TPT_OK && use_y && !fy) {
+            bool same = (use_x && !fx && nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
             if (same) { p->lamy = p->lamx; p->qy = p->qx; }
             else if (tpt::eigen_decompose(oy, p->lamy, p->qy) != 0) rc = TPT_ENUMERIC;
         }
-        if (rc == TPT_OK && use_x) {
+        if (rc == TPT_OK && use_x && !fx) {
             std::vector<double> m((size_t)nx * nx);
             for (int i = 0; i < nx; ++i) {
                 const double s = x_scale * std::sqrt(ox.w[i]);
@@ -298,7 +357,7 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
                 rc = upload(&p->d_xinv, m);
             }
         }
-        if (rc == TPT_OK && use_y) {
+        if (rc == TPT_OK && use_y && !fy) {
             std::vector<double> m((size_t)ny * ny, 0.0);
             if (rc == TPT_OK) {
                 for (int j = 0; j < ny; ++j) {
@@ -362,7 +421,8 @@ int tpt_plan_create_dirs(tpt_plan **plan_out, int nx, int ny, int nz, const doub
         cudaError_t e = cudaMalloc(&p->d_work, p->points() * sizeof(double));
         if (e != cudaSuccess) { cudaGetLastError(); rc = (e == cudaErrorMemoryAllocation) ? TPT_ENOMEM : TPT_ECUDA; }
     }
-    if (rc == TPT_OK && (tpt::gemm_configure() != cudaSuccess || tpt::gemm_tma_configure() != cudaSuccess)) {
+    if (rc == TPT_OK && (tpt::gemm_configure() != cudaSuccess || tpt::gemm_tma_configure() != cudaSuccess ||
+                         tpt::fft_configure() != cudaSuccess)) {
         cudaGetLastError();
         rc = TPT_ECUDA;
     }
@@ -558,7 +618,8 @@ int tpt_plan_get_eigen(const tpt_plan *p, int dir, double *lambda_host, double *
     if (!p || (dir != 0 && dir != 1)) return TPT_EINVAL;
     const std::vector<double> &l = dir == 0 ? p->lamx : p->lamy;
     const std::vector<double> &q = dir == 0 ? p->qx : p->qy;
-    if (q.empty()) return TPT_EINVAL;   // this plan does not diagonalise that direction
+    if (!(p->dirs & (1 << dir))) return TPT_EINVAL;   // this plan does not diagonalise that direction
+    if (qtilde_host && q.empty()) return TPT_EINVAL;   // fast-transform direction: the basis is not stored (closed form, fft.cu)
     if (lambda_host) std::memcpy(lambda_host, l.data(), l.size() * sizeof(double));
     if (qtilde_host) std::memcpy(qtilde_host, q.data(), q.size() * sizeof(double));
     return TPT_OK;

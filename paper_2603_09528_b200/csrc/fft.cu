@@ -1,0 +1,322 @@
+// fft.cu — the eigenbasis transforms of a UNIFORM direction by fast transforms instead of GEMMs ("a
+// uniform direction may use either FFT-based transforms or numerical eigenbasis transforms evaluated with GEMM",
+// :211 "for a uniform direction, the analytical eigenvalues are stored", :221 O(N log N) per line).
+//
+// On a uniform direction the eigenvectors of the 1-D operator (Eq. 3-5 with the boundary rows of DESIGN.md A3) are
+// known in closed form:   Neumann    q_k(i) ~ cos(pi k (2i+1) / 2N)            (DCT-II / DCT-III pair)
+//                         Dirichlet  q_k(i) ~ sin(pi (k+1) (2i+1) / 2N)        (DST-II / DST-III pair)
+//                         periodic   1, cos(2 pi j i / N), sin(2 pi j i / N), (-1)^i   (real DFT)
+// so  p^ = Q~^T D^{1/2} f  and  phi = D^{-1/2} Q~ x^  (Eq. 10, 12) are one complex FFT of length N per PAIR of lines:
+//   * two real lines ride in the real and imaginary parts of one complex sequence and are untangled afterwards
+//     (V1_k = (Z_k + conj Z_{N-k})/2, V2_k = (Z_k - conj Z_{N-k})/2i);
+//   * the cosine transforms use Makhoul's reordering v_n = f_{2n}, v_{N-1-n} = f_{2n+1}, C_k = Re(e^{-i pi k/2N} V_k);
+//     the sine transforms are cosine transforms of (-1)^i f_i read backwards; the inverse transforms run the same
+//     steps in reverse (Hermitian-symmetrised coefficients -> inverse FFT -> real part);
+//   * the FFT is a Stockham autosort FFT in shared memory (radix 8/4/2 passes, ping-pong buffers, one barrier per
+//     pass); a CTA owns several pairs of lines: contiguous rows for the x direction, a 16-column tile (128-byte rows)
+//     for the y direction, so both directions run in the field's native layout without transposes.
+// HBM-bound: 16 B/pt (read once, write once) against 2N flop/pt for the GEMM form.  N = 2^m, 16 <= N <= 2048.
+#include "kernels.cuh"
+
+namespace tpt {
+
+namespace {
+
+struct cplx { double x, y; };
+__device__ __forceinline__ cplx operator+(cplx a, cplx b) { return {a.x + b.x, a.y + b.y}; }
+__device__ __forceinline__ cplx operator-(cplx a, cplx b) { return {a.x - b.x, a.y - b.y}; }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return {fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x)}; }
+__device__ __forceinline__ cplx conj(cplx a) { return {a.x, -a.y}; }
+// multiply by -i (forward) or +i (inverse)
+template <int INV>
+__device__ __forceinline__ cplx mul_mi(cplx a) { return INV ? cplx{-a.y, a.x} : cplx{a.y, -a.x}; }
+
+template <int INV>
+__device__ __forceinline__ void fft2(cplx *v) {
+    const cplx a = v[0], b = v[1];
+    v[0] = a + b;
+    v[1] = a - b;
+}
+template <int INV>
+__device__ __forceinline__ void fft4(cplx &v0, cplx &v1, cplx &v2, cplx &v3) {
+    const cplx t0 = v0 + v2, t1 = v0 - v2, t2 = v1 + v3, t3 = mul_mi<INV>(v1 - v3);
+    v0 = t0 + t2;
+    v1 = t1 + t3;
+    v2 = t0 - t2;
+    v3 = t1 - t3;
+}
+template <int INV>
+__device__ __forceinline__ void fft8(cplx *v) {
+    fft4<INV>(v[0], v[2], v[4], v[6]);      // even inputs -> E_0..E_3 in v[0], v[2], v[4], v[6]
+    fft4<INV>(v[1], v[3], v[5], v[7]);      // odd inputs  -> O_0..O_3 in v[1], v[3], v[5], v[7]
+    constexpr double h = 0.70710678118654752440;
+    const cplx o0 = v[1];
+    const cplx o1 = INV ? cplx{h * (v[3].x - v[3].y), h * (v[3].x + v[3].y)} : cplx{h * (v[3].x + v[3].y), h * (v[3].y - v[3].x)};
+    const cplx o2 = mul_mi<INV>(v[5]);
+    const cplx o3 = INV ? cplx{-h * (v[7].x + v[7].y), h * (v[7].x - v[7].y)} : cplx{h * (v[7].y - v[7].x), -h * (v[7].x + v[7].y)};
+    const cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+    v[0] = e0 + o0; v[4] = e0 - o0;
+    v[1] = e1 + o1; v[5] = e1 - o1;
+    v[2] = e2 + o2; v[6] = e2 - o2;
+    v[3] = e3 + o3; v[7] = e3 - o3;
+}
+
+// shared-memory index with one padding element per 8 (keeps the stride-R stores of the first pass conflict-free)
+__device__ __forceinline__ int pad(int i) { return i + (i >> 3); }
+
+// One Stockham pass of radix R over `pairs` sequences of length N: src -> dst (both padded, `npad` elements apart).
+// Work item j of a sequence: k = j mod Ns;  v_r = src[j + r N/R] W^{r k N/(Ns R)};  radix-R butterfly;
+// dst[(j / Ns) Ns R + k + r Ns] = v_r.   W[t] = e^{-2 pi i t / N} (conjugated for the inverse).
+template <int R, int INV>
+__device__ __forceinline__ void stockham_pass(const cplx *__restrict__ src, cplx *__restrict__ dst, int N, int Ns, int pairs,
+                                              int npad, const double2 *__restrict__ W) {
+    const int per = N / R;
+    const int tstep = N / (Ns * R);
+    for (int item = threadIdx.x; item < pairs * per; item += blockDim.x) {
+        const int pr = item / per, j = item - pr * per;
+        const cplx *s = src + pr * npad;
+        cplx *d = dst + pr * npad;
+        const int k = j & (Ns - 1);
+        cplx v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            v[r] = s[pad(j + r * per)];
+            if (Ns > 1 && r > 0) {
+                const double2 w = __ldg(W + ((r * k * tstep) & (N - 1)));
+                v[r] = cmul(v[r], cplx{w.x, INV ? -w.y : w.y});
+            }
+        }
+        if (R == 2) fft2<INV>(v);
+        else if (R == 4) fft4<INV>(v[0], v[1], v[2], v[3]);
+        else fft8<INV>(v);
+        const int j0 = (j - k) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; ++r) d[pad(j0 + r * Ns)] = v[r];
+    }
+}
+
+struct FftParams {
+    const double *in;
+    double *out;
+    const double2 *W;     // e^{-2 pi i t / N},  t = 0..N-1
+    const double2 *T4;    // e^{-i pi k / 2N},   k = 0..N-1
+    int N;                // transform length (nx for the x direction, ny for y)
+    int bc;               // 0 Neumann, 1 Dirichlet, 2 periodic
+    int nx, ny;           // field row length and rows per plane
+    int lines;            // x: rows to transform (ny * planes); y: unused
+    int radix[4];         // pass radices (0-terminated)
+    double s0, s1;        // forward: output scale of the two special slots / of the others; inverse: input scales
+};
+
+// Input position of sample i in the complex sequence, and its sign (Makhoul reordering; DST: alternate signs).
+__device__ __forceinline__ int seq_index(int bc, int i, int N, double &sign) {
+    sign = 1.0;
+    if (bc == 2) return i;
+    if (bc == 1 && (i & 1)) sign = -1.0;
+    return (i & 1) ? N - 1 - (i >> 1) : (i >> 1);
+}
+// slots whose basis vector has norm^2 N instead of N/2
+__device__ __forceinline__ bool special_slot(int bc, int slot, int N) {
+    return bc == 0 ? slot == 0 : (bc == 1 ? slot == N - 1 : (slot == 0 || slot == N - 1));
+}
+
+// Line / element addressing.  X: a CTA owns `nl` consecutive rows (lines contiguous in memory, N = nx).
+// Y: a CTA owns `nl` neighbouring columns of one z-plane (lines strided by nx, N = ny; rows of nl*8 bytes).
+template <bool YP>
+struct Lines {
+    size_t base;     // element offset of the CTA's first line
+    int nl, valid;   // lines of this CTA, and how many of them exist
+    int nx, N;
+    __device__ Lines(const FftParams &p, int nlines) : nl(nlines), nx(p.nx), N(p.N) {
+        if (YP) {
+            base = (size_t)blockIdx.y * p.nx * p.ny + (size_t)blockIdx.x * nl;
+            valid = nl;
+        } else {
+            const int first = blockIdx.x * nl;
+            base = (size_t)first * p.nx;
+            valid = min(nl, p.lines - first);
+        }
+    }
+    // e-th element of the CTA's chunk in memory order -> (line, index along the line)
+    __device__ void decode(int e, int &l, int &idx) const {
+        if (YP) { idx = e / nl; l = e - idx * nl; }
+        else { l = e / N; idx = e - l * N; }
+    }
+    __device__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + (size_t)l * N + idx; }
+};
+
+template <int INV>
+__device__ __forceinline__ cplx *run_passes(cplx *b0, cplx *b1, const FftParams &p, int pairs, int npad) {
+    cplx *src = b0, *dst = b1;
+    int Ns = 1;
+    for (int q = 0; q < 4 && p.radix[q]; ++q) {
+        const int R = p.radix[q];
+        if (R == 8) stockham_pass<8, INV>(src, dst, p.N, Ns, pairs, npad, p.W);
+        else if (R == 4) stockham_pass<4, INV>(src, dst, p.N, Ns, pairs, npad, p.W);
+        else stockham_pass<2, INV>(src, dst, p.N, Ns, pairs, npad, p.W);
+        __syncthreads();
+        cplx *t = src; src = dst; dst = t;
+        Ns *= R;
+    }
+    return src;
+}
+
+// Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
+template <bool YP>
+__global__ void __launch_bounds__(512)
+fft_forward_kernel(const FftParams p, int nlines) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = p.N, npad = pad(N), pairs = nlines >> 1, bc = p.bc;
+    cplx *b0 = reinterpret_cast<cplx *>(smem_raw), *b1 = b0 + pairs * npad;
+    const Lines<YP> L(p, nlines);
+    const int total = nlines * N;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int l, i;
+        L.decode(e, l, i);
+        double sign;
+        const int n = seq_index(bc, i, N, sign);
+        const double val = l < L.valid ? p.in[L.addr(l, i)] : 0.0;
+        reinterpret_cast<double *>(b0 + (l >> 1) * npad + pad(n))[l & 1] = sign * val;
+    }
+    __syncthreads();
+    const cplx *Z = run_passes<0>(b0, b1, p, pairs, npad);
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int l, slot;
+        L.decode(e, l, slot);
+        if (l >= L.valid) continue;
+        const cplx *z = Z + (l >> 1) * npad;
+        const int k = bc == 2 ? (slot + 1) >> 1 : (bc == 0 ? slot : N - 1 - slot);
+        const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
+        // untangle the two real lines of the pair
+        const cplx V = (l & 1) ? cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)} : cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)};
+        double val;
+        if (bc == 2) val = (slot == 0 || (slot & 1)) ? V.x : -V.y;       // cos rows: Re X_j, sin rows: -Im X_j
+        else {
+            const double2 t = __ldg(p.T4 + k);                            // C_k = Re(e^{-i pi k / 2N} V_k)
+            val = fma(t.x, V.x, -t.y * V.y);
+        }
+        p.out[L.addr(l, slot)] = (special_slot(bc, slot, N) ? p.s0 : p.s1) * val;
+    }
+}
+
+// Inverse: out[line][i] = sum_slot q_slot(i) s(slot) in[line][slot]   (Eq. 12 with Q = D^{-1/2} Q~)
+template <bool YP>
+__global__ void __launch_bounds__(512)
+fft_inverse_kernel(const FftParams p, int nlines) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = p.N, npad = pad(N), pairs = nlines >> 1, bc = p.bc;
+    cplx *b0 = reinterpret_cast<cplx *>(smem_raw), *b1 = b0 + pairs * npad;
+    double *Rr = reinterpret_cast<double *>(b1);                          // staged coefficients [line][slot]
+    const Lines<YP> L(p, nlines);
+    const int total = nlines * N;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int l, slot;
+        L.decode(e, l, slot);
+        Rr[l * N + slot] = l < L.valid ? (special_slot(bc, slot, N) ? p.s0 : p.s1) * p.in[L.addr(l, slot)] : 0.0;
+    }
+    __syncthreads();
+    // Hermitian-symmetrised spectrum B of each line (its inverse DFT is real); the pair rides as Z = B_even + i B_odd
+    for (int item = threadIdx.x; item < pairs * N; item += blockDim.x) {
+        const int pr = item / N, k = item - pr * N;
+        cplx B[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const double *a = Rr + (2 * pr + h) * N;
+            if (bc == 2) {
+                const int j = k <= N / 2 ? k : N - k;                      // B_k = b_k / 2, B_{N-k} = conj(b_k) / 2
+                if (j == 0) B[h] = {a[0], 0.0};
+                else if (j == N / 2) B[h] = {a[N - 1], 0.0};
+                else B[h] = {0.5 * a[2 * j - 1], (k < N / 2 ? -0.5 : 0.5) * a[2 * j]};
+            } else if (k == 0) {
+                B[h] = {bc == 0 ? a[0] : a[N - 1], 0.0};
+            } else {
+                const double ak = bc == 0 ? a[k] : a[N - 1 - k], am = bc == 0 ? a[N - k] : a[k - 1];
+                const double2 t = __ldg(p.T4 + k);                         // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
+                B[h] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak, -am});
+            }
+        }
+        b0[pr * npad + pad(k)] = cplx{B[0].x - B[1].y, B[0].y + B[1].x};
+    }
+    __syncthreads();
+    const cplx *Z = run_passes<1>(b0, b1, p, pairs, npad);
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int l, i;
+        L.decode(e, l, i);
+        if (l >= L.valid) continue;
+        double sign;
+        const int n = seq_index(bc, i, N, sign);
+        const cplx z = Z[(l >> 1) * npad + pad(n)];
+        p.out[L.addr(l, i)] = sign * ((l & 1) ? z.y : z.x);
+    }
+}
+
+}  // namespace
+
+bool fft_supported(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
+
+// Host side of the twiddle tables: W[t] = e^{-2 pi i t / N}, T4[k] = e^{-i pi k / 2N}, interleaved (re, im).
+void fft_tables(int n, std::vector<double> &out) {
+    out.resize((size_t)4 * n);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int t = 0; t < n; ++t) {
+        const long double a = -2.0L * pi * t / n, b = -pi * t / (2.0L * n);
+        out[2 * t] = (double)cosl(a);
+        out[2 * t + 1] = (double)sinl(a);
+        out[2 * n + 2 * t] = (double)cosl(b);
+        out[2 * n + 2 * t + 1] = (double)sinl(b);
+    }
+}
+
+cudaError_t fft_configure() {
+    const int big = 200 * 1024;
+    cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_forward_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    return e;
+}
+
+cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
+    const int N = a.dir == 0 ? a.nx : a.ny;
+    if (!fft_supported(N) || a.planes < 1) return cudaErrorInvalidValue;
+    FftParams p{};
+    p.in = a.in; p.out = a.out;
+    p.W = reinterpret_cast<const double2 *>(a.tables);
+    p.T4 = p.W + N;
+    p.N = N; p.bc = a.bc; p.nx = a.nx; p.ny = a.ny;
+    p.s0 = a.s0; p.s1 = a.s1;
+    int m = 0;
+    while ((1 << m) < N) ++m;
+    int q = 0;
+    const int n8 = m / 3, rem = m % 3;
+    if (rem == 1) {   // 8^(a-1) * 4 * 4
+        for (int r = 0; r < n8 - 1; ++r) p.radix[q++] = 8;
+        p.radix[q++] = 4; p.radix[q++] = 4;
+    } else {
+        for (int r = 0; r < n8; ++r) p.radix[q++] = 8;
+        if (rem == 2) p.radix[q++] = 4;
+    }
+    const int npad = N + (N >> 3);
+    if (a.dir == 0) {
+        const int pairs = N >= 2048 ? 1 : 2048 / N;
+        const int nl = 2 * pairs;
+        p.lines = a.ny * a.planes;
+        const size_t smem = (size_t)2 * pairs * npad * 16;
+        const int grid = (p.lines + nl - 1) / nl;
+        if (a.inverse) fft_inverse_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
+        else fft_forward_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
+    } else {
+        int cols = 8192 / N;
+        if (cols > 16) cols = 16;
+        if (a.nx % cols) return cudaErrorInvalidValue;
+        const size_t smem = (size_t)2 * (cols / 2) * npad * 16;
+        int threads = (cols / 2) * (N / 8);
+        threads = threads > 512 ? 512 : (threads < 64 ? 64 : threads);
+        dim3 grid(a.nx / cols, a.planes);
+        if (a.inverse) fft_inverse_kernel<true><<<grid, threads, smem, stream>>>(p, cols);
+        else fft_forward_kernel<true><<<grid, threads, smem, stream>>>(p, cols);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace tpt

@@ -79,6 +79,22 @@ cudaError_t launch_divergence(const double *u, const double *v, const double *w,
 cudaError_t launch_correct(const double *phi, double *u, double *v, double *w, double *p, const ProjGeom &g, double c,
                            double alpha, int dirs, cudaStream_t stream);
 
+// Fast transforms of a uniform direction (fft.cu): the same Eq. 10 / 12 as the GEMM kernels, in the
+// field's natural layout.  dir 0: along x for ny*planes rows; dir 1: along y for `planes` z-planes (nx % 16 == 0).
+// s0 / s1: scale of the special slots (norm^2 N) / of the others — forward: applied to the outputs, inverse: to the inputs.
+struct FftArgs {
+    const double *in;
+    double *out;
+    const double *tables;   // device copy of fft_tables(N)
+    int dir, inverse, bc;
+    int nx, ny, planes;
+    double s0, s1;
+};
+bool fft_supported(int n);                                   // 2^m, 16 <= n <= 2048
+void fft_tables(int n, std::vector<double> &out);            // 4n doubles: e^{-2 pi i t/n} | e^{-i pi k/2n}
+cudaError_t fft_configure();
+cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream);
+
 // FP64 pipe microbenchmarks (kind 0: DFMA, 1: DMMA).  Returns TFLOP/s.
 cudaError_t run_fp64_peak(int kind, double *tflops);
 

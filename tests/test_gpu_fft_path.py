@@ -1,0 +1,138 @@
+"""GPU parity of the fast-transform path for uniform directions (the paper's FF / FG / GF
+variants) against the CPU oracle, which knows nothing of FFTs: it eigen-solves the same operator with
+Jacobi and applies dense transforms.  phi is unique, so both must agree whatever basis each side uses.
+Grids use power-of-two lengths so that the face coordinates L i / N are exact and "uniform" holds bit for bit."""
+import itertools
+
+import numpy as np
+import pytest
+
+from paper_2603_09528_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+PARITY_TOL = 1e-10
+RESID_TOL = 1e-11
+N_, D_, P_ = I.NEUMANN, I.DIRICHLET, I.PERIODIC
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def tpt(torch):
+    from paper_2603_09528_b200 import api
+
+    api.lib()
+    return api
+
+
+def _rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def _solve(torch, plan, f):
+    d_f = torch.from_numpy(np.ascontiguousarray(f)).cuda()
+    d_o = torch.empty_like(d_f)
+    plan.solve(d_f, d_o)
+    torch.cuda.synchronize()
+    return d_o.cpu().numpy()
+
+
+def _check(tpt, torch, orc, n, L, beta, bc, alpha, transform, seed=3):
+    P = I.Problem("fft", n, L, beta, bc, alpha, seed)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, alpha, transform=transform)
+    phi = _solve(torch, plan, f)
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha).solve(f)
+    assert _rel(phi, ref) <= PARITY_TOL
+    r = orc.residual_norms(xf, yf, zf, bc, alpha, f, phi)
+    assert r["relL2vol"] <= RESID_TOL
+    return plan, phi, (xf, yf, zf)
+
+
+# every boundary type in each fast direction, both directions, several radix factorizations (16 = 4.4, 32 = 8.4,
+# 64 = 8.8, 128 = 8.4.4, 256 = 8.8.4), ragged line counts (ny * nz not a multiple of the lines per CTA)
+@pytest.mark.parametrize("bcx,bcy", list(itertools.product((N_, D_, P_), repeat=2)))
+def test_ff_all_boundary_types(tpt, torch, orc, bcx, bcy):
+    plan, _, _ = _check(tpt, torch, orc, (64, 32, 19), (2.0, 1.0, 1.0), (0.0, 0.0, 2.0), (bcx, bcy, D_), 0.0,
+                        (tpt.TRANSFORM_FFT, tpt.TRANSFORM_FFT))
+    plan.destroy()
+
+
+@pytest.mark.parametrize("n,transform", [
+    ((16, 128, 21), (1, 1)), ((128, 16, 24), (1, 1)), ((256, 64, 17), (1, 1)),
+    ((128, 128, 40), (1, 0)),      # FG: fast x, stretched y through the TMA GEMM and the blocked layout
+    ((128, 128, 40), (0, 1)),      # GF: stretched x, fast y
+    ((40, 64, 33), (0, 1)),        # ragged stretched x (generic GEMM) ... nx % 16 != 0 is rejected below instead
+])
+def test_sizes_and_mixed_variants(tpt, torch, orc, n, transform):
+    if n[0] % 16 and transform[1]:
+        with pytest.raises(tpt.TptError):
+            tpt.plan_create(*n, *I.Problem("x", n, (1.0, 1.0, 1.0), (2.0, 0.0, 2.0), (N_, N_, D_), 0.0, 1).faces(),
+                            (N_, N_, D_), 0.0, transform=transform)
+        return
+    beta = (0.0 if transform[0] else 2.0, 0.0 if transform[1] else 1.5, 2.5)
+    plan, _, _ = _check(tpt, torch, orc, n, (4.0, 1.0, 2.0), beta, (N_, N_, D_), 0.0, transform)
+    plan.destroy()
+
+
+def test_singular_and_helmholtz_and_paper_benchmark_bcs(tpt, torch, orc):
+    # all-Neumann Poisson (gauge), Helmholtz (the -1/alpha scale rides in the forward-x scales), and the paper's
+    # benchmark BCs: periodic x, Neumann y and z with uniform x, y and a stretched z
+    for bc, alpha in (((N_, N_, N_), 0.0), ((N_, D_, N_), 2e-3), ((P_, N_, N_), 0.0)):
+        plan, phi, (xf, yf, zf) = _check(tpt, torch, orc, (128, 64, 36), (8.0, 2.0, 1.0), (0.0, 0.0, 2.0), bc, alpha,
+                                         (tpt.TRANSFORM_FFT, tpt.TRANSFORM_FFT))
+        if alpha == 0.0:
+            assert plan.singular
+            V = np.diff(zf)[:, None, None] * np.diff(yf)[None, :, None] * np.diff(xf)[None, None, :]
+            assert abs((V * phi).sum()) < 1e-13 * np.abs(phi).max() * V.sum()
+        plan.destroy()
+
+
+def test_fast_plan_equals_gemm_plan_and_reports_analytical_eigenvalues(tpt, torch):
+    n, L = (256, 128, 48), (8.0, 2.0, 2.0)
+    P = I.Problem("c4-like", n, L, (0.0, 0.0, 3.0), (N_, D_, D_), 0.0, 9)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    gg = tpt.plan_create(*n, xf, yf, zf, P.bc, 0.0)
+    ff = tpt.plan_create(*n, xf, yf, zf, P.bc, 0.0, transform=(tpt.TRANSFORM_FFT, tpt.TRANSFORM_FFT))
+    assert _rel(_solve(torch, ff, f), _solve(torch, gg, f)) <= 1e-11
+    for d, (m, ln, bc) in enumerate(((n[0], L[0], N_), (n[1], L[1], D_))):
+        lam = ff.eigenvalues(d)
+        k = np.arange(m) + (1 if bc == D_ else 0)
+        closed = -(4.0 / (ln / m) ** 2) * np.sin(np.pi * k / (2 * m)) ** 2          # BJ north_star closed form
+        assert np.abs(lam - closed).max() <= 1e-13 * np.abs(closed).max()
+        assert np.abs(lam - gg.eigenvalues(d)).max() <= 1e-11 * np.abs(closed).max()   # numerical eigen-solve agrees
+        with pytest.raises(tpt.TptError):
+            ff.eigen(d)                                                                # the basis is not stored
+    # stage-wise: forward then inverse of one direction is the identity
+    d_f = torch.from_numpy(f).cuda()
+    a, b = torch.empty_like(d_f), torch.empty_like(d_f)
+    for fwd, inv in ((tpt.K_FWD_X, tpt.K_INV_X), (tpt.K_FWD_Y, tpt.K_INV_Y)):
+        ff.stage(fwd, d_f, a)
+        ff.stage(inv, a, b)
+        torch.cuda.synchronize()
+        assert float((b - d_f).abs().max()) <= 1e-13
+    gg.destroy()
+    ff.destroy()
+
+
+def test_fast_transform_is_refused_where_it_does_not_apply(tpt, torch):
+    n = (64, 64, 16)
+    P = I.Problem("bad", n, (1.0, 1.0, 1.0), (2.0, 0.0, 1.0), (N_, N_, D_), 1e-3, 1)
+    xf, yf, zf = P.faces()
+    with pytest.raises(tpt.TptError):      # x is stretched
+        tpt.plan_create(*n, xf, yf, zf, P.bc, 0.0, transform=(1, 0))
+    with pytest.raises(tpt.TptError):      # y is not diagonalised by a z-only plan
+        tpt.plan_create(*n, xf, yf, zf, P.bc, 1e-3, dirs=tpt.DIRS_Z, transform=(0, 1))
+    Q = I.Problem("bad2", (48, 64, 16), (1.0, 1.0, 1.0), (0.0, 0.0, 1.0), (N_, N_, D_), 0.0, 1)
+    with pytest.raises(tpt.TptError):      # 48 is not a power of two
+        tpt.plan_create(*Q.n, *Q.faces(), Q.bc, 0.0, transform=(1, 0))
+    tpt.plan_create(*Q.n, *Q.faces(), Q.bc, 0.0, transform=(0, 1)).destroy()   # y = 64 uniform: fine
