@@ -66,14 +66,15 @@ __device__ __forceinline__ int pad(int i) { return i + (i >> 3); }
 
 // One Stockham pass of radix R over `pairs` sequences of length N: src -> dst (both padded, `npad` elements apart).
 // Work item j of a sequence: k = j mod Ns;  v_r = src[j + r N/R] W^{r k N/(Ns R)};  radix-R butterfly;
-// dst[(j / Ns) Ns R + k + r Ns] = v_r.   W[t] = e^{-2 pi i t / N} (conjugated for the inverse).
+// dst[(j / Ns) Ns R + k + r Ns] = v_r.   The twiddles of a pass come from its own table Wq[(r-1) Ns + k] =
+// e^{-2 pi i r k / (Ns R)} (conjugated for the inverse): lanes with consecutive k read consecutive entries.
 template <int R, int INV>
-__device__ __forceinline__ void stockham_pass(const cplx *__restrict__ src, cplx *__restrict__ dst, int N, int Ns, int pairs,
-                                              int npad, const double2 *__restrict__ W) {
-    const int per = N / R;
-    const int tstep = N / (Ns * R);
-    for (int item = threadIdx.x; item < pairs * per; item += blockDim.x) {
-        const int pr = item / per, j = item - pr * per;
+__device__ __forceinline__ void stockham_pass(const cplx *__restrict__ src, cplx *__restrict__ dst, int N, int logN, int Ns, int pairs,
+                                              int npad, const double2 *__restrict__ Wq) {
+    constexpr int LOGR = R == 8 ? 3 : (R == 4 ? 2 : 1);
+    const int logper = logN - LOGR, per = 1 << logper;
+    for (int item = threadIdx.x; item < (pairs << logper); item += blockDim.x) {
+        const int pr = item >> logper, j = item & (per - 1);
         const cplx *s = src + pr * npad;
         cplx *d = dst + pr * npad;
         const int k = j & (Ns - 1);
@@ -82,7 +83,7 @@ __device__ __forceinline__ void stockham_pass(const cplx *__restrict__ src, cplx
         for (int r = 0; r < R; ++r) {
             v[r] = s[pad(j + r * per)];
             if (Ns > 1 && r > 0) {
-                const double2 w = __ldg(W + ((r * k * tstep) & (N - 1)));
+                const double2 w = __ldg(Wq + (r - 1) * Ns + k);
                 v[r] = cmul(v[r], cplx{w.x, INV ? -w.y : w.y});
             }
         }
@@ -98,9 +99,9 @@ __device__ __forceinline__ void stockham_pass(const cplx *__restrict__ src, cplx
 struct FftParams {
     const double *in;
     double *out;
-    const double2 *W;     // e^{-2 pi i t / N},  t = 0..N-1
+    const double2 *Wq[4]; // per-pass twiddle tables (see stockham_pass)
     const double2 *T4;    // e^{-i pi k / 2N},   k = 0..N-1
-    int N;                // transform length (nx for the x direction, ny for y)
+    int N, logN;          // transform length (nx for the x direction, ny for y) = 2^logN
     int bc;               // 0 Neumann, 1 Dirichlet, 2 periodic
     int nx, ny;           // field row length and rows per plane
     int lines;            // x: rows to transform (ny * planes); y: unused
@@ -120,14 +121,17 @@ __device__ __forceinline__ bool special_slot(int bc, int slot, int N) {
     return bc == 0 ? slot == 0 : (bc == 1 ? slot == N - 1 : (slot == 0 || slot == N - 1));
 }
 
-// Line / element addressing.  X: a CTA owns `nl` consecutive rows (lines contiguous in memory, N = nx).
-// Y: a CTA owns `nl` neighbouring columns of one z-plane (lines strided by nx, N = ny; rows of nl*8 bytes).
+// Line / element addressing, two neighbouring memory elements (one 16-byte access) per step.
+// X: a CTA owns `nl` consecutive rows (lines contiguous in memory, N = nx); step e2 -> line l, samples i, i+1.
+// Y: a CTA owns `nl` neighbouring columns of one z-plane (lines strided by nx, N = ny; rows of nl*8 bytes);
+//    step e2 -> sample idx of the two lines 2c, 2c+1 — which are exactly the two halves of one complex sequence.
 template <bool YP>
 struct Lines {
     size_t base;     // element offset of the CTA's first line
     int nl, valid;   // lines of this CTA, and how many of them exist
-    int nx, N;
-    __device__ Lines(const FftParams &p, int nlines) : nl(nlines), nx(p.nx), N(p.N) {
+    int nx, N, logN, lognl;
+    __device__ Lines(const FftParams &p, int nlines) : nl(nlines), nx(p.nx), N(p.N), logN(p.logN) {
+        lognl = 31 - __clz(nlines);
         if (YP) {
             base = (size_t)blockIdx.y * p.nx * p.ny + (size_t)blockIdx.x * nl;
             valid = nl;
@@ -137,12 +141,13 @@ struct Lines {
             valid = min(nl, p.lines - first);
         }
     }
-    // e-th element of the CTA's chunk in memory order -> (line, index along the line)
-    __device__ void decode(int e, int &l, int &idx) const {
-        if (YP) { idx = e / nl; l = e - idx * nl; }
-        else { l = e / N; idx = e - l * N; }
+    __device__ int steps() const { return (nl << logN) >> 1; }
+    // X: (line, even sample index);  Y: (first line of the pair, sample index)
+    __device__ void decode(int e2, int &l, int &idx) const {
+        if (YP) { idx = e2 >> (lognl - 1); l = (e2 & ((nl >> 1) - 1)) << 1; }
+        else { l = e2 >> (logN - 1); idx = (e2 & ((N >> 1) - 1)) << 1; }
     }
-    __device__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + (size_t)l * N + idx; }
+    __device__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + ((size_t)l << logN) + idx; }
 };
 
 template <int INV>
@@ -151,9 +156,9 @@ __device__ __forceinline__ cplx *run_passes(cplx *b0, cplx *b1, const FftParams 
     int Ns = 1;
     for (int q = 0; q < 4 && p.radix[q]; ++q) {
         const int R = p.radix[q];
-        if (R == 8) stockham_pass<8, INV>(src, dst, p.N, Ns, pairs, npad, p.W);
-        else if (R == 4) stockham_pass<4, INV>(src, dst, p.N, Ns, pairs, npad, p.W);
-        else stockham_pass<2, INV>(src, dst, p.N, Ns, pairs, npad, p.W);
+        if (R == 8) stockham_pass<8, INV>(src, dst, p.N, p.logN, Ns, pairs, npad, p.Wq[q]);
+        else if (R == 4) stockham_pass<4, INV>(src, dst, p.N, p.logN, Ns, pairs, npad, p.Wq[q]);
+        else stockham_pass<2, INV>(src, dst, p.N, p.logN, Ns, pairs, npad, p.Wq[q]);
         __syncthreads();
         cplx *t = src; src = dst; dst = t;
         Ns *= R;
@@ -161,41 +166,70 @@ __device__ __forceinline__ cplx *run_passes(cplx *b0, cplx *b1, const FftParams 
     return src;
 }
 
+// spectrum slot -> (FFT bin k, which real combination): value of one line at `slot` from its untangled bin V_k
+__device__ __forceinline__ int slot_bin(int bc, int slot, int N) {
+    return bc == 2 ? (slot + 1) >> 1 : (bc == 0 ? slot : N - 1 - slot);
+}
+__device__ __forceinline__ double slot_value(int bc, int slot, cplx V, double2 t4) {
+    if (bc == 2) return (slot == 0 || (slot & 1)) ? V.x : -V.y;          // cos rows: Re X_j, sin rows: -Im X_j
+    return fma(t4.x, V.x, -t4.y * V.y);                                  // C_k = Re(e^{-i pi k / 2N} V_k)
+}
+
 // Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
 template <bool YP>
 __global__ void __launch_bounds__(512)
 fft_forward_kernel(const FftParams p, int nlines) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = p.N, npad = pad(N), pairs = nlines >> 1, bc = p.bc;
+    const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc;   // + 1: neighbouring sequences start in different banks
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw), *b1 = b0 + pairs * npad;
     const Lines<YP> L(p, nlines);
-    const int total = nlines * N;
-    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+    const int steps = L.steps();
+#pragma unroll 4
+    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, i;
-        L.decode(e, l, i);
-        double sign;
-        const int n = seq_index(bc, i, N, sign);
-        const double val = l < L.valid ? p.in[L.addr(l, i)] : 0.0;
-        reinterpret_cast<double *>(b0 + (l >> 1) * npad + pad(n))[l & 1] = sign * val;
+        L.decode(e2, l, i);
+        double2 v = make_double2(0.0, 0.0);
+        if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + L.addr(l, i));
+        if (YP) {            // v = sample i of lines l, l+1: one complex element
+            double sign;
+            const int n = seq_index(bc, i, N, sign);
+            b0[(l >> 1) * npad + pad(n)] = cplx{sign * v.x, sign * v.y};
+        } else {             // v = samples i (even), i+1 of line l
+            double s0, s1;
+            const int n0 = seq_index(bc, i, N, s0), n1 = seq_index(bc, i + 1, N, s1);
+            double *z = reinterpret_cast<double *>(b0 + (l >> 1) * npad) + (l & 1);
+            z[2 * pad(n0)] = s0 * v.x;
+            z[2 * pad(n1)] = s1 * v.y;
+        }
     }
     __syncthreads();
     const cplx *Z = run_passes<0>(b0, b1, p, pairs, npad);
-    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+#pragma unroll 4
+    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, slot;
-        L.decode(e, l, slot);
+        L.decode(e2, l, slot);
         if (l >= L.valid) continue;
         const cplx *z = Z + (l >> 1) * npad;
-        const int k = bc == 2 ? (slot + 1) >> 1 : (bc == 0 ? slot : N - 1 - slot);
-        const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
-        // untangle the two real lines of the pair
-        const cplx V = (l & 1) ? cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)} : cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)};
-        double val;
-        if (bc == 2) val = (slot == 0 || (slot & 1)) ? V.x : -V.y;       // cos rows: Re X_j, sin rows: -Im X_j
-        else {
-            const double2 t = __ldg(p.T4 + k);                            // C_k = Re(e^{-i pi k / 2N} V_k)
-            val = fma(t.x, V.x, -t.y * V.y);
+        double2 o;
+        if (YP) {            // one slot, both lines of the pair
+            const int k = slot_bin(bc, slot, N);
+            const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
+            const double2 t4 = __ldg(p.T4 + k);
+            const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
+            o.x = sc * slot_value(bc, slot, cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, t4);
+            o.y = sc * slot_value(bc, slot, cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)}, t4);
+        } else {             // slots `slot`, `slot + 1` of line l
+            double r[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int sl = slot + h, k = slot_bin(bc, sl, N);
+                const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
+                const cplx V = (l & 1) ? cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)} : cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)};
+                r[h] = (special_slot(bc, sl, N) ? p.s0 : p.s1) * slot_value(bc, sl, V, __ldg(p.T4 + k));
+            }
+            o = make_double2(r[0], r[1]);
         }
-        p.out[L.addr(l, slot)] = (special_slot(bc, slot, N) ? p.s0 : p.s1) * val;
+        *reinterpret_cast<double2 *>(p.out + L.addr(l, slot)) = o;
     }
 }
 
@@ -204,24 +238,36 @@ template <bool YP>
 __global__ void __launch_bounds__(512)
 fft_inverse_kernel(const FftParams p, int nlines) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = p.N, npad = pad(N), pairs = nlines >> 1, bc = p.bc;
+    const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc, logN = p.logN;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw), *b1 = b0 + pairs * npad;
     double *Rr = reinterpret_cast<double *>(b1);                          // staged coefficients [line][slot]
     const Lines<YP> L(p, nlines);
-    const int total = nlines * N;
-    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+    const int steps = L.steps();
+#pragma unroll 4
+    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, slot;
-        L.decode(e, l, slot);
-        Rr[l * N + slot] = l < L.valid ? (special_slot(bc, slot, N) ? p.s0 : p.s1) * p.in[L.addr(l, slot)] : 0.0;
+        L.decode(e2, l, slot);
+        double2 v = make_double2(0.0, 0.0);
+        if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + L.addr(l, slot));
+        if (YP) {            // slot of lines l, l+1
+            const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
+            Rr[(l << logN) + slot] = sc * v.x;
+            Rr[((l + 1) << logN) + slot] = sc * v.y;
+        } else {             // slots slot, slot+1 of line l
+            v.x *= special_slot(bc, slot, N) ? p.s0 : p.s1;
+            v.y *= special_slot(bc, slot + 1, N) ? p.s0 : p.s1;
+            *reinterpret_cast<double2 *>(Rr + (l << logN) + slot) = v;
+        }
     }
     __syncthreads();
     // Hermitian-symmetrised spectrum B of each line (its inverse DFT is real); the pair rides as Z = B_even + i B_odd
-    for (int item = threadIdx.x; item < pairs * N; item += blockDim.x) {
-        const int pr = item / N, k = item - pr * N;
+    for (int item = threadIdx.x; item < (pairs << logN); item += blockDim.x) {
+        const int pr = item >> logN, k = item & (N - 1);
         cplx B[2];
+        const double2 t = __ldg(p.T4 + k);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const double *a = Rr + (2 * pr + h) * N;
+            const double *a = Rr + ((2 * pr + h) << logN);
             if (bc == 2) {
                 const int j = k <= N / 2 ? k : N - k;                      // B_k = b_k / 2, B_{N-k} = conj(b_k) / 2
                 if (j == 0) B[h] = {a[0], 0.0};
@@ -231,39 +277,77 @@ fft_inverse_kernel(const FftParams p, int nlines) {
                 B[h] = {bc == 0 ? a[0] : a[N - 1], 0.0};
             } else {
                 const double ak = bc == 0 ? a[k] : a[N - 1 - k], am = bc == 0 ? a[N - k] : a[k - 1];
-                const double2 t = __ldg(p.T4 + k);                         // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
-                B[h] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak, -am});
+                B[h] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak, -am});   // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
             }
         }
         b0[pr * npad + pad(k)] = cplx{B[0].x - B[1].y, B[0].y + B[1].x};
     }
     __syncthreads();
     const cplx *Z = run_passes<1>(b0, b1, p, pairs, npad);
-    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+#pragma unroll 4
+    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, i;
-        L.decode(e, l, i);
+        L.decode(e2, l, i);
         if (l >= L.valid) continue;
-        double sign;
-        const int n = seq_index(bc, i, N, sign);
-        const cplx z = Z[(l >> 1) * npad + pad(n)];
-        p.out[L.addr(l, i)] = sign * ((l & 1) ? z.y : z.x);
+        const cplx *z = Z + (l >> 1) * npad;
+        double2 o;
+        if (YP) {
+            double sign;
+            const cplx c = z[pad(seq_index(bc, i, N, sign))];
+            o = make_double2(sign * c.x, sign * c.y);
+        } else {
+            double s0, s1;
+            const cplx c0 = z[pad(seq_index(bc, i, N, s0))], c1 = z[pad(seq_index(bc, i + 1, N, s1))];
+            o = (l & 1) ? make_double2(s0 * c0.y, s1 * c1.y) : make_double2(s0 * c0.x, s1 * c1.x);
+        }
+        *reinterpret_cast<double2 *>(p.out + L.addr(l, i)) = o;
     }
 }
 
 }  // namespace
 
+// pass radices of a length-2^m transform: as many 8s as possible, then 4 (or 4, 4); at most 4 passes for n <= 2048
+static int fft_radices(int n, int radix[4]) {
+    int m = 0;
+    while ((1 << m) < n) ++m;
+    int q = 0;
+    const int n8 = m / 3, rem = m % 3;
+    radix[0] = radix[1] = radix[2] = radix[3] = 0;
+    if (rem == 1) {
+        for (int r = 0; r < n8 - 1; ++r) radix[q++] = 8;
+        radix[q++] = 4; radix[q++] = 4;
+    } else {
+        for (int r = 0; r < n8; ++r) radix[q++] = 8;
+        if (rem == 2) radix[q++] = 4;
+    }
+    return m;
+}
+
 bool fft_supported(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
 
-// Host side of the twiddle tables: W[t] = e^{-2 pi i t / N}, T4[k] = e^{-i pi k / 2N}, interleaved (re, im).
+// Host side of the twiddle tables, interleaved (re, im): T4[k] = e^{-i pi k / 2N} (n entries), then for every pass
+// after the first its table e^{-2 pi i r k / (Ns R)}, r = 1..R-1, k = 0..Ns-1.
 void fft_tables(int n, std::vector<double> &out) {
-    out.resize((size_t)4 * n);
     const long double pi = 3.14159265358979323846264338327950288L;
+    out.clear();
     for (int t = 0; t < n; ++t) {
-        const long double a = -2.0L * pi * t / n, b = -pi * t / (2.0L * n);
-        out[2 * t] = (double)cosl(a);
-        out[2 * t + 1] = (double)sinl(a);
-        out[2 * n + 2 * t] = (double)cosl(b);
-        out[2 * n + 2 * t + 1] = (double)sinl(b);
+        const long double b = -pi * t / (2.0L * n);
+        out.push_back((double)cosl(b));
+        out.push_back((double)sinl(b));
+    }
+    int radix[4];
+    fft_radices(n, radix);
+    int Ns = 1;
+    for (int q = 0; q < 4 && radix[q]; ++q) {
+        const int R = radix[q];
+        if (q > 0)
+            for (int r = 1; r < R; ++r)
+                for (int k = 0; k < Ns; ++k) {
+                    const long double a = -2.0L * pi * r * k / ((long double)Ns * R);
+                    out.push_back((double)cosl(a));
+                    out.push_back((double)sinl(a));
+                }
+        Ns *= R;
     }
 }
 
@@ -281,24 +365,22 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
     if (!fft_supported(N) || a.planes < 1) return cudaErrorInvalidValue;
     FftParams p{};
     p.in = a.in; p.out = a.out;
-    p.W = reinterpret_cast<const double2 *>(a.tables);
-    p.T4 = p.W + N;
+    p.T4 = reinterpret_cast<const double2 *>(a.tables);
     p.N = N; p.bc = a.bc; p.nx = a.nx; p.ny = a.ny;
     p.s0 = a.s0; p.s1 = a.s1;
-    int m = 0;
-    while ((1 << m) < N) ++m;
-    int q = 0;
-    const int n8 = m / 3, rem = m % 3;
-    if (rem == 1) {   // 8^(a-1) * 4 * 4
-        for (int r = 0; r < n8 - 1; ++r) p.radix[q++] = 8;
-        p.radix[q++] = 4; p.radix[q++] = 4;
-    } else {
-        for (int r = 0; r < n8; ++r) p.radix[q++] = 8;
-        if (rem == 2) p.radix[q++] = 4;
+    p.logN = fft_radices(N, p.radix);
+    {
+        const double2 *w = p.T4 + N;
+        int Ns = 1;
+        for (int q = 0; q < 4 && p.radix[q]; ++q) {
+            p.Wq[q] = w;
+            if (q > 0) w += (p.radix[q] - 1) * Ns;
+            Ns *= p.radix[q];
+        }
     }
-    const int npad = N + (N >> 3);
+    const int npad = N + (N >> 3) + 1;
     if (a.dir == 0) {
-        const int pairs = N >= 2048 ? 1 : 2048 / N;
+        const int pairs = N >= 2048 ? 1 : 2048 / N;          // 4096 samples per CTA, 256 threads, three CTAs per SM
         const int nl = 2 * pairs;
         p.lines = a.ny * a.planes;
         const size_t smem = (size_t)2 * pairs * npad * 16;
@@ -306,8 +388,9 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
         if (a.inverse) fft_inverse_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
         else fft_forward_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
     } else {
-        int cols = 8192 / N;
+        int cols = 4096 / N;                                  // 4096 samples per CTA: 8-column tiles at N = 512
         if (cols > 16) cols = 16;
+        if (cols < 2) cols = 2;
         if (a.nx % cols) return cudaErrorInvalidValue;
         const size_t smem = (size_t)2 * (cols / 2) * npad * 16;
         int threads = (cols / 2) * (N / 8);

@@ -91,7 +91,7 @@ struct FftArgs {
     double s0, s1;
 };
 bool fft_supported(int n);                                   // 2^m, 16 <= n <= 2048
-void fft_tables(int n, std::vector<double> &out);            // 4n doubles: e^{-2 pi i t/n} | e^{-i pi k/2n}
+void fft_tables(int n, std::vector<double> &out);            // e^{-i pi k/2n} (n entries) | per-pass twiddle tables
 cudaError_t fft_configure();
 cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream);
 
