@@ -37,6 +37,9 @@ UNIT = "Gpts/s"
 # DFMA microbenchmarks of the library are reported next to it.
 SM_COUNT, FP64_FMA_PER_CLK_SM = 148, 64
 ORACLE_SAMPLE_NZ = 64
+# transform type per diagonalised direction (x, y): the paper's GG / FG / GF / FF variants; FFT needs a
+# uniform power-of-two direction.  BASELINE.json's metric is quoted on GG.
+TRANSFORMS = {"gg": (0, 0), "fg": (1, 0), "gf": (0, 1), "ff": (1, 1)}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (gemm_tma_kernel), from the one
 # `ncu --set full` capture summarised in profiles/r1c_blocked_layout_projection.md (config c3; bytes).  Other configs: null.
 NCU_TRAFFIC_BYTES = {"c3": 1.077565e9 + 1.031300e9}
@@ -217,7 +220,7 @@ def run_gpu(args):
         xf, yf, zf = P.faces()
         key = (P.n, P.bc, P.alpha, P.beta, P.length)
         if key not in plan_cache:
-            plan_cache[key] = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
+            plan_cache[key] = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=TRANSFORMS[args.transform])
         plans.append(plan_cache[key])
         f = replica_problem(P, rank).rhs()
         h_rhs.append(f)
@@ -334,14 +337,16 @@ def run_gpu(args):
         kernels = {}
         for slot, name in enumerate(api.KERNEL_NAMES):
             entry = {"ms": ms0[slot]}
-            if name == "thomas":
+            fast = (name.endswith("_x") and TRANSFORMS[args.transform][0]) or (name.endswith("_y") and TRANSFORMS[args.transform][1])
+            if name == "thomas" or fast:
                 gbs = 16.0 * pts / (ms0[slot] * 1e-3) / 1e9
                 entry.update({"bound": "hbm", "achieved_gbs_16B_per_pt": gbs, "frac_of_hbm_peak": gbs / peaks["hbm_gbs"]})
             else:
                 tf = flops[name] / (ms0[slot] * 1e-3) / 1e12
                 entry.update({"bound": "tensor", "achieved_tflops": tf, "frac_of_fp64_peak": tf / fp64_peak})
             kernels[name] = entry
-        dom = max(("fwd_x", "fwd_y", "inv_y", "inv_x"), key=lambda n: kernels[n]["ms"])
+        gemm_slots = [n for n in ("fwd_x", "fwd_y", "inv_y", "inv_x") if kernels[n]["bound"] == "tensor"]
+        dom = max(gemm_slots or ("fwd_x", "fwd_y", "inv_y", "inv_x"), key=lambda n: kernels[n]["ms"])
         traffic = NCU_TRAFFIC_BYTES.get(args.config)
         roofline = {
             "kernel": f"gemm_tma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
@@ -353,13 +358,21 @@ def run_gpu(args):
             "algorithmic_flops_per_launch": flops[dom], "algorithmic_dram_bytes_per_launch": 16.0 * pts,
             "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1c_*.md)",
         }
+        if not gemm_slots:   # FF: no GEMM left — the dominant kernel is the slowest fast transform, HBM-bound at 16 B/pt
+            roofline = {
+                "kernel": f"fft kernel ({dom})", "bound": "hbm", "achieved": kernels[dom]["achieved_gbs_16B_per_pt"],
+                "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": kernels[dom]["frac_of_hbm_peak"], "traffic": None,
+                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})",
+                "algorithmic_dram_bytes_per_launch": 16.0 * pts,
+            }
         cpu = _oracle_sample(probs, 1, 1)
         n20 = per_step[: min(20, len(per_step))]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": _config_json(args.config, probs, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
+            "config": _config_json(args.config, probs, {"parallelism": "replicas only" if world > 1 else "single GPU",
+                                                          "transform_xy": args.transform}),
             "clocks": clocks,
             "projection": projection,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * pts_step, "d2h_bytes_per_step": 8 * pts_step,
@@ -386,6 +399,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c3", choices=sorted(I.CONFIGS))
+    ap.add_argument("--transform", default="gg", choices=sorted(TRANSFORMS),
+                    help="transform type in x, y: g = eigenbasis GEMM (BASELINE metric), f = fast transform (uniform directions)")
     ap.add_argument("--no-projection", dest="no_projection", action="store_true",
                     help="skip the (untimed-region) pressure-projection measurement")
     args = ap.parse_args()

@@ -205,7 +205,7 @@ int tpt_plan_get_kernel_times(tpt_plan *plan, float *ms_host, int *launches_out,
 int tpt_plan_set_gemm_variant(tpt_plan *plan, int variant);
 
 /* Select the z-sweep kernel: 1 = on-chip partitioned Thomas kernel (column tiles resident in shared memory,
- * 16 B/pt of HBM traffic; used where nx*ny % 16 == 0 and nz <= 768, default), 0 = streaming one-thread-per-column
+ * 16 B/pt of HBM traffic; used where nx*ny % 16 == 0 and nz <= 1056, default), 0 = streaming one-thread-per-column
  * kernel that spills c' to the plan workspace (any shape).  Both solve step 2.3 exactly. */
 int tpt_plan_set_thomas_variant(tpt_plan *plan, int variant);
 

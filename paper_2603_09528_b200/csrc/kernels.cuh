@@ -54,7 +54,7 @@ cudaError_t launch_thomas(double *x, double *cprime, const double *az, const dou
 // Reads the right-hand sides from `in` and writes the solution to `x` (in == x: in place).
 // tab: device copy of the two tables thomas_onchip_tables() builds (8 * (nz + THOMAS_TABLE_PAD) doubles).
 // sms = SM count.
-constexpr int THOMAS_TABLE_PAD = 128;   // >= the rows by which S*M can exceed nz in any launch shape
+constexpr int THOMAS_TABLE_PAD = 160;   // >= the rows by which S*M can exceed nz in any launch shape
 bool thomas_onchip_supported(int nx, int ny, int nz);
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out);
 cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,

@@ -273,7 +273,7 @@ cudaError_t launch_m(const double *in, double *x, const double *tab, const doubl
 }  // namespace
 
 bool thomas_onchip_supported(int nx, int ny, int nz) {
-    return ((size_t)nx * ny) % 16 == 0 && nz >= 2 && nz <= 768;
+    return ((size_t)nx * ny) % 16 == 0 && nz >= 2 && nz <= 1056;
 }
 
 cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
@@ -290,7 +290,9 @@ cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab,
     // rounding — on a natural-layout field (tpt_solve_host, whose results equal tpt_solve's bit for bit).
     if ((blocked || blocked_shape) && nz <= 544) return TPT_GO(17, 8, 256, 2);
     if (nz <= 512) return TPT_GO(16, 16, 512, 1);
-    return TPT_GO(32, 16, 384, 1);
+    if (nz <= 768) return TPT_GO(32, 16, 384, 1);
+    // up to 1056 rows: 8-column tiles of 33-row segments (three 66 KB buffers), one CTA per SM
+    return TPT_GO(33, 8, 256, 1);
 #undef TPT_GO
 }
 
