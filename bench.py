@@ -61,7 +61,8 @@ def _workload(name: str):
 def _config_json(name: str, probs, extra=None):
     P = probs[0]
     cfg = {
-        "workload": f"BASELINE.json configs[{int(name[1]) - 1}] ({name}): " + ", ".join(p.name for p in probs),
+        "workload": (f"BASELINE.json configs[{int(name[1]) - 1}] ({name}): " if name[0] == "c" else
+                     f"the paper's single-GPU benchmark case, PAPER.md:294 ({name}): ") + ", ".join(p.name for p in probs),
         "grid": list(P.n), "tanh_beta": list(P.beta), "bc": ["N" if b == 0 else "D" for b in P.bc],
         "solves_per_step": len(probs), "helmholtz_alpha": [p.alpha for p in probs],
         "points_per_step": sum(p.points for p in probs),
@@ -348,16 +349,17 @@ def run_gpu(args):
         gemm_slots = [n for n in ("fwd_x", "fwd_y", "inv_y", "inv_x") if kernels[n]["bound"] == "tensor"]
         dom = max(gemm_slots or ("fwd_x", "fwd_y", "inv_y", "inv_x"), key=lambda n: kernels[n]["ms"])
         traffic = NCU_TRAFFIC_BYTES.get(args.config)
-        roofline = {
-            "kernel": f"gemm_tma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
-            "peak": fp64_peak, "unit": "TFLOP/s", "frac": kernels[dom]["achieved_tflops"] / fp64_peak, "traffic": traffic,
-            "peak_source": f"148 SMs x 64 FP64 FMA/clk x 2 x {sm_max:.0f} MHz ({peak_kind} sm_max_mhz); FP64 is absent from "
-                           "MEASURED_PEAKS.json",
-            "peak_measured_dmma_loop": dmma_meas, "peak_measured_dfma_loop": dfma_meas,
-            "frac_of_measured_dmma_loop": kernels[dom]["achieved_tflops"] / dmma_meas,
-            "algorithmic_flops_per_launch": flops[dom], "algorithmic_dram_bytes_per_launch": 16.0 * pts,
-            "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1c_*.md)",
-        }
+        if gemm_slots:
+            roofline = {
+                "kernel": f"gemm_tma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
+                "peak": fp64_peak, "unit": "TFLOP/s", "frac": kernels[dom]["achieved_tflops"] / fp64_peak, "traffic": traffic,
+                "peak_source": f"148 SMs x 64 FP64 FMA/clk x 2 x {sm_max:.0f} MHz ({peak_kind} sm_max_mhz); FP64 is absent from "
+                               "MEASURED_PEAKS.json",
+                "peak_measured_dmma_loop": dmma_meas, "peak_measured_dfma_loop": dfma_meas,
+                "frac_of_measured_dmma_loop": kernels[dom]["achieved_tflops"] / dmma_meas,
+                "algorithmic_flops_per_launch": flops[dom], "algorithmic_dram_bytes_per_launch": 16.0 * pts,
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1c_*.md)",
+            }
         if not gemm_slots:   # FF: no GEMM left — the dominant kernel is the slowest fast transform, HBM-bound at 16 B/pt
             roofline = {
                 "kernel": f"fft kernel ({dom})", "bound": "hbm", "achieved": kernels[dom]["achieved_gbs_16B_per_pt"],

@@ -127,4 +127,7 @@ CONFIGS = {
            for s in (4, 5, 6)]
           + [Problem("c5-poisson-768-neumann", (768, 768, 768), (1.0, 1.0, 1.0), (3.0, 3.0, 3.0), (N_, N_, N_), 0.0, 7)],
     "p1024": [PAPER_GG],
+    # the same case with y uniform as well, so that all four transform variants FF / FG / GF / GG
+    # can be timed on one grid (bench.py --transform)
+    "p1024u": [dataclasses.replace(PAPER_GG, name="paper-1024-periodic-x-uniform-xy", beta=(0.0, 0.0, 2.0))],
 }
