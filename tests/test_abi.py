@@ -61,7 +61,18 @@ def test_argument_validation_needs_no_gpu(tpt):
     assert e.value.status == -1
     with pytest.raises(ValueError):
         tpt.plan_create(8, 8, 8, good[:-1], good, good, (0, 0, 1), 0.0)
+    # fast transforms: only for diagonalised, uniform, power-of-two directions
+    u16, s16 = np.linspace(0, 1, 17), np.linspace(0, 1, 17) ** 2
+    for args, kw in (((16, 16, 16, s16, u16, u16, (0, 0, 1), 0.0), dict(transform=(1, 0))),        # x stretched
+                     ((8, 16, 16, good, u16, u16, (0, 0, 1), 0.0), dict(transform=(1, 0))),        # 8 cells: below 16
+                     ((16, 16, 16, u16, u16, u16, (0, 0, 1), 1e-3), dict(transform=(0, 1), dirs=tpt.DIRS_Z)),
+                     ((16, 16, 16, u16, u16, u16, (0, 0, 1), 0.0), dict(transform=(0, 7)))):
+        with pytest.raises(tpt.TptError) as e:
+            tpt.plan_create(*args, **kw)
+        assert e.value.status == -1
     L = tpt.lib()
+    assert L.tpt_project(None, None, None, None, 1.0, None, None, 0.0, 7, None) == -1
+    assert L.tpt_divergence(None, None, None, None, 1.0, None, None) == -1
     assert L.tpt_solve(None, None, None, None) == -1
     assert L.tpt_plan_destroy(None) == 0
     assert L.tpt_plan_is_singular(None) == -1

@@ -136,3 +136,23 @@ def test_fast_transform_is_refused_where_it_does_not_apply(tpt, torch):
     with pytest.raises(tpt.TptError):      # 48 is not a power of two
         tpt.plan_create(*Q.n, *Q.faces(), Q.bc, 0.0, transform=(1, 0))
     tpt.plan_create(*Q.n, *Q.faces(), Q.bc, 0.0, transform=(0, 1)).destroy()   # y = 64 uniform: fine
+
+
+def test_c4_full_size_grids_fg_parity_and_residual(tpt, torch, orc):
+    # BASELINE.json configs[3]: x is uniform with 1024 cells — here on the fast path (FG) instead of the GEMM
+    P = I.CONFIGS["c4"][0].thin_z(16)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=(tpt.TRANSFORM_FFT, tpt.TRANSFORM_GEMM))
+    phi = _solve(torch, plan, f)
+    plan.destroy()
+    assert _rel(phi, orc.OraclePlan(xf, yf, zf, P.bc, P.alpha).solve(f)) <= PARITY_TOL
+    # full size: flux-form residual at round-off
+    P = I.CONFIGS["c4"][0]
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=(tpt.TRANSFORM_FFT, tpt.TRANSFORM_GEMM))
+    phi = _solve(torch, plan, f)
+    plan.destroy()
+    r = orc.residual_norms(xf, yf, zf, P.bc, P.alpha, f, phi)
+    assert r["rel2"] <= RESID_TOL and r["relL2vol"] <= RESID_TOL
