@@ -127,9 +127,13 @@ cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st)
 // The mode-space field (between steps 2.2 and 2.4) is kept tile-blocked when the kernels on both sides of it can:
 // the TMA GEMM for the y transforms and the on-chip sweep.  tpt_stage always uses the natural layout.
 bool use_blocked(const tpt_plan *p) {
-    if (p->gemm_variant != 2 || p->thomas_variant != 1 || !(p->dirs & 2) || p->transform[1] != TPT_TRANSFORM_GEMM) return false;
+    if (p->thomas_variant != 1 || !(p->dirs & 2)) return false;
     if (!tpt::blocked_layout_supported(p->nx, p->ny, p->nz) || !tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) return false;
-    return p->ny % 128 == 0 && p->nx % 128 == 0;   // the TMA GEMM's tile shape (M = K = ny, N = nx)
+    // the fast y transform addresses either layout, but pays for the scattered 64-byte pieces: measured, the blocked
+    // layout wins only where the natural-layout sweep is weak (long columns: 43.8 -> 41.6 ms per 1024^3 FF solve,
+    // but 3.94 -> 4.02 ms at 512^3)
+    if (p->transform[1] == TPT_TRANSFORM_FFT) return p->nz > 544;
+    return p->gemm_variant == 2 && p->ny % 128 == 0 && p->nx % 128 == 0;   // the TMA GEMM's tile shape (M = K = ny, N = nx)
 }
 
 // Step 2.3 on one field: in -> out (in == out allowed); `scratch` is a free field (used by the streaming kernel only).
@@ -160,11 +164,18 @@ int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t 
              bool blocked = false) {
     cudaError_t e = cudaSuccess;
     const int d = (slot == TPT_K_FWD_X || slot == TPT_K_INV_X) ? 0 : 1;
-    if (p->transform[d] == TPT_TRANSFORM_FFT) {   // uniform direction: fast transform in the natural layout
+    if (p->transform[d] == TPT_TRANSFORM_FFT) {   // uniform direction: fast transform, no transposes
         const bool inv = slot == TPT_K_INV_X || slot == TPT_K_INV_Y;
         const size_t off = (size_t)p->nx * p->ny * k0;
-        tpt::FftArgs a{in + off, out + off, p->d_fft[d], d, inv ? 1 : 0, p->bc[d], p->nx, p->ny, nk,
-                       p->fft_s[d][inv ? 2 : 0], p->fft_s[d][inv ? 3 : 1]};
+        const bool blk = blocked && d == 1;          // mode-space side of a y transform: tile-blocked (offset by k0 inside)
+        tpt::FftArgs a{};
+        a.in = (blk && inv) ? in : in + off;
+        a.out = (blk && !inv) ? out : out + off;
+        a.tables = p->d_fft[d];
+        a.dir = d; a.inverse = inv ? 1 : 0; a.bc = p->bc[d];
+        a.nx = p->nx; a.ny = p->ny; a.planes = nk;
+        a.s0 = p->fft_s[d][inv ? 2 : 0]; a.s1 = p->fft_s[d][inv ? 3 : 1];
+        a.blocked = blk ? 1 : 0; a.nz = p->nz; a.k0 = k0;
         ++*launches;
         return tpt::launch_fft(a, st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
     }

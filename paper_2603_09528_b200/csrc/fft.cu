@@ -64,36 +64,52 @@ __device__ __forceinline__ void fft8(cplx *v) {
 // shared-memory index with one padding element per 8 (keeps the stride-R stores of the first pass conflict-free)
 __device__ __forceinline__ int pad(int i) { return i + (i >> 3); }
 
-// One Stockham pass of radix R over `pairs` sequences of length N: src -> dst (both padded, `npad` elements apart).
-// Work item j of a sequence: k = j mod Ns;  v_r = src[j + r N/R] W^{r k N/(Ns R)};  radix-R butterfly;
-// dst[(j / Ns) Ns R + k + r Ns] = v_r.   The twiddles of a pass come from its own table Wq[(r-1) Ns + k] =
+// One Stockham pass of radix R over `pairs` sequences of length N, in place (sequences `npad` elements apart).
+// Work item j of a sequence: k = j mod Ns;  v_r = buf[j + r N/R] W^{r k N/(Ns R)};  radix-R butterfly;
+// buf[(j / Ns) Ns R + k + r Ns] = v_r.   A thread keeps all its items (at most ITEMS) in registers across the barrier
+// that separates the reads of a pass from its writes, so one buffer suffices (half the shared memory of a ping-pong
+// scheme: more CTAs per SM).  The twiddles of a pass come from its own table Wq[(r-1) Ns + k] =
 // e^{-2 pi i r k / (Ns R)} (conjugated for the inverse): lanes with consecutive k read consecutive entries.
 template <int R, int INV>
-__device__ __forceinline__ void stockham_pass(const cplx *__restrict__ src, cplx *__restrict__ dst, int N, int logN, int Ns, int pairs,
-                                              int npad, const double2 *__restrict__ Wq) {
+__device__ __forceinline__ void stockham_pass(cplx *__restrict__ buf, int logN, int Ns, int pairs, int npad,
+                                              const double2 *__restrict__ Wq) {
     constexpr int LOGR = R == 8 ? 3 : (R == 4 ? 2 : 1);
+    constexpr int ITEMS = 8 / R;                 // 4096 samples and >= 256 threads per CTA: one radix-8 item, two radix-4
     const int logper = logN - LOGR, per = 1 << logper;
-    for (int item = threadIdx.x; item < (pairs << logper); item += blockDim.x) {
+    const int total = pairs << logper;
+    cplx v[ITEMS][R];
+#pragma unroll
+    for (int it = 0; it < ITEMS; ++it) {
+        const int item = threadIdx.x + it * blockDim.x;
+        if (item >= total) continue;
         const int pr = item >> logper, j = item & (per - 1);
-        const cplx *s = src + pr * npad;
-        cplx *d = dst + pr * npad;
+        const cplx *s = buf + pr * npad;
         const int k = j & (Ns - 1);
-        cplx v[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            v[r] = s[pad(j + r * per)];
+            v[it][r] = s[pad(j + r * per)];
             if (Ns > 1 && r > 0) {
                 const double2 w = __ldg(Wq + (r - 1) * Ns + k);
-                v[r] = cmul(v[r], cplx{w.x, INV ? -w.y : w.y});
+                v[it][r] = cmul(v[it][r], cplx{w.x, INV ? -w.y : w.y});
             }
         }
-        if (R == 2) fft2<INV>(v);
-        else if (R == 4) fft4<INV>(v[0], v[1], v[2], v[3]);
-        else fft8<INV>(v);
+        if (R == 2) fft2<INV>(v[it]);
+        else if (R == 4) fft4<INV>(v[it][0], v[it][1], v[it][2], v[it][3]);
+        else fft8<INV>(v[it]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < ITEMS; ++it) {
+        const int item = threadIdx.x + it * blockDim.x;
+        if (item >= total) continue;
+        const int pr = item >> logper, j = item & (per - 1);
+        cplx *d = buf + pr * npad;
+        const int k = j & (Ns - 1);
         const int j0 = (j - k) * R + k;
 #pragma unroll
-        for (int r = 0; r < R; ++r) d[pad(j0 + r * Ns)] = v[r];
+        for (int r = 0; r < R; ++r) d[pad(j0 + r * Ns)] = v[it][r];
     }
+    __syncthreads();
 }
 
 struct FftParams {
@@ -105,6 +121,8 @@ struct FftParams {
     int bc;               // 0 Neumann, 1 Dirichlet, 2 periodic
     int nx, ny;           // field row length and rows per plane
     int lines;            // x: rows to transform (ny * planes); y: unused
+    int blk_in, blk_out;  // y only: that side is the tile-blocked mode-space layout (kernels.cuh); needs nz, k0
+    int nz, k0;           // field depth and the z index of the launch's first plane
     int radix[4];         // pass radices (0-terminated)
     double s0, s1;        // forward: output scale of the two special slots / of the others; inverse: input scales
 };
@@ -148,22 +166,23 @@ struct Lines {
         else { l = e2 >> (logN - 1); idx = (e2 & ((N >> 1) - 1)) << 1; }
     }
     __device__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + ((size_t)l << logN) + idx; }
+    // y only: mode `idx` of column line l in the tile-blocked layout ((m (nx/16) + i/16) nz + k) 16 + i mod 16
+    __device__ size_t addr_blocked(const FftParams &p, int l, int idx) const {
+        const int i = blockIdx.x * nl + l, k = p.k0 + blockIdx.y;
+        return (((size_t)idx * (p.nx >> 4) + (i >> 4)) * p.nz + k) * 16 + (i & 15);
+    }
 };
 
 template <int INV>
-__device__ __forceinline__ cplx *run_passes(cplx *b0, cplx *b1, const FftParams &p, int pairs, int npad) {
-    cplx *src = b0, *dst = b1;
+__device__ __forceinline__ void run_passes(cplx *buf, const FftParams &p, int pairs, int npad) {
     int Ns = 1;
     for (int q = 0; q < 4 && p.radix[q]; ++q) {
         const int R = p.radix[q];
-        if (R == 8) stockham_pass<8, INV>(src, dst, p.N, p.logN, Ns, pairs, npad, p.Wq[q]);
-        else if (R == 4) stockham_pass<4, INV>(src, dst, p.N, p.logN, Ns, pairs, npad, p.Wq[q]);
-        else stockham_pass<2, INV>(src, dst, p.N, p.logN, Ns, pairs, npad, p.Wq[q]);
-        __syncthreads();
-        cplx *t = src; src = dst; dst = t;
+        if (R == 8) stockham_pass<8, INV>(buf, p.logN, Ns, pairs, npad, p.Wq[q]);
+        else if (R == 4) stockham_pass<4, INV>(buf, p.logN, Ns, pairs, npad, p.Wq[q]);
+        else stockham_pass<2, INV>(buf, p.logN, Ns, pairs, npad, p.Wq[q]);
         Ns *= R;
     }
-    return src;
 }
 
 // spectrum slot -> (FFT bin k, which real combination): value of one line at `slot` from its untangled bin V_k
@@ -177,11 +196,11 @@ __device__ __forceinline__ double slot_value(int bc, int slot, cplx V, double2 t
 
 // Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
 template <bool YP>
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(256, 4)
 fft_forward_kernel(const FftParams p, int nlines) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc;   // + 1: neighbouring sequences start in different banks
-    cplx *b0 = reinterpret_cast<cplx *>(smem_raw), *b1 = b0 + pairs * npad;
+    cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
     const Lines<YP> L(p, nlines);
     const int steps = L.steps();
 #pragma unroll 4
@@ -203,7 +222,8 @@ fft_forward_kernel(const FftParams p, int nlines) {
         }
     }
     __syncthreads();
-    const cplx *Z = run_passes<0>(b0, b1, p, pairs, npad);
+    run_passes<0>(b0, p, pairs, npad);
+    const cplx *Z = b0;
 #pragma unroll 4
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, slot;
@@ -229,18 +249,18 @@ fft_forward_kernel(const FftParams p, int nlines) {
             }
             o = make_double2(r[0], r[1]);
         }
-        *reinterpret_cast<double2 *>(p.out + L.addr(l, slot)) = o;
+        *reinterpret_cast<double2 *>(p.out + ((YP && p.blk_out) ? L.addr_blocked(p, l, slot) : L.addr(l, slot))) = o;
     }
 }
 
 // Inverse: out[line][i] = sum_slot q_slot(i) s(slot) in[line][slot]   (Eq. 12 with Q = D^{-1/2} Q~)
 template <bool YP>
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(256, 4)
 fft_inverse_kernel(const FftParams p, int nlines) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc, logN = p.logN;
-    cplx *b0 = reinterpret_cast<cplx *>(smem_raw), *b1 = b0 + pairs * npad;
-    double *Rr = reinterpret_cast<double *>(b1);                          // staged coefficients [line][slot]
+    cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
+    double *Rr = reinterpret_cast<double *>(b0);                          // staged coefficients [line][slot], overwritten by Z
     const Lines<YP> L(p, nlines);
     const int steps = L.steps();
 #pragma unroll 4
@@ -248,7 +268,7 @@ fft_inverse_kernel(const FftParams p, int nlines) {
         int l, slot;
         L.decode(e2, l, slot);
         double2 v = make_double2(0.0, 0.0);
-        if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + L.addr(l, slot));
+        if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + ((YP && p.blk_in) ? L.addr_blocked(p, l, slot) : L.addr(l, slot)));
         if (YP) {            // slot of lines l, l+1
             const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
             Rr[(l << logN) + slot] = sc * v.x;
@@ -260,8 +280,14 @@ fft_inverse_kernel(const FftParams p, int nlines) {
         }
     }
     __syncthreads();
-    // Hermitian-symmetrised spectrum B of each line (its inverse DFT is real); the pair rides as Z = B_even + i B_odd
-    for (int item = threadIdx.x; item < (pairs << logN); item += blockDim.x) {
+    // Hermitian-symmetrised spectrum B of each line (its inverse DFT is real); the pair rides as Z = B_even + i B_odd.
+    // Built in registers (at most ZITEMS elements per thread), then written over the staged coefficients.
+    constexpr int ZITEMS = 8;
+    cplx zreg[ZITEMS];
+#pragma unroll
+    for (int it = 0; it < ZITEMS; ++it) {
+        const int item = threadIdx.x + it * blockDim.x;
+        if (item >= (pairs << logN)) continue;
         const int pr = item >> logN, k = item & (N - 1);
         cplx B[2];
         const double2 t = __ldg(p.T4 + k);
@@ -280,10 +306,18 @@ fft_inverse_kernel(const FftParams p, int nlines) {
                 B[h] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak, -am});   // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
             }
         }
-        b0[pr * npad + pad(k)] = cplx{B[0].x - B[1].y, B[0].y + B[1].x};
+        zreg[it] = cplx{B[0].x - B[1].y, B[0].y + B[1].x};
     }
     __syncthreads();
-    const cplx *Z = run_passes<1>(b0, b1, p, pairs, npad);
+#pragma unroll
+    for (int it = 0; it < ZITEMS; ++it) {
+        const int item = threadIdx.x + it * blockDim.x;
+        if (item >= (pairs << logN)) continue;
+        b0[(item >> logN) * npad + pad(item & (N - 1))] = zreg[it];
+    }
+    __syncthreads();
+    run_passes<1>(b0, p, pairs, npad);
+    const cplx *Z = b0;
 #pragma unroll 4
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, i;
@@ -368,6 +402,8 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
     p.T4 = reinterpret_cast<const double2 *>(a.tables);
     p.N = N; p.bc = a.bc; p.nx = a.nx; p.ny = a.ny;
     p.s0 = a.s0; p.s1 = a.s1;
+    p.blk_in = a.dir == 1 && a.inverse && a.blocked; p.blk_out = a.dir == 1 && !a.inverse && a.blocked;
+    p.nz = a.nz; p.k0 = a.k0;
     p.logN = fft_radices(N, p.radix);
     {
         const double2 *w = p.T4 + N;
@@ -383,7 +419,7 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
         const int pairs = N >= 2048 ? 1 : 2048 / N;          // 4096 samples per CTA, 256 threads, three CTAs per SM
         const int nl = 2 * pairs;
         p.lines = a.ny * a.planes;
-        const size_t smem = (size_t)2 * pairs * npad * 16;
+        const size_t smem = (size_t)pairs * npad * 16;
         const int grid = (p.lines + nl - 1) / nl;
         if (a.inverse) fft_inverse_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
         else fft_forward_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
@@ -392,9 +428,9 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
         if (cols > 16) cols = 16;
         if (cols < 2) cols = 2;
         if (a.nx % cols) return cudaErrorInvalidValue;
-        const size_t smem = (size_t)2 * (cols / 2) * npad * 16;
+        const size_t smem = (size_t)(cols / 2) * npad * 16;
         int threads = (cols / 2) * (N / 8);
-        threads = threads > 512 ? 512 : (threads < 64 ? 64 : threads);
+        threads = threads > 256 ? 256 : (threads < 64 ? 64 : threads);
         dim3 grid(a.nx / cols, a.planes);
         if (a.inverse) fft_inverse_kernel<true><<<grid, threads, smem, stream>>>(p, cols);
         else fft_forward_kernel<true><<<grid, threads, smem, stream>>>(p, cols);

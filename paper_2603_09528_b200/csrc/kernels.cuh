@@ -89,6 +89,9 @@ struct FftArgs {
     int dir, inverse, bc;
     int nx, ny, planes;
     double s0, s1;
+    // y only: the mode-space side (output of the forward, input of the inverse transform) is tile-blocked; in / out
+    // then point at the FIELD on that side, nz = field depth, k0 = z index of the first plane of this launch
+    int blocked = 0, nz = 0, k0 = 0;
 };
 bool fft_supported(int n);                                   // 2^m, 16 <= n <= 2048
 void fft_tables(int n, std::vector<double> &out);            // e^{-i pi k/2n} (n entries) | per-pass twiddle tables

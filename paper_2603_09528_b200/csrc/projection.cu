@@ -7,8 +7,8 @@
 // prescribed value), Dirichlet = ghost value -Phi at one cell width, periodic = faces 0 and n are one face (entry n
 // ignored on input, written as a copy of entry 0).
 //
-// Both kernels are HBM-bound stencils: one thread per (i, j) column marching over a chunk of KZ z-levels, x
-// contiguous across the warp (coalesced 8-byte accesses), the z neighbour carried in a register, the x / y
+// Both kernels are HBM-bound stencils: one thread per two x-neighbouring cells of one z-level (16-byte accesses; the
+// one-cell-per-thread kernels serve odd nx), x contiguous across the warp, the x / y / z
 // neighbours re-read through L1/L2.  Algorithmic traffic: divergence 32 B/pt (three face arrays in, one cell array
 // out), correction 56 B/pt (Phi in, three face arrays read-modify-write) + 16 B/pt with the pressure update.
 #include "kernels.cuh"

@@ -129,5 +129,7 @@ CONFIGS = {
     "p1024": [PAPER_GG],
     # the same case with y uniform as well, so that all four transform variants FF / FG / GF / GG
     # can be timed on one grid (bench.py --transform)
+    # 512^3 with uniform x and y (Neumann) and a stretched z (Dirichlet): the grid on which the FF variant is profiled
+    "ff512": [Problem("ff512-poisson-uniform-xy", (512, 512, 512), (8.0, 2.0, 2.0), (0.0, 0.0, 3.0), (N_, N_, D_), 0.0, 9)],
     "p1024u": [dataclasses.replace(PAPER_GG, name="paper-1024-periodic-x-uniform-xy", beta=(0.0, 0.0, 2.0))],
 }
