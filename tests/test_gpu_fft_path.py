@@ -70,6 +70,8 @@ def test_ff_all_boundary_types(tpt, torch, orc, bcx, bcy):
     ((16, 128, 21), (1, 1)), ((128, 16, 24), (1, 1)), ((256, 64, 17), (1, 1)),
     ((128, 128, 40), (1, 0)),      # FG: fast x, stretched y through the TMA GEMM and the blocked layout
     ((128, 128, 40), (0, 1)),      # GF: stretched x, fast y
+    ((64, 32, 600), (1, 1)),       # long columns: the fast y transform writes / reads the tile-blocked layout
+    ((128, 64, 777), (0, 1)),      # the same with a stretched x through the GEMM
     ((40, 64, 33), (0, 1)),        # ragged stretched x (generic GEMM) ... nx % 16 != 0 is rejected below instead
 ])
 def test_sizes_and_mixed_variants(tpt, torch, orc, n, transform):
