@@ -195,8 +195,8 @@ __device__ __forceinline__ double slot_value(int bc, int slot, cplx V, double2 t
 }
 
 // Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
-template <bool YP>
-__global__ void __launch_bounds__(256, 4)
+template <bool YP, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
 fft_forward_kernel(const FftParams p, int nlines) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc;   // + 1: neighbouring sequences start in different banks
@@ -254,8 +254,8 @@ fft_forward_kernel(const FftParams p, int nlines) {
 }
 
 // Inverse: out[line][i] = sum_slot q_slot(i) s(slot) in[line][slot]   (Eq. 12 with Q = D^{-1/2} Q~)
-template <bool YP>
-__global__ void __launch_bounds__(256, 4)
+template <bool YP, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
 fft_inverse_kernel(const FftParams p, int nlines) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc, logN = p.logN;
@@ -387,10 +387,12 @@ void fft_tables(int n, std::vector<double> &out) {
 
 cudaError_t fft_configure() {
     const int big = 200 * 1024;
-    cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_forward_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<false, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_forward_kernel<true, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_forward_kernel<true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<false, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<true, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     return e;
 }
 
@@ -421,19 +423,28 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
         p.lines = a.ny * a.planes;
         const size_t smem = (size_t)pairs * npad * 16;
         const int grid = (p.lines + nl - 1) / nl;
-        if (a.inverse) fft_inverse_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
-        else fft_forward_kernel<false><<<grid, 256, smem, stream>>>(p, nl);
+        if (a.inverse) fft_inverse_kernel<false, 256><<<grid, 256, smem, stream>>>(p, nl);
+        else fft_forward_kernel<false, 256><<<grid, 256, smem, stream>>>(p, nl);
     } else {
-        int cols = 4096 / N;                                  // 4096 samples per CTA: 8-column tiles at N = 512
+        // 4096 samples per CTA (8-column tiles at N = 512), but never rows narrower than 64 bytes: 8192 samples and
+        // 512 threads for N >= 1024
+        int cols = 4096 / N;
+        if (cols < 8) cols = N <= 1024 ? 8 : 4;
         if (cols > 16) cols = 16;
         if (cols < 2) cols = 2;
         if (a.nx % cols) return cudaErrorInvalidValue;
         const size_t smem = (size_t)(cols / 2) * npad * 16;
         int threads = (cols / 2) * (N / 8);
-        threads = threads > 256 ? 256 : (threads < 64 ? 64 : threads);
+        threads = threads < 64 ? 64 : threads;                // (cols / 2)(N / 8) <= 512
         dim3 grid(a.nx / cols, a.planes);
-        if (a.inverse) fft_inverse_kernel<true><<<grid, threads, smem, stream>>>(p, cols);
-        else fft_forward_kernel<true><<<grid, threads, smem, stream>>>(p, cols);
+        if (threads > 512) return cudaErrorInvalidValue;
+        if (threads > 256) {
+            if (a.inverse) fft_inverse_kernel<true, 512><<<grid, threads, smem, stream>>>(p, cols);
+            else fft_forward_kernel<true, 512><<<grid, threads, smem, stream>>>(p, cols);
+        } else {
+            if (a.inverse) fft_inverse_kernel<true, 256><<<grid, threads, smem, stream>>>(p, cols);
+            else fft_forward_kernel<true, 256><<<grid, threads, smem, stream>>>(p, cols);
+        }
     }
     return cudaGetLastError();
 }

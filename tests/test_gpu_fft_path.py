@@ -178,3 +178,15 @@ def test_batched_and_host_solves_on_fast_plans(tpt, torch, nz):
     plan.solve_host(fs[1], out)
     assert np.array_equal(out, singles[1])
     plan.destroy()
+
+
+def test_long_y_lines_use_the_512_thread_tiles(tpt, torch, orc):
+    # ny = 1024: 8-column tiles of 8192 samples, 512 threads per CTA (the y grid is c4's x grid, so the oracle's
+    # 1024-point eigen-decomposition is shared with the c4 tests)
+    P = I.Problem("ylong", (32, 1024, 6), (1.0, 8.0, 1.0), (1.5, 0.0, 2.0), (D_, N_, D_), 0.0, 17)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0, transform=(tpt.TRANSFORM_GEMM, tpt.TRANSFORM_FFT))
+    phi = _solve(torch, plan, f)
+    plan.destroy()
+    assert _rel(phi, orc.OraclePlan(xf, yf, zf, P.bc, 0.0).solve(f)) <= PARITY_TOL
