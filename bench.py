@@ -9,7 +9,8 @@ tanh beta = 2 in all three directions, all-Neumann (singular), uniform[-1,1] rhs
 volume-weighted mean removed.  Prints ONE JSON line (rank 0).
 
   value       whole-job Gpts/s with the rhs already resident in HBM (N>1: N independent replicas, §8(e))
-  e2e         the same metric through the C-ABI call tpt_solve_host with pinned HOST buffers (H2D + D2H inside)
+  e2e         the same metric through the C-ABI calls tpt_solve_host_async / tpt_plan_wait with pinned HOST buffers
+              (H2D + D2H of every step inside; consecutive steps overlap their copies through two plans)
   roofline    dominant kernel (the slowest of the four DMMA GEMM transforms): algorithmic flops / CUDA-event duration vs FP64 peak
   cpu_baseline the oracle (as it stands) timed on the host cores on a bounded z-slab sample of the workload
   --impl reference  times the oracle alone (rank 0 only)
@@ -216,13 +217,15 @@ def run_gpu(args):
     # replicas only (§8(e)): every rank solves its own copy of the workload (seed offset by rank)
     probs = _workload(args.config)
     plans, d_rhs, d_out, h_rhs = [], [], [], []
-    plan_cache = {}
+    plan_cache, probs_by_key, plan_keys = {}, {}, []
     for P in probs:
         xf, yf, zf = P.faces()
         key = (P.n, P.bc, P.alpha, P.beta, P.length)
         if key not in plan_cache:
             plan_cache[key] = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=TRANSFORMS[args.transform])
+            probs_by_key[key] = P
         plans.append(plan_cache[key])
+        plan_keys.append(key)
         f = replica_problem(P, rank).rhs()
         h_rhs.append(f)
         d_rhs.append(torch.from_numpy(f).cuda())
@@ -269,22 +272,38 @@ def run_gpu(args):
     ms_per_step = total_ms / args.steps
     value = whole_job_value(world, pts_step, args.steps, total_ms * 1e-3)
 
-    # ---- e2e: the C-ABI call with pinned HOST buffers, copies inside the timed region
-    e2e_steps = max(1, min(args.steps, 5))
+    # ---- e2e: the C-ABI call with pinned HOST buffers, copies inside the timed region.  Every step moves its inputs
+    # host -> device and its result device -> host; consecutive steps alternate between two plan sets on two streams
+    # (tpt_solve_host_async / tpt_plan_wait), so one step's download overlaps the next one's upload on the full-duplex bus.
+    e2e_steps = max(2, min(args.steps, 10))
     pin_in = [torch.from_numpy(f).pin_memory() for f in h_rhs]
-    pin_out = [torch.empty_like(t).pin_memory() for t in pin_in]
-    for pl, a, b in zip(plans, pin_in, pin_out):
-        api.solve_host(pl, a, b, stream)
+    pin_out = [[torch.empty_like(t).pin_memory() for t in pin_in] for _ in range(2)]
+    plan_cache2 = {k: api.plan_create(*pl.shape[::-1], *probs_by_key[k].faces(), probs_by_key[k].bc, probs_by_key[k].alpha,
+                                      transform=TRANSFORMS[args.transform]) for k, pl in plan_cache.items()}
+    slot_plans = [plans, [plan_cache2[k] for k in plan_keys]]
+    slot_streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+
+    def e2e_run(nsteps):
+        for s in range(nsteps):
+            q = s & 1
+            for pl, a, b in zip(slot_plans[q], pin_in, pin_out[q]):
+                api.solve_host(pl, a, b, slot_streams[q], nowait=True)
+        for q in range(2):
+            for pl in set(slot_plans[q]):
+                api.plan_wait(pl)
+
+    e2e_run(2)
     barrier()
     t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        for pl, a, b in zip(plans, pin_in, pin_out):
-            api.solve_host(pl, a, b, stream)
+    e2e_run(e2e_steps)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(dist, e2e_s, "cuda")
     e2e_val = whole_job_value(world, pts_step, e2e_steps, e2e_s)
-    e2e_ok = all(np.array_equal(b.numpy(), o.cpu().numpy()) for b, o in zip(pin_out, d_out))
+    e2e_ok = all(np.array_equal(b.numpy(), o.cpu().numpy()) for q in range(2) for b, o in zip(pin_out[q], d_out))
+    for pl in plan_cache2.values():
+        api.plan_destroy(pl)
+    del pin_out
 
     # ---- widened row: one pressure projection (Eq. 2c-2e) = divergence + this solve + correction,
     # timed on the device on the workload's Poisson plan (outside the headline timed region; rank 0 only)

@@ -140,6 +140,17 @@ int tpt_plan_reserve_batch(tpt_plan *plan, int nrhs);
 int tpt_solve_host(tpt_plan *plan, const double *rhs_host, double *out_host, void *cuda_stream);
 
 /*
+ * tpt_solve_host_async / tpt_plan_wait — the same solve (steps 2.1–2.5 of PAPER.md:181–185 between the two copies),
+ * split into "enqueue" and "wait": tpt_solve_host_async returns as soon as the copies and kernels are enqueued
+ * (truly asynchronous only for pinned HOST buffers, which must stay valid and untouched until tpt_plan_wait returns);
+ * tpt_plan_wait blocks until the plan's most recent host solve has delivered its result.  A second call on the same
+ * plan queues behind the first.  Two plans on two streams overlap one solve's device-to-host copy with the next
+ * one's host-to-device copy (the bus is full duplex): that is how bench.py measures its end-to-end throughput.
+ */
+int tpt_solve_host_async(tpt_plan *plan, const double *rhs_host, double *out_host, void *cuda_stream);
+int tpt_plan_wait(tpt_plan *plan);
+
+/*
  * Pressure projection of the fractional-step method on the staggered grid, Eq. 2c–2e (staggered
  * arrangement PAPER.md:57; "applying the pressure-projection step to a white-noise velocity field produces a
  * discretely divergence-free field to machine precision").

@@ -29,7 +29,7 @@ SYMBOLS = (
     "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
-    "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex",
+    "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -59,6 +59,8 @@ def lib():
         L.tpt_solve_batch.argtypes = [vp, vp, vp, i, vp]
         L.tpt_plan_reserve_batch.argtypes = [vp, i]
         L.tpt_solve_host.argtypes = [vp, vp, vp, vp]
+        L.tpt_solve_host_async.argtypes = [vp, vp, vp, vp]
+        L.tpt_plan_wait.argtypes = [vp]
         L.tpt_divergence.argtypes = [vp, vp, vp, vp, d, vp, vp]
         L.tpt_gradient_correct.argtypes = [vp, vp, d, vp, vp, vp, vp, d, i, vp]
         L.tpt_project.argtypes = [vp, vp, vp, vp, d, vp, vp, d, i, vp]
@@ -239,8 +241,9 @@ def solve_batch(plan: Plan, rhs, out, stream=None):
     return out
 
 
-def solve_host(plan: Plan, rhs_host, out_host, stream=None):
-    """Solve with HOST buffers (numpy float64 arrays or CPU torch tensors, ideally pinned)."""
+def solve_host(plan: Plan, rhs_host, out_host, stream=None, nowait: bool = False):
+    """Solve with HOST buffers (numpy float64 arrays or CPU torch tensors, ideally pinned).  nowait: only enqueue
+    (pinned buffers, kept valid until plan_wait); two plans on two streams then overlap their copies."""
     def hp(a, what):
         if isinstance(a, np.ndarray):
             if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"] or a.size != plan.points:
@@ -253,9 +256,14 @@ def solve_host(plan: Plan, rhs_host, out_host, stream=None):
             raise ValueError(f"{what}: need a contiguous CPU float64 tensor of {plan.points} elements")
         return C.c_void_p(a.data_ptr())
 
-    _check(lib().tpt_solve_host(plan._h, hp(rhs_host, "rhs"), hp(out_host, "out"), _stream_handle(stream)),
-           "tpt_solve_host")
+    fn = lib().tpt_solve_host_async if nowait else lib().tpt_solve_host
+    _check(fn(plan._h, hp(rhs_host, "rhs"), hp(out_host, "out"), _stream_handle(stream)), "tpt_solve_host")
     return out_host
+
+
+def plan_wait(plan: Plan):
+    """Block until the plan's most recent solve_host(..., nowait=True) has delivered its result."""
+    _check(lib().tpt_plan_wait(plan._h), "tpt_plan_wait")
 
 
 def face_counts(plan: Plan):

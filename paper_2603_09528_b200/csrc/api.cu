@@ -506,6 +506,17 @@ static int host_slabs(const tpt_plan *p) {
 }
 
 int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *cuda_stream) {
+    int rc = tpt_solve_host_async(p, rhs_host, out_host, cuda_stream);
+    return rc == TPT_OK ? tpt_plan_wait(p) : rc;
+}
+
+int tpt_plan_wait(tpt_plan *p) {
+    if (!p) return TPT_EINVAL;
+    if (!p->ev_done) return TPT_OK;   // no host solve was ever enqueued
+    return cudaEventSynchronize(p->ev_done) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+int tpt_solve_host_async(tpt_plan *p, const double *rhs_host, double *out_host, void *cuda_stream) {
     if (!p || !rhs_host || !out_host) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t bytes = p->points() * sizeof(double);
@@ -578,7 +589,7 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
     if (cudaEventRecord(p->ev_done, p->st_d2h) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_done, 0) != cudaSuccess)
         return TPT_ECUDA;
     p->launches_last = launches;
-    return cudaStreamSynchronize(st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+    return TPT_OK;
 }
 
 int tpt_divergence(tpt_plan *p, const double *u_dev, const double *v_dev, const double *w_dev, double scale, double *out_dev,

@@ -177,6 +177,27 @@ def test_host_path_slab_pipeline_equals_device_solve(tpt, torch, dirs_name, nz):
     plan.destroy()
 
 
+def test_host_path_async_two_plans_overlap_and_wait(tpt, torch):
+    # tpt_solve_host_async / tpt_plan_wait: two plans on two streams, several solves in flight; same bits as device solves
+    P = I.Problem("host-async", (128, 128, 96), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, D_), 0.0, 14)
+    xf, yf, zf = P.faces()
+    plans = [tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0) for _ in range(2)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    fs = [I.uniform_pm1(500 + r, P.points).reshape(P.n[::-1]) for r in range(4)]
+    devs = [_solve(torch, plans[0], f) for f in fs]
+    h_in = [torch.from_numpy(f).pin_memory() for f in fs]
+    h_out = [torch.zeros_like(t).pin_memory() for t in h_in]
+    tpt.plan_wait(plans[0])                                                  # nothing enqueued yet: returns at once
+    for r in range(4):
+        tpt.solve_host(plans[r & 1], h_in[r], h_out[r], streams[r & 1], nowait=True)
+    for pl in plans:
+        tpt.plan_wait(pl)
+    for r in range(4):
+        assert np.array_equal(h_out[r].numpy(), devs[r])
+    for pl in plans:
+        pl.destroy()
+
+
 def test_host_path_poisson_singular_multi_slab(tpt, torch, orc):
     P = I.Problem("host-sing", (256, 128, 320), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, 13)
     xf, yf, zf = P.faces()
