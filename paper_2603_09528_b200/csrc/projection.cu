@@ -138,7 +138,7 @@ correct_kernel(const double *__restrict__ phi, double *__restrict__ u, double *_
 // are 16-byte aligned); the u rows have odd length nx + 1, so the two u faces are 8-byte accesses.  One z-level per
 // thread (the z neighbours come from L2, which holds many planes).
 template <bool WITH_P>
-__global__ void __launch_bounds__(PX)
+__global__ void __launch_bounds__(PX, 12)
 correct2_kernel(const double *__restrict__ phi, double *__restrict__ u, double *__restrict__ v, double *__restrict__ w,
                 double *__restrict__ p, const double *__restrict__ gfx, const double *__restrict__ gfy,
                 const double *__restrict__ gfz, const double *__restrict__ rwx, const double *__restrict__ rwy,
