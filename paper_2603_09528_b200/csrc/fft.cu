@@ -261,6 +261,7 @@ fft_inverse_kernel(const FftParams p, int nlines) {
     const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc, logN = p.logN;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
     double *Rr = reinterpret_cast<double *>(b0);                          // staged coefficients [line][slot], overwritten by Z
+    const int rstr = N + 2;                                               // line stride: neighbouring lines in different banks
     const Lines<YP> L(p, nlines);
     const int steps = L.steps();
 #pragma unroll 4
@@ -271,12 +272,12 @@ fft_inverse_kernel(const FftParams p, int nlines) {
         if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + ((YP && p.blk_in) ? L.addr_blocked(p, l, slot) : L.addr(l, slot)));
         if (YP) {            // slot of lines l, l+1
             const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
-            Rr[(l << logN) + slot] = sc * v.x;
-            Rr[((l + 1) << logN) + slot] = sc * v.y;
+            Rr[l * rstr + slot] = sc * v.x;
+            Rr[(l + 1) * rstr + slot] = sc * v.y;
         } else {             // slots slot, slot+1 of line l
             v.x *= special_slot(bc, slot, N) ? p.s0 : p.s1;
             v.y *= special_slot(bc, slot + 1, N) ? p.s0 : p.s1;
-            *reinterpret_cast<double2 *>(Rr + (l << logN) + slot) = v;
+            *reinterpret_cast<double2 *>(Rr + l * rstr + slot) = v;
         }
     }
     __syncthreads();
@@ -293,7 +294,7 @@ fft_inverse_kernel(const FftParams p, int nlines) {
         const double2 t = __ldg(p.T4 + k);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const double *a = Rr + ((2 * pr + h) << logN);
+            const double *a = Rr + (2 * pr + h) * rstr;
             if (bc == 2) {
                 const int j = k <= N / 2 ? k : N - k;                      // B_k = b_k / 2, B_{N-k} = conj(b_k) / 2
                 if (j == 0) B[h] = {a[0], 0.0};
