@@ -177,6 +177,39 @@ def test_host_path_slab_pipeline_equals_device_solve(tpt, torch, dirs_name, nz):
     plan.destroy()
 
 
+def test_solve_is_capturable_in_a_cuda_graph(tpt, torch, orc):
+    # tpt_solve only enqueues kernels (no allocation, no synchronisation; the TMA descriptors travel as kernel
+    # parameters), so a launch-bound small solve can be captured once and replayed: BASELINE configs[1] (128^3 Helmholtz)
+    P = I.CONFIGS["c2"][0]
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
+    d_f = torch.from_numpy(P.rhs()).cuda()
+    d_o = torch.empty_like(d_f)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        tpt.solve(plan, d_f, d_o, side)                                      # warm-up outside the capture
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        tpt.solve(plan, d_f, d_o, torch.cuda.current_stream())
+    ref = orc.OraclePlan(xf, yf, zf, P.bc, P.alpha).solve(P.rhs())
+    for seed in (0, 1):                                                      # replay on new right-hand sides, same buffers
+        f = I.uniform_pm1(900 + seed, P.points).reshape(P.n[::-1])
+        d_f.copy_(torch.from_numpy(f))
+        d_o.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        direct = _solve(torch, plan, f)
+        assert np.array_equal(d_o.cpu().numpy(), direct)
+    d_f.copy_(torch.from_numpy(P.rhs()))
+    graph.replay()
+    torch.cuda.synchronize()
+    assert _rel(d_o.cpu().numpy(), ref) <= PARITY_TOL
+    plan.destroy()
+
+
 def test_host_path_async_two_plans_overlap_and_wait(tpt, torch):
     # tpt_solve_host_async / tpt_plan_wait: two plans on two streams, several solves in flight; same bits as device solves
     P = I.Problem("host-async", (128, 128, 96), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, D_), 0.0, 14)
