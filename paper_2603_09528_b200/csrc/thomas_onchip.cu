@@ -1,9 +1,11 @@
 // thomas_onchip.cu — step 2.3 (Eq. 11 at PAPER.md:161–163) with the whole z-column resident on chip:
 // every point of the field is read from HBM once and written once (16 B/pt, the algorithmic minimum).
 //
-// A CTA owns tiles of 16 neighbouring (kx,ky) columns x nz rows, staged in shared memory by 2-D tiled TMA
-// (boxes of 16 columns x up to 256 rows; 128-byte rows) through an NBUF-deep ring, so the load of the next tile
-// and the store of the previous one overlap the arithmetic of the current one (persistent CTAs).
+// A CTA owns tiles of 16 (or 8) neighbouring (kx,ky) columns x nz rows, staged in shared memory by tiled TMA
+// (boxes of up to 256 rows of 128 or 64 bytes) through an NBUF-deep ring, so the load of the next tile and the
+// store of the previous one overlap the arithmetic of the current one (persistent CTAs).  The field may be in the
+// natural layout (rows nx*ny apart) or in the tile-blocked mode-space layout of kernels.cuh, where a 16-column tile
+// is one dense block of nz*128 bytes; the tensor map hides the difference.  Launch shapes: launch_thomas_onchip.
 // (Row-by-row 1-D bulk copies were measured first: the TMA unit then sustains only ~1 copy / 17 cycles per SM,
 // 2.2 TB/s chip-wide — hence the tensor map.)
 //
