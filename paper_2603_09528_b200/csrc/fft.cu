@@ -148,7 +148,7 @@ struct Lines {
     size_t base;     // element offset of the CTA's first line
     int nl, valid;   // lines of this CTA, and how many of them exist
     int nx, N, logN, lognl;
-    __device__ Lines(const FftParams &p, int nlines) : nl(nlines), nx(p.nx), N(p.N), logN(p.logN) {
+    __device__ __forceinline__ Lines(const FftParams &p, int nlines, int logn) : nl(nlines), nx(p.nx), N(1 << logn), logN(logn) {
         lognl = 31 - __clz(nlines);
         if (YP) {
             base = (size_t)blockIdx.y * p.nx * p.ny + (size_t)blockIdx.x * nl;
@@ -159,29 +159,47 @@ struct Lines {
             valid = min(nl, p.lines - first);
         }
     }
-    __device__ int steps() const { return (nl << logN) >> 1; }
+    __device__ __forceinline__ int steps() const { return (nl << logN) >> 1; }
     // X: (line, even sample index);  Y: (first line of the pair, sample index)
-    __device__ void decode(int e2, int &l, int &idx) const {
+    __device__ __forceinline__ void decode(int e2, int &l, int &idx) const {
         if (YP) { idx = e2 >> (lognl - 1); l = (e2 & ((nl >> 1) - 1)) << 1; }
         else { l = e2 >> (logN - 1); idx = (e2 & ((N >> 1) - 1)) << 1; }
     }
-    __device__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + ((size_t)l << logN) + idx; }
+    __device__ __forceinline__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + ((size_t)l << logN) + idx; }
     // y only: mode `idx` of column line l in the tile-blocked layout ((m (nx/16) + i/16) nz + k) 16 + i mod 16
-    __device__ size_t addr_blocked(const FftParams &p, int l, int idx) const {
+    __device__ __forceinline__ size_t addr_blocked(const FftParams &p, int l, int idx) const {
         const int i = blockIdx.x * nl + l, k = p.k0 + blockIdx.y;
         return (((size_t)idx * (p.nx >> 4) + (i >> 4)) * p.nz + k) * 16 + (i & 15);
     }
 };
 
-template <int INV>
+// Everything that depends only on the transform length is a compile-time constant of the kernel (template LOGN): the
+// pass radices, the lines and threads per CTA, every shift, mask and padded offset — index arithmetic was most of the
+// instruction count when these were run-time values (profiles/r1d_fft_path.md).
+__host__ __device__ constexpr int radix_at(int logn, int q) {            // as many 8s as possible, then 4 (or 4, 4)
+    const int n8 = logn / 3, rem = logn % 3;
+    if (rem == 1) return q < n8 - 1 ? 8 : (q < n8 + 1 ? 4 : 0);
+    return q < n8 ? 8 : ((rem == 2 && q == n8) ? 4 : 0);
+}
+__host__ __device__ constexpr int lines_of(bool yp, int logn) {          // lines (real sequences) per CTA
+    const int n = 1 << logn;
+    if (!yp) return n >= 2048 ? 2 : 2 * (2048 / n);                       // x: 4096 samples
+    int cols = 4096 / n;                                                  // y: 4096 samples, rows of at least 64 bytes
+    if (cols > 16) cols = 16;
+    if (cols < 8) cols = n <= 1024 ? 8 : 4;
+    return cols;
+}
+__host__ __device__ constexpr int threads_of(bool yp, int logn) {
+    if (!yp) return 256;
+    const int t = (lines_of(true, logn) / 2) * ((1 << logn) / 8);
+    return t < 64 ? 64 : t;
+}
+template <int LOGN, int INV, int Q = 0, int NS = 1>
 __device__ __forceinline__ void run_passes(cplx *buf, const FftParams &p, int pairs, int npad) {
-    int Ns = 1;
-    for (int q = 0; q < 4 && p.radix[q]; ++q) {
-        const int R = p.radix[q];
-        if (R == 8) stockham_pass<8, INV>(buf, p.logN, Ns, pairs, npad, p.Wq[q]);
-        else if (R == 4) stockham_pass<4, INV>(buf, p.logN, Ns, pairs, npad, p.Wq[q]);
-        else stockham_pass<2, INV>(buf, p.logN, Ns, pairs, npad, p.Wq[q]);
-        Ns *= R;
+    constexpr int R = radix_at(LOGN, Q);
+    if constexpr (R != 0) {
+        stockham_pass<R, INV>(buf, LOGN, NS, pairs, npad, p.Wq[Q]);
+        run_passes<LOGN, INV, Q + 1, NS * R>(buf, p, pairs, npad);
     }
 }
 
@@ -195,13 +213,15 @@ __device__ __forceinline__ double slot_value(int bc, int slot, cplx V, double2 t
 }
 
 // Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
-template <bool YP, int THREADS>
-__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
-fft_forward_kernel(const FftParams p, int nlines) {
+template <bool YP, int LOGN>
+__global__ void __launch_bounds__(threads_of(YP, LOGN), threads_of(YP, LOGN) > 256 ? 2 : 4)
+fft_forward_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc;   // + 1: neighbouring sequences start in different banks
+    constexpr int N = 1 << LOGN, nlines = lines_of(YP, LOGN), pairs = nlines >> 1;
+    constexpr int npad = N + (N >> 3) + 1;       // padded length + 1: neighbouring sequences start in different banks
+    const int bc = p.bc;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
-    const Lines<YP> L(p, nlines);
+    const Lines<YP> L(p, nlines, LOGN);
     const int steps = L.steps();
 #pragma unroll 4
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
@@ -222,7 +242,7 @@ fft_forward_kernel(const FftParams p, int nlines) {
         }
     }
     __syncthreads();
-    run_passes<0>(b0, p, pairs, npad);
+    run_passes<LOGN, 0>(b0, p, pairs, npad);
     const cplx *Z = b0;
 #pragma unroll 4
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
@@ -254,15 +274,17 @@ fft_forward_kernel(const FftParams p, int nlines) {
 }
 
 // Inverse: out[line][i] = sum_slot q_slot(i) s(slot) in[line][slot]   (Eq. 12 with Q = D^{-1/2} Q~)
-template <bool YP, int THREADS>
-__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
-fft_inverse_kernel(const FftParams p, int nlines) {
+template <bool YP, int LOGN>
+__global__ void __launch_bounds__(threads_of(YP, LOGN), threads_of(YP, LOGN) > 256 ? 2 : 4)
+fft_inverse_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = p.N, npad = pad(N) + 1, pairs = nlines >> 1, bc = p.bc, logN = p.logN;
+    constexpr int N = 1 << LOGN, logN = LOGN, nlines = lines_of(YP, LOGN), pairs = nlines >> 1;
+    constexpr int npad = N + (N >> 3) + 1;
+    const int bc = p.bc;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
     double *Rr = reinterpret_cast<double *>(b0);                          // staged coefficients [line][slot], overwritten by Z
-    const int rstr = N + 2;                                               // line stride: neighbouring lines in different banks
-    const Lines<YP> L(p, nlines);
+    constexpr int rstr = N + 2;                                             // line stride: neighbouring lines in different banks
+    const Lines<YP> L(p, nlines, LOGN);
     const int steps = L.steps();
 #pragma unroll 4
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
@@ -317,7 +339,7 @@ fft_inverse_kernel(const FftParams p, int nlines) {
         b0[(item >> logN) * npad + pad(item & (N - 1))] = zreg[it];
     }
     __syncthreads();
-    run_passes<1>(b0, p, pairs, npad);
+    run_passes<LOGN, 1>(b0, p, pairs, npad);
     const cplx *Z = b0;
 #pragma unroll 4
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
@@ -386,16 +408,43 @@ void fft_tables(int n, std::vector<double> &out) {
     }
 }
 
-cudaError_t fft_configure() {
-    const int big = 200 * 1024;
-    cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<false, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_forward_kernel<true, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_forward_kernel<true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<false, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<true, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    return e;
+cudaError_t fft_configure() { return cudaSuccess; }   // shared-memory opt-in happens per instantiation at first launch
+
+namespace {
+
+template <bool YP, int LOGN>
+cudaError_t launch_one(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
+    constexpr int N = 1 << LOGN, nl = lines_of(YP, LOGN), threads = threads_of(YP, LOGN);
+    constexpr size_t smem = (size_t)(nl / 2) * (N + (N >> 3) + 1) * 16;
+    static bool configured = false;
+    if (!configured && smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<YP, LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<YP, LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    configured = true;
+    const dim3 grid(grid_x, grid_y);
+    if (inverse) fft_inverse_kernel<YP, LOGN><<<grid, threads, smem, stream>>>(p);
+    else fft_forward_kernel<YP, LOGN><<<grid, threads, smem, stream>>>(p);
+    return cudaGetLastError();
 }
+
+template <bool YP>
+cudaError_t launch_len(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
+    switch (p.logN) {
+        case 4: return launch_one<YP, 4>(p, inverse, grid_x, grid_y, stream);
+        case 5: return launch_one<YP, 5>(p, inverse, grid_x, grid_y, stream);
+        case 6: return launch_one<YP, 6>(p, inverse, grid_x, grid_y, stream);
+        case 7: return launch_one<YP, 7>(p, inverse, grid_x, grid_y, stream);
+        case 8: return launch_one<YP, 8>(p, inverse, grid_x, grid_y, stream);
+        case 9: return launch_one<YP, 9>(p, inverse, grid_x, grid_y, stream);
+        case 10: return launch_one<YP, 10>(p, inverse, grid_x, grid_y, stream);
+        case 11: return launch_one<YP, 11>(p, inverse, grid_x, grid_y, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
 
 cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
     const int N = a.dir == 0 ? a.nx : a.ny;
@@ -417,37 +466,14 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
             Ns *= p.radix[q];
         }
     }
-    const int npad = N + (N >> 3) + 1;
     if (a.dir == 0) {
-        const int pairs = N >= 2048 ? 1 : 2048 / N;          // 4096 samples per CTA, 256 threads, three CTAs per SM
-        const int nl = 2 * pairs;
+        const int nl = lines_of(false, p.logN);
         p.lines = a.ny * a.planes;
-        const size_t smem = (size_t)pairs * npad * 16;
-        const int grid = (p.lines + nl - 1) / nl;
-        if (a.inverse) fft_inverse_kernel<false, 256><<<grid, 256, smem, stream>>>(p, nl);
-        else fft_forward_kernel<false, 256><<<grid, 256, smem, stream>>>(p, nl);
-    } else {
-        // 4096 samples per CTA (8-column tiles at N = 512), but never rows narrower than 64 bytes: 8192 samples and
-        // 512 threads for N >= 1024
-        int cols = 4096 / N;
-        if (cols < 8) cols = N <= 1024 ? 8 : 4;
-        if (cols > 16) cols = 16;
-        if (cols < 2) cols = 2;
-        if (a.nx % cols) return cudaErrorInvalidValue;
-        const size_t smem = (size_t)(cols / 2) * npad * 16;
-        int threads = (cols / 2) * (N / 8);
-        threads = threads < 64 ? 64 : threads;                // (cols / 2)(N / 8) <= 512
-        dim3 grid(a.nx / cols, a.planes);
-        if (threads > 512) return cudaErrorInvalidValue;
-        if (threads > 256) {
-            if (a.inverse) fft_inverse_kernel<true, 512><<<grid, threads, smem, stream>>>(p, cols);
-            else fft_forward_kernel<true, 512><<<grid, threads, smem, stream>>>(p, cols);
-        } else {
-            if (a.inverse) fft_inverse_kernel<true, 256><<<grid, threads, smem, stream>>>(p, cols);
-            else fft_forward_kernel<true, 256><<<grid, threads, smem, stream>>>(p, cols);
-        }
+        return launch_len<false>(p, a.inverse, (p.lines + nl - 1) / nl, 1, stream);
     }
-    return cudaGetLastError();
+    const int cols = lines_of(true, p.logN);
+    if (a.nx % cols) return cudaErrorInvalidValue;
+    return launch_len<true>(p, a.inverse, a.nx / cols, a.planes, stream);
 }
 
 }  // namespace tpt
