@@ -213,13 +213,13 @@ __device__ __forceinline__ double slot_value(int bc, int slot, cplx V, double2 t
 }
 
 // Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
-template <bool YP, int LOGN>
+template <bool YP, int LOGN, int BC>
 __global__ void __launch_bounds__(threads_of(YP, LOGN), threads_of(YP, LOGN) > 256 ? 2 : 4)
 fft_forward_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 1 << LOGN, nlines = lines_of(YP, LOGN), pairs = nlines >> 1;
     constexpr int npad = N + (N >> 3) + 1;       // padded length + 1: neighbouring sequences start in different banks
-    const int bc = p.bc;
+    constexpr int bc = BC;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
     const Lines<YP> L(p, nlines, LOGN);
     const int steps = L.steps();
@@ -274,13 +274,13 @@ fft_forward_kernel(const FftParams p) {
 }
 
 // Inverse: out[line][i] = sum_slot q_slot(i) s(slot) in[line][slot]   (Eq. 12 with Q = D^{-1/2} Q~)
-template <bool YP, int LOGN>
+template <bool YP, int LOGN, int BC>
 __global__ void __launch_bounds__(threads_of(YP, LOGN), threads_of(YP, LOGN) > 256 ? 2 : 4)
 fft_inverse_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 1 << LOGN, logN = LOGN, nlines = lines_of(YP, LOGN), pairs = nlines >> 1;
     constexpr int npad = N + (N >> 3) + 1;
-    const int bc = p.bc;
+    constexpr int bc = BC;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
     double *Rr = reinterpret_cast<double *>(b0);                          // staged coefficients [line][slot], overwritten by Z
     constexpr int rstr = N + 2;                                             // line stride: neighbouring lines in different banks
@@ -412,21 +412,28 @@ cudaError_t fft_configure() { return cudaSuccess; }   // shared-memory opt-in ha
 
 namespace {
 
-template <bool YP, int LOGN>
-cudaError_t launch_one(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
+template <bool YP, int LOGN, int BC>
+cudaError_t launch_bc(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
     constexpr int N = 1 << LOGN, nl = lines_of(YP, LOGN), threads = threads_of(YP, LOGN);
     constexpr size_t smem = (size_t)(nl / 2) * (N + (N >> 3) + 1) * 16;
     static bool configured = false;
     if (!configured && smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<YP, LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<YP, LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<YP, LOGN, BC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<YP, LOGN, BC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
     configured = true;
     const dim3 grid(grid_x, grid_y);
-    if (inverse) fft_inverse_kernel<YP, LOGN><<<grid, threads, smem, stream>>>(p);
-    else fft_forward_kernel<YP, LOGN><<<grid, threads, smem, stream>>>(p);
+    if (inverse) fft_inverse_kernel<YP, LOGN, BC><<<grid, threads, smem, stream>>>(p);
+    else fft_forward_kernel<YP, LOGN, BC><<<grid, threads, smem, stream>>>(p);
     return cudaGetLastError();
+}
+
+template <bool YP, int LOGN>
+cudaError_t launch_one(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
+    if (p.bc == 0) return launch_bc<YP, LOGN, 0>(p, inverse, grid_x, grid_y, stream);
+    if (p.bc == 1) return launch_bc<YP, LOGN, 1>(p, inverse, grid_x, grid_y, stream);
+    return launch_bc<YP, LOGN, 2>(p, inverse, grid_x, grid_y, stream);
 }
 
 template <bool YP>
