@@ -140,7 +140,8 @@ __device__ __forceinline__ bool special_slot(int bc, int slot, int N) {
 }
 
 // Line / element addressing, two neighbouring memory elements (one 16-byte access) per step.
-// X: a CTA owns `nl` consecutive rows (lines contiguous in memory, N = nx); step e2 -> line l, samples i, i+1.
+// X: a CTA owns `nl` consecutive rows (lines contiguous in memory, N = nx); step e2 -> samples i, i+1 of the two lines
+//    l, l+1 of a pair (two 16-byte accesses, two whole complex elements).
 // Y: a CTA owns `nl` neighbouring columns of one z-plane (lines strided by nx, N = ny; rows of nl*8 bytes);
 //    step e2 -> sample idx of the two lines 2c, 2c+1 — which are exactly the two halves of one complex sequence.
 template <bool YP>
@@ -159,11 +160,11 @@ struct Lines {
             valid = min(nl, p.lines - first);
         }
     }
-    __device__ __forceinline__ int steps() const { return (nl << logN) >> 1; }
-    // X: (line, even sample index);  Y: (first line of the pair, sample index)
+    __device__ __forceinline__ int steps() const { return YP ? (nl << logN) >> 1 : (nl << logN) >> 2; }
+    // (first line of a pair, sample index): X steps over two samples of both lines, Y over one sample of both lines
     __device__ __forceinline__ void decode(int e2, int &l, int &idx) const {
         if (YP) { idx = e2 >> (lognl - 1); l = (e2 & ((nl >> 1) - 1)) << 1; }
-        else { l = e2 >> (logN - 1); idx = (e2 & ((N >> 1) - 1)) << 1; }
+        else { l = (e2 >> (logN - 1)) << 1; idx = (e2 & ((N >> 1) - 1)) << 1; }
     }
     __device__ __forceinline__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + ((size_t)l << logN) + idx; }
     // y only: mode `idx` of column line l in the tile-blocked layout ((m (nx/16) + i/16) nz + k) 16 + i mod 16
@@ -227,18 +228,20 @@ fft_forward_kernel(const FftParams p) {
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, i;
         L.decode(e2, l, i);
-        double2 v = make_double2(0.0, 0.0);
-        if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + L.addr(l, i));
         if (YP) {            // v = sample i of lines l, l+1: one complex element
+            const double2 v = *reinterpret_cast<const double2 *>(p.in + L.addr(l, i));
             double sign;
             const int n = seq_index(bc, i, N, sign);
             b0[(l >> 1) * npad + pad(n)] = cplx{sign * v.x, sign * v.y};
-        } else {             // v = samples i (even), i+1 of line l
+        } else {             // samples i (even), i+1 of lines l and l+1: two complex elements
+            double2 va = make_double2(0.0, 0.0), vb = va;
+            if (l < L.valid) va = *reinterpret_cast<const double2 *>(p.in + L.addr(l, i));
+            if (l + 1 < L.valid) vb = *reinterpret_cast<const double2 *>(p.in + L.addr(l + 1, i));
             double s0, s1;
             const int n0 = seq_index(bc, i, N, s0), n1 = seq_index(bc, i + 1, N, s1);
-            double *z = reinterpret_cast<double *>(b0 + (l >> 1) * npad) + (l & 1);
-            z[2 * pad(n0)] = s0 * v.x;
-            z[2 * pad(n1)] = s1 * v.y;
+            cplx *z = b0 + (l >> 1) * npad;
+            z[pad(n0)] = cplx{s0 * va.x, s0 * vb.x};
+            z[pad(n1)] = cplx{s1 * va.y, s1 * vb.y};
         }
     }
     __syncthreads();
@@ -258,16 +261,19 @@ fft_forward_kernel(const FftParams p) {
             const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
             o.x = sc * slot_value(bc, slot, cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, t4);
             o.y = sc * slot_value(bc, slot, cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)}, t4);
-        } else {             // slots `slot`, `slot + 1` of line l
-            double r[2];
+        } else {             // slots `slot`, `slot + 1` of both lines of the pair
+            double ra[2], rb[2];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int sl = slot + h, k = slot_bin(bc, sl, N);
                 const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
-                const cplx V = (l & 1) ? cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)} : cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)};
-                r[h] = (special_slot(bc, sl, N) ? p.s0 : p.s1) * slot_value(bc, sl, V, __ldg(p.T4 + k));
+                const double2 t4 = __ldg(p.T4 + k);
+                const double sc = special_slot(bc, sl, N) ? p.s0 : p.s1;
+                ra[h] = sc * slot_value(bc, sl, cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, t4);
+                rb[h] = sc * slot_value(bc, sl, cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)}, t4);
             }
-            o = make_double2(r[0], r[1]);
+            o = make_double2(ra[0], ra[1]);
+            if (l + 1 < L.valid) *reinterpret_cast<double2 *>(p.out + L.addr(l + 1, slot)) = make_double2(rb[0], rb[1]);
         }
         *reinterpret_cast<double2 *>(p.out + ((YP && p.blk_out) ? L.addr_blocked(p, l, slot) : L.addr(l, slot))) = o;
     }
@@ -290,16 +296,18 @@ fft_inverse_kernel(const FftParams p) {
     for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
         int l, slot;
         L.decode(e2, l, slot);
-        double2 v = make_double2(0.0, 0.0);
-        if (l < L.valid) v = *reinterpret_cast<const double2 *>(p.in + ((YP && p.blk_in) ? L.addr_blocked(p, l, slot) : L.addr(l, slot)));
         if (YP) {            // slot of lines l, l+1
+            const double2 v = *reinterpret_cast<const double2 *>(p.in + (p.blk_in ? L.addr_blocked(p, l, slot) : L.addr(l, slot)));
             const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
             Rr[l * rstr + slot] = sc * v.x;
             Rr[(l + 1) * rstr + slot] = sc * v.y;
-        } else {             // slots slot, slot+1 of line l
-            v.x *= special_slot(bc, slot, N) ? p.s0 : p.s1;
-            v.y *= special_slot(bc, slot + 1, N) ? p.s0 : p.s1;
-            *reinterpret_cast<double2 *>(Rr + l * rstr + slot) = v;
+        } else {             // slots slot, slot+1 of lines l and l+1
+            double2 va = make_double2(0.0, 0.0), vb = va;
+            if (l < L.valid) va = *reinterpret_cast<const double2 *>(p.in + L.addr(l, slot));
+            if (l + 1 < L.valid) vb = *reinterpret_cast<const double2 *>(p.in + L.addr(l + 1, slot));
+            const double sc0 = special_slot(bc, slot, N) ? p.s0 : p.s1, sc1 = special_slot(bc, slot + 1, N) ? p.s0 : p.s1;
+            *reinterpret_cast<double2 *>(Rr + l * rstr + slot) = make_double2(sc0 * va.x, sc1 * va.y);
+            *reinterpret_cast<double2 *>(Rr + (l + 1) * rstr + slot) = make_double2(sc0 * vb.x, sc1 * vb.y);
         }
     }
     __syncthreads();
@@ -355,7 +363,8 @@ fft_inverse_kernel(const FftParams p) {
         } else {
             double s0, s1;
             const cplx c0 = z[pad(seq_index(bc, i, N, s0))], c1 = z[pad(seq_index(bc, i + 1, N, s1))];
-            o = (l & 1) ? make_double2(s0 * c0.y, s1 * c1.y) : make_double2(s0 * c0.x, s1 * c1.x);
+            o = make_double2(s0 * c0.x, s1 * c1.x);              // line l: real parts; line l + 1: imaginary parts
+            if (l + 1 < L.valid) *reinterpret_cast<double2 *>(p.out + L.addr(l + 1, i)) = make_double2(s0 * c0.y, s1 * c1.y);
         }
         *reinterpret_cast<double2 *>(p.out + L.addr(l, i)) = o;
     }
