@@ -26,7 +26,6 @@ struct cplx { double x, y; };
 __device__ __forceinline__ cplx operator+(cplx a, cplx b) { return {a.x + b.x, a.y + b.y}; }
 __device__ __forceinline__ cplx operator-(cplx a, cplx b) { return {a.x - b.x, a.y - b.y}; }
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return {fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x)}; }
-__device__ __forceinline__ cplx conj(cplx a) { return {a.x, -a.y}; }
 // multiply by -i (forward) or +i (inverse)
 template <int INV>
 __device__ __forceinline__ cplx mul_mi(cplx a) { return INV ? cplx{-a.y, a.x} : cplx{a.y, -a.x}; }
