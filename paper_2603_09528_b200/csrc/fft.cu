@@ -184,7 +184,7 @@ __host__ __device__ constexpr int radix_at(int logn, int q) {            // as m
 __host__ __device__ constexpr int lines_of(bool yp, int logn) {          // lines (real sequences) per CTA
     const int n = 1 << logn;
     if (!yp) return n >= 2048 ? 2 : 2 * (2048 / n);                       // x: 4096 samples
-    int cols = 4096 / n;                                                  // y: 4096 samples, rows of at least 64 bytes
+    int cols = 8192 / n;                                                  // y: 8192 samples, rows of at least 64 bytes
     if (cols > 16) cols = 16;
     if (cols < 8) cols = n <= 1024 ? 8 : 4;
     return cols;
