@@ -287,8 +287,11 @@ fft_inverse_kernel(const FftParams p) {
     constexpr int npad = N + (N >> 3) + 1;
     constexpr int bc = BC;
     cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
-    double *Rr = reinterpret_cast<double *>(b0);                          // staged coefficients [line][slot], overwritten by Z
-    constexpr int rstr = N + 2;                                             // line stride: neighbouring lines in different banks
+    cplx *Cc = b0;                   // staged scaled coefficients [pair][slot] = (line 2 pr, line 2 pr + 1), overwritten by Z
+    constexpr int cstr = N + 1;      // pair stride: neighbouring pairs in different banks
+    // (x keeps the two lines of a pair as two real arrays, `rstr` apart: its 16-byte stores are then conflict-free)
+    double *Rr = reinterpret_cast<double *>(b0);
+    constexpr int rstr = N + 2;
     const Lines<YP> L(p, nlines, LOGN);
     const int steps = L.steps();
 #pragma unroll 4
@@ -298,8 +301,7 @@ fft_inverse_kernel(const FftParams p) {
         if (YP) {            // slot of lines l, l+1
             const double2 v = *reinterpret_cast<const double2 *>(p.in + (p.blk_in ? L.addr_blocked(p, l, slot) : L.addr(l, slot)));
             const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
-            Rr[l * rstr + slot] = sc * v.x;
-            Rr[(l + 1) * rstr + slot] = sc * v.y;
+            Cc[(l >> 1) * cstr + slot] = cplx{sc * v.x, sc * v.y};
         } else {             // slots slot, slot+1 of lines l and l+1
             double2 va = make_double2(0.0, 0.0), vb = va;
             if (l < L.valid) va = *reinterpret_cast<const double2 *>(p.in + L.addr(l, slot));
@@ -320,21 +322,32 @@ fft_inverse_kernel(const FftParams p) {
         if (item >= (pairs << logN)) continue;
         const int pr = item >> logN, k = item & (N - 1);
         cplx B[2];
-        const double2 t = __ldg(p.T4 + k);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const double *a = Rr + (2 * pr + h) * rstr;
-            if (bc == 2) {
-                const int j = k <= N / 2 ? k : N - k;                      // B_k = b_k / 2, B_{N-k} = conj(b_k) / 2
-                if (j == 0) B[h] = {a[0], 0.0};
-                else if (j == N / 2) B[h] = {a[N - 1], 0.0};
-                else B[h] = {0.5 * a[2 * j - 1], (k < N / 2 ? -0.5 : 0.5) * a[2 * j]};
-            } else if (k == 0) {
-                B[h] = {bc == 0 ? a[0] : a[N - 1], 0.0};
+        // scaled coefficient q of both lines of the pair
+        auto c = [&](int q) -> cplx {
+            if (YP) return Cc[pr * cstr + q];
+            return cplx{Rr[2 * pr * rstr + q], Rr[(2 * pr + 1) * rstr + q]};
+        };
+        if (bc == 2) {
+            const int j = k <= N / 2 ? k : N - k;                          // B_k = b_k / 2, B_{N-k} = conj(b_k) / 2
+            if (j == 0 || j == N / 2) {
+                const cplx a = c(j == 0 ? 0 : N - 1);
+                B[0] = {a.x, 0.0};
+                B[1] = {a.y, 0.0};
             } else {
-                const double ak = bc == 0 ? a[k] : a[N - 1 - k], am = bc == 0 ? a[N - k] : a[k - 1];
-                B[h] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak, -am});   // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
+                const cplx ar = c(2 * j - 1), ai = c(2 * j);
+                const double sg = k < N / 2 ? -0.5 : 0.5;
+                B[0] = {0.5 * ar.x, sg * ai.x};
+                B[1] = {0.5 * ar.y, sg * ai.y};
             }
+        } else if (k == 0) {
+            const cplx a = c(bc == 0 ? 0 : N - 1);
+            B[0] = {a.x, 0.0};
+            B[1] = {a.y, 0.0};
+        } else {
+            const cplx ak = c(bc == 0 ? k : N - 1 - k), am = c(bc == 0 ? N - k : k - 1);
+            const double2 t = __ldg(p.T4 + k);                             // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
+            B[0] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak.x, -am.x});
+            B[1] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak.y, -am.y});
         }
         zreg[it] = cplx{B[0].x - B[1].y, B[0].y + B[1].x};
     }
