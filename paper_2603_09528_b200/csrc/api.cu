@@ -129,10 +129,8 @@ cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st)
 bool use_blocked(const tpt_plan *p) {
     if (p->thomas_variant != 1 || !(p->dirs & 2)) return false;
     if (!tpt::blocked_layout_supported(p->nx, p->ny, p->nz) || !tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) return false;
-    // the fast y transform addresses either layout, but pays for the scattered 64-byte pieces: measured, the blocked
-    // layout wins only where the natural-layout sweep is weak (long columns: 43.8 -> 41.6 ms per 1024^3 FF solve,
-    // but 3.94 -> 4.02 ms at 512^3)
-    if (p->transform[1] == TPT_TRANSFORM_FFT) return p->nz > 544;
+    // the fast y transform addresses either layout (its tiles write whole 128-byte lines of the blocked field)
+    if (p->transform[1] == TPT_TRANSFORM_FFT) return true;
     return p->gemm_variant == 2 && p->ny % 128 == 0 && p->nx % 128 == 0;   // the TMA GEMM's tile shape (M = K = ny, N = nx)
 }
 
