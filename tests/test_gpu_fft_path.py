@@ -190,3 +190,41 @@ def test_long_y_lines_use_the_512_thread_tiles(tpt, torch, orc):
     phi = _solve(torch, plan, f)
     plan.destroy()
     assert _rel(phi, orc.OraclePlan(xf, yf, zf, P.bc, 0.0).solve(f)) <= PARITY_TOL
+
+
+@pytest.mark.parametrize("direction,bc", [(0, N_), (0, D_), (0, P_), (1, N_), (1, P_)])
+def test_longest_lines_against_the_closed_form_basis(tpt, torch, direction, bc):
+    # 2048-long lines (radices 8.8.8.4; x: one pair per CTA, y: 4-column tiles with 512 threads).  The oracle's Jacobi
+    # would take minutes at this length, so the stage outputs are compared with the closed-form orthonormal bases
+    # themselves (BJ north_star: DCT-II for Neumann; sine / Fourier for Dirichlet / periodic): p^ = sqrt(w) Q^T f.
+    n = (2048, 16, 3) if direction == 0 else (16, 2048, 3)
+    N, L = 2048, 4.0
+    bcs = (bc, N_, D_) if direction == 0 else (N_, bc, D_)
+    P = I.Problem("long", n, (L, 1.0, 1.0) if direction == 0 else (1.0, L, 1.0), (0.0, 0.0, 1.5), bcs, 0.0, 33)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*n, xf, yf, zf, bcs, 0.0, transform=(tpt.TRANSFORM_FFT, tpt.TRANSFORM_FFT))
+    i = np.arange(N)[:, None]
+    s = np.arange(N)[None, :]
+    if bc == N_:
+        Q = np.cos(np.pi * s * (2 * i + 1) / (2 * N))
+    elif bc == D_:
+        Q = np.sin(np.pi * (s + 1) * (2 * i + 1) / (2 * N))
+    else:
+        j = (s + 1) // 2
+        Q = np.where((s == 0) | (s % 2 == 1), np.cos(2 * np.pi * j * i / N), np.sin(2 * np.pi * j * i / N))
+    Q = Q / np.linalg.norm(Q, axis=0)
+    w = L / N
+    f = P.rhs()
+    d_f = torch.from_numpy(f).cuda()
+    a, b = torch.empty_like(d_f), torch.empty_like(d_f)
+    plan.stage(tpt.K_FWD_X if direction == 0 else tpt.K_FWD_Y, d_f, a)
+    plan.stage(tpt.K_INV_X if direction == 0 else tpt.K_INV_Y, a, b)
+    torch.cuda.synchronize()
+    expect = np.sqrt(w) * (np.einsum("im,kji->kjm", Q, f) if direction == 0 else np.einsum("jm,kji->kmi", Q, f))
+    assert np.abs(a.cpu().numpy() - expect).max() <= 1e-12 * np.abs(expect).max()
+    assert float((b - d_f).abs().max()) <= 1e-12
+    lam = plan.eigenvalues(direction)
+    k = np.arange(N)
+    arg = {N_: np.pi * k / (2 * N), D_: np.pi * (k + 1) / (2 * N), P_: np.pi * ((k + 1) // 2) / N}[bc]
+    assert np.abs(lam + 4.0 / w**2 * np.sin(arg) ** 2).max() <= 1e-13 * 4.0 / w**2
+    plan.destroy()
