@@ -42,7 +42,7 @@ def _solve(torch, plan, f):
 
 
 # nz picks the sweep's launch shape: <=128: 8-row segments; <=256: 16 rows, two CTAs per SM; 257..544 (blocked):
-# 8-column tiles with 17-row segments; 545..768: 32-row segments; 769..1056: 8-column tiles with 33-row segments.  Ragged nz exercises the zero-filled tail rows.
+# 8-column tiles with 17-row segments; 545..768: 32-row segments; 769..1056: 8-column tiles with 17-row segments and 512 threads.  Ragged nz exercises the zero-filled tail rows.
 SHAPES = [
     ("nz24", (128, 128, 24), (N_, N_, D_), 0.0),
     ("nz130", (128, 256, 130), (N_, N_, D_), 0.0),

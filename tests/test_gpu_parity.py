@@ -181,7 +181,7 @@ THOMAS_SHAPES = [
     (64, 32, 512, N_, 0.0),      # M = 32, S = 16 (the bench configuration), singular
     (64, 32, 768, D_, 5e-4),     # M = 32, S = 24, two-slot ring
     (48, 24, 700, N_, 0.0),      # M = 32, ragged, S = 22, singular
-    (64, 32, 1000, N_, 0.0),     # M = 33, 8-column tiles in the natural layout, ragged, singular
+    (64, 32, 1000, N_, 0.0),     # M = 17, S = 60 -> 64, 8-column tiles in the natural layout, ragged, singular
     (32, 16, 1056, D_, 1e-3),    # the longest column the on-chip kernel takes
     (40, 6, 33, D_, 0.0),        # nx*ny % 16 == 0 with nx % 16 != 0: tiles straddle y rows
 ]
