@@ -16,7 +16,7 @@
  *   - "HOST" / "DEVICE" below says where a pointer must live.  Device pointers must be 16-byte
  *     aligned (any cudaMalloc / torch allocation is).
  *   - the CUDA device is the one current at tpt_plan_create; the same device must be current in
- *     later calls on that plan.  There is no CPU fallback: without a usable CUDA device
+ *     later calls on that plan (TPT_EINVAL otherwise).  There is no CPU fallback: without a usable CUDA device
  *     tpt_plan_create fails with TPT_ECUDA.
  */
 #ifndef TPT_H
@@ -169,7 +169,10 @@ int tpt_plan_wait(tpt_plan *plan);
  *                     The plan must be a Poisson plan of the full operator (helmholtz_alpha == 0, TPT_DIRS_XYZ):
  *                     TPT_EINVAL otherwise.  On a singular plan the velocity field must be compatible (zero net flux
  *                     through the walls), as in the paper's solver; Phi then has zero volume-weighted mean.
- * All DEVICE pointers, 16-byte aligned, no aliasing between arguments; phi_dev / out_dev: nx*ny*nz doubles.
+ * All DEVICE pointers, no aliasing between arguments; phi_dev / out_dev: nx*ny*nz doubles.  Alignment: 8 bytes is
+ * enough for tpt_divergence and tpt_gradient_correct (a view into a larger buffer is fine: arrays that are not 16-byte
+ * aligned take the one-cell-per-thread kernels instead of the two-cell ones); tpt_project needs a 16-byte aligned
+ * phi_dev because it runs tpt_solve on it.  Anything less is TPT_EINVAL, never a fault.
  * Asynchronous on cuda_stream, no allocation, no host synchronisation.  gamma_dt, c > 0; alpha_p >= 0.
  */
 int tpt_divergence(tpt_plan *plan, const double *u_dev, const double *v_dev, const double *w_dev, double scale,

@@ -2,10 +2,12 @@
 
 Usage: python -m paper_2603_09528_b200.build [--force] [--verbose]
 nvcc cross-compiles without a GPU.  The library is built IN-TREE (it is git-ignored but travels to the
-GPU box with the repo snapshot).
+GPU box with the repo snapshot).  Each source is compiled to its own object (in parallel, only when stale) under
+paper_2603_09528_b200/build/, then linked.
 """
 from __future__ import annotations
 
+import concurrent.futures
 import os
 import shutil
 import subprocess
@@ -14,15 +16,17 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
+OBJ = os.path.join(PKG, "build")
 LIB = os.path.join(PKG, "libtpt.so")
-SOURCES = ["api.cu", "kernels.cu", "gemm_tma.cu", "thomas_onchip.cu", "projection.cu", "fft.cu", "plan_host.cpp"]
-HEADERS = [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "tmap.hpp"), os.path.join(CSRC, "plan_host.hpp"), os.path.join(ROOT, "include", "tpt.h")]
+SOURCES = ["api.cu", "kernels.cu", "gemm_tma.cu", "thomas_onchip.cu", "projection.cu", "fft.cu", "plan_host.cpp",
+           "sharded.cu", "fused_small.cu"]
+HEADERS = [os.path.join(CSRC, h) for h in ("kernels.cuh", "ptx.cuh", "tmap.hpp", "plan_host.hpp", "devonce.hpp", "plan.hpp")] + \
+          [os.path.join(ROOT, "include", "tpt.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC,-fopenmp,-O3",
-    "-shared",
 ]
 
 
@@ -33,26 +37,53 @@ def nvcc() -> str:
     return exe
 
 
+def _sources():
+    return [s for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
+
+
+def _deps_mtime() -> float:
+    deps = [h for h in HEADERS if os.path.exists(h)] + [os.path.abspath(__file__)]
+    return max(os.path.getmtime(d) for d in deps)
+
+
 def is_fresh() -> bool:
     if not os.path.exists(LIB):
         return False
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
-    return all(os.path.getmtime(d) <= t for d in deps)
+    return all(os.path.getmtime(os.path.join(CSRC, s)) <= t for s in _sources()) and _deps_mtime() <= t
+
+
+def _compile(src: str, verbose: bool) -> str:
+    obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+    cmd = [nvcc(), *NVCC_FLAGS]
+    if verbose:
+        cmd += ["-Xptxas", "-v"]
+    cmd += ["-c", "-o", obj, os.path.join(CSRC, src)]
+    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
+    return res.stdout + res.stderr
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if is_fresh() and not force:
         return LIB
-    cmd = [nvcc(), *NVCC_FLAGS]
+    os.makedirs(OBJ, exist_ok=True)
+    hdr_t = _deps_mtime()
+    stale = []
+    for s in _sources():
+        obj = os.path.join(OBJ, os.path.splitext(s)[0] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_t, os.path.getmtime(os.path.join(CSRC, s))):
+            stale.append(s)
+    with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, max(1, len(stale)))) as pool:
+        logs = list(pool.map(lambda s: _compile(s, verbose), stale))
     if verbose:
-        cmd += ["-Xptxas", "-v"]
-    cmd += ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lgomp"]
+        print("".join(logs))
+    objs = [os.path.join(OBJ, os.path.splitext(s)[0] + ".o") for s in _sources()]
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC", "-o", LIB, *objs, "-lgomp"]
     res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
-    if verbose:
-        print(res.stdout + res.stderr)
+        raise RuntimeError("link failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
     return LIB
 
 

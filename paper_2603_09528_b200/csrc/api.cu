@@ -46,6 +46,7 @@ struct tpt_plan {
     cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
     cudaEvent_t ev_start = nullptr, ev_done = nullptr;
     std::vector<cudaEvent_t> ev_slab;   // 2 per z-slab: slab arrived, slab ready to leave
+    bool host_ready = false;            // all of the above exist (set last, tpt_solve_host_async)
     // profiling: one set of TPT_K_COUNT+1 events per profiled solve since the last read-out
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;           // events handed out since the last read-out
@@ -229,6 +230,15 @@ int run_pipeline(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream
 }
 
 bool aligned16(const void *q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; }
+bool aligned8(const void *q) { return (reinterpret_cast<uintptr_t>(q) & 7) == 0; }
+
+// tpt.h: "the same device must be current in later calls on that plan" — a launch on another device would read the
+// plan's matrices through an invalid context; refuse instead.
+bool on_plan_device(const tpt_plan *p) {
+    int d = -1;
+    if (cudaGetDevice(&d) != cudaSuccess) { cudaGetLastError(); return false; }
+    return d == p->device;
+}
 
 }  // namespace
 
@@ -441,7 +451,7 @@ int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double
 }
 
 int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_stream) {
-    if (!p || !rhs_dev || !out_dev || !aligned16(rhs_dev) || !aligned16(out_dev)) return TPT_EINVAL;
+    if (!p || !rhs_dev || !out_dev || !aligned16(rhs_dev) || !aligned16(out_dev) || !on_plan_device(p)) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int launches = 0;
     const bool prof = p->profiling != 0;
@@ -467,7 +477,7 @@ int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_st
 }
 
 int tpt_plan_reserve_batch(tpt_plan *p, int nrhs) {
-    if (!p || nrhs < 1 || (double)nrhs * (double)p->points() > 8.0e9) return TPT_EINVAL;
+    if (!p || nrhs < 1 || (double)nrhs * (double)p->points() > 8.0e9 || !on_plan_device(p)) return TPT_EINVAL;
     if (nrhs <= p->work_fields) return TPT_OK;
     if (cudaDeviceSynchronize() != cudaSuccess) return TPT_ECUDA;
     double *w = nullptr;
@@ -480,7 +490,7 @@ int tpt_plan_reserve_batch(tpt_plan *p, int nrhs) {
 }
 
 int tpt_solve_batch(tpt_plan *p, const double *rhs_dev, double *out_dev, int nrhs, void *cuda_stream) {
-    if (!p || !rhs_dev || !out_dev || nrhs < 1 || !aligned16(rhs_dev) || !aligned16(out_dev)) return TPT_EINVAL;
+    if (!p || !rhs_dev || !out_dev || nrhs < 1 || !aligned16(rhs_dev) || !aligned16(out_dev) || !on_plan_device(p)) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int launches = 0;
     const size_t pts = p->points();
@@ -510,12 +520,12 @@ int tpt_solve_host(tpt_plan *p, const double *rhs_host, double *out_host, void *
 
 int tpt_plan_wait(tpt_plan *p) {
     if (!p) return TPT_EINVAL;
-    if (!p->ev_done) return TPT_OK;   // no host solve was ever enqueued
+    if (!p->host_ready) return TPT_OK;   // no host solve was ever enqueued
     return cudaEventSynchronize(p->ev_done) == cudaSuccess ? TPT_OK : TPT_ECUDA;
 }
 
 int tpt_solve_host_async(tpt_plan *p, const double *rhs_host, double *out_host, void *cuda_stream) {
-    if (!p || !rhs_host || !out_host) return TPT_EINVAL;
+    if (!p || !rhs_host || !out_host || !on_plan_device(p)) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t bytes = p->points() * sizeof(double);
     if (!p->d_stage) {
@@ -523,17 +533,31 @@ int tpt_solve_host_async(tpt_plan *p, const double *rhs_host, double *out_host, 
         if (e != cudaSuccess) { cudaGetLastError(); p->d_stage = nullptr; return e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
     }
     const int ns = host_slabs(p);
-    if (!p->st_h2d) {
-        if (cudaStreamCreateWithFlags(&p->st_h2d, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) != cudaSuccess)
+    if (!p->host_ready) {
+        // every stream and event is created into locals and committed to the plan only when all of them exist: a
+        // partial failure leaves the plan as it was (no null stream silently becoming the legacy default stream)
+        cudaStream_t s_in = nullptr, s_out = nullptr;
+        cudaEvent_t e_start = nullptr, e_done = nullptr;
+        std::vector<cudaEvent_t> slab;
+        bool ok = true;
+        try { slab.assign(2 * 16, nullptr); } catch (const std::bad_alloc &) { return TPT_ENOMEM; }
+        ok = cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) == cudaSuccess &&
+             cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&e_start, cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&e_done, cudaEventDisableTiming) == cudaSuccess;
+        for (size_t q = 0; ok && q < slab.size(); ++q) ok = cudaEventCreateWithFlags(&slab[q], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            for (auto &e : slab) if (e) cudaEventDestroy(e);
+            if (e_start) cudaEventDestroy(e_start);
+            if (e_done) cudaEventDestroy(e_done);
+            if (s_in) cudaStreamDestroy(s_in);
+            if (s_out) cudaStreamDestroy(s_out);
             return TPT_ECUDA;
-        try {
-            p->ev_slab.resize(2 * 16, nullptr);
-        } catch (const std::bad_alloc &) { return TPT_ENOMEM; }
-        for (auto &e : p->ev_slab)
-            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return TPT_ECUDA;
+        }
+        p->st_h2d = s_in; p->st_d2h = s_out; p->ev_start = e_start; p->ev_done = e_done;
+        p->ev_slab.swap(slab);
+        p->host_ready = true;
     }
     // Slab pipeline: the transforms act plane by plane, so slab s is transformed (2.1, 2.2) while slab s+1 is still
     // on the bus; after the sweep (which needs every plane) slab s leaves while slab s+1 is transformed back.
@@ -592,7 +616,8 @@ int tpt_solve_host_async(tpt_plan *p, const double *rhs_host, double *out_host, 
 
 int tpt_divergence(tpt_plan *p, const double *u_dev, const double *v_dev, const double *w_dev, double scale, double *out_dev,
                    void *cuda_stream) {
-    if (!p || !u_dev || !v_dev || !w_dev || !out_dev || !std::isfinite(scale)) return TPT_EINVAL;
+    if (!p || !u_dev || !v_dev || !w_dev || !out_dev || !std::isfinite(scale) || !on_plan_device(p)) return TPT_EINVAL;
+    if (!aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(out_dev)) return TPT_EINVAL;
     cudaError_t e = tpt::launch_divergence(u_dev, v_dev, w_dev, p->geo, scale, out_dev, static_cast<cudaStream_t>(cuda_stream));
     p->launches_last = 1;
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
@@ -602,7 +627,8 @@ static bool dirs_valid(int d) { return d == TPT_DIRS_XYZ || d == TPT_DIRS_YZ || 
 
 int tpt_gradient_correct(tpt_plan *p, const double *phi_dev, double c, double *u_dev, double *v_dev, double *w_dev, double *p_dev,
                          double alpha_p, int implicit_dirs, void *cuda_stream) {
-    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c)) return TPT_EINVAL;
+    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c) || !on_plan_device(p)) return TPT_EINVAL;
+    if (!aligned8(phi_dev) || !aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(p_dev)) return TPT_EINVAL;
     if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
     cudaError_t e = tpt::launch_correct(phi_dev, u_dev, v_dev, w_dev, p_dev, p->geo, c, alpha_p, implicit_dirs,
                                         static_cast<cudaStream_t>(cuda_stream));
@@ -612,7 +638,8 @@ int tpt_gradient_correct(tpt_plan *p, const double *phi_dev, double c, double *u
 
 int tpt_project(tpt_plan *p, double *u_dev, double *v_dev, double *w_dev, double gamma_dt, double *phi_dev, double *p_dev,
                 double alpha_p, int implicit_dirs, void *cuda_stream) {
-    if (!p || !u_dev || !v_dev || !w_dev || !phi_dev || !aligned16(phi_dev)) return TPT_EINVAL;
+    if (!p || !u_dev || !v_dev || !w_dev || !phi_dev || !aligned16(phi_dev) || !on_plan_device(p)) return TPT_EINVAL;
+    if (!aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(p_dev)) return TPT_EINVAL;
     if (p->alpha != 0.0 || p->dirs != TPT_DIRS_XYZ) return TPT_EINVAL;       // Eq. 2c carries the full Laplacian
     if (!(gamma_dt > 0.0) || !std::isfinite(gamma_dt)) return TPT_EINVAL;
     if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
@@ -661,7 +688,7 @@ int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
 
 int tpt_stage(tpt_plan *p, int slot, const double *in_dev, double *out_dev, void *cuda_stream) {
     if (!p || !in_dev || !out_dev || slot < 0 || slot >= TPT_K_COUNT) return TPT_EINVAL;
-    if (!aligned16(in_dev) || !aligned16(out_dev)) return TPT_EINVAL;
+    if (!aligned16(in_dev) || !aligned16(out_dev) || !on_plan_device(p)) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int launches = 0;
     if (!slot_active(p, slot)) return TPT_EINVAL;   // this plan does not diagonalise that direction

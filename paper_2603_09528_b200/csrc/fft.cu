@@ -16,6 +16,7 @@
 //     pass); a CTA owns several pairs of lines: contiguous rows for the x direction, a 16-column tile (128-byte rows)
 //     for the y direction, so both directions run in the field's native layout without transposes.
 // HBM-bound: 16 B/pt (read once, write once) against 2N flop/pt for the GEMM form.  N = 2^m, 16 <= N <= 2048.
+#include "devonce.hpp"
 #include "kernels.cuh"
 
 namespace tpt {
@@ -437,13 +438,15 @@ template <bool YP, int LOGN, int BC>
 cudaError_t launch_bc(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
     constexpr int N = 1 << LOGN, nl = lines_of(YP, LOGN), threads = threads_of(YP, LOGN);
     constexpr size_t smem = (size_t)(nl / 2) * (N + (N >> 3) + 1) * 16;
-    static bool configured = false;
-    if (!configured && smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(fft_forward_kernel<YP, LOGN, BC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(fft_inverse_kernel<YP, LOGN, BC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem > 48 * 1024) {
+        static DeviceOnce configured;                        // per device, thread-safe (devonce.hpp)
+        cudaError_t e = configured.run([&] {
+            cudaError_t q = cudaFuncSetAttribute(fft_forward_kernel<YP, LOGN, BC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (q == cudaSuccess) q = cudaFuncSetAttribute(fft_inverse_kernel<YP, LOGN, BC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            return q;
+        });
         if (e != cudaSuccess) return e;
     }
-    configured = true;
     const dim3 grid(grid_x, grid_y);
     if (inverse) fft_inverse_kernel<YP, LOGN, BC><<<grid, threads, smem, stream>>>(p);
     else fft_forward_kernel<YP, LOGN, BC><<<grid, threads, smem, stream>>>(p);

@@ -186,6 +186,13 @@ bool gemm_tma_supported(const GemmArgs &g) {
 }
 
 cudaError_t gemm_tma_configure() {
+    // setmaxnreg.inc<112> in the consumers can only be granted from the CTA's own launch allocation:
+    // THREADS x numRegs >= 128 x 24 + 512 x 112, i.e. 96 registers per thread at launch (what ptxas gives under
+    // __launch_bounds__(640, 1) today).  A toolchain that allocated fewer would hang the kernel: refuse instead.
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, gemm_tma_kernel);
+    if (e != cudaSuccess) return e;
+    if (fa.numRegs * THREADS < 128 * 24 + CONSUMER_WARPS * 32 * 112) return cudaErrorLaunchOutOfResources;
     return cudaFuncSetAttribute(gemm_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
 }
 

@@ -11,8 +11,6 @@
 #include "kernels.cuh"
 #include "ptx.cuh"
 
-#include <cstdio>
-
 namespace tpt {
 
 using ptx::cp_async16;

@@ -219,9 +219,13 @@ correct2_kernel(const double *__restrict__ phi, double *__restrict__ u, double *
 
 }  // namespace
 
+// The two-cells-per-thread kernels make 16-byte accesses to every array but u (whose rows have odd length nx + 1);
+// a pointer that is only 8-byte aligned (a view into a larger buffer) takes the one-cell kernels instead of faulting.
+static bool aligned16(const void *q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; }
+
 cudaError_t launch_divergence(const double *u, const double *v, const double *w, const ProjGeom &g, double scale,
                               double *out, cudaStream_t stream) {
-    if (g.nx % 2 == 0) {
+    if (g.nx % 2 == 0 && aligned16(v) && aligned16(w) && aligned16(out)) {
         dim3 grid2((g.nx / 2 + PX - 1) / PX, g.ny, g.nz);
         divergence2_kernel<<<grid2, PX, 0, stream>>>(u, v, w, g.rwx, g.rwy, g.rwz, out, g.nx, g.ny, g.nz, g.bc[0] == 2,
                                                      g.bc[1] == 2, scale);
@@ -235,7 +239,7 @@ cudaError_t launch_divergence(const double *u, const double *v, const double *w,
 
 cudaError_t launch_correct(const double *phi, double *u, double *v, double *w, double *p, const ProjGeom &g, double c,
                            double alpha, int dirs, cudaStream_t stream) {
-    if (g.nx % 2 == 0) {   // two cells per thread, 16-byte accesses
+    if (g.nx % 2 == 0 && aligned16(phi) && aligned16(v) && aligned16(w) && aligned16(p)) {   // two cells per thread, 16-byte accesses
         dim3 grid((g.nx / 2 + PX - 1) / PX, g.ny, g.nz);
         if (p)
             correct2_kernel<true><<<grid, PX, 0, stream>>>(phi, u, v, w, p, g.gfx, g.gfy, g.gfz, g.rwx, g.rwy, g.rwz, g.nx, g.ny,

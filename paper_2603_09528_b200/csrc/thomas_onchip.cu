@@ -24,6 +24,7 @@
 
 #include <vector>
 
+#include "devonce.hpp"
 #include "kernels.cuh"
 #include "ptx.cuh"
 #include "tmap.hpp"
@@ -31,7 +32,6 @@
 namespace tpt {
 
 namespace {
-
 
 template <int M, int TCOLS, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
@@ -243,29 +243,21 @@ cudaError_t launch_m(const double *in, double *x, const double *tab, const doubl
     if (nbuf < 2) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)nbuf * tile_bytes + fixed;
     auto kern = thomas_onchip_kernel<M, TC, MAXT, CTAS>;
-    static bool configured = false;
-    static int per_sm_cache[2] = {0, 0};                     // {threads*2^20 + smem key, blocks per SM}
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CTA_MAX);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static DeviceOnce configured;                            // per device, thread-safe (devonce.hpp)
+    static OccupancyCache occupancy;
+    cudaError_t e = configured.run([&] { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CTA_MAX); });
+    if (e != cudaSuccess) return e;
     const int threads = TC * S;
     if (threads > MAXT) return cudaErrorInvalidConfiguration;
-    const int key = threads * 4096 + (int)(smem / 64);
-    if (per_sm_cache[0] != key) {
-        int per_sm = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem);
-        if (e != cudaSuccess) return e;
-        if (per_sm < 1) return cudaErrorInvalidConfiguration;
-        per_sm_cache[0] = key;
-        per_sm_cache[1] = per_sm;
-    }
+    int per_sm = 0;
+    e = occupancy.get(kern, threads, smem, &per_sm);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorInvalidConfiguration;
     CUtensorMap tmap, tmap_out;
     if (!make_field_map(&tmap, in, (size_t)nx * ny, nz, TC, box_rows, blocked)) return cudaErrorUnknown;
     if (!make_field_map(&tmap_out, x, (size_t)nx * ny, nz, TC, box_rows, blocked)) return cudaErrorUnknown;
     const int ntiles = (int)(((size_t)nx * ny) / TC);
-    int grid = sms * per_sm_cache[1];
+    int grid = sms * per_sm;
     if (grid > ntiles) grid = ntiles;
     kern<<<grid, threads, smem, stream>>>(tmap, tmap_out, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf,
                                           box_rows, nbox, buf_rows, shift0, singular, ntiles);

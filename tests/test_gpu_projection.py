@@ -156,3 +156,40 @@ def test_project_argument_checks(tpt, torch):
     torch.cuda.synchronize()
     assert float(phi.abs().max()) == 0.0 and float(u.abs().max()) == 0.0
     pois.destroy()
+
+
+def test_views_that_are_only_8_byte_aligned_are_taken_not_faulted(tpt, torch, orc):
+    # tpt.h: 8-byte alignment is enough for tpt_divergence / tpt_gradient_correct; a view buf[1:1+n] into a larger
+    # buffer must give the same result as a 16-byte aligned array (it takes the one-cell kernels), never a sticky
+    # misaligned-address fault.  tpt_solve / tpt_project on a misaligned field are refused with TPT_EINVAL.
+    n, bc = (64, 12, 10), (N_, D_, D_)          # even nx: the aligned path is the two-cell kernel
+    P = I.Problem("misaligned", n, (1.0, 2.0, 1.5), (2.0, 1.5, 2.5), bc, 0.0, 5)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, 0.0)
+    u, v, w = _velocity(orc, n, bc, 40)
+    phi = I.uniform_pm1(50, P.points).reshape(n[::-1])
+    p0 = I.uniform_pm1(51, P.points).reshape(n[::-1])
+
+    def shifted(a):
+        buf = torch.zeros(a.size + 2, dtype=torch.float64, device="cuda")
+        view = buf[1:1 + a.size]
+        view.copy_(torch.from_numpy(a.ravel()).cuda())
+        assert view.data_ptr() % 16 == 8
+        return view
+
+    results = []
+    for make in (lambda a: torch.from_numpy(a.ravel().copy()).cuda(), shifted):
+        du, dv, dw, dphi, dp = (make(a) for a in (u, v, w, phi, p0))
+        out = make(np.zeros(P.points))
+        tpt.divergence(plan, du, dv, dw, out, scale=2.5)
+        tpt.gradient_correct(plan, dphi, 0.7, du, dv, dw, p=dp, alpha_p=2e-3, dirs=tpt.DIRS_XYZ)
+        torch.cuda.synchronize()
+        results.append([t.cpu().numpy().copy() for t in (out, du, dv, dw, dp)])
+    ref = orc.divergence(xf, yf, zf, bc, u, v, w, scale=2.5)
+    assert _rel(results[1][0].reshape(ref.shape), ref) <= STENCIL_TOL
+    for a, b in zip(*results):
+        assert np.abs(a - b).max() <= 1e-13 * max(1.0, np.abs(a).max())   # one-cell vs two-cell kernels: same arithmetic
+    bad = shifted(phi)
+    with pytest.raises(tpt.TptError):
+        tpt.solve(plan, bad, bad)
+    plan.destroy()
