@@ -37,13 +37,12 @@ UNIT = "Gpts/s"
 # FP64 peak of one B200: 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1.965 GHz; the DMMA and
 # DFMA microbenchmarks of the library are reported next to it.
 SM_COUNT, FP64_FMA_PER_CLK_SM = 148, 64
-ORACLE_SAMPLE_NZ = 64
 # transform type per diagonalised direction (x, y): the paper's GG / FG / GF / FF variants; FFT needs a
 # uniform power-of-two direction.  BASELINE.json's metric is quoted on GG.
 TRANSFORMS = {"gg": (0, 0), "fg": (1, 0), "gf": (0, 1), "ff": (1, 1)}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (gemm_tma_kernel), from the one
 # `ncu --set full` capture summarised in profiles/r1c_blocked_layout_projection.md (config c3; bytes).  Other configs: null.
-NCU_TRAFFIC_BYTES = {"c3": 1.077565e9 + 1.031300e9}
+NCU_TRAFFIC = {"commit": "757b0f5", "capture": "profiles/r1c_blocked_layout_projection.md", "bytes": {"c3": 1.077565e9 + 1.031300e9}}
 
 
 def _peaks():
@@ -120,17 +119,36 @@ class ClockSampler(threading.Thread):
 BAD_REASONS = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
 
 
-def _oracle_sample(probs, steps: int, warmup: int):
-    """Times the oracle's solve (plan excluded, like the GPU's) on a z-slab sample of each problem."""
+def _oracle_time(probs, steps: int, warmup: int, budget_s: float):
+    """Times the oracle's solve (plan excluded, like the GPU's) on the workload.  The FULL workload is timed whenever
+    (steps + warmup) passes of it fit `budget_s` of host time (configs c1-c4 on the box's 16 cores); otherwise every
+    problem is cut to a z-slab of as many planes as fit (same x/y grids, eigenbases and per-point transform work;
+    c5: ~3e12 flop per solve), and `sample` says so.  The plane count is chosen from an untimed 8-plane calibration."""
     import oracle   # test infrastructure; allowed here (cpu_baseline / --impl reference)
 
-    plans, rhs, pts = [], [], 0
+    passes = steps + warmup
+    t_plane = 0.0
+    cal = []
     for P in probs:
-        S = P.thin_z(min(ORACLE_SAMPLE_NZ, P.n[2]))
+        C = P.thin_z(min(8, P.n[2]))
+        xf, yf, zf = C.faces()
+        pl, f = oracle.OraclePlan(xf, yf, zf, C.bc, C.alpha), C.rhs()
+        pl.solve(f)
+        t0 = time.perf_counter()
+        pl.solve(f)
+        cal.append((time.perf_counter() - t0) / C.n[2])
+        pl.close()
+    full_s = sum(c * P.n[2] for c, P in zip(cal, probs)) * passes
+    frac = min(1.0, budget_s / max(full_s, 1e-9))
+    plans, rhs, pts, planes = [], [], 0, []
+    for P in probs:
+        nzs = P.n[2] if frac >= 1.0 else max(8, min(P.n[2], int(P.n[2] * frac) // 8 * 8))
+        S = P if nzs == P.n[2] else P.thin_z(nzs)
         xf, yf, zf = S.faces()
         plans.append(oracle.OraclePlan(xf, yf, zf, S.bc, S.alpha))
         rhs.append(S.rhs())
         pts += S.points
+        planes.append(nzs)
     for _ in range(warmup):
         for pl, f in zip(plans, rhs):
             pl.solve(f)
@@ -139,11 +157,19 @@ def _oracle_sample(probs, steps: int, warmup: int):
         for pl, f in zip(plans, rhs):
             pl.solve(f)
     dt = (time.perf_counter() - t0) / steps
+    for pl in plans:
+        pl.close()
     P = probs[0]
-    sample = (f"oracle solve on a z-slab of each problem: {P.n[0]}x{P.n[1]}x{min(ORACLE_SAMPLE_NZ, P.n[2])} cells "
-              f"(same x/y grids and eigenbases, {min(ORACLE_SAMPLE_NZ, P.n[2])}/{P.n[2]} of the points; per-point "
-              f"transform work identical); plan (eigendecomposition) excluded")
+    if all(n == Q.n[2] for n, Q in zip(planes, probs)):
+        sample = (f"the FULL workload ({len(probs)} solve(s) of {P.n[0]}x{P.n[1]}x{P.n[2]} cells per step), {steps} timed step(s) "
+                  f"after {warmup} warm-up; plan (eigendecomposition) excluded")
+    else:
+        sample = (f"oracle solve on a z-slab of each problem: {P.n[0]}x{P.n[1]}x{planes[0]} of {P.n[2]} planes (same x/y grids "
+                  f"and eigenbases, per-point transform work identical; the full workload would take ~{full_s:.0f} s for "
+                  f"{passes} passes, budget {budget_s:.0f} s), {steps} timed step(s) after {warmup} warm-up; plan excluded")
     return {"value": pts / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample,
+            "note": "the parity oracle as it stands: naive OpenMP loops, no BLAS, never tuned — a reported baseline, not a "
+                    "tuned CPU implementation and not the target",
             "ms_per_sample_step": dt * 1e3, "sample_points": pts}
 
 
@@ -152,14 +178,15 @@ def run_reference(args):
     if rank != 0:
         return
     probs = _workload(args.config)
-    steps = max(1, min(args.steps, 5))
-    base = _oracle_sample(probs, steps, min(args.warmup, 1))
+    steps, warmup = max(1, args.steps), max(0, args.warmup)      # honoured as given (the driver compares them)
+    base = _oracle_time(probs, steps, warmup, budget_s=300.0)
     line = {
         "impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
-        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": base["ms_per_sample_step"],
+        "steps": steps, "warmup": warmup, "ms_per_step": base["ms_per_sample_step"],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": _config_json(args.config, probs, {"note": "CPU oracle on the host cores; a step is the bounded sample"}),
-        "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "config": _config_json(args.config, probs, {"parallelism": "replicas only" if args.gpus > 1 else "single GPU",
+                                                      "transform_xy": args.transform}),
+        "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample", "note")},
         "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -187,6 +214,80 @@ def max_over_ranks(dist, value: float, device="cpu") -> float:
 def whole_job_value(world: int, pts_step: int, steps: int, seconds: float) -> float:
     """Gpts/s over all replicas: every rank processed pts_step * steps points in `seconds` (max over ranks)."""
     return world * pts_step * steps / seconds / 1e9
+
+
+def device_rhs(api, torch, P, stream=None):
+    """The problem's right-hand side generated on the device: the same counter-based white noise as Problem.rhs()
+    (bit-identical, tests/test_gpu_variants.py) and, for singular problems, the volume-weighted mean removed (A8)."""
+    nx, ny, nz = P.n
+    f = torch.empty((nz, ny, nx), dtype=torch.float64, device="cuda")
+    api.fill_uniform(f, P.seed, 0, stream)
+    if P.singular:
+        wx, wy, wz = (torch.from_numpy(np.diff(a)).cuda() for a in P.faces())
+        mean = torch.einsum("k,j,i,kji->", wz, wy, wx, f) / (wx.sum() * wy.sum() * wz.sum())
+        f -= mean
+    return f
+
+
+def measure_config(api, torch, name, fp64_peak, hbm_gbs, steps=6, warmup=3):
+    """Device-timed numbers of one BASELINE config (GG transforms): ms per step, Gpts/s, the slowest GEMM transform's
+    fraction of the FP64 peak and the sweep's fraction of the HBM peak, from `steps` timed steps after `warmup`."""
+    probs = I.CONFIGS[name]
+    stream = torch.cuda.current_stream()
+    plan_cache, plans, rhs, outs = {}, [], [], []
+    for P in probs:
+        key = (P.n, P.bc, P.alpha, P.beta, P.length)
+        if key not in plan_cache:
+            plan_cache[key] = api.plan_create(*P.n, *P.faces(), P.bc, P.alpha)
+        plans.append(plan_cache[key])
+        rhs.append(device_rhs(api, torch, P, stream))
+        outs.append(torch.empty_like(rhs[-1]))
+    # the small configs fit the 126 MB L2: flush it between steps (outside the per-step events) by rewriting a 256 MB buffer
+    small = sum(P.points for P in probs) * 8 * 3 < 256e6
+    flush = torch.empty(32 << 20, dtype=torch.float64, device="cuda") if small else None
+
+    def step():
+        for pl, r, o in zip(plans, rhs, outs):
+            api.solve(pl, r, o, stream)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    for pl in plan_cache.values():
+        pl.set_profiling(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        if flush is not None:
+            flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sorted(a.elapsed_time(b) for a, b in ev)
+    ms_step = float(np.mean(ms))
+    P0, pl0 = probs[0], plans[0]
+    kms, launches, _ = pl0.kernel_times()
+    for pl in plan_cache.values():
+        pl.set_profiling(False)
+    nx, ny, nz = P0.n
+    gemm = {"fwd_x": 2.0 * nx, "fwd_y": 2.0 * ny, "inv_y": 2.0 * ny, "inv_x": 2.0 * nx}
+    fr = {k: gemm[k] * P0.points / (kms[i] * 1e-3) / 1e12 / fp64_peak for i, k in enumerate(api.KERNEL_NAMES) if k in gemm}
+    slow = min(fr, key=fr.get)
+    th = kms[api.K_THOMAS]
+    out = {
+        "workload": ", ".join(P.name for P in probs), "grid": list(P0.n), "solves_per_step": len(probs),
+        "ms_per_step": ms_step, "ms_per_step_min": ms[0], "gpts_per_s": sum(P.points for P in probs) / ms_step / 1e6,
+        "timed_steps": steps, "warmup": warmup, "l2_flushed_between_steps": bool(small),
+        "kernel_ms_first_plan": dict(zip(api.KERNEL_NAMES, kms)),
+        "gemm_frac_of_fp64_peak": {"slowest": slow, "frac": fr[slow], "all": fr},
+        "thomas_frac_of_hbm_peak_16B_per_pt": 16.0 * P0.points / (th * 1e-3) / 1e9 / hbm_gbs,
+        "gpu_launches_first_plan": launches,
+    }
+    for pl in plan_cache.values():
+        pl.destroy()
+    del rhs, outs, flush
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_gpu(args):
@@ -347,6 +448,14 @@ def run_gpu(args):
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         fp64_peak = SM_COUNT * FP64_FMA_PER_CLK_SM * 2 * sm_max * 1e6 / 1e12
         dmma_meas, dfma_meas = api.fp64_peak(1), api.fp64_peak(0)
+        # ---- the other BASELINE configs (device-timed, GG), so that the driver-run record carries all five
+        other_configs = None
+        if not args.no_other_configs and args.transform == "gg":
+            for t in (d_rhs, d_out):
+                t.clear()
+            torch.cuda.empty_cache()
+            other_configs = {n: measure_config(api, torch, n, fp64_peak, peaks["hbm_gbs"])
+                             for n in ("c1", "c2", "c3", "c4", "c5") if n != args.config}
         # per-kernel: mean event durations over the timed region (dominant plan = first)
         key0 = next(iter(kt))
         ms0, _ = kt[key0]
@@ -367,7 +476,7 @@ def run_gpu(args):
             kernels[name] = entry
         gemm_slots = [n for n in ("fwd_x", "fwd_y", "inv_y", "inv_x") if kernels[n]["bound"] == "tensor"]
         dom = max(gemm_slots or ("fwd_x", "fwd_y", "inv_y", "inv_x"), key=lambda n: kernels[n]["ms"])
-        traffic = NCU_TRAFFIC_BYTES.get(args.config)
+        traffic = NCU_TRAFFIC["bytes"].get(args.config)
         if gemm_slots:
             roofline = {
                 "kernel": f"gemm_tma_kernel ({dom})", "bound": "tensor", "achieved": kernels[dom]["achieved_tflops"],
@@ -377,8 +486,10 @@ def run_gpu(args):
                 "peak_measured_dmma_loop": dmma_meas, "peak_measured_dfma_loop": dfma_meas,
                 "frac_of_measured_dmma_loop": kernels[dom]["achieved_tflops"] / dmma_meas,
                 "algorithmic_flops_per_launch": flops[dom], "algorithmic_dram_bytes_per_launch": 16.0 * pts,
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1c_*.md)",
             }
+            if traffic is not None:
+                roofline["traffic_unit"] = (f"bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum; capture "
+                                            f"{NCU_TRAFFIC['capture']}, kernel source as of commit {NCU_TRAFFIC['commit']})")
         if not gemm_slots:   # FF: no GEMM left — the dominant kernel is the slowest fast transform, HBM-bound at 16 B/pt
             roofline = {
                 "kernel": f"fft kernel ({dom})", "bound": "hbm", "achieved": kernels[dom]["achieved_gbs_16B_per_pt"],
@@ -386,7 +497,7 @@ def run_gpu(args):
                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})",
                 "algorithmic_dram_bytes_per_launch": 16.0 * pts,
             }
-        cpu = _oracle_sample(probs, 1, 1)
+        cpu = _oracle_time(probs, 3, 1, budget_s=60.0)
         n20 = per_step[: min(20, len(per_step))]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -401,7 +512,8 @@ def run_gpu(args):
             "gpu_launches": launches,
             "roofline": roofline,
             "kernels": kernels,
-            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "note")},
+            "other_configs": other_configs,
             "solve_ms_mean_20_fastest": float(np.mean(n20)) / len(probs), "solve_ms_min": per_step[0] / len(probs),
             "hbm_peak_gbs": peaks["hbm_gbs"], "peaks": peak_kind,
         }
@@ -422,6 +534,8 @@ def main():
     ap.add_argument("--config", default="c3", choices=sorted(I.CONFIGS))
     ap.add_argument("--transform", default="gg", choices=sorted(TRANSFORMS),
                     help="transform type in x, y: g = eigenbasis GEMM (BASELINE metric), f = fast transform (uniform directions)")
+    ap.add_argument("--no-other-configs", dest="no_other_configs", action="store_true",
+                    help="skip the device-timed numbers of the other BASELINE configs (c1, c2, c4, c5)")
     ap.add_argument("--no-projection", dest="no_projection", action="store_true",
                     help="skip the (untimed-region) pressure-projection measurement")
     args = ap.parse_args()

@@ -192,6 +192,15 @@ int tpt_plan_destroy(tpt_plan *plan);
  * mode m of the orthogonal Q~ (Eq. 5).  Either output may be NULL.  HOST pointers. */
 int tpt_plan_get_eigen(const tpt_plan *plan, int dir, double *lambda_host, double *qtilde_host);
 
+/* The plan-time eigen-solver alone, on the HOST (no device needed): steps 1.1-1.2 of PAPER.md:175-176 for one direction —
+ * operator of Eq. 3-4 from the n+1 faces, symmetrisation (Eq. 5), base solver, two guarded factored-form refinement
+ * steps (A9) — with the output conventions of tpt_plan_get_eigen.  base_kind 0 = the plan's implicit-QL base
+ * solver; 1 = a deliberately crude one (normwise deflation, 64x looser): the accuracy rule says the refinement must
+ * absorb the difference (SURVEY 8(c.5) cross-solver check).  tpt_debug_set_eigen_base selects the base solver of every
+ * plan created afterwards in this process (test only; 0 restores the default).  HOST pointers; either output may be NULL. */
+int tpt_host_eigen(int n, const double *faces_host, int bc, int base_kind, double *lambda_host, double *qtilde_host);
+int tpt_debug_set_eigen_base(int base_kind);
+
 /* 1 if the plan is singular (all-Neumann Poisson), 0 if not, < 0 on error. */
 int tpt_plan_is_singular(const tpt_plan *plan);
 
@@ -222,6 +231,12 @@ int tpt_plan_set_gemm_variant(tpt_plan *plan, int variant);
  * 16 B/pt of HBM traffic; used where nx*ny % 16 == 0 and nz <= 1056, default), 0 = streaming one-thread-per-column
  * kernel that spills c' to the plan workspace (any shape).  Both solve step 2.3 exactly. */
 int tpt_plan_set_thomas_variant(tpt_plan *plan, int variant);
+
+/* Synthetic input generator on the device ("white-noise" fields; recipe in DESIGN.md §4): out_dev[t] =
+ * 2u - 1, u = top 53 bits of the splitmix64 finaliser of (offset + t + (seed + 1) * 0x9E3779B97F4A7C15 mod 2^64) * 2^-53 —
+ * bit-identical to the host generator the tests and the oracle use, so large right-hand sides need not cross the bus.
+ * Holds none of the method's arithmetic.  out_dev: DEVICE, count doubles, 8-byte aligned.  Asynchronous on cuda_stream. */
+int tpt_fill_uniform(double *out_dev, size_t count, unsigned long long seed, unsigned long long offset, void *cuda_stream);
 
 /* FP64 arithmetic-pipe microbenchmarks used as roofline denominators: kind 0 = register-resident
  * DFMA loop, kind 1 = register-resident DMMA (m8n8k4) loop.  Runs on the current device, returns

@@ -30,6 +30,7 @@ SYMBOLS = (
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
+    "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_fill_uniform",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -67,6 +68,8 @@ def lib():
         L.tpt_plan_destroy.argtypes = [vp]
         L.tpt_plan_get_eigen.argtypes = [vp, i, _dp, _dp]
         L.tpt_plan_is_singular.argtypes = [vp]
+        L.tpt_host_eigen.argtypes = [i, _dp, i, i, _dp, _dp]
+        L.tpt_debug_set_eigen_base.argtypes = [i]
         L.tpt_plan_device_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
         L.tpt_stage.argtypes = [vp, i, vp, vp, vp]
         L.tpt_plan_set_profiling.argtypes = [vp, i]
@@ -74,6 +77,7 @@ def lib():
         L.tpt_plan_set_gemm_variant.argtypes = [vp, i]
         L.tpt_plan_set_thomas_variant.argtypes = [vp, i]
         L.tpt_fp64_peak.argtypes = [i, _dp]
+        L.tpt_fill_uniform.argtypes = [vp, C.c_size_t, C.c_ulonglong, C.c_ulonglong, vp]
         L.tpt_strerror.argtypes = [i]
         L.tpt_strerror.restype = C.c_char_p
         L.tpt_version.argtypes = []
@@ -299,6 +303,27 @@ def project(plan: Plan, u, v, w, gamma_dt: float, phi, p=None, alpha_p: float = 
 
 def plan_destroy(plan: Plan):
     plan.destroy()
+
+
+def host_eigen(faces, bc: int, base_kind: int = 0):
+    """(lambda[n], qtilde[n, n]) from the plan-time eigen-solver alone (host only, no device needed)."""
+    fa, fp = _faces(faces)
+    n = fa.size - 1
+    lam, q = np.empty(n), np.empty((n, n))
+    _check(lib().tpt_host_eigen(n, fp, int(bc), int(base_kind), lam.ctypes.data_as(_dp), q.ctypes.data_as(_dp)), "tpt_host_eigen")
+    return lam, q
+
+
+def debug_set_eigen_base(base_kind: int):
+    """Base eigen-solver of plans created from now on: 0 = default, 1 = deliberately crude (tests only)."""
+    _check(lib().tpt_debug_set_eigen_base(int(base_kind)), "tpt_debug_set_eigen_base")
+
+
+def fill_uniform(out, seed: int, offset: int = 0, stream=None):
+    """out[t] = seeded uniform[-1,1) white noise, bit-identical to inputs.uniform_pm1(seed, n, offset)."""
+    _check(lib().tpt_fill_uniform(_dev_ptr(out, out.numel(), "out"), out.numel(), int(seed), int(offset),
+                                  _stream_handle(stream)), "tpt_fill_uniform")
+    return out
 
 
 def fp64_peak(kind: int) -> float:

@@ -56,6 +56,8 @@ struct tpt_plan {
 
 namespace {
 
+int g_eigen_base = 0;   // tpt_debug_set_eigen_base: base eigen-solver of plans created from now on (test only)
+
 bool bc_valid(int b) { return b == TPT_BC_NEUMANN || b == TPT_BC_DIRICHLET || b == TPT_BC_PERIODIC; }
 
 void free_plan(tpt_plan *p) {
@@ -355,11 +357,11 @@ int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double
         };
         if (fx) rc = setup_fft(0, nx, xf, bc[0], x_scale, p->lamx);
         if (rc == TPT_OK && fy) rc = setup_fft(1, ny, yf, bc[1], y_scale, p->lamy);
-        if (rc == TPT_OK && use_x && !fx && tpt::eigen_decompose(ox, p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
+        if (rc == TPT_OK && use_x && !fx && tpt::eigen_decompose(ox, p->lamx, p->qx, g_eigen_base) != 0) rc = TPT_ENUMERIC;
         if (rc == TPT_OK && use_y && !fy) {
             bool same = (use_x && !fx && nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
             if (same) { p->lamy = p->lamx; p->qy = p->qx; }
-            else if (tpt::eigen_decompose(oy, p->lamy, p->qy) != 0) rc = TPT_ENUMERIC;
+            else if (tpt::eigen_decompose(oy, p->lamy, p->qy, g_eigen_base) != 0) rc = TPT_ENUMERIC;
         }
         if (rc == TPT_OK && use_x && !fx) {
             std::vector<double> m((size_t)nx * nx);
@@ -674,6 +676,30 @@ int tpt_plan_get_eigen(const tpt_plan *p, int dir, double *lambda_host, double *
 
 int tpt_plan_is_singular(const tpt_plan *p) { return p ? p->singular : TPT_EINVAL; }
 
+int tpt_host_eigen(int n, const double *faces, int bc, int base_kind, double *lambda_host, double *qtilde_host) {
+    if (!tpt::faces_valid(n, faces) || !bc_valid(bc) || (bc == TPT_BC_PERIODIC && n < 3)) return TPT_EINVAL;
+    if (base_kind != 0 && base_kind != 1) return TPT_EINVAL;
+    try {
+        tpt::Operator1D op;
+        tpt::build_operator(n, faces, bc, op);
+        std::vector<double> lam, q;
+        if (tpt::eigen_decompose(op, lam, q, base_kind) != 0) return TPT_ENUMERIC;
+        if (lambda_host) std::memcpy(lambda_host, lam.data(), lam.size() * sizeof(double));
+        if (qtilde_host) std::memcpy(qtilde_host, q.data(), q.size() * sizeof(double));
+    } catch (const std::bad_alloc &) {
+        return TPT_ENOMEM;
+    } catch (...) {
+        return TPT_ENUMERIC;
+    }
+    return TPT_OK;
+}
+
+int tpt_debug_set_eigen_base(int base_kind) {
+    if (base_kind != 0 && base_kind != 1) return TPT_EINVAL;
+    g_eigen_base = base_kind;
+    return TPT_OK;
+}
+
 int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
     if (!p || !bytes_out) return TPT_EINVAL;
     size_t b = 2 * ((size_t)p->nx * p->nx + (size_t)p->ny * p->ny) * sizeof(double);
@@ -734,6 +760,13 @@ int tpt_plan_set_gemm_variant(tpt_plan *p, int variant) {
 int tpt_plan_set_thomas_variant(tpt_plan *p, int variant) {
     if (!p || (variant != 0 && variant != 1)) return TPT_EINVAL;
     p->thomas_variant = variant;
+    return TPT_OK;
+}
+
+int tpt_fill_uniform(double *out_dev, size_t count, unsigned long long seed, unsigned long long offset, void *cuda_stream) {
+    if ((!out_dev && count) || !aligned8(out_dev)) return TPT_EINVAL;
+    cudaError_t e = tpt::launch_fill_uniform(out_dev, count, seed, offset, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
     return TPT_OK;
 }
 

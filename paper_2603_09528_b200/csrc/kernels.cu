@@ -357,6 +357,33 @@ cudaError_t launch_gauge(double *x, const double *wz, size_t stride, int nz, cud
 }
 
 // ------------------------------------------------------------------------------------------------
+// Seeded white-noise input generator on the device (the same counter-based recipe as
+// paper_2603_09528_b200/inputs.py, restated): element t = 2u - 1 with u the top 53 bits of the splitmix64
+// finaliser of (offset + t + (seed + 1) * 0x9E3779B97F4A7C15).  No solver arithmetic.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fill_uniform_kernel(double *out, size_t count, unsigned long long base) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
+        unsigned long long z = base + t;
+        z ^= z >> 30;
+        z *= 0xBF58476D1CE4E5B9ull;
+        z ^= z >> 27;
+        z *= 0x94D049BB133111EBull;
+        z ^= z >> 31;
+        out[t] = (double)(z >> 11) * 0x1.0p-52 - 1.0;
+    }
+}
+
+cudaError_t launch_fill_uniform(double *out, size_t count, unsigned long long seed, unsigned long long offset, cudaStream_t stream) {
+    if (count == 0) return cudaSuccess;
+    const unsigned long long base = (seed + 1ull) * 0x9E3779B97F4A7C15ull + offset;
+    size_t blocks = (count + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    fill_uniform_kernel<<<(unsigned)blocks, 256, 0, stream>>>(out, count, base);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
 // FP64 pipe microbenchmarks (roofline denominators; MEASURED_PEAKS.json has no FP64 entry).
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(512) peak_dfma_kernel(double *out, int iters, double x, double y) {

@@ -98,6 +98,9 @@ void fft_tables(int n, std::vector<double> &out);            // e^{-i pi k/2n} (
 cudaError_t fft_configure();
 cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream);
 
+// Seeded uniform[-1,1) white noise, element t a pure function of (seed, offset + t): the input recipe of DESIGN.md §4.
+cudaError_t launch_fill_uniform(double *out, size_t count, unsigned long long seed, unsigned long long offset, cudaStream_t stream);
+
 // FP64 pipe microbenchmarks (kind 0: DFMA, 1: DMMA).  Returns TFLOP/s.
 cudaError_t run_fp64_peak(int kind, double *tflops);
 

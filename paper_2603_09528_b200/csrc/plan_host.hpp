@@ -27,6 +27,8 @@ void build_operator(int n, const double *xf, int bc, Operator1D &op);
 // q[n*n] row-major with q[i*n+m] = component i of mode m; Neumann null pair set analytically;
 // sign convention sum_i q_im sqrt(w_i) >= 0.  Returns 0 on success, <0 if QL failed to converge or
 // the refined basis misses the accuracy rule (orthogonality defect > 1e-11).
-int eigen_decompose(const Operator1D &op, std::vector<double> &lambda, std::vector<double> &q);
+// base_kind: 0 = implicit QL with the local relative deflation test (the plan's solver); 1 = the same iteration with a
+// deliberately crude normwise deflation test (test only: the refinement must absorb the difference).
+int eigen_decompose(const Operator1D &op, std::vector<double> &lambda, std::vector<double> &q, int base_kind = 0);
 
 }  // namespace tpt
