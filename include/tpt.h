@@ -185,6 +185,74 @@ int tpt_project(tpt_plan *plan, double *u_dev, double *v_dev, double *w_dev, dou
 /* tpt_plan_destroy — frees everything the plan owns (synchronises the device). NULL is a no-op. */
 int tpt_plan_destroy(tpt_plan *plan);
 
+/* ---- the solve sharded across the GPUs of one NVLink domain ------------------------------------------
+ *
+ * PAPER.md:197-207 (pencil layouts, collective transposes between them), Algorithm 1 steps 2, 4, 6, 8.
+ * The paper moves the field between x-, y- and z-aligned pencils with four all-to-alls per solve.  Here rank r of
+ * nranks (<= 8, one process per GPU) owns
+ *   - the z-SLAB [k0, k1) of the physical field: rhs and solution are nx*ny*(k1-k0) doubles, element (i, j, k - k0) at
+ *     i + nx*(j + ny*(k - k0)).  Steps 2.1, 2.2, 2.4, 2.5 act plane by plane, so both transforms are local to a slab;
+ *   - the y-MODE rows [m0, m1) (all kx, all z) of the mode-space field, on which it runs step 2.3.
+ * The two remaining exchanges are the STORES of kernels that touch the data anyway: the forward-y GEMM's epilogue writes
+ * each mode row into its owner's memory, the z sweep's TMA store writes each z-range of a solved tile into its slab
+ * owner's memory — peer-mapped pointers over NVLink, no pack/unpack kernel, no collective.  Per solve a rank sends
+ * nvlink_bytes_per_solve bytes (2 * 8 * nx * (m1-m0) * (nz - (k1-k0))), two device-side flag barriers order the phases.
+ *
+ * Shapes: nx, ny multiples of 128; 2*nranks <= nz <= 1056; ny/16 >= nranks; x and y by GEMM or (x only) fast transform;
+ * bc and alpha as tpt_plan_create (periodic z: TPT_EINVAL); anything else TPT_EINVAL.  Slab boundaries are even numbers.
+ *
+ * tpt_shard_layout      HOST only, needs no device: the split every rank computes identically.
+ * tpt_shard_create      plan-time setup of rank `rank` on the current device (full-grid eigenproblems: every rank solves
+ *                       the same ones — they are tiny beside a solve and avoid a broadcast) + one "symmetric" allocation
+ *                       of sym_bytes: [mode buffer | slab buffer | signal pad], same offsets on every rank.
+ * tpt_shard_sym         that allocation (DEVICE pointer) and its size.
+ * tpt_shard_set_peers   sym_dev[r] = rank r's allocation as addressable from THIS device (HOST array of nranks DEVICE
+ *                       pointers): same-process peers ("virtual ranks" on one device, or cudaDeviceEnablePeerAccess), or
+ *                       pointers the caller mapped itself.  sym_dev[rank] must be the shard's own.
+ * tpt_shard_ipc_export  writes the TPT_IPC_HANDLE_BYTES-byte CUDA IPC handle of the allocation to handle_out (HOST);
+ * tpt_shard_ipc_import  takes the nranks handles (HOST, rank-major, own entry ignored) all-gathered by the caller over
+ *                       its own control plane (torch.distributed) and maps the peers; closes them at destroy.
+ * tpt_solve_sharded     the whole solve of this rank's slab: rhs_slab_dev -> out_slab_dev (DEVICE, 16-byte aligned, may
+ *                       alias), asynchronous on cuda_stream.  EVERY rank must call it the same number of times; the
+ *                       barrier kernels spin until all ranks arrive (so all ranks' kernels must be able to run
+ *                       concurrently: one GPU per rank).
+ * tpt_shard_solve_phase one phase without any waiting kernel (0: steps 2.1-2.2 + exchange 1; 1: step 2.3 + exchange 2;
+ *                       2: steps 2.4-2.5), for callers that order the phases themselves — run phase p of every rank, then
+ *                       phase p+1 (virtual ranks sharing one device and stream, the tests' setting).  Unused slab
+ *                       arguments may be NULL.
+ * tpt_shard_barrier     one flag barrier on cuda_stream (exposed for tests and for callers composing their own phases).
+ * tpt_shard_barrier_all  the flag barrier of ALL n = nranks virtual ranks of one device (shards[r] = rank r, peers set to one
+ *                       another's allocations) as ONE cooperative launch, block r acting as rank r — kernels that wait on
+ *                       one another must not be separate launches on one GPU.  HOST array of handles.  Test / one-GPU use.
+ * tpt_shard_launches    kernels the last solve / phase call launched.
+ * tpt_shard_destroy     synchronises, unmaps peers, frees.  Call it on every rank only after all ranks' solves are done.
+ */
+#define TPT_IPC_HANDLE_BYTES 64
+typedef struct tpt_shard tpt_shard; /* opaque */
+typedef struct tpt_shard_layout_t {
+    int rank, nranks;
+    int k0, k1;                     /* owned z-planes */
+    int m0, m1;                     /* owned y-mode rows */
+    size_t mode_bytes, slab_bytes;  /* the two parts of the symmetric allocation (sized for the largest rank) */
+    size_t sym_bytes;
+    size_t slab_points;             /* nx * ny * (k1 - k0) */
+    size_t nvlink_bytes_per_solve;  /* bytes this rank writes into OTHER ranks' memory per solve (both exchanges) */
+} tpt_shard_layout_t;
+int tpt_shard_layout(int nranks, int rank, int nx, int ny, int nz, tpt_shard_layout_t *out);
+int tpt_shard_create(tpt_shard **shard_out, int rank, int nranks, int nx, int ny, int nz, const double *xf, const double *yf,
+                     const double *zf, const int bc[3], double helmholtz_alpha, int transform_x);
+int tpt_shard_get_layout(const tpt_shard *shard, tpt_shard_layout_t *out);
+int tpt_shard_sym(const tpt_shard *shard, void **sym_dev_out, size_t *bytes_out);
+int tpt_shard_set_peers(tpt_shard *shard, void *const *sym_dev);
+int tpt_shard_ipc_export(const tpt_shard *shard, void *handle_out);
+int tpt_shard_ipc_import(tpt_shard *shard, const void *handles);
+int tpt_solve_sharded(tpt_shard *shard, const double *rhs_slab_dev, double *out_slab_dev, void *cuda_stream);
+int tpt_shard_solve_phase(tpt_shard *shard, int phase, const double *rhs_slab_dev, double *out_slab_dev, void *cuda_stream);
+int tpt_shard_barrier(tpt_shard *shard, void *cuda_stream);
+int tpt_shard_barrier_all(tpt_shard *const *shards, int n, void *cuda_stream);
+int tpt_shard_launches(const tpt_shard *shard);
+int tpt_shard_destroy(tpt_shard *shard);
+
 /* ---- inspection / test entry points ------------------------------------------------------------ */
 
 /* Eigen-decomposition of direction dir (0 = x, 1 = y) as used by the plan: lambda_host[n]

@@ -31,7 +31,18 @@ SYMBOLS = (
     "tpt_plan_get_kernel_times", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
     "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_fill_uniform",
+    "tpt_shard_layout", "tpt_shard_create", "tpt_shard_get_layout", "tpt_shard_sym", "tpt_shard_set_peers", "tpt_shard_ipc_export",
+    "tpt_shard_ipc_import", "tpt_solve_sharded", "tpt_shard_solve_phase", "tpt_shard_barrier", "tpt_shard_barrier_all", "tpt_shard_launches", "tpt_shard_destroy",
 )
+IPC_HANDLE_BYTES = 64
+
+
+class ShardLayout(C.Structure):
+    """tpt_shard_layout_t of include/tpt.h."""
+    _fields_ = [("rank", C.c_int), ("nranks", C.c_int), ("k0", C.c_int), ("k1", C.c_int), ("m0", C.c_int), ("m1", C.c_int),
+                ("mode_bytes", C.c_size_t), ("slab_bytes", C.c_size_t), ("sym_bytes", C.c_size_t), ("slab_points", C.c_size_t),
+                ("nvlink_bytes_per_solve", C.c_size_t)]
+
 
 _dp = C.POINTER(C.c_double)
 _lib = None
@@ -78,6 +89,19 @@ def lib():
         L.tpt_plan_set_thomas_variant.argtypes = [vp, i]
         L.tpt_fp64_peak.argtypes = [i, _dp]
         L.tpt_fill_uniform.argtypes = [vp, C.c_size_t, C.c_ulonglong, C.c_ulonglong, vp]
+        L.tpt_shard_layout.argtypes = [i, i, i, i, i, C.POINTER(ShardLayout)]
+        L.tpt_shard_create.argtypes = [C.POINTER(vp), i, i, i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i]
+        L.tpt_shard_get_layout.argtypes = [vp, C.POINTER(ShardLayout)]
+        L.tpt_shard_sym.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_size_t)]
+        L.tpt_shard_set_peers.argtypes = [vp, C.POINTER(vp)]
+        L.tpt_shard_ipc_export.argtypes = [vp, vp]
+        L.tpt_shard_ipc_import.argtypes = [vp, vp]
+        L.tpt_solve_sharded.argtypes = [vp, vp, vp, vp]
+        L.tpt_shard_solve_phase.argtypes = [vp, i, vp, vp, vp]
+        L.tpt_shard_barrier.argtypes = [vp, vp]
+        L.tpt_shard_barrier_all.argtypes = [C.POINTER(vp), i, vp]
+        L.tpt_shard_launches.argtypes = [vp]
+        L.tpt_shard_destroy.argtypes = [vp]
         L.tpt_strerror.argtypes = [i]
         L.tpt_strerror.restype = C.c_char_p
         L.tpt_version.argtypes = []
@@ -303,6 +327,120 @@ def project(plan: Plan, u, v, w, gamma_dt: float, phi, p=None, alpha_p: float = 
 
 def plan_destroy(plan: Plan):
     plan.destroy()
+
+
+# ---- sharded solve (include/tpt.h "the solve sharded across the GPUs of one NVLink domain") ----------
+
+def shard_layout(nranks: int, rank: int, nx: int, ny: int, nz: int) -> ShardLayout:
+    """The z-slab / y-mode split of rank `rank` (host only, needs no device)."""
+    lay = ShardLayout()
+    _check(lib().tpt_shard_layout(int(nranks), int(rank), nx, ny, nz, C.byref(lay)), "tpt_shard_layout")
+    return lay
+
+
+class Shard:
+    """Handle of a tpt_shard: rank `rank` of a solve sharded over `nranks` GPUs.  rhs / out are this rank's z-slab,
+    float64 CUDA tensors of nx*ny*(k1-k0) elements, shape (k1-k0, ny, nx)."""
+
+    def __init__(self, handle, nx, ny, nz):
+        self._h = handle
+        self.nx, self.ny, self.nz = nx, ny, nz
+        lay = ShardLayout()
+        _check(lib().tpt_shard_get_layout(handle, C.byref(lay)), "tpt_shard_get_layout")
+        self.layout = lay
+
+    @property
+    def slab_shape(self):
+        return (self.layout.k1 - self.layout.k0, self.ny, self.nx)
+
+    @property
+    def slab_points(self) -> int:
+        return int(self.layout.slab_points)
+
+    def sym(self):
+        """(device pointer, bytes) of the symmetric allocation."""
+        ptr, n = C.c_void_p(), C.c_size_t()
+        _check(lib().tpt_shard_sym(self._h, C.byref(ptr), C.byref(n)), "tpt_shard_sym")
+        return int(ptr.value), int(n.value)
+
+    def set_peers(self, sym_ptrs):
+        arr = (C.c_void_p * len(sym_ptrs))(*[C.c_void_p(int(q)) for q in sym_ptrs])
+        _check(lib().tpt_shard_set_peers(self._h, arr), "tpt_shard_set_peers")
+
+    def ipc_export(self) -> bytes:
+        buf = C.create_string_buffer(IPC_HANDLE_BYTES)
+        _check(lib().tpt_shard_ipc_export(self._h, buf), "tpt_shard_ipc_export")
+        return buf.raw
+
+    def ipc_import(self, handles):
+        """handles: the nranks exported handles in rank order (bytes each)."""
+        blob = b"".join(bytes(h) for h in handles)
+        if len(blob) != IPC_HANDLE_BYTES * self.layout.nranks:
+            raise ValueError("need one IPC handle per rank")
+        _check(lib().tpt_shard_ipc_import(self._h, C.c_char_p(blob)), "tpt_shard_ipc_import")
+
+    def _slab(self, t, what):
+        return None if t is None else _dev_ptr(t, self.slab_points, what)
+
+    def solve(self, rhs, out, stream=None):
+        """The whole sharded solve of this rank's slab; every rank must call it (device-side barriers)."""
+        _check(lib().tpt_solve_sharded(self._h, self._slab(rhs, "rhs"), self._slab(out, "out"), _stream_handle(stream)),
+               "tpt_solve_sharded")
+        return out
+
+    def solve_phase(self, phase: int, rhs=None, out=None, stream=None):
+        """One phase (0 forward + exchange 1, 1 sweep + exchange 2, 2 inverse) without any waiting kernel."""
+        _check(lib().tpt_shard_solve_phase(self._h, int(phase), self._slab(rhs, "rhs"), self._slab(out, "out"),
+                                           _stream_handle(stream)), "tpt_shard_solve_phase")
+
+    def barrier(self, stream=None):
+        _check(lib().tpt_shard_barrier(self._h, _stream_handle(stream)), "tpt_shard_barrier")
+
+    def launches(self) -> int:
+        return int(lib().tpt_shard_launches(self._h))
+
+    def destroy(self):
+        if self._h is not None:
+            h, self._h = self._h, None
+            _check(lib().tpt_shard_destroy(h), "tpt_shard_destroy")
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def shard_create(rank: int, nranks: int, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0,
+                 transform_x: int = TRANSFORM_GEMM) -> Shard:
+    xa, xp = _faces(xf)
+    ya, yp = _faces(yf)
+    za, zp = _faces(zf)
+    if (xa.size, ya.size, za.size) != (nx + 1, ny + 1, nz + 1):
+        raise ValueError("face arrays must have n+1 entries per direction")
+    bca = (C.c_int * 3)(*[int(b) for b in bc])
+    h = C.c_void_p()
+    _check(lib().tpt_shard_create(C.byref(h), int(rank), int(nranks), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha),
+                                  int(transform_x)), "tpt_shard_create")
+    return Shard(h, nx, ny, nz)
+
+
+def shard_barrier_all(shards, stream=None):
+    """The flag barrier of all virtual ranks of one device as one cooperative launch (tpt_shard_barrier_all)."""
+    arr = (C.c_void_p * len(shards))(*[s._h for s in shards])
+    _check(lib().tpt_shard_barrier_all(arr, len(shards), _stream_handle(stream)), "tpt_shard_barrier_all")
+
+
+def virtual_ranks_solve(shards, rhs_slabs, out_slabs, stream=None, barriers: bool = False):
+    """Sharded solve with all ranks living on ONE device (virtual ranks): phase p of every rank, then phase p+1, on one
+    stream — stream order stands in for the two flag barriers (barriers=True runs them as well, all ranks in one
+    cooperative launch).  Pure call ordering; no arithmetic."""
+    for ph in range(3):
+        for s, r, o in zip(shards, rhs_slabs, out_slabs):
+            s.solve_phase(ph, r if ph == 0 else None, o if ph == 2 else None, stream)
+        if barriers and ph < 2:
+            shard_barrier_all(shards, stream)
+    return out_slabs
 
 
 def host_eigen(faces, bc: int, base_kind: int = 0):

@@ -6,57 +6,46 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <deque>
+#include <mutex>
 #include <new>
 #include <vector>
 
 #include "kernels.cuh"
+#include "plan.hpp"
 #include "plan_host.hpp"
-
-struct tpt_plan {
-    int nx = 0, ny = 0, nz = 0;
-    int bc[3] = {0, 0, 0};
-    double alpha = 0.0;
-    int singular = 0;
-    int dirs = TPT_DIRS_XYZ;      // implicitly treated directions: bit 0 = x, 1 = y, 2 = z
-    int work_fields = 1;          // fields the workspace holds (tpt_plan_reserve_batch)
-    int device = 0;
-    double shift0 = 0.0;          // 0 (Poisson) or -1/alpha (Helmholtz, A5)
-    int transform[2] = {0, 0};    // per diagonalised direction: TPT_TRANSFORM_GEMM / TPT_TRANSFORM_FFT (uniform directions)
-    double fft_s[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};   // [dir]: forward s0, s1, inverse s0, s1 (fft.cu)
-    double *d_fft[2] = {nullptr, nullptr};   // twiddle tables
-    int gemm_variant = 2;
-    int thomas_variant = 1;       // 1 = on-chip partitioned kernel where supported, 0 = streaming kernel
-    int sms = 0;
-    int profiling = 0;
-    int launches_last = 0;
-    std::vector<double> lamx, lamy, qx, qy;   // host copies (inspection)
-    // device: pre-scaled transform matrices, all row-major
-    double *d_xfwd = nullptr;   // [i][m]  = s * sqrt(wx_i) Q~x[i][m]      B-operand of step 2.1
-    double *d_xinv = nullptr;   // [m][i]  = Q~x[i][m] / sqrt(wx_i)         B-operand of step 2.5
-    double *d_yfwd = nullptr;   // [m][j]  = sqrt(wy_j) Q~y[j][m]           A-operand of step 2.2
-    double *d_yinv = nullptr;   // [j][m]  = Q~y[j][m] / sqrt(wy_j)         A-operand of step 2.4
-    double *d_vec = nullptr;    // lamx | lamy | az | bz | cz | wz
-    double *d_geo = nullptr;    // rwx | gfx | rwy | gfy | rwz | gfz: 1/width per cell, 1/centre spacing per face (projection.cu)
-    tpt::ProjGeom geo{};
-    double *d_abc = nullptr;    // coefficient tables of the on-chip Thomas kernel (thomas_onchip_tables)
-    double *d_lamx = nullptr, *d_lamy = nullptr, *d_az = nullptr, *d_bz = nullptr, *d_cz = nullptr, *d_wz = nullptr;
-    double *d_work = nullptr;   // one field
-    double *d_stage = nullptr;  // staging field for tpt_solve_host (lazy)
-    // tpt_solve_host pipeline (lazy): copy streams and per-slab events
-    cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
-    cudaEvent_t ev_start = nullptr, ev_done = nullptr;
-    std::vector<cudaEvent_t> ev_slab;   // 2 per z-slab: slab arrived, slab ready to leave
-    bool host_ready = false;            // all of the above exist (set last, tpt_solve_host_async)
-    // profiling: one set of TPT_K_COUNT+1 events per profiled solve since the last read-out
-    std::vector<cudaEvent_t> ev_pool;
-    size_t ev_used = 0;           // events handed out since the last read-out
-    long launches_accum = 0;
-    size_t points() const { return (size_t)nx * ny * nz; }
-};
 
 namespace {
 
 int g_eigen_base = 0;   // tpt_debug_set_eigen_base: base eigen-solver of plans created from now on (test only)
+
+// Plan-time eigen-decompositions are O(N^3) host work and depend only on (faces, bc): the last few are kept, so that
+// a second plan on the same grid (the two plans of a config-5 step, the e2e double buffer, the P shards of a sharded
+// plan in one process) does not repeat them ("reused for every right-hand side").
+struct EigenEntry {
+    int n, bc, base;
+    std::vector<double> faces, lam, q;
+};
+std::mutex g_eigen_mutex;
+std::deque<EigenEntry> g_eigen_cache;
+
+int cached_eigen(const tpt::Operator1D &op, int n, const double *faces, int bc, std::vector<double> &lam, std::vector<double> &q) {
+    {
+        std::lock_guard<std::mutex> lock(g_eigen_mutex);
+        for (const EigenEntry &e : g_eigen_cache)
+            if (e.n == n && e.bc == bc && e.base == g_eigen_base && std::memcmp(e.faces.data(), faces, sizeof(double) * (n + 1)) == 0) {
+                lam = e.lam;
+                q = e.q;
+                return 0;
+            }
+    }
+    const int rc = tpt::eigen_decompose(op, lam, q, g_eigen_base);
+    if (rc != 0) return rc;
+    std::lock_guard<std::mutex> lock(g_eigen_mutex);
+    g_eigen_cache.push_front(EigenEntry{n, bc, g_eigen_base, std::vector<double>(faces, faces + n + 1), lam, q});
+    if (g_eigen_cache.size() > 4) g_eigen_cache.pop_back();
+    return 0;
+}
 
 bool bc_valid(int b) { return b == TPT_BC_NEUMANN || b == TPT_BC_DIRICHLET || b == TPT_BC_PERIODIC; }
 
@@ -140,20 +129,22 @@ bool use_blocked(const tpt_plan *p) {
 // Step 2.3 on one field: in -> out (in == out allowed); `scratch` is a free field (used by the streaming kernel only).
 int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches, bool blocked = false,
                bool blocked_shape = false) {
-    cudaError_t e;
     if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) {
-        e = tpt::launch_thomas_onchip(in, out, p->d_abc, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz, p->shift0,
-                                      p->singular, blocked, blocked_shape, p->sms, st);
-    } else {   // streaming kernel: in place on `out`, c' spilled to `scratch`
-        if (blocked) return TPT_ECUDA;
-        if (in != out && cudaMemcpyAsync(out, in, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
-            return TPT_ECUDA;
-        e = tpt::launch_thomas(out, scratch, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
-                               p->shift0, p->singular, st);
+        // on-chip kernel; the null-mode gauge of a singular plan is fused into it
+        cudaError_t e = tpt::launch_thomas_onchip(in, out, p->d_abc, p->d_lamx, p->d_lamy, p->d_wz, p->nx, p->ny, p->nz, p->shift0,
+                                                  p->singular, blocked, blocked_shape, p->sms, st);
+        ++*launches;
+        return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
     }
+    // streaming kernel: in place on `out`, c' spilled to `scratch`; separate gauge kernel
+    if (blocked) return TPT_ECUDA;
+    if (in != out && cudaMemcpyAsync(out, in, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return TPT_ECUDA;
+    cudaError_t e = tpt::launch_thomas(out, scratch, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
+                                       p->shift0, p->singular, st);
     ++*launches;
     if (e == cudaSuccess && p->singular) {
-        e = tpt::launch_gauge(out, p->d_wz, blocked ? (size_t)16 : (size_t)p->nx * p->ny, p->nz, st);
+        e = tpt::launch_gauge(out, p->d_wz, (size_t)p->nx * p->ny, p->nz, st);
         ++*launches;
     }
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
@@ -244,6 +235,23 @@ bool on_plan_device(const tpt_plan *p) {
 
 }  // namespace
 
+namespace tpt {
+namespace detail {
+GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *mat, int k0, int nk) {
+    return ::gemm_x(p, in, out, mat, k0, nk);
+}
+GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat, int k0, int nk, bool in_blocked,
+                bool out_blocked) {
+    return ::gemm_y(p, in, out, mat, k0, nk, in_blocked, out_blocked);
+}
+cudaError_t run_gemm(const tpt_plan *p, const GemmArgs &g, cudaStream_t st) { return ::run_gemm(p, g, st); }
+int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int k0, int nk, bool blocked) {
+    return ::run_slot(p, slot, in, out, st, launches, k0, nk, blocked);
+}
+bool on_plan_device(const tpt_plan *p) { return ::on_plan_device(p); }
+}  // namespace detail
+}  // namespace tpt
+
 extern "C" {
 
 int tpt_plan_create(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
@@ -268,6 +276,14 @@ static bool direction_uniform(int n, const double *f) {
 
 int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
                        const double *zf, const int bc[3], double helmholtz_alpha, int implicit_dirs, const int transform[2]) {
+    return tpt::detail::plan_create_sized(plan_out, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha, implicit_dirs, transform, 0);
+}
+
+}  // extern "C"
+
+int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, const double *xf, const double *yf,
+                                   const double *zf, const int bc[3], double helmholtz_alpha, int implicit_dirs,
+                                   const int transform[2], size_t work_points) {
     if (!plan_out || !bc || !transform) return TPT_EINVAL;
     for (int d = 0; d < 2; ++d)
         if (transform[d] != TPT_TRANSFORM_GEMM && transform[d] != TPT_TRANSFORM_FFT) return TPT_EINVAL;
@@ -357,11 +373,11 @@ int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double
         };
         if (fx) rc = setup_fft(0, nx, xf, bc[0], x_scale, p->lamx);
         if (rc == TPT_OK && fy) rc = setup_fft(1, ny, yf, bc[1], y_scale, p->lamy);
-        if (rc == TPT_OK && use_x && !fx && tpt::eigen_decompose(ox, p->lamx, p->qx, g_eigen_base) != 0) rc = TPT_ENUMERIC;
+        if (rc == TPT_OK && use_x && !fx && cached_eigen(ox, nx, xf, bc[0], p->lamx, p->qx) != 0) rc = TPT_ENUMERIC;
         if (rc == TPT_OK && use_y && !fy) {
             bool same = (use_x && !fx && nx == ny && bc[0] == bc[1] && std::memcmp(xf, yf, sizeof(double) * (nx + 1)) == 0);
             if (same) { p->lamy = p->lamx; p->qy = p->qx; }
-            else if (tpt::eigen_decompose(oy, p->lamy, p->qy, g_eigen_base) != 0) rc = TPT_ENUMERIC;
+            else if (cached_eigen(oy, ny, yf, bc[1], p->lamy, p->qy) != 0) rc = TPT_ENUMERIC;
         }
         if (rc == TPT_OK && use_x && !fx) {
             std::vector<double> m((size_t)nx * nx);
@@ -439,7 +455,7 @@ int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double
         rc = TPT_ECUDA;
     }
     if (rc == TPT_OK) {
-        cudaError_t e = cudaMalloc(&p->d_work, p->points() * sizeof(double));
+        cudaError_t e = cudaMalloc(&p->d_work, (work_points ? work_points : p->points()) * sizeof(double));
         if (e != cudaSuccess) { cudaGetLastError(); rc = (e == cudaErrorMemoryAllocation) ? TPT_ENOMEM : TPT_ECUDA; }
     }
     if (rc == TPT_OK && (tpt::gemm_configure() != cudaSuccess || tpt::gemm_tma_configure() != cudaSuccess ||
@@ -451,6 +467,8 @@ int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz, const double
     *plan_out = p;
     return TPT_OK;
 }
+
+extern "C" {
 
 int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_stream) {
     if (!p || !rhs_dev || !out_dev || !aligned16(rhs_dev) || !aligned16(out_dev) || !on_plan_device(p)) return TPT_EINVAL;

@@ -40,6 +40,10 @@ struct TmaGemmParams {
     int ntiles;          // tiles_mn * batch
     int a_batch_rows;    // rows of the A tensor per batch (0: shared by all batches)
     int b_batch_rows;    // rows of the B tensor per batch (0: shared)
+    // sharded solve: rows of C scattered to their owners' memory (GemmArgs::peerC); row m belongs to rank
+    // ((m/16 + 1) * npeers - 1) / units, the inverse of the unit split [units*q/npeers, units*(q+1)/npeers)
+    int npeers, units;
+    double *peerC[MAX_PEERS];
 };
 
 __global__ void __launch_bounds__(THREADS, 1)
@@ -156,14 +160,19 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         const int b = tile / p.tiles_mn;
         const int mn = tile - b * p.tiles_mn;
         const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
-        double *Cw = p.C + (int64_t)b * p.strideC + ((int64_t)mt * BM + wm0 + rho) * p.ldc +
-                     (int64_t)(nt * (BN / 16) + wn0 / 16) * p.ldg + ((t >> 1) << 1) + ((t & 1) << 3);
+        const int row0 = mt * BM + wm0 + rho;
+        const int64_t off = (int64_t)b * p.strideC + (int64_t)(nt * (BN / 16) + wn0 / 16) * p.ldg + ((t >> 1) << 1) + ((t & 1) << 3);
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 4; ++i) {
+            const int row = row0 + 8 * i;
+            // sharded solve: the owner of mode row `row` receives it straight from this epilogue (16-byte stores to
+            // peer-mapped memory travel over NVLink while the next tile's DMMAs run) — no pack kernel, no collective
+            double *base = p.npeers ? p.peerC[(((row >> 4) + 1) * p.npeers - 1) / p.units] : p.C;
+            double *Cw = base + off + (int64_t)row * p.ldc;
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                *reinterpret_cast<double2 *>(Cw + (int64_t)(8 * i) * p.ldc + (int64_t)(j >> 1) * p.ldg + (j & 1) * 4) =
-                    make_double2(acc[i][j][0], acc[i][j][1]);
+                *reinterpret_cast<double2 *>(Cw + (int64_t)(j >> 1) * p.ldg + (j & 1) * 4) = make_double2(acc[i][j][0], acc[i][j][1]);
+        }
     }
 }
 
@@ -175,6 +184,9 @@ bool gemm_tma_supported(const GemmArgs &g) {
     if (g.M % BM || g.N % BN || g.K % BK || g.K < BK) return false;
     if (g.lda % 2 || g.ldb % 2 || g.ldc % 2 || g.strideC % 2) return false;
     if (!aligned16(g.A) || !aligned16(g.B) || !aligned16(g.C)) return false;
+    if (g.npeers < 0 || g.npeers > MAX_PEERS) return false;
+    for (int q = 0; q < g.npeers; ++q)
+        if (!g.peerC[q] || !aligned16(g.peerC[q])) return false;
     // batches are folded into the row dimension of the operand tensors: a batched operand must be densely stacked
     if (g.batch > 1) {
         if (g.strideA != 0 && g.strideA != (int64_t)g.M * g.lda) return false;
@@ -226,6 +238,9 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
     p.ntiles = p.tiles_mn * g.batch;
     p.a_batch_rows = a_batched ? g.M : 0;
     p.b_batch_rows = b_batched ? g.K : 0;
+    p.npeers = g.npeers;
+    p.units = g.M / 16;
+    for (int q = 0; q < MAX_PEERS; ++q) p.peerC[q] = q < g.npeers ? g.peerC[q] : nullptr;
     const int grid = p.ntiles < sms ? p.ntiles : sms;
     gemm_tma_kernel<<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);
     return cudaGetLastError();

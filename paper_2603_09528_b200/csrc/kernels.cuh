@@ -10,6 +10,8 @@ namespace tpt {
 
 // Row-major batched GEMM  C[b] = A[b] * B[b],  A: M x K (lda), B: K x N (ldb), C: M x N (ldc),
 // batch strides in elements (0 = operand shared by all batches).
+constexpr int MAX_PEERS = 8;   // ranks of a sharded plan: one NVLink domain of 8 GPUs
+
 struct GemmArgs {
     const double *A;
     const double *B;
@@ -22,6 +24,12 @@ struct GemmArgs {
     // 0 or 16 = plain row-major.  Anything else is the tile-blocked mode-space layout of the y transforms (below);
     // only the TMA kernel (variant 2) takes it.
     int64_t ldgB = 0, ldgC = 0;
+    // Sharded solve (sharded.cu): the rows of C are owned by `npeers` ranks in blocks of 16-row units
+    // (rank q owns units [units*q/npeers, units*(q+1)/npeers), units = M/16); row m is then written through peerC[q]
+    // instead of C — a pointer into rank q's memory (peer-mapped over NVLink), with the owner's row offset and this
+    // rank's batch offset already folded in.  npeers == 0: plain single-destination C.  TMA kernel only.
+    int npeers = 0;
+    double *peerC[MAX_PEERS] = {};
 };
 
 // Tile-blocked layout of the mode-space field between steps 2.2 and 2.4 (the z sweep's input and output):
@@ -57,8 +65,25 @@ cudaError_t launch_thomas(double *x, double *cprime, const double *az, const dou
 constexpr int THOMAS_TABLE_PAD = 160;   // >= the rows by which S*M can exceed nz in any launch shape
 bool thomas_onchip_supported(int nx, int ny, int nz);
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out);
-cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
-                                 int nz, double shift0, int singular, bool blocked, bool blocked_shape, int sms, cudaStream_t stream);
+// wz: the nz cell widths of the z direction — on a singular plan the kernel itself removes the dz-weighted mean of the
+// null column (0,0) before the tile leaves the chip (A7): no separate gauge launch.
+cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, const double *wz,
+                                 int nx, int ny, int nz, double shift0, int singular, bool blocked, bool blocked_shape, int sms,
+                                 cudaStream_t stream);
+
+// Sharded solve (sharded.cu): the sweep over the `rows` y-modes this rank owns (field `in`: tile-blocked, rows * nx
+// columns, full nz), the solution rows [k0[r], k0[r+1]) of every tile stored into rank r's z-slab buffer slab[r]
+// (tile-blocked over ALL total_cols = nx*ny columns with that rank's nz_r rows; peer-mapped memory).
+struct ThomasPeers {
+    int npeers = 0;
+    int k0[MAX_PEERS + 1] = {};       // slab boundaries; k0[npeers] = nz; even (see launch_thomas_onchip_sharded)
+    double *slab[MAX_PEERS] = {};
+    size_t total_cols = 0;            // nx * ny
+    int group0 = 0;                   // (first owned row) * nx / 16
+};
+cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &peers, const double *tab, const double *lamx,
+                                         const double *lamy_owned, const double *wz, int nx, int rows, int nz, double shift0,
+                                         int singular, int sms, cudaStream_t stream);
 
 // Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean); `stride` = distance
 // between consecutive z levels of that column (nx*ny in the natural layout, 16 in the tile-blocked one).

@@ -22,6 +22,7 @@
 // dominant so no pivoting is needed, A13).  c'_t and g_t stay in registers, d_t / x_t in the tile.
 #include <cuda.h>
 
+#include <type_traits>
 #include <vector>
 
 #include "devonce.hpp"
@@ -33,13 +34,27 @@ namespace tpt {
 
 namespace {
 
-template <int M, int TCOLS, int MAXT, int MINB>
+// Destination of the solution tiles.  Plain solve: one tensor map over the output field.  Sharded solve (sharded.cu;
+// PAPER.md:197-207, Algorithm 1 step 6): rows [k0[r], k0[r+1]) of every tile belong to rank r, whose z-slab buffer
+// (tile-blocked, peer-mapped over NVLink) they are stored into directly — the transpose back to z-slabs is this
+// kernel's own TMA store, not a collective.
+struct StoreOne { CUtensorMap map; };
+struct StorePeers {
+    CUtensorMap map[MAX_PEERS];   // rank r's slab buffer as [16-column group][tile of the group][local z][columns]
+    int k0[MAX_PEERS + 1];        // z-slab boundaries (even numbers, so 8-column rows stay 128-byte aligned in shared memory)
+    int npeers;
+    int box_rows;                 // rows per store box
+    int group0;                   // index of this rank's first 16-column group in the peers' (global) group numbering
+};
+
+template <int M, int TCOLS, int MAXT, int MINB, bool SH>
 __global__ void __launch_bounds__(MAXT, MINB)
-thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_out,
+thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
+                     const __grid_constant__ typename std::conditional<SH, StorePeers, StoreOne>::type dst,
                      const double *__restrict__ tab_reg,
                      const double *__restrict__ tab_null, const double *__restrict__ lamx,
-                     const double *__restrict__ lamy, int nx, int nz, int S, int nbuf, int box_rows, int nbox,
-                     int buf_rows, double shift0, int singular, int ntiles) {
+                     const double *__restrict__ lamy, const double *__restrict__ wz, int nx, int nz, int S, int nbuf,
+                     int box_rows, int nbox, int buf_rows, double shift0, int singular, int ntiles) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const size_t tile_elems = (size_t)buf_rows * TCOLS;             // buf_rows = max(S*M, nbox*box_rows) >= nz
     double *bufs = reinterpret_cast<double *>(smem_raw);            // nbuf x tile_elems
@@ -54,7 +69,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
 
     if (tid == 0) {
         ptx::tma_prefetch_desc(&tmap);
-        ptx::tma_prefetch_desc(&tmap_out);
+        if constexpr (SH) {
+            for (int r = 0; r < dst.npeers; ++r) ptx::tma_prefetch_desc(&dst.map[r]);
+        } else {
+            ptx::tma_prefetch_desc(&dst.map);
+        }
         for (int b = 0; b < nbuf; ++b) ptx::mbar_init(&full[b], 1);
         ptx::fence_mbar_init();
     }
@@ -193,12 +212,47 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             xk = fma(-cp[t], xk, fma(-g[t], xl, buf[t * TCOLS]));
             buf[t * TCOLS] = xk;
         }
+        // ---- null-mode gauge (A7), fused: the tile that holds column (0,0) of a singular
+        // plan subtracts the dz-weighted mean of that column before it leaves the chip (block-uniform branch)
+        if (singular && tile == 0) {
+            __syncthreads();
+            double ps = 0.0, pl = 0.0;
+            if (col == 0) {
+#pragma unroll
+                for (int t = 0; t < M; ++t)
+                    if (k0 + t < nz) {
+                        const double w = __ldg(wz + k0 + t);
+                        ps = fma(w, buf[t * TCOLS], ps);
+                        pl += w;
+                    }
+            }
+            set0[me] = ps;
+            set0[STR + me] = pl;
+            __syncthreads();
+            double sum = 0.0, len = 0.0;
+            for (int q = 0; q < S; ++q) {
+                sum += set0[q * TCOLS];
+                len += set0[STR + q * TCOLS];
+            }
+            const double mean = sum / len;
+            if (col == 0) {
+#pragma unroll
+                for (int t = 0; t < M; ++t)
+                    if (k0 + t < nz) buf[t * TCOLS] -= mean;
+            }
+        }
         ptx::fence_proxy_async();
         __syncthreads();
         if (tid == 0) {                        // rows past nz are clipped by the tensor map
             const double *src = bufs + (size_t)b * tile_elems;
-            for (int q = 0; q < nbox; ++q)
-                ptx::tma_store_4d(&tmap_out, 0, q * box_rows, tile % SUB, tile / SUB, src + (size_t)q * box_rows * TCOLS);
+            if constexpr (SH) {
+                for (int r = 0; r < dst.npeers; ++r)
+                    for (int kk = dst.k0[r]; kk < dst.k0[r + 1]; kk += dst.box_rows)
+                        ptx::tma_store_4d(&dst.map[r], 0, kk - dst.k0[r], tile % SUB, dst.group0 + tile / SUB, src + (size_t)kk * TCOLS);
+            } else {
+                for (int q = 0; q < nbox; ++q)
+                    ptx::tma_store_4d(&dst.map, 0, q * box_rows, tile % SUB, tile / SUB, src + (size_t)q * box_rows * TCOLS);
+            }
             ptx::bulk_commit();
         }
         if (++b == nbuf) {
@@ -223,10 +277,13 @@ bool make_field_map(CUtensorMap *map, const double *x, size_t plane, int nz, int
 
 constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_CTA_RESERVED = 1024, SMEM_CTA_MAX = 227 * 1024;
 
-// M rows per segment, TC columns per tile, CTAS co-resident CTAs per SM (their barrier phases interleave).
+// Launch geometry shared by the plain and the sharded launch.
+struct ThomasGeom {
+    int S, nbox, box_rows, buf_rows, nbuf, threads;
+    size_t smem;
+};
 template <int M, int TC, int MAXT, int CTAS>
-cudaError_t launch_m(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny, int nz,
-                     double shift0, int singular, bool blocked, int sms, cudaStream_t stream) {
+bool thomas_geometry(int nz, ThomasGeom &g) {
     constexpr int ROW_BYTES = TC * (int)sizeof(double);
     int S = (nz + M - 1) / M;
     while ((S * TC) % 32) ++S;                               // whole warps
@@ -240,27 +297,59 @@ cudaError_t launch_m(const double *in, double *x, const double *tab, const doubl
     if (budget > SMEM_CTA_MAX) budget = SMEM_CTA_MAX;
     int nbuf = (int)((budget - fixed) / tile_bytes);
     if (nbuf > 3) nbuf = 3;
-    if (nbuf < 2) return cudaErrorInvalidConfiguration;
-    const size_t smem = (size_t)nbuf * tile_bytes + fixed;
-    auto kern = thomas_onchip_kernel<M, TC, MAXT, CTAS>;
+    if (nbuf < 2 || TC * S > MAXT) return false;
+    g = {S, nbox, box_rows, buf_rows, nbuf, TC * S, (size_t)nbuf * tile_bytes + fixed};
+    return true;
+}
+
+// M rows per segment, TC columns per tile, CTAS co-resident CTAs per SM (their barrier phases interleave).
+// `cols` = number of (kx,ky) columns of the field at `in` (nx*ny, or the rows a rank owns times nx).
+// peers == nullptr: plain solve into the field x (same layout as `in`); else the sharded store of StorePeers.
+template <int M, int TC, int MAXT, int CTAS, bool SH>
+cudaError_t launch_m(const double *in, double *x, const ThomasPeers *peers, const double *tab, const double *lamx, const double *lamy,
+                     const double *wz, int nx, size_t cols, int nz, double shift0, int singular, bool blocked, int sms, cudaStream_t stream) {
+    ThomasGeom g;
+    if (!thomas_geometry<M, TC, MAXT, CTAS>(nz, g)) return cudaErrorInvalidConfiguration;
+    auto kern = thomas_onchip_kernel<M, TC, MAXT, CTAS, SH>;
     static DeviceOnce configured;                            // per device, thread-safe (devonce.hpp)
     static OccupancyCache occupancy;
     cudaError_t e = configured.run([&] { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CTA_MAX); });
     if (e != cudaSuccess) return e;
-    const int threads = TC * S;
-    if (threads > MAXT) return cudaErrorInvalidConfiguration;
     int per_sm = 0;
-    e = occupancy.get(kern, threads, smem, &per_sm);
+    e = occupancy.get(kern, g.threads, g.smem, &per_sm);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorInvalidConfiguration;
-    CUtensorMap tmap, tmap_out;
-    if (!make_field_map(&tmap, in, (size_t)nx * ny, nz, TC, box_rows, blocked)) return cudaErrorUnknown;
-    if (!make_field_map(&tmap_out, x, (size_t)nx * ny, nz, TC, box_rows, blocked)) return cudaErrorUnknown;
-    const int ntiles = (int)(((size_t)nx * ny) / TC);
+    CUtensorMap tmap;
+    if (!make_field_map(&tmap, in, cols, nz, TC, g.box_rows, blocked)) return cudaErrorUnknown;
+    const int ntiles = (int)(cols / TC);
     int grid = sms * per_sm;
     if (grid > ntiles) grid = ntiles;
-    kern<<<grid, threads, smem, stream>>>(tmap, tmap_out, tab, tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD), lamx, lamy, nx, nz, S, nbuf,
-                                          box_rows, nbox, buf_rows, shift0, singular, ntiles);
+    const double *tab_null = tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD);
+    if constexpr (SH) {
+        StorePeers dst{};
+        dst.npeers = peers->npeers;
+        dst.group0 = peers->group0;
+        int longest = 0;
+        for (int r = 0; r <= peers->npeers; ++r) dst.k0[r] = peers->k0[r];
+        for (int r = 0; r < peers->npeers; ++r) longest = peers->k0[r + 1] - peers->k0[r] > longest ? peers->k0[r + 1] - peers->k0[r] : longest;
+        const int nb = (longest + 255) / 256;
+        dst.box_rows = (longest + nb - 1) / nb;
+        if (dst.box_rows & 1) ++dst.box_rows;                // even: 8-column rows stay 128-byte aligned in shared memory
+        if (dst.box_rows < 1) dst.box_rows = 2;
+        for (int r = 0; r < peers->npeers; ++r) {
+            const int nzl = peers->k0[r + 1] - peers->k0[r];
+            if (nzl <= 0) continue;                          // an empty slab receives nothing
+            if ((peers->k0[r] & 1) && TC < 16) return cudaErrorInvalidValue;
+            if (!make_field_map(&dst.map[r], peers->slab[r], peers->total_cols, nzl, TC, dst.box_rows, true)) return cudaErrorUnknown;
+        }
+        kern<<<grid, g.threads, g.smem, stream>>>(tmap, dst, tab, tab_null, lamx, lamy, wz, nx, nz, g.S, g.nbuf, g.box_rows, g.nbox,
+                                                  g.buf_rows, shift0, singular, ntiles);
+    } else {
+        StoreOne dst;
+        if (!make_field_map(&dst.map, x, cols, nz, TC, g.box_rows, blocked)) return cudaErrorUnknown;
+        kern<<<grid, g.threads, g.smem, stream>>>(tmap, dst, tab, tab_null, lamx, lamy, wz, nx, nz, g.S, g.nbuf, g.box_rows, g.nbox,
+                                                  g.buf_rows, shift0, singular, ntiles);
+    }
     return cudaGetLastError();
 }
 
@@ -270,10 +359,13 @@ bool thomas_onchip_supported(int nx, int ny, int nz) {
     return ((size_t)nx * ny) % 16 == 0 && nz >= 2 && nz <= 1056;
 }
 
-cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, int nx, int ny,
-                                 int nz, double shift0, int singular, bool blocked, bool blocked_shape, int sms, cudaStream_t stream) {
-    if (!thomas_onchip_supported(nx, ny, nz)) return cudaErrorInvalidValue;
-#define TPT_GO(M, TC, MAXT, CTAS) launch_m<M, TC, MAXT, CTAS>(in, x, tab, lamx, lamy, nx, ny, nz, shift0, singular, blocked, sms, stream)
+namespace {
+template <bool SH>
+cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, const double *tab, const double *lamx, const double *lamy,
+                     const double *wz, int nx, size_t cols, int nz, double shift0, int singular, bool blocked, bool blocked_shape,
+                     int sms, cudaStream_t stream) {
+#define TPT_GO(M, TC, MAXT, CTAS) \
+    launch_m<M, TC, MAXT, CTAS, SH>(in, x, peers, tab, lamx, lamy, wz, nx, cols, nz, shift0, singular, blocked, sms, stream)
     // Measured on the box (profiles/r1c_*.md): the sweep is bound by the FP64 + shared-memory pipes of the 16 warps the
     // register file admits per SM, so the shapes differ only in how well the phases of co-resident CTAs interleave.
     if (nz <= 128) return TPT_GO(8, 16, 256, 2);
@@ -289,6 +381,21 @@ cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab,
     // (33-row segments with 256 threads and 242 registers: 4.25 instead of 3.69 ms at 1024^3)
     return TPT_GO(17, 8, 512, 1);
 #undef TPT_GO
+}
+}  // namespace
+
+cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, const double *wz,
+                                 int nx, int ny, int nz, double shift0, int singular, bool blocked, bool blocked_shape, int sms,
+                                 cudaStream_t stream) {
+    if (!thomas_onchip_supported(nx, ny, nz)) return cudaErrorInvalidValue;
+    return dispatch<false>(in, x, nullptr, tab, lamx, lamy, wz, nx, (size_t)nx * ny, nz, shift0, singular, blocked, blocked_shape, sms, stream);
+}
+
+cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &peers, const double *tab, const double *lamx,
+                                         const double *lamy_owned, const double *wz, int nx, int rows, int nz, double shift0,
+                                         int singular, int sms, cudaStream_t stream) {
+    if (rows < 1 || nx % 16 || nz < 2 || nz > 1056 || peers.npeers < 1 || peers.npeers > MAX_PEERS) return cudaErrorInvalidValue;
+    return dispatch<true>(in, nullptr, &peers, tab, lamx, lamy_owned, wz, nx, (size_t)nx * rows, nz, shift0, singular, true, false, sms, stream);
 }
 
 // Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows

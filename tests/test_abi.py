@@ -102,3 +102,36 @@ def test_product_does_not_import_the_oracle():
             src = open(os.path.join(orc, f)).read()
             assert "paper_2603_09528_b200" not in src.replace("under paper_2603_09528_b200/", ""), f
             assert "tpt.h" not in src, f
+
+
+def test_shard_layout_partitions_planes_and_mode_rows():
+    # tpt_shard_layout is host-only: the z-slabs tile [0, nz) with even boundaries, the mode rows tile [0, ny) in units of
+    # 16, the symmetric allocation is sized for the largest rank, and the NVLink byte count is what leaves the rank
+    # (every element of the mode-space field crosses once per exchange, except the part that stays).
+    from paper_2603_09528_b200 import api
+
+    for (nx, ny, nz, P) in [(512, 512, 512, 8), (1024, 256, 512, 8), (128, 128, 21, 5), (256, 128, 35, 3), (128, 256, 300, 8),
+                            (128, 128, 16, 1), (768, 768, 768, 7), (1024, 1024, 1024, 8)]:
+        lays = [api.shard_layout(P, r, nx, ny, nz) for r in range(P)]
+        assert lays[0].k0 == 0 and lays[-1].k1 == nz and lays[0].m0 == 0 and lays[-1].m1 == ny
+        sent = 0
+        for r, l in enumerate(lays):
+            assert (l.rank, l.nranks) == (r, P)
+            assert l.k0 % 2 == 0 and l.k1 > l.k0 and l.m0 % 16 == 0 and l.m1 > l.m0 and (l.m1 - l.m0) % 16 == 0
+            if r:
+                assert l.k0 == lays[r - 1].k1 and l.m0 == lays[r - 1].m1
+            assert l.slab_points == nx * ny * (l.k1 - l.k0)
+            assert l.mode_bytes == 8 * nx * nz * max(q.m1 - q.m0 for q in lays)
+            assert l.slab_bytes == 8 * nx * ny * max(q.k1 - q.k0 for q in lays)
+            assert l.sym_bytes >= l.mode_bytes + l.slab_bytes and l.sym_bytes == lays[0].sym_bytes
+            assert l.nvlink_bytes_per_solve == 2 * 8 * nx * (l.m1 - l.m0) * (nz - (l.k1 - l.k0))
+            sent += l.nvlink_bytes_per_solve
+        # balanced to within one unit
+        assert max(q.k1 - q.k0 for q in lays) - min(q.k1 - q.k0 for q in lays) <= 2
+        assert max(q.m1 - q.m0 for q in lays) - min(q.m1 - q.m0 for q in lays) <= 16
+        if P > 1 and nz % (2 * P) == 0 and ny % (16 * P) == 0:
+            assert sent == 2 * 8 * nx * ny * nz * (P - 1) // P
+    for bad in [(9, 0, 128, 128, 64), (2, 2, 128, 128, 64), (2, 0, 96, 128, 64), (2, 0, 128, 192, 64), (8, 0, 128, 128, 12),
+                (2, 0, 128, 128, 2000)]:
+        with pytest.raises(api.TptError):
+            api.shard_layout(*bad)
