@@ -290,6 +290,129 @@ def measure_config(api, torch, name, fp64_peak, hbm_gbs, steps=6, warmup=3):
     return out
 
 
+def shard_slab(f, lay):
+    """This rank's z-slab of the (nz, ny, nx) field f (the field is distributed, each rank holds a part)."""
+    return np.ascontiguousarray(f[lay.k0:lay.k1])
+
+
+def exchange_ipc_handles(dist, shard):
+    """Control plane of the sharded solve: all-gather the CUDA IPC handles of the symmetric allocations (64 bytes per rank,
+    through torch.distributed's object collective — not a data-path collective) and map the peers."""
+    handles = [None] * dist.get_world_size()
+    dist.all_gather_object(handles, shard.ipc_export())
+    shard.ipc_import(handles)
+    return handles
+
+
+def sharded_strong_value(pts_step: int, steps: int, seconds: float) -> float:
+    """Strong scaling: the job is ONE workload whatever the number of ranks."""
+    return pts_step * steps / seconds / 1e9
+
+
+def measure_sharded(api, torch, dist, args, probs, rank, world, stream, barrier):
+    """the workload's solves sharded over the `world` GPUs (tpt_solve_sharded: two exchanges fused into the
+    forward-y GEMM epilogue and the sweep's TMA store, two flag barriers).  Strong scaling; device-timed, max over ranks.
+    Every rank also solves the same right-hand side on its own with the single-GPU plan and compares its slab bit by bit."""
+    shards, rhs, out, ok, nvl = [], [], [], True, 0
+    cache = {}
+    for P in probs:
+        key = (P.n, P.bc, P.alpha, P.beta, P.length)
+        if key not in cache:
+            xf, yf, zf = P.faces()
+            sh = api.shard_create(rank, world, *P.n, xf, yf, zf, P.bc, P.alpha, TRANSFORMS[args.transform][0])
+            exchange_ipc_handles(dist, sh)
+            cache[key] = sh
+        sh = cache[key]
+        shards.append(sh)
+        f = P.rhs()
+        rhs.append(torch.from_numpy(shard_slab(f, sh.layout)).cuda())
+        out.append(torch.empty_like(rhs[-1]))
+        nvl += int(sh.layout.nvlink_bytes_per_solve)
+        del f
+    barrier()
+
+    def step():
+        for sh, r, o in zip(shards, rhs, out):
+            sh.solve(r, o, stream)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = max_over_ranks(dist, e0.elapsed_time(e1), "cuda")
+    # parity of the sharded result with the single-GPU solve of the same right-hand side (first problem), slab by slab
+    P = probs[0]
+    xf, yf, zf = P.faces()
+    plan = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=(TRANSFORMS[args.transform][0], 0))
+    full = torch.from_numpy(P.rhs()).cuda()
+    api.solve(plan, full, full, stream)
+    torch.cuda.synchronize()
+    lay = shards[0].layout
+    ok = bool(torch.equal(full.view(P.n[2], P.n[1], P.n[0])[lay.k0:lay.k1].reshape(-1), out[0].reshape(-1)))
+    flag = torch.tensor([1 if ok else 0], device="cuda")
+    dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+    plan.destroy()
+    del full
+    barrier()
+    for sh in cache.values():
+        sh.destroy()
+    pts_step = sum(P.points for P in probs)
+    secs = ms * 1e-3
+    return {"what": "tpt_solve_sharded: z-slab + y-mode-row ownership, exchanges fused into the GEMM epilogue and the sweep's "
+                    "TMA store over NVLink peer memory (PAPER.md:197-207)",
+            "scaling": "strong", "ranks": world, "value": sharded_strong_value(pts_step, args.steps, secs), "unit": UNIT,
+            "ms_per_step": ms / args.steps, "nvlink_bytes_per_step_per_rank": nvl,
+            "nvlink_gbs_per_rank_per_direction": nvl / (ms / args.steps * 1e-3) / 1e9,
+            "launches_per_solve": 7, "matches_single_gpu_bitwise": bool(flag.item())}
+
+
+def measure_sharded_virtual(api, torch, P, nranks, stream, steps=5, warmup=3):
+    """One-GPU leg of SURVEY 8(f).4: `nranks` virtual ranks on this device (peer pointers = local pointers), phases ordered
+    by the stream.  All ranks' work runs on one GPU, so the time is comparable with one single-plan solve: the difference is
+    what the fused exchanges (scattered epilogue rows, per-owner TMA stores) cost on the device."""
+    xf, yf, zf = P.faces()
+    shards = [api.shard_create(r, nranks, *P.n, xf, yf, zf, P.bc, P.alpha) for r in range(nranks)]
+    syms = [sh.sym()[0] for sh in shards]
+    for sh in shards:
+        sh.set_peers(syms)
+    full = device_rhs(api, torch, P, stream).view(P.n[2], P.n[1], P.n[0])
+    rhs = [full[sh.layout.k0:sh.layout.k1].reshape(-1) for sh in shards]      # z-slabs are contiguous views
+    out = [torch.empty_like(r) for r in rhs]
+    for _ in range(warmup):
+        api.virtual_ranks_solve(shards, rhs, out, stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        api.virtual_ranks_solve(shards, rhs, out, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    plan = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha)
+    ref = torch.empty_like(full).reshape(-1)
+    api.solve(plan, full.reshape(-1), ref, stream)
+    torch.cuda.synchronize()
+    same = bool(torch.equal(torch.cat(out), ref))
+    e0.record(stream)
+    for _ in range(steps):
+        api.solve(plan, full.reshape(-1), ref, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_one = e0.elapsed_time(e1) / steps
+    plan.destroy()
+    for sh in shards:
+        sh.destroy()
+    return {"what": f"{nranks} virtual ranks of the sharded solve on one device ({P.name}); all ranks' kernels run on this GPU",
+            "virtual_ranks": nranks, "ms_per_solve_all_ranks": ms, "ms_single_plan_solve": ms_one,
+            "device_overhead_of_fused_exchanges": ms / ms_one - 1.0, "matches_single_plan_bitwise": same,
+            "launches": 5 * nranks}
+
+
 def run_gpu(args):
     import torch
 
@@ -406,6 +529,14 @@ def run_gpu(args):
         api.plan_destroy(pl)
     del pin_out
 
+    # ---- the same workload sharded over the ranks (strong scaling), beside the replica number
+    sharded = None
+    if world > 1 and not args.no_sharded:
+        try:
+            sharded = measure_sharded(api, torch, dist, args, probs, rank, world, stream, barrier)
+        except api.TptError as exc:      # e.g. a grid the sharded layout does not take: reported, never silently skipped
+            sharded = {"unavailable": str(exc)}
+
     # ---- widened row: one pressure projection (Eq. 2c-2e) = divergence + this solve + correction,
     # timed on the device on the workload's Poisson plan (outside the headline timed region; rank 0 only)
     projection = None
@@ -456,6 +587,11 @@ def run_gpu(args):
             torch.cuda.empty_cache()
             other_configs = {n: measure_config(api, torch, n, fp64_peak, peaks["hbm_gbs"])
                              for n in ("c1", "c2", "c3", "c4", "c5") if n != args.config}
+        if world == 1 and not args.no_sharded and args.transform == "gg":
+            try:
+                sharded = measure_sharded_virtual(api, torch, I.CONFIGS["c3"][0], 4, stream)
+            except api.TptError as exc:
+                sharded = {"unavailable": str(exc)}
         # per-kernel: mean event durations over the timed region (dominant plan = first)
         key0 = next(iter(kt))
         ms0, _ = kt[key0]
@@ -514,6 +650,7 @@ def run_gpu(args):
             "kernels": kernels,
             "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "note")},
             "other_configs": other_configs,
+            "sharded": sharded,
             "solve_ms_mean_20_fastest": float(np.mean(n20)) / len(probs), "solve_ms_min": per_step[0] / len(probs),
             "hbm_peak_gbs": peaks["hbm_gbs"], "peaks": peak_kind,
         }
@@ -536,6 +673,8 @@ def main():
                     help="transform type in x, y: g = eigenbasis GEMM (BASELINE metric), f = fast transform (uniform directions)")
     ap.add_argument("--no-other-configs", dest="no_other_configs", action="store_true",
                     help="skip the device-timed numbers of the other BASELINE configs (c1, c2, c4, c5)")
+    ap.add_argument("--no-sharded", dest="no_sharded", action="store_true",
+                    help="skip the sharded-solve leg (N > 1: strong scaling over the ranks; N = 1: four virtual ranks on one GPU)")
     ap.add_argument("--no-projection", dest="no_projection", action="store_true",
                     help="skip the (untimed-region) pressure-projection measurement")
     args = ap.parse_args()

@@ -66,3 +66,60 @@ def test_reference_arm_runs_on_rank0_only():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] == line["value"] > 0
     assert line["e2e"] == {"value": line["value"], "unit": "Gpts/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert line["vs_baseline"] is None and np.isfinite(line["ms_per_step"])
+
+
+class _FakeShard:
+    """Stands in for api.Shard on a CPU-only box: the host logic under test is the handle exchange, not CUDA."""
+
+    def __init__(self, rank):
+        self.rank, self.imported = rank, None
+
+    def ipc_export(self):
+        return bytes([self.rank]) * 64
+
+    def ipc_import(self, handles):
+        self.imported = list(handles)
+
+
+def _shard_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    from paper_2603_09528_b200 import api, inputs as I
+
+    sh = _FakeShard(rank)
+    bench.exchange_ipc_handles(dist, sh)
+    nx, ny, nz = 128, 128, 22
+    lay = api.shard_layout(world, rank, nx, ny, nz)            # host-only entry point of the library
+    f = I.uniform_pm1(3, nx * ny * nz).reshape(nz, ny, nx)
+    slab = bench.shard_slab(f, lay)
+    q.put((rank, [h[0] for h in sh.imported], lay.k0, lay.k1, slab.shape, float(slab.sum()), float(f.sum()),
+           int(lay.nvlink_bytes_per_solve)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_sharded_host_logic_gloo_world2():
+    # SURVEY 8(f).4 host side: IPC handles all-gathered in rank order on every rank; the z-slabs of the ranks tile the
+    # field; the byte count that crosses NVLink is 2 * 8 * pts * (P-1)/P over all ranks; strong-scaling value
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    a, b = out
+    assert a[1] == b[1] == [0, 1]
+    assert a[2] == 0 and a[3] == b[2] and b[3] == 22 and a[3] % 2 == 0
+    assert a[4] == (a[3], 128, 128) and b[4] == (22 - a[3], 128, 128)
+    assert abs(a[5] + b[5] - a[6]) < 1e-9
+    assert a[7] == 2 * 8 * 128 * 64 * (22 - a[3]) and b[7] == 2 * 8 * 128 * 64 * a[3]
+    assert a[7] + b[7] == 2 * 8 * 128 * 128 * 22 // 2
+
+    import bench
+
+    assert bench.sharded_strong_value(10 ** 9, 4, 2.0) == 2.0

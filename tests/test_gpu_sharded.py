@@ -177,3 +177,61 @@ def test_shard_argument_errors(tpt, torch):
     with pytest.raises(tpt.TptError):          # own entry must be the shard's own allocation
         s.set_peers([s.sym()[0] + 256, s.sym()[0]])
     s.destroy()
+
+
+def _ipc_worker(rank, world, port, q):
+    # One PROCESS per rank, as under torchrun — here both on GPU 0 (the box has one).  The peers' allocations are mapped
+    # through CUDA IPC exactly as bench.py --gpus N does it; the phases are ordered by HOST barriers (gloo) after a device
+    # synchronise, so no kernel ever waits on another process's kernel.
+    import os
+
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch
+    import torch.distributed as dist
+
+    import bench
+    from paper_2603_09528_b200 import api
+
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    P = I.Problem("ipc", (128, 128, 36), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, seed=11)
+    xf, yf, zf = P.faces()
+    sh = api.shard_create(rank, world, *P.n, xf, yf, zf, P.bc, P.alpha)
+    handles = bench.exchange_ipc_handles(dist, sh)
+    f = P.rhs()
+    rhs = torch.from_numpy(bench.shard_slab(f, sh.layout)).cuda()
+    out = torch.empty_like(rhs)
+    for _ in range(2):
+        for ph in range(3):
+            sh.solve_phase(ph, rhs if ph == 0 else None, out if ph == 2 else None)
+            torch.cuda.synchronize()
+            dist.barrier()
+    q.put((rank, sh.layout.k0, sh.layout.k1, out.cpu().numpy(), len(set(handles))))
+    dist.barrier()
+    sh.destroy()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_solve_across_processes_with_cuda_ipc(tpt, torch, orc, world):
+    import os
+
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29600 + os.getpid() % 2000 + world
+    procs = [ctx.Process(target=_ipc_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    P = I.Problem("ipc", (128, 128, 36), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, seed=11)
+    xf, yf, zf = P.faces()
+    ref = orc.OraclePlan(xf, yf, zf, P.bc, P.alpha).solve(P.rhs())
+    assert res[0][1] == 0 and res[-1][2] == P.n[2] and all(a[2] == b[1] for a, b in zip(res, res[1:]))
+    assert all(r[4] == world for r in res)                 # every rank saw `world` distinct handles
+    phi = np.concatenate([r[3].reshape(-1) for r in res]).reshape(ref.shape)
+    assert float(np.abs(phi - ref).max() / np.abs(ref).max()) <= PARITY_TOL
