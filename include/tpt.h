@@ -290,10 +290,26 @@ int tpt_plan_set_profiling(tpt_plan *plan, int enabled);
 int tpt_plan_get_kernel_times(tpt_plan *plan, float *ms_host, int *launches_out, int *solves_out);
 
 /* Select the GEMM kernel for the transforms: 2 = persistent warp-specialised DMMA kernel fed by TMA through an
- * mbarrier ring (default; used where M and N are multiples of 128 and K of 16), 1 = cp.async-pipelined DMMA kernel
- * (M, N multiples of 64), 0 = generic FP64-FMA tile kernel (any shape).  A variant falls back to the next lower one
+ * mbarrier ring (default; any grid with even nx and ny — "non-uniform grids in any direction", any N_x, N_y, PAPER.md:187:
+ * edge tiles through TMA's out-of-bounds zero fill), 1 = cp.async-pipelined DMMA kernel (M, N multiples of 64),
+ * 0 = generic FP64-FMA tile kernel (any shape, odd sizes included).  A variant falls back to the next lower one
  * for shapes it does not take.  For A/B measurement and tests; all are this library's own sm_100a kernels. */
 int tpt_plan_set_gemm_variant(tpt_plan *plan, int variant);
+
+/* Which kernel tpt_solve runs in each slot of this plan with its current variant settings (one code
+ * per step 2.1-2.5): paths_out[TPT_K_COUNT], HOST.  For tests and the bench record — e.g. that a 1000 x 200 grid really
+ * runs on the tensor-path GEMM. */
+enum {
+    TPT_PATH_NONE = 0,            /* slot inactive (direction not diagonalised, tpt_plan_create_dirs) */
+    TPT_PATH_GEMM_GENERIC = 1,    /* DFMA tile kernel */
+    TPT_PATH_GEMM_CPASYNC = 2,    /* cp.async-pipelined DMMA kernel */
+    TPT_PATH_GEMM_TMA = 3,        /* persistent TMA / mbarrier DMMA kernel */
+    TPT_PATH_FFT = 4,             /* fast transform of a uniform direction */
+    TPT_PATH_THOMAS_STREAM = 5,   /* one thread per column, c' spilled to the workspace */
+    TPT_PATH_THOMAS_ONCHIP = 6,   /* on-chip partitioned sweep, natural layout */
+    TPT_PATH_THOMAS_BLOCKED = 7   /* on-chip partitioned sweep on the tile-blocked mode-space layout */
+};
+int tpt_plan_get_paths(const tpt_plan *plan, int *paths_out);
 
 /* Select the z-sweep kernel: 1 = on-chip partitioned Thomas kernel (column tiles resident in shared memory,
  * 16 B/pt of HBM traffic; used where nx*ny % 16 == 0 and nz <= 1056, default), 0 = streaming one-thread-per-column

@@ -123,7 +123,7 @@ bool use_blocked(const tpt_plan *p) {
     if (!tpt::blocked_layout_supported(p->nx, p->ny, p->nz) || !tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) return false;
     // the fast y transform addresses either layout (its tiles write whole 128-byte lines of the blocked field)
     if (p->transform[1] == TPT_TRANSFORM_FFT) return true;
-    return p->gemm_variant == 2 && p->ny % 128 == 0 && p->nx % 128 == 0;   // the TMA GEMM's tile shape (M = K = ny, N = nx)
+    return p->gemm_variant == 2 && p->ny % 2 == 0;   // the TMA GEMM (M = K = ny any even size, N = nx a multiple of 16)
 }
 
 // Step 2.3 on one field: in -> out (in == out allowed); `scratch` is a free field (used by the streaming kernel only).
@@ -766,6 +766,32 @@ int tpt_plan_get_kernel_times(tpt_plan *p, float *ms_host, int *launches_out, in
     if (solves_out) *solves_out = (int)solves;
     p->ev_used = 0;
     p->launches_accum = 0;
+    return TPT_OK;
+}
+
+int tpt_plan_get_paths(const tpt_plan *p, int *paths_out) {
+    if (!p || !paths_out) return TPT_EINVAL;
+    const bool blk = use_blocked(p);
+    double *w = p->d_work;   // stands for any 16-byte aligned field
+    for (int s = 0; s < TPT_K_COUNT; ++s) {
+        int path = TPT_PATH_NONE;
+        if (s == TPT_K_THOMAS) {
+            const bool onchip = p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz);
+            path = !onchip ? TPT_PATH_THOMAS_STREAM : (blk ? TPT_PATH_THOMAS_BLOCKED : TPT_PATH_THOMAS_ONCHIP);
+        } else if (slot_active(p, s)) {
+            const int d = (s == TPT_K_FWD_X || s == TPT_K_INV_X) ? 0 : 1;
+            if (p->transform[d] == TPT_TRANSFORM_FFT) {
+                path = TPT_PATH_FFT;
+            } else {
+                const tpt::GemmArgs g = d == 0 ? gemm_x(p, w, w, p->d_xfwd, 0, p->nz)
+                                               : gemm_y(p, w, w, p->d_yfwd, 0, p->nz, blk && s == TPT_K_INV_Y, blk && s == TPT_K_FWD_Y);
+                if (p->gemm_variant == 2 && tpt::gemm_tma_supported(g)) path = TPT_PATH_GEMM_TMA;
+                else if (p->gemm_variant >= 1 && tpt::gemm_dmma_supported(g)) path = TPT_PATH_GEMM_CPASYNC;
+                else path = TPT_PATH_GEMM_GENERIC;
+            }
+        }
+        paths_out[s] = path;
+    }
     return TPT_OK;
 }
 

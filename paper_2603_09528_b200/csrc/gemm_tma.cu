@@ -10,7 +10,10 @@
 //     every 16-column group are assigned to MMA lanes through fixed permutations (rho, nu below) that make every
 //     64-bit fragment load bank-conflict free without padding.
 //
-// Row-major C[b] (M x N) = A[b] (M x K, k contiguous) * B[b] (K x N, n contiguous).  M % 128 == N % 128 == 0, K % 16 == 0.
+// Row-major C[b] (M x N) = A[b] (M x K, k contiguous) * B[b] (K x N, n contiguous).  Any M and K, any even N ("the
+// framework supports non-uniform grids in any direction", PAPER.md:187 — any N_x, N_y): ragged edge tiles are loaded
+// with TMA's out-of-bounds zero fill (a zero row of A or column of B contributes nothing), warps whose 32x32 sub-tile
+// lies wholly outside skip their DMMAs, and the epilogue stores are predicated.
 #include <cuda.h>
 
 #include "kernels.cuh"
@@ -34,10 +37,12 @@ struct TmaGemmParams {
     double *C;
     int64_t ldc, strideC;
     int64_t ldg;         // stride between 16-column groups of C (16 = plain row-major)
-    int KT;              // K / 16
-    int tiles_n;         // N / 128
-    int tiles_mn;        // (M / 128) * (N / 128)
+    int M, N;            // extents of C (edge tiles: predicated stores)
+    int KT;              // ceil(K / 16)
+    int tiles_n;         // ceil(N / 128)
+    int tiles_mn;        // ceil(M / 128) * ceil(N / 128)
     int ntiles;          // tiles_mn * batch
+    int b_split;         // N % 16 != 0: mapB is the plain 3-D tensor [batch][K][N], one load per 16-column group
     int a_batch_rows;    // rows of the A tensor per batch (0: shared by all batches)
     int b_batch_rows;    // rows of the B tensor per batch (0: shared)
     // sharded solve: rows of C scattered to their owners' memory (GemmArgs::peerC); row m belongs to rank
@@ -85,7 +90,13 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                     unsigned char *st = smem + (size_t)slot * STAGE_BYTES;
                     ptx::mbar_arrive_expect_tx(&full[slot], STAGE_BYTES);
                     ptx::tma_load_2d(st, &mapA, kt * BK, a_row, &full[slot]);
-                    ptx::tma_load_4d(st + A_BYTES, &mapB, 0, kt * BK, nt * (BN / 16), b_sel, &full[slot]);
+                    if (!p.b_split) {
+                        ptx::tma_load_4d(st + A_BYTES, &mapB, 0, kt * BK, nt * (BN / 16), b_sel, &full[slot]);
+                    } else {     // same shared-memory image, built from eight boxes clipped at column N
+#pragma unroll
+                        for (int q = 0; q < BN / 16; ++q)
+                            ptx::tma_load_3d(st + A_BYTES + q * 2048, &mapB, nt * BN + q * 16, kt * BK, b_sel, &full[slot]);
+                    }
                     if (++slot == STAGES) { slot = 0; phase ^= 1; }
                 }
             }
@@ -132,6 +143,11 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        const int b = tile / p.tiles_mn;
+        const int mn = tile - b * p.tiles_mn;
+        const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
+        // edge tiles: a warp whose sub-tile lies wholly past M or N only keeps the ring's bookkeeping going
+        const bool inside = mt * BM + wm0 < p.M && nt * BN + wn0 < p.N;
 
         for (int kt = 0; kt < KT; ++kt) {
             ptx::mbar_wait(&full[slot], phase);
@@ -141,6 +157,7 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             }
             const uint32_t sa = smem_base + (uint32_t)slot * STAGE_BYTES;
             const uint32_t sb = sa + A_BYTES;
+            if (inside) {
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
                 double af[4], bf[4];
@@ -153,25 +170,28 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
 #pragma unroll
                     for (int j = 0; j < 4; ++j) ptx::dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
             }
+            }
             prev_slot = slot;
             if (++slot == STAGES) { slot = 0; phase ^= 1; }
         }
         // epilogue: lane holds rows 8i + rho, columns nu(2t), nu(2t)+1 of each MMA tile -> 16-byte stores
-        const int b = tile / p.tiles_mn;
-        const int mn = tile - b * p.tiles_mn;
-        const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
+        if (!inside) continue;
         const int row0 = mt * BM + wm0 + rho;
-        const int64_t off = (int64_t)b * p.strideC + (int64_t)(nt * (BN / 16) + wn0 / 16) * p.ldg + ((t >> 1) << 1) + ((t & 1) << 3);
+        const int cin = ((t >> 1) << 1) + ((t & 1) << 3);          // first of my two columns inside a 16-column group
+        const int col0 = nt * BN + wn0 + cin;
+        const int64_t off = (int64_t)b * p.strideC + (int64_t)(nt * (BN / 16) + wn0 / 16) * p.ldg + cin;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int row = row0 + 8 * i;
+            if (row >= p.M) break;
             // sharded solve: the owner of mode row `row` receives it straight from this epilogue (16-byte stores to
             // peer-mapped memory travel over NVLink while the next tile's DMMAs run) — no pack kernel, no collective
             double *base = p.npeers ? p.peerC[(((row >> 4) + 1) * p.npeers - 1) / p.units] : p.C;
             double *Cw = base + off + (int64_t)row * p.ldc;
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                *reinterpret_cast<double2 *>(Cw + (int64_t)(j >> 1) * p.ldg + (j & 1) * 4) = make_double2(acc[i][j][0], acc[i][j][1]);
+                if (col0 + (j >> 1) * 16 + (j & 1) * 4 < p.N)         // N is even: a column pair is inside or outside as a whole
+                    *reinterpret_cast<double2 *>(Cw + (int64_t)(j >> 1) * p.ldg + (j & 1) * 4) = make_double2(acc[i][j][0], acc[i][j][1]);
         }
     }
 }
@@ -181,19 +201,23 @@ bool aligned16(const void *q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 
 }  // namespace
 
 bool gemm_tma_supported(const GemmArgs &g) {
-    if (g.M % BM || g.N % BN || g.K % BK || g.K < BK) return false;
+    if (g.M < 1 || g.N < 2 || g.N % 2 || g.K < 1 || g.batch < 1) return false;
     if (g.lda % 2 || g.ldb % 2 || g.ldc % 2 || g.strideC % 2) return false;
+    // the blocked layouts address whole 16-column groups; the peer scatter owns rows in 16-row units
+    if ((g.ldgB > 16 || g.ldgC > 16 || g.npeers) && g.N % 16) return false;
+    if (g.npeers && g.M % 16) return false;
     if (!aligned16(g.A) || !aligned16(g.B) || !aligned16(g.C)) return false;
     if (g.npeers < 0 || g.npeers > MAX_PEERS) return false;
     for (int q = 0; q < g.npeers; ++q)
         if (!g.peerC[q] || !aligned16(g.peerC[q])) return false;
     // batches are folded into the row dimension of the operand tensors: a batched operand must be densely stacked
     if (g.batch > 1) {
-        if (g.strideA != 0 && g.strideA != (int64_t)g.M * g.lda) return false;
+        // a batched A is one tall tensor: its edge tiles would run into the next batch
+        if (g.strideA != 0 && (g.strideA != (int64_t)g.M * g.lda || g.M % BM)) return false;
         if (g.strideB != 0 && g.strideB % 2) return false;
     }
     if (g.ldgB % 2 || g.ldgC % 2) return false;
-    const int64_t tiles = (int64_t)(g.M / BM) * (g.N / BN) * g.batch;
+    const int64_t tiles = (int64_t)((g.M + BM - 1) / BM) * ((g.N + BN - 1) / BN) * g.batch;
     return tiles < (int64_t)1 << 30;
 }
 
@@ -219,7 +243,14 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
         const uint32_t box[2] = {BK, BM};
         if (!make_f64_map(&mapA, g.A, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) return cudaErrorUnknown;
     }
-    {
+    const bool b_split = g.N % 16 != 0;
+    if (b_split) {
+        // plain [batch][K][N]: a box is one 16 k x 16 n sub-tile, clipped (zero-filled) at column N
+        const uint64_t dims[3] = {(uint64_t)g.N, (uint64_t)g.K, (uint64_t)(b_batched ? g.batch : 1)};
+        const uint64_t strides[2] = {(uint64_t)g.ldb * 8, (uint64_t)(b_batched ? g.strideB : (int64_t)g.K * g.ldb) * 8};
+        const uint32_t box[3] = {16, BK, 1};
+        if (!make_f64_map(&mapB, g.B, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) return cudaErrorUnknown;
+    } else {
         // B viewed as [batch][N/16 groups][K rows][16 columns]: one box = 8 sub-tiles of 16 k x 16 n (128-byte rows)
         const uint64_t ldg = g.ldgB ? (uint64_t)g.ldgB : 16;
         const uint64_t dims[4] = {16, (uint64_t)g.K, (uint64_t)g.N / 16, (uint64_t)(b_batched ? g.batch : 1)};
@@ -232,14 +263,17 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
     p.ldc = g.ldc;
     p.strideC = g.strideC;
     p.ldg = g.ldgC ? g.ldgC : 16;
-    p.KT = g.K / BK;
-    p.tiles_n = g.N / BN;
-    p.tiles_mn = (g.M / BM) * (g.N / BN);
+    p.M = g.M;
+    p.N = g.N;
+    p.KT = (g.K + BK - 1) / BK;
+    p.tiles_n = (g.N + BN - 1) / BN;
+    p.tiles_mn = ((g.M + BM - 1) / BM) * p.tiles_n;
     p.ntiles = p.tiles_mn * g.batch;
+    p.b_split = b_split ? 1 : 0;
     p.a_batch_rows = a_batched ? g.M : 0;
     p.b_batch_rows = b_batched ? g.K : 0;
     p.npeers = g.npeers;
-    p.units = g.M / 16;
+    p.units = g.M / 16 > 0 ? g.M / 16 : 1;
     for (int q = 0; q < MAX_PEERS; ++q) p.peerC[q] = q < g.npeers ? g.peerC[q] : nullptr;
     const int grid = p.ntiles < sms ? p.ntiles : sms;
     gemm_tma_kernel<<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);

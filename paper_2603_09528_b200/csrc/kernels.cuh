@@ -46,7 +46,8 @@ bool gemm_dmma_supported(const GemmArgs &g);
 cudaError_t gemm_configure();   // one-time cudaFuncSetAttribute for the dynamic-smem kernels
 
 // variant 2 (gemm_tma.cu): persistent warp-specialised DMMA kernel fed by TMA through an mbarrier ring.
-// M % 128 == N % 128 == 0, K % 16 == 0, batched operands densely stacked.  sms = SM count.
+// Any M, K and even N (edge tiles through TMA's out-of-bounds zero fill and predicated stores), even leading dimensions,
+// 16-byte aligned bases, batched operands densely stacked; the blocked layouts need N % 16 == 0.  sms = SM count.
 bool gemm_tma_supported(const GemmArgs &g);
 cudaError_t gemm_tma_configure();
 cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream);

@@ -82,6 +82,51 @@ def test_parity_small_cases(tpt, torch, orc, case, variant):
     plan.destroy()
 
 
+# Grids whose sizes are not multiples of the GEMM's 128 x 128 tile (any N_x, N_y): the tensor-path TMA
+# kernel takes them through out-of-bounds zero fill (16-multiples keep the tile-blocked sweep layout; 8- and 2-multiples
+# load B in clipped 16-column boxes), never the DFMA fallback.
+RAGGED_TMA = [
+    ("r192", (192, 320, 24), (1.0, 2.0, 1.0), (2.0, 2.5, 2.0), (N_, N_, D_), 0.0, True),
+    ("r1000", (1000, 200, 40), (4.0, 1.0, 1.0), (0.0, 2.0, 2.5), (N_, D_, N_), 0.0, False),
+    ("r144", (144, 80, 33), (1.0, 1.0, 2.0), (2.0, 1.5, 2.5), (N_, N_, N_), 0.0, True),
+    ("r-even", (134, 90, 18), (1.0, 1.0, 1.0), (1.5, 2.0, 2.0), (D_, N_, D_), 1e-3, False),
+    ("r-periodic", (208, 176, 20), (2.0, 1.0, 1.0), (0.0, 2.0, 2.0), (I.PERIODIC, N_, N_), 0.0, True),
+]
+
+
+@pytest.mark.parametrize("case", RAGGED_TMA, ids=[c[0] for c in RAGGED_TMA])
+def test_ragged_grids_run_on_the_tma_gemm(tpt, torch, orc, case):
+    name, n, L, beta, bc, alpha, blocked = case
+    P = I.Problem(name, n, L, beta, bc, alpha, seed=len(name) + n[1])
+    plan, f, phi = _gpu_solve(tpt, torch, P, 2)
+    paths = plan.paths()
+    assert [paths[s] for s in (tpt.K_FWD_X, tpt.K_FWD_Y, tpt.K_INV_Y, tpt.K_INV_X)] == [tpt.PATH_GEMM_TMA] * 4
+    assert paths[tpt.K_THOMAS] == (tpt.PATH_THOMAS_BLOCKED if blocked else tpt.PATH_THOMAS_ONCHIP)
+    xf, yf, zf = P.faces()
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha).solve(f)
+    assert _rel(phi, ref) <= PARITY_TOL
+    r = orc.residual_norms(xf, yf, zf, bc, alpha, f, phi)
+    assert r["rel2"] <= RESID_TOL and r["relL2vol"] <= RESID_TOL
+    # the DFMA tile kernel (an independent implementation of the same contraction) agrees to rounding
+    plan.set_gemm_variant(0)
+    assert plan.paths()[tpt.K_FWD_X] == tpt.PATH_GEMM_GENERIC
+    d_f = torch.from_numpy(f).cuda()
+    d_o = torch.empty_like(d_f)
+    plan.solve(d_f, d_o)
+    torch.cuda.synchronize()
+    assert _rel(d_o.cpu().numpy(), phi) <= 1e-11
+    plan.destroy()
+
+
+def test_odd_sizes_fall_back_to_the_generic_gemm(tpt, torch):
+    P = I.Problem("odd", (33, 17, 8), (1.0, 1.0, 1.0), (1.0, 1.0, 1.0), (N_, N_, D_), 0.0, 3)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0)
+    paths = plan.paths()
+    assert paths[tpt.K_FWD_X] == tpt.PATH_GEMM_GENERIC and paths[tpt.K_THOMAS] == tpt.PATH_THOMAS_STREAM
+    plan.destroy()
+
+
 @pytest.mark.parametrize("cfg", ["c1", "c2"])
 def test_parity_baseline_small_configs(tpt, torch, orc, cfg):
     P = I.CONFIGS[cfg][0]
@@ -275,7 +320,7 @@ def test_profiling_reports_five_kernels(tpt, torch):
         plan.solve(d, o)
     ms, launches, solves = plan.kernel_times()
     assert len(ms) == 5 and all(m > 0 for m in ms) and solves == 3
-    assert launches == 18                                                # (5 kernels + gauge) x 3, singular plan
+    assert launches == 15                                                # 5 kernels x 3: the gauge of a singular plan is fused into the sweep
     plan.set_profiling(False)
     plan.solve(d, o)
     with pytest.raises(tpt.TptError):
