@@ -79,7 +79,9 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         if (warp == CONSUMER_WARPS && lane == 0) {
             int slot = 0;
             uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x) {
+            for (int round = 0, base = 0; base < p.ntiles; ++round, base += gridDim.x) {
+                const int tile = base + (int)((blockIdx.x + round) % gridDim.x);
+                if (tile >= p.ntiles) continue;
                 const int b = tile / p.tiles_mn;
                 const int mn = tile - b * p.tiles_mn;
                 const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
@@ -107,7 +109,10 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     // ---------------- consumers ---------------------------------------------------------------------
     ptx::setmaxnreg_inc<112>();   // 640 x 96 registers at launch = 128 x 24 + 512 x 112 (the pool is the CTA's own)
     const int g = lane >> 2, t = lane & 3;
-    const int wm0 = (warp >> 2) * 32, wn0 = (warp & 3) * 32;
+    // Warp w runs on SM sub-partition w % 4.  The 4 x 4 grid of 32 x 32 warp tiles is handed out as a Latin square: every
+    // sub-partition holds one warp of each row block AND of each column block, so on an edge tile (rows or columns past
+    // M / N skipped) the remaining DMMAs still spread evenly over the four FP64 tensor pipes.
+    const int wm0 = (warp >> 2) * 32, wn0 = (((warp & 3) + (warp >> 2)) & 3) * 32;
     const int rho = ((g & 3) << 1) | (g >> 2);                 // MMA row g  <-> tile row 8i + rho
     // A fragment (row 8i + rho, k = 4kk + t):  byte = row*128 + (((k>>1) ^ rho) << 4) + (k&1)*8
     uint32_t a_off[4];
@@ -137,7 +142,12 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     // queueing shared-memory loads the read itself can still be pending when an L2-hit TMA refill lands.
     int slot = 0, prev_slot = -1;
     uint32_t phase = 0;
-    for (int tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x) {
+    // Static schedule: round r hands tiles [r grid, (r+1) grid) to the CTAs rotated by r — with a plain stride-grid walk a
+    // CTA would meet the same (mt, nt) every round whenever grid is a multiple of tiles_mn, i.e. some CTAs only cheap edge
+    // tiles and others only full ones.
+    for (int round = 0, base = 0; base < p.ntiles; ++round, base += gridDim.x) {
+        const int tile = base + (int)((blockIdx.x + round) % gridDim.x);
+        if (tile >= p.ntiles) continue;
         double acc[4][4][2];
 #pragma unroll
         for (int i = 0; i < 4; ++i)

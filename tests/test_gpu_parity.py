@@ -89,7 +89,7 @@ RAGGED_TMA = [
     ("r192", (192, 320, 24), (1.0, 2.0, 1.0), (2.0, 2.5, 2.0), (N_, N_, D_), 0.0, True),
     ("r1000", (1000, 200, 40), (4.0, 1.0, 1.0), (0.0, 2.0, 2.5), (N_, D_, N_), 0.0, False),
     ("r144", (144, 80, 33), (1.0, 1.0, 2.0), (2.0, 1.5, 2.5), (N_, N_, N_), 0.0, True),
-    ("r-even", (134, 90, 18), (1.0, 1.0, 1.0), (1.5, 2.0, 2.0), (D_, N_, D_), 1e-3, False),
+    ("r-even", (136, 90, 18), (1.0, 1.0, 1.0), (1.5, 2.0, 2.0), (D_, N_, D_), 1e-3, False),
     ("r-periodic", (208, 176, 20), (2.0, 1.0, 1.0), (0.0, 2.0, 2.0), (I.PERIODIC, N_, N_), 0.0, True),
 ]
 
