@@ -307,9 +307,21 @@ enum {
     TPT_PATH_FFT = 4,             /* fast transform of a uniform direction */
     TPT_PATH_THOMAS_STREAM = 5,   /* one thread per column, c' spilled to the workspace */
     TPT_PATH_THOMAS_ONCHIP = 6,   /* on-chip partitioned sweep, natural layout */
-    TPT_PATH_THOMAS_BLOCKED = 7   /* on-chip partitioned sweep on the tile-blocked mode-space layout */
+    TPT_PATH_THOMAS_BLOCKED = 7,  /* on-chip partitioned sweep on the tile-blocked mode-space layout */
+    TPT_PATH_FUSED_SMALL = 8      /* all five steps in one cluster launch (grids that fit on chip) */
 };
 int tpt_plan_get_paths(const tpt_plan *plan, int *paths_out);
+
+/* Kernel launches the last tpt_solve / tpt_solve_batch / tpt_solve_host[_async] / tpt_project on this plan enqueued
+ * (>= 0), < 0 on error. */
+int tpt_plan_launches(const tpt_plan *plan);
+
+/* Small-grid execution path (BASELINE.json configs[0]): with the default kernel variants, a grid of at most 16384 points
+ * whose z-plane slabs fit the shared memory of a thread-block cluster of 8 runs steps 2.1-2.5 and the
+ * gauge as ONE launch — the planes stay on chip through both transforms of each side, the sweep's change of ownership
+ * goes through the workspace in L2 between two cluster barriers.  GEMM transforms only.  enabled = 0 forces the five
+ * separate kernels (default 1).  tpt_stage and the host-buffer solves always use the separate kernels. */
+int tpt_plan_set_fused_small(tpt_plan *plan, int enabled);
 
 /* Select the z-sweep kernel: 1 = on-chip partitioned Thomas kernel (column tiles resident in shared memory,
  * 16 B/pt of HBM traffic; used where nx*ny % 16 == 0 and nz <= 1056, default), 0 = streaming one-thread-per-column

@@ -23,7 +23,7 @@ K_FWD_X, K_FWD_Y, K_THOMAS, K_INV_Y, K_INV_X, K_COUNT = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")
 # tpt_plan_get_paths codes
 (PATH_NONE, PATH_GEMM_GENERIC, PATH_GEMM_CPASYNC, PATH_GEMM_TMA, PATH_FFT, PATH_THOMAS_STREAM, PATH_THOMAS_ONCHIP,
- PATH_THOMAS_BLOCKED) = range(8)
+ PATH_THOMAS_BLOCKED, PATH_FUSED_SMALL) = range(9)
 
 # every symbol include/tpt.h declares (tests check the library exports exactly these)
 TRANSFORM_GEMM, TRANSFORM_FFT = 0, 1   # per diagonalised direction: eigenbasis GEMM / fast transform
@@ -31,7 +31,7 @@ TRANSFORM_GEMM, TRANSFORM_FFT = 0, 1   # per diagonalised direction (PAPER.md:20
 SYMBOLS = (
     "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
-    "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
+    "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_launches", "tpt_plan_set_fused_small", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
     "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_fill_uniform",
     "tpt_shard_layout", "tpt_shard_create", "tpt_shard_get_layout", "tpt_shard_sym", "tpt_shard_set_peers", "tpt_shard_ipc_export",
@@ -90,6 +90,8 @@ def lib():
         L.tpt_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i), C.POINTER(i)]
         L.tpt_plan_get_paths.argtypes = [vp, C.POINTER(C.c_int)]
         L.tpt_plan_set_gemm_variant.argtypes = [vp, i]
+        L.tpt_plan_set_fused_small.argtypes = [vp, i]
+        L.tpt_plan_launches.argtypes = [vp]
         L.tpt_plan_set_thomas_variant.argtypes = [vp, i]
         L.tpt_fp64_peak.argtypes = [i, _dp]
         L.tpt_fill_uniform.argtypes = [vp, C.c_size_t, C.c_ulonglong, C.c_ulonglong, vp]
@@ -222,6 +224,16 @@ class Plan:
         out = (C.c_int * K_COUNT)()
         _check(lib().tpt_plan_get_paths(self._h, out), "tpt_plan_get_paths")
         return [int(v) for v in out]
+
+    def launches_last(self) -> int:
+        """Kernel launches enqueued by the last solve on this plan."""
+        n = lib().tpt_plan_launches(self._h)
+        if n < 0:
+            raise TptError(n, "tpt_plan_launches")
+        return int(n)
+
+    def set_fused_small(self, enabled: bool):
+        _check(lib().tpt_plan_set_fused_small(self._h, int(bool(enabled))), "tpt_plan_set_fused_small")
 
     def set_gemm_variant(self, variant: int):
         _check(lib().tpt_plan_set_gemm_variant(self._h, int(variant)), "tpt_plan_set_gemm_variant")

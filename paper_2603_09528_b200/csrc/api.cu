@@ -187,6 +187,29 @@ bool slot_active(const tpt_plan *p, int slot) {
     return slot == TPT_K_THOMAS;
 }
 
+// Grids that fit on chip run the whole solve as one cluster launch (fused_small.cu) — with the default kernel variants
+// only, so that selecting a variant still exercises that kernel.
+bool use_fused_small(const tpt_plan *p) {
+    if (!p->fused_small || p->gemm_variant != 2 || p->thomas_variant != 1) return false;
+    if (!(p->dirs & 3)) return false;     // sweep only ("z"): already a single launch
+    if (((p->dirs & 1) && p->transform[0] != TPT_TRANSFORM_GEMM) || ((p->dirs & 2) && p->transform[1] != TPT_TRANSFORM_GEMM)) return false;
+    return tpt::fused_small_supported(p->nx, p->ny, p->nz);
+}
+
+int run_fused_small(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream_t st, int *launches) {
+    const size_t pts = p->points();
+    for (int f = 0; f < nf; ++f) {
+        tpt::FusedSmallArgs a{};
+        a.rhs = rhs + f * pts; a.out = out + f * pts; a.work = p->d_work + f * pts;
+        a.xfwd = p->d_xfwd; a.xinv = p->d_xinv; a.yfwd = p->d_yfwd; a.yinv = p->d_yinv;
+        a.az = p->d_az; a.bz = p->d_bz; a.cz = p->d_cz; a.wz = p->d_wz; a.lamx = p->d_lamx; a.lamy = p->d_lamy;
+        a.nx = p->nx; a.ny = p->ny; a.nz = p->nz; a.dirs = p->dirs; a.singular = p->singular; a.shift0 = p->shift0;
+        if (tpt::launch_fused_small(a, st) != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
+        ++*launches;
+    }
+    return TPT_OK;
+}
+
 // Steps 2.1-2.5 on nf stacked fields (nf <= work_fields).  Buffers: the transforms are out of place and alternate
 // between the plan workspace W and `out`, starting with W (rhs may alias out); the sweep works in place on whichever
 // holds the data — or straight from rhs to out when no transform is active (the "z" choice of PAPER.md:209) — so the
@@ -198,6 +221,13 @@ int run_pipeline(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream
     const int nk = p->nz * nf;
     const bool blk = use_blocked(p);
     if (ev && cudaEventRecord(ev[0], st) != cudaSuccess) return TPT_ECUDA;
+    if (use_fused_small(p)) {      // one launch: its time is reported in the first slot
+        int rc = run_fused_small(p, rhs, out, nf, st, launches);
+        if (rc != TPT_OK) return rc;
+        for (int s = 0; ev && s < TPT_K_COUNT; ++s)
+            if (cudaEventRecord(ev[s + 1], st) != cudaSuccess) return TPT_ECUDA;
+        return TPT_OK;
+    }
     for (int s = 0; s < TPT_K_COUNT; ++s) {
         int rc = TPT_OK;
         if (s == TPT_K_THOMAS) {
@@ -772,10 +802,13 @@ int tpt_plan_get_kernel_times(tpt_plan *p, float *ms_host, int *launches_out, in
 int tpt_plan_get_paths(const tpt_plan *p, int *paths_out) {
     if (!p || !paths_out) return TPT_EINVAL;
     const bool blk = use_blocked(p);
+    const bool fused = use_fused_small(p);
     double *w = p->d_work;   // stands for any 16-byte aligned field
     for (int s = 0; s < TPT_K_COUNT; ++s) {
         int path = TPT_PATH_NONE;
-        if (s == TPT_K_THOMAS) {
+        if (fused) {
+            path = (s == TPT_K_THOMAS || slot_active(p, s)) ? TPT_PATH_FUSED_SMALL : TPT_PATH_NONE;
+        } else if (s == TPT_K_THOMAS) {
             const bool onchip = p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz);
             path = !onchip ? TPT_PATH_THOMAS_STREAM : (blk ? TPT_PATH_THOMAS_BLOCKED : TPT_PATH_THOMAS_ONCHIP);
         } else if (slot_active(p, s)) {
@@ -798,6 +831,14 @@ int tpt_plan_get_paths(const tpt_plan *p, int *paths_out) {
 int tpt_plan_set_gemm_variant(tpt_plan *p, int variant) {
     if (!p || variant < 0 || variant > 2) return TPT_EINVAL;
     p->gemm_variant = variant;
+    return TPT_OK;
+}
+
+int tpt_plan_launches(const tpt_plan *p) { return p ? p->launches_last : TPT_EINVAL; }
+
+int tpt_plan_set_fused_small(tpt_plan *p, int enabled) {
+    if (!p) return TPT_EINVAL;
+    p->fused_small = enabled ? 1 : 0;
     return TPT_OK;
 }
 

@@ -86,6 +86,19 @@ cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &pe
                                          const double *lamy_owned, const double *wz, int nx, int rows, int nz, double shift0,
                                          int singular, int sms, cudaStream_t stream);
 
+// The whole solve in one cluster launch for grids that fit on chip (fused_small.cu): steps 2.1-2.5 + gauge, GEMM
+// transforms only.  work: a field-sized scratch in global memory (the plan's workspace); rhs == out allowed.
+struct FusedSmallArgs {
+    const double *rhs;
+    double *out, *work;
+    const double *xfwd, *xinv, *yfwd, *yinv;                  // pre-scaled matrices of the plan (plan.hpp); unused ones may be null
+    const double *az, *bz, *cz, *wz, *lamx, *lamy;
+    int nx, ny, nz, dirs, singular;
+    double shift0;
+};
+bool fused_small_supported(int nx, int ny, int nz);
+cudaError_t launch_fused_small(const FusedSmallArgs &a, cudaStream_t stream);
+
 // Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean); `stride` = distance
 // between consecutive z levels of that column (nx*ny in the natural layout, 16 in the tile-blocked one).
 cudaError_t launch_gauge(double *x, const double *wz, size_t stride, int nz, cudaStream_t stream);

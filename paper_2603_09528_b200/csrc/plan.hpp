@@ -23,6 +23,7 @@ struct tpt_plan {
     double *d_fft[2] = {nullptr, nullptr};   // twiddle tables
     int gemm_variant = 2;
     int thomas_variant = 1;       // 1 = on-chip partitioned kernel where supported, 0 = streaming kernel
+    int fused_small = 1;          // grids that fit on chip: the whole solve in one cluster launch (fused_small.cu)
     int sms = 0;
     int profiling = 0;
     int launches_last = 0;

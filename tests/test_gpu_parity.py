@@ -119,7 +119,7 @@ def test_ragged_grids_run_on_the_tma_gemm(tpt, torch, orc, case):
 
 
 def test_odd_sizes_fall_back_to_the_generic_gemm(tpt, torch):
-    P = I.Problem("odd", (33, 17, 8), (1.0, 1.0, 1.0), (1.0, 1.0, 1.0), (N_, N_, D_), 0.0, 3)
+    P = I.Problem("odd", (65, 33, 20), (1.0, 1.0, 1.0), (1.0, 1.0, 1.0), (N_, N_, D_), 0.0, 3)
     xf, yf, zf = P.faces()
     plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0)
     paths = plan.paths()

@@ -89,6 +89,9 @@ def test_partial_dirs_argument_checks_and_skipped_slots(tpt, torch):
         plan.stage(tpt.K_FWD_X, d, o)
     plan.set_profiling(True)
     plan.solve(d, o)
+    assert plan.kernel_times()[1:] == (1, 1)                                 # 8192 points: the one-launch small-grid path
+    plan.set_fused_small(False)
+    plan.solve(d, o)
     ms, launches, solves = plan.kernel_times()
     assert launches == 3 and solves == 1                                     # fwd y, sweep, inv y
     plan.destroy()
