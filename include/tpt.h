@@ -312,6 +312,15 @@ enum {
 };
 int tpt_plan_get_paths(const tpt_plan *plan, int *paths_out);
 
+/* L2-resident slab pipeline of steps 2.2 -> 2.3 -> 2.4 (BASELINE north_star "Fusion"): the forward-y
+ * transform, the z sweep and the inverse-y transform run x-slab by x-slab (G 16-column groups x ny x nz) through two
+ * plan-owned slab buffers that stay in the 126 MB L2, so the mode-space field never travels to HBM (4 of a solve's 10
+ * field-sized HBM passes).  groups: -1 = automatic (default: one-group slabs where the y transform is a fast transform,
+ * the field is at least 256 MiB and a slab at most 40 MiB), 0 = off, G > 0 = force slabs of G groups (the slab buffers,
+ * 2 * G * 16 * ny * nz doubles, are allocated at the next solve).  Needs the tile-blocked layout (nx % 16 == 0, default
+ * kernel variants); ignored otherwise.  Results equal the unslabbed solve's bit for bit. */
+int tpt_plan_set_slab_groups(tpt_plan *plan, int groups);
+
 /* Kernel launches the last tpt_solve / tpt_solve_batch / tpt_solve_host[_async] / tpt_project on this plan enqueued
  * (>= 0), < 0 on error. */
 int tpt_plan_launches(const tpt_plan *plan);

@@ -31,7 +31,7 @@ TRANSFORM_GEMM, TRANSFORM_FFT = 0, 1   # per diagonalised direction (PAPER.md:20
 SYMBOLS = (
     "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
-    "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_launches", "tpt_plan_set_fused_small", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
+    "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_launches", "tpt_plan_set_slab_groups", "tpt_plan_set_fused_small", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
     "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_fill_uniform",
     "tpt_shard_layout", "tpt_shard_create", "tpt_shard_get_layout", "tpt_shard_sym", "tpt_shard_set_peers", "tpt_shard_ipc_export",
@@ -92,6 +92,7 @@ def lib():
         L.tpt_plan_set_gemm_variant.argtypes = [vp, i]
         L.tpt_plan_set_fused_small.argtypes = [vp, i]
         L.tpt_plan_launches.argtypes = [vp]
+        L.tpt_plan_set_slab_groups.argtypes = [vp, i]
         L.tpt_plan_set_thomas_variant.argtypes = [vp, i]
         L.tpt_fp64_peak.argtypes = [i, _dp]
         L.tpt_fill_uniform.argtypes = [vp, C.c_size_t, C.c_ulonglong, C.c_ulonglong, vp]
@@ -231,6 +232,10 @@ class Plan:
         if n < 0:
             raise TptError(n, "tpt_plan_launches")
         return int(n)
+
+    def set_slab_groups(self, groups: int):
+        """-1 automatic, 0 off, G > 0: run steps 2.2-2.4 through L2-resident slabs of G 16-column groups."""
+        _check(lib().tpt_plan_set_slab_groups(self._h, int(groups)), "tpt_plan_set_slab_groups")
 
     def set_fused_small(self, enabled: bool):
         _check(lib().tpt_plan_set_fused_small(self._h, int(bool(enabled))), "tpt_plan_set_fused_small")

@@ -62,6 +62,10 @@ void free_plan(tpt_plan *p) {
     cudaFree(p->d_fft[1]);
     cudaFree(p->d_work);
     cudaFree(p->d_stage);
+    cudaFree(p->d_slab);
+    if (p->ev_slab_fork) cudaEventDestroy(p->ev_slab_fork);
+    if (p->ev_slab_join) cudaEventDestroy(p->ev_slab_join);
+    if (p->st_slab) cudaStreamDestroy(p->st_slab);
     for (auto &e : p->ev_pool) cudaEventDestroy(e);
     for (auto &e : p->ev_slab) cudaEventDestroy(e);
     if (p->ev_start) cudaEventDestroy(p->ev_start);
@@ -94,18 +98,21 @@ tpt::GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const dou
 
 // steps 2.2 / 2.4: per z-plane, out_k = mat * in_k  (strided-batched, no transposes).  in_blocked / out_blocked: that
 // side is the mode-space field in the tile-blocked layout (kernels.cuh), whose z index has stride 16.
+// x0 / ncols: only the columns [x0, x0 + ncols) of every plane (ncols = 0: all); a blocked side is then a slab buffer of
+// its own, ncols columns wide (the L2-resident slab pipeline below), a natural side the full field.
 tpt::GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat, int k0, int nk,
-                     bool in_blocked, bool out_blocked) {
+                     bool in_blocked, bool out_blocked, int x0 = 0, int ncols = 0) {
     const int64_t plane = (int64_t)p->nx * p->ny;
+    const int w = ncols ? ncols : p->nx;
     tpt::GemmArgs g{};
     g.A = mat;
-    g.M = p->ny; g.N = p->nx; g.K = p->ny;
+    g.M = p->ny; g.N = w; g.K = p->ny;
     g.lda = p->ny; g.strideA = 0;
     g.batch = nk;
-    if (in_blocked) { g.B = in + (size_t)16 * k0; g.ldb = (int64_t)p->nx * p->nz; g.strideB = 16; g.ldgB = (int64_t)16 * p->nz; }
-    else { g.B = in + (size_t)plane * k0; g.ldb = p->nx; g.strideB = plane; }
-    if (out_blocked) { g.C = out + (size_t)16 * k0; g.ldc = (int64_t)p->nx * p->nz; g.strideC = 16; g.ldgC = (int64_t)16 * p->nz; }
-    else { g.C = out + (size_t)plane * k0; g.ldc = p->nx; g.strideC = plane; }
+    if (in_blocked) { g.B = in + (size_t)16 * k0; g.ldb = (int64_t)w * p->nz; g.strideB = 16; g.ldgB = (int64_t)16 * p->nz; }
+    else { g.B = in + (size_t)plane * k0 + x0; g.ldb = p->nx; g.strideB = plane; }
+    if (out_blocked) { g.C = out + (size_t)16 * k0; g.ldc = (int64_t)w * p->nz; g.strideC = 16; g.ldgC = (int64_t)16 * p->nz; }
+    else { g.C = out + (size_t)plane * k0 + x0; g.ldc = p->nx; g.strideC = plane; }
     return g;
 }
 
@@ -153,7 +160,7 @@ int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cuda
 // Runs one transform slot on z-planes [k0, k0 + nk) of the fields at in / out; *launches incremented by the kernels
 // enqueued.  `blocked`: the mode-space side of a y transform (output of 2.2, input of 2.4) is tile-blocked.
 int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int k0, int nk,
-             bool blocked = false) {
+             bool blocked = false, int x0 = 0, int ncols = 0) {
     cudaError_t e = cudaSuccess;
     const int d = (slot == TPT_K_FWD_X || slot == TPT_K_INV_X) ? 0 : 1;
     if (p->transform[d] == TPT_TRANSFORM_FFT) {   // uniform direction: fast transform, no transposes
@@ -168,14 +175,15 @@ int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t 
         a.nx = p->nx; a.ny = p->ny; a.planes = nk;
         a.s0 = p->fft_s[d][inv ? 2 : 0]; a.s1 = p->fft_s[d][inv ? 3 : 1];
         a.blocked = blk ? 1 : 0; a.nz = p->nz; a.k0 = k0;
+        if (d == 1) { a.x0 = x0; a.ncols = ncols; }
         ++*launches;
         return tpt::launch_fft(a, st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
     }
     switch (slot) {
         case TPT_K_FWD_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xfwd, k0, nk), st); ++*launches; break;
         case TPT_K_INV_X: e = run_gemm(p, gemm_x(p, in, out, p->d_xinv, k0, nk), st); ++*launches; break;
-        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd, k0, nk, false, blocked), st); ++*launches; break;
-        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv, k0, nk, blocked, false), st); ++*launches; break;
+        case TPT_K_FWD_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yfwd, k0, nk, false, blocked, x0, ncols), st); ++*launches; break;
+        case TPT_K_INV_Y: e = run_gemm(p, gemm_y(p, in, out, p->d_yinv, k0, nk, blocked, false, x0, ncols), st); ++*launches; break;
         default: return TPT_EINVAL;
     }
     return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
@@ -185,6 +193,80 @@ bool slot_active(const tpt_plan *p, int slot) {
     if (slot == TPT_K_FWD_X || slot == TPT_K_INV_X) return (p->dirs & 1) != 0;
     if (slot == TPT_K_FWD_Y || slot == TPT_K_INV_Y) return (p->dirs & 2) != 0;
     return slot == TPT_K_THOMAS;
+}
+
+// ---- L2-resident slab pipeline of steps 2.2 -> 2.3 -> 2.4 (BASELINE north_star "Fusion") -----------------
+// The mode-space field between the forward-y transform, the z sweep and the inverse-y transform is only ever needed one
+// x-slab at a time: the y transforms act column by column in x, the sweep column by column in (kx, ky).  So instead of
+// writing the whole field to HBM and reading it back twice, the three steps run slab by slab through two small slab
+// buffers (G 16-column groups x ny x nz, tile-blocked) that stay resident in the 126 MB L2: 4 of the 10 field-sized HBM
+// passes of a solve disappear.  Even and odd slabs alternate between the caller's stream and a second one, so the tail of
+// one slab's kernels overlaps the next slab's.  Pays where those steps are HBM-bound (fast y transforms); with GEMM y
+// transforms they are FP64-bound and a slab narrow enough for L2 would starve the 128-column GEMM tiles.
+size_t slab_bytes(const tpt_plan *p, int groups) { return (size_t)groups * 16 * p->ny * p->nz * sizeof(double); }
+
+int slab_groups_of(const tpt_plan *p) {
+    if (!use_blocked(p)) return 0;
+    if (p->slab_groups >= 0) return p->slab_groups > p->nx / 16 ? p->nx / 16 : p->slab_groups;
+    // automatic: off — measured on the box (profiles/r2_*.md) the slab pipeline does not pay with the present kernels
+    return 0;
+}
+
+int slab_setup(tpt_plan *p, int groups) {
+    const size_t need = slab_bytes(p, groups) / sizeof(double);
+    if (p->slab_elems < need) {
+        if (cudaDeviceSynchronize() != cudaSuccess) return TPT_ECUDA;
+        cudaFree(p->d_slab);
+        p->d_slab = nullptr;
+        p->slab_elems = 0;
+        cudaError_t e = cudaMalloc(&p->d_slab, 2 * need * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
+        p->slab_elems = need;
+    }
+    if (!p->st_slab) {
+        cudaStream_t s2 = nullptr;
+        cudaEvent_t ef = nullptr, ej = nullptr;
+        if (cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ef, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ej, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            if (ef) cudaEventDestroy(ef);
+            if (ej) cudaEventDestroy(ej);
+            if (s2) cudaStreamDestroy(s2);
+            return TPT_ECUDA;
+        }
+        p->st_slab = s2; p->ev_slab_fork = ef; p->ev_slab_join = ej;
+    }
+    return TPT_OK;
+}
+
+// steps 2.2-2.4 of one field, slab by slab: src (natural layout) -> dst (natural layout; src == dst allowed, a slab's
+// columns are read completely before they are written)
+int run_slabs(tpt_plan *p, const double *src, double *dst, int groups, cudaStream_t st, int *launches) {
+    int rc = slab_setup(p, groups);
+    if (rc != TPT_OK) return rc;
+    const int total = p->nx / 16;
+    const int nslabs = (total + groups - 1) / groups;
+    const bool two = nslabs > 1;
+    if (two && (cudaEventRecord(p->ev_slab_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->st_slab, p->ev_slab_fork, 0) != cudaSuccess))
+        return TPT_ECUDA;
+    for (int s = 0; s < nslabs; ++s) {
+        cudaStream_t q = (s & 1) ? p->st_slab : st;                 // buffer s & 1 belongs to stream s & 1: in-order reuse
+        double *buf = p->d_slab + (size_t)(s & 1) * p->slab_elems;
+        const int g0 = s * groups, ng = (total - g0 < groups) ? total - g0 : groups;
+        const int x0 = g0 * 16, ncols = ng * 16;
+        rc = run_slot(p, TPT_K_FWD_Y, src, buf, q, launches, 0, p->nz, true, x0, ncols);
+        if (rc != TPT_OK) return rc;
+        cudaError_t e = tpt::launch_thomas_onchip(buf, buf, p->d_abc, p->d_lamx + x0, p->d_lamy, p->d_wz, ncols, p->ny, p->nz, p->shift0,
+                                                  p->singular && x0 == 0, true, false, p->sms, q);
+        ++*launches;
+        if (e != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
+        rc = run_slot(p, TPT_K_INV_Y, buf, dst, q, launches, 0, p->nz, true, x0, ncols);
+        if (rc != TPT_OK) return rc;
+    }
+    if (two && (cudaEventRecord(p->ev_slab_join, p->st_slab) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_slab_join, 0) != cudaSuccess))
+        return TPT_ECUDA;
+    return TPT_OK;
 }
 
 // Grids that fit on chip run the whole solve as one cluster launch (fused_small.cu) — with the default kernel variants
@@ -226,6 +308,25 @@ int run_pipeline(tpt_plan *p, const double *rhs, double *out, int nf, cudaStream
         if (rc != TPT_OK) return rc;
         for (int s = 0; ev && s < TPT_K_COUNT; ++s)
             if (cudaEventRecord(ev[s + 1], st) != cudaSuccess) return TPT_ECUDA;
+        return TPT_OK;
+    }
+    const int slabs = slab_groups_of(p);
+    if (slabs > 0) {
+        // xyz: rhs -> W (2.1) -> slabs: W -> W (2.2-2.4) -> out (2.5);   yz: slabs: rhs -> out
+        const bool use_x = (p->dirs & 1) != 0;
+        int rc = TPT_OK;
+        if (use_x) rc = run_slot(p, TPT_K_FWD_X, rhs, W, st, launches, 0, nk);
+        if (rc != TPT_OK) return rc;
+        if (ev && cudaEventRecord(ev[TPT_K_FWD_X + 1], st) != cudaSuccess) return TPT_ECUDA;
+        for (int f = 0; f < nf && rc == TPT_OK; ++f)
+            rc = run_slabs(p, (use_x ? W : rhs) + f * pts, (use_x ? W : out) + f * pts, slabs, st, launches);
+        if (rc != TPT_OK) return rc;
+        // the three steps interleave slab by slab: their time is reported in the forward-y slot
+        for (int s = TPT_K_FWD_Y; ev && s <= TPT_K_INV_Y; ++s)
+            if (cudaEventRecord(ev[s + 1], st) != cudaSuccess) return TPT_ECUDA;
+        if (use_x) rc = run_slot(p, TPT_K_INV_X, W, out, st, launches, 0, nk);
+        if (rc != TPT_OK) return rc;
+        if (ev && cudaEventRecord(ev[TPT_K_INV_X + 1], st) != cudaSuccess) return TPT_ECUDA;
         return TPT_OK;
     }
     for (int s = 0; s < TPT_K_COUNT; ++s) {
@@ -272,11 +373,11 @@ GemmArgs gemm_x(const tpt_plan *p, const double *in, double *out, const double *
 }
 GemmArgs gemm_y(const tpt_plan *p, const double *in, double *out, const double *mat, int k0, int nk, bool in_blocked,
                 bool out_blocked) {
-    return ::gemm_y(p, in, out, mat, k0, nk, in_blocked, out_blocked);
+    return ::gemm_y(p, in, out, mat, k0, nk, in_blocked, out_blocked, 0, 0);
 }
 cudaError_t run_gemm(const tpt_plan *p, const GemmArgs &g, cudaStream_t st) { return ::run_gemm(p, g, st); }
 int run_slot(tpt_plan *p, int slot, const double *in, double *out, cudaStream_t st, int *launches, int k0, int nk, bool blocked) {
-    return ::run_slot(p, slot, in, out, st, launches, k0, nk, blocked);
+    return ::run_slot(p, slot, in, out, st, launches, k0, nk, blocked, 0, 0);
 }
 bool on_plan_device(const tpt_plan *p) { return ::on_plan_device(p); }
 }  // namespace detail
@@ -831,6 +932,12 @@ int tpt_plan_get_paths(const tpt_plan *p, int *paths_out) {
 int tpt_plan_set_gemm_variant(tpt_plan *p, int variant) {
     if (!p || variant < 0 || variant > 2) return TPT_EINVAL;
     p->gemm_variant = variant;
+    return TPT_OK;
+}
+
+int tpt_plan_set_slab_groups(tpt_plan *p, int groups) {
+    if (!p || groups < -1) return TPT_EINVAL;
+    p->slab_groups = groups;
     return TPT_OK;
 }
 

@@ -64,322 +64,457 @@ __device__ __forceinline__ void fft8(cplx *v) {
 // shared-memory index with one padding element per 8 (keeps the stride-R stores of the first pass conflict-free)
 __device__ __forceinline__ int pad(int i) { return i + (i >> 3); }
 
-// One Stockham pass of radix R over `pairs` sequences of length N, in place (sequences `npad` elements apart).
-// Work item j of a sequence: k = j mod Ns;  v_r = buf[j + r N/R] W^{r k N/(Ns R)};  radix-R butterfly;
-// buf[(j / Ns) Ns R + k + r Ns] = v_r.   A thread keeps all its items (at most ITEMS) in registers across the barrier
-// that separates the reads of a pass from its writes, so one buffer suffices (half the shared memory of a ping-pong
-// scheme: more CTAs per SM).  The twiddles of a pass come from its own table Wq[(r-1) Ns + k] =
-// e^{-2 pi i r k / (Ns R)} (conjugated for the inverse): lanes with consecutive k read consecutive entries.
-template <int R, int INV>
-__device__ __forceinline__ void stockham_pass(cplx *__restrict__ buf, int logN, int Ns, int pairs, int npad,
-                                              const double2 *__restrict__ Wq) {
-    constexpr int LOGR = R == 8 ? 3 : (R == 4 ? 2 : 1);
-    constexpr int ITEMS = 8 / R;                 // 4096 samples and >= 256 threads per CTA: one radix-8 item, two radix-4
-    const int logper = logN - LOGR, per = 1 << logper;
-    const int total = pairs << logper;
-    cplx v[ITEMS][R];
-#pragma unroll
-    for (int it = 0; it < ITEMS; ++it) {
-        const int item = threadIdx.x + it * blockDim.x;
-        if (item >= total) continue;
-        const int pr = item >> logper, j = item & (per - 1);
-        const cplx *s = buf + pr * npad;
-        const int k = j & (Ns - 1);
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            v[it][r] = s[pad(j + r * per)];
-            if (Ns > 1 && r > 0) {
-                const double2 w = __ldg(Wq + (r - 1) * Ns + k);
-                v[it][r] = cmul(v[it][r], cplx{w.x, INV ? -w.y : w.y});
-            }
-        }
-        if (R == 2) fft2<INV>(v[it]);
-        else if (R == 4) fft4<INV>(v[it][0], v[it][1], v[it][2], v[it][3]);
-        else fft8<INV>(v[it]);
-    }
-    __syncthreads();
-#pragma unroll
-    for (int it = 0; it < ITEMS; ++it) {
-        const int item = threadIdx.x + it * blockDim.x;
-        if (item >= total) continue;
-        const int pr = item >> logper, j = item & (per - 1);
-        cplx *d = buf + pr * npad;
-        const int k = j & (Ns - 1);
-        const int j0 = (j - k) * R + k;
-#pragma unroll
-        for (int r = 0; r < R; ++r) d[pad(j0 + r * Ns)] = v[it][r];
-    }
-    __syncthreads();
-}
-
 struct FftParams {
     const double *in;
     double *out;
-    const double2 *Wq[4]; // per-pass twiddle tables (see stockham_pass)
+    const double2 *Wq[4]; // per-pass twiddle tables: Wq[q][(r-1) Ns + k] = e^{-2 pi i r k / (Ns R)}
     const double2 *T4;    // e^{-i pi k / 2N},   k = 0..N-1
     int N, logN;          // transform length (nx for the x direction, ny for y) = 2^logN
     int bc;               // 0 Neumann, 1 Dirichlet, 2 periodic
     int nx, ny;           // field row length and rows per plane
-    int lines;            // x: rows to transform (ny * planes); y: unused
+    int lines;            // x: rows to transform (ny * planes)
+    int planes;           // y: z-planes of this launch
     int blk_in, blk_out;  // y only: that side is the tile-blocked mode-space layout (kernels.cuh); needs nz, k0
     int nz, k0;           // field depth and the z index of the launch's first plane
+    int bgroups;          // y only: 16-column groups per mode row of the blocked side (nx/16, or the slab width / 16)
     int radix[4];         // pass radices (0-terminated)
     double s0, s1;        // forward: output scale of the two special slots / of the others; inverse: input scales
 };
 
-// Input position of sample i in the complex sequence, and its sign (Makhoul reordering; DST: alternate signs).
-__device__ __forceinline__ int seq_index(int bc, int i, int N, double &sign) {
-    sign = 1.0;
-    if (bc == 2) return i;
-    if (bc == 1 && (i & 1)) sign = -1.0;
-    return (i & 1) ? N - 1 - (i >> 1) : (i >> 1);
-}
-// slots whose basis vector has norm^2 N instead of N/2
-__device__ __forceinline__ bool special_slot(int bc, int slot, int N) {
-    return bc == 0 ? slot == 0 : (bc == 1 ? slot == N - 1 : (slot == 0 || slot == N - 1));
-}
-
-// Line / element addressing, two neighbouring memory elements (one 16-byte access) per step.
-// X: a CTA owns `nl` consecutive rows (lines contiguous in memory, N = nx); step e2 -> samples i, i+1 of the two lines
-//    l, l+1 of a pair (two 16-byte accesses, two whole complex elements).
-// Y: a CTA owns `nl` neighbouring columns of one z-plane (lines strided by nx, N = ny; rows of nl*8 bytes);
-//    step e2 -> sample idx of the two lines 2c, 2c+1 — which are exactly the two halves of one complex sequence.
-template <bool YP>
-struct Lines {
-    size_t base;     // element offset of the CTA's first line
-    int nl, valid;   // lines of this CTA, and how many of them exist
-    int nx, N, logN, lognl;
-    __device__ __forceinline__ Lines(const FftParams &p, int nlines, int logn) : nl(nlines), nx(p.nx), N(1 << logn), logN(logn) {
-        lognl = 31 - __clz(nlines);
-        if (YP) {
-            base = (size_t)blockIdx.y * p.nx * p.ny + (size_t)blockIdx.x * nl;
-            valid = nl;
-        } else {
-            const int first = blockIdx.x * nl;
-            base = (size_t)first * p.nx;
-            valid = min(nl, p.lines - first);
-        }
-    }
-    __device__ __forceinline__ int steps() const { return YP ? (nl << logN) >> 1 : (nl << logN) >> 2; }
-    // (first line of a pair, sample index): X steps over two samples of both lines, Y over one sample of both lines
-    __device__ __forceinline__ void decode(int e2, int &l, int &idx) const {
-        if (YP) { idx = e2 >> (lognl - 1); l = (e2 & ((nl >> 1) - 1)) << 1; }
-        else { l = (e2 >> (logN - 1)) << 1; idx = (e2 & ((N >> 1) - 1)) << 1; }
-    }
-    __device__ __forceinline__ size_t addr(int l, int idx) const { return YP ? base + (size_t)idx * nx + l : base + ((size_t)l << logN) + idx; }
-    // y only: mode `idx` of column line l in the tile-blocked layout ((m (nx/16) + i/16) nz + k) 16 + i mod 16
-    __device__ __forceinline__ size_t addr_blocked(const FftParams &p, int l, int idx) const {
-        const int i = blockIdx.x * nl + l, k = p.k0 + blockIdx.y;
-        return (((size_t)idx * (p.nx >> 4) + (i >> 4)) * p.nz + k) * 16 + (i & 15);
-    }
-};
-
 // Everything that depends only on the transform length is a compile-time constant of the kernel (template LOGN): the
-// pass radices, the lines and threads per CTA, every shift, mask and padded offset — index arithmetic was most of the
-// instruction count when these were run-time values (profiles/r1d_fft_path.md).
+// pass radices, the lines per CTA, every shift, mask and padded offset.
 __host__ __device__ constexpr int radix_at(int logn, int q) {            // as many 8s as possible, then 4 (or 4, 4)
     const int n8 = logn / 3, rem = logn % 3;
     if (rem == 1) return q < n8 - 1 ? 8 : (q < n8 + 1 ? 4 : 0);
     return q < n8 ? 8 : ((rem == 2 && q == n8) ? 4 : 0);
 }
-__host__ __device__ constexpr int lines_of(bool yp, int logn) {          // lines (real sequences) per CTA
-    const int n = 1 << logn;
-    if (!yp) return n >= 2048 ? 2 : 2 * (2048 / n);                       // x: 4096 samples
-    int cols = 8192 / n;                                                  // y: 8192 samples, rows of at least 64 bytes
-    if (cols > 16) cols = 16;
-    if (cols < 8) cols = n <= 1024 ? 8 : 4;
-    return cols;
+__host__ __device__ constexpr int npasses(int logn) { return radix_at(logn, 1) == 0 ? 1 : (radix_at(logn, 2) == 0 ? 2 : (radix_at(logn, 3) == 0 ? 3 : 4)); }
+
+// Geometry of one CTA: every thread holds 16 complex values (two real lines ride in one complex sequence).
+//   x: 4096 / N consecutive rows, 128 threads (four CTAs per SM interleave their load / compute / store phases).
+//   y: 8192 samples, 256 threads: a tile of COLS neighbouring columns (128-byte rows up to N = 512, 64 / 32 bytes
+//   for N = 1024 / 2048) of PL consecutive z-planes.
+// Thread t holds the 16 values of its work items in registers through every pass.  Thread <-> (pair of lines pr, slice u
+// of the sequence, u in [0, N/16)):  y: pr fastest — the 8 lanes of a quarter-warp are the 8 column pairs of one row, so
+// every global access is a whole 128-byte row and every shared-memory access hits 8 different sequences (NPAD keeps
+// them in different banks);  x: u fastest — consecutive lanes hold consecutive sequence elements.
+template <bool YP, int LOGN>
+struct Geo {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int COLS = N <= 512 ? 16 : (N == 1024 ? 8 : 4);
+    static constexpr int PL = N >= 512 ? 1 : 512 / N;
+    static constexpr int LINES = YP ? COLS * PL : (N >= 2048 ? 2 : 4096 / N);
+    static constexpr int PAIRS = LINES / 2;
+    static constexpr int UPP = N / 16;
+    static constexpr int THREADS = PAIRS * UPP;                          // y: 256, x: 128
+    static constexpr int MINB = 512 / THREADS;                           // CTAs per SM the 128-register budget admits
+    static constexpr int BANKSTEP = !YP ? 1 : (COLS == 16 ? 1 : (COLS == 8 ? 2 : 4));
+    static constexpr int NPAD = ((N + (N >> 3) + 7) & ~7) + BANKSTEP;    // padded sequence length (complex elements)
+    static constexpr size_t SMEM = (size_t)PAIRS * NPAD * 16;
+};
+
+template <int R, int INV>
+__device__ __forceinline__ void bfly(cplx *v) {
+    if (R == 8) fft8<INV>(v);
+    else fft4<INV>(v[0], v[1], v[2], v[3]);
 }
-__host__ __device__ constexpr int threads_of(bool yp, int logn) {
-    if (!yp) return 256;
-    const int t = (lines_of(true, logn) / 2) * ((1 << logn) / 8);
-    return t < 64 ? 64 : t;
-}
-template <int LOGN, int INV, int Q = 0, int NS = 1>
-__device__ __forceinline__ void run_passes(cplx *buf, const FftParams &p, int pairs, int npad) {
-    constexpr int R = radix_at(LOGN, Q);
-    if constexpr (R != 0) {
-        stockham_pass<R, INV>(buf, LOGN, NS, pairs, npad, p.Wq[Q]);
-        run_passes<LOGN, INV, Q + 1, NS * R>(buf, p, pairs, npad);
+template <int R, int INV>
+__device__ __forceinline__ void twiddle(cplx *v, const double2 *__restrict__ Wq, int Ns, int k) {
+#pragma unroll
+    for (int r = 1; r < R; ++r) {
+        const double2 w = __ldg(Wq + (r - 1) * Ns + k);
+        v[r] = cmul(v[r], cplx{w.x, INV ? -w.y : w.y});
     }
 }
 
-// spectrum slot -> (FFT bin k, which real combination): value of one line at `slot` from its untangled bin V_k
-__device__ __forceinline__ int slot_bin(int bc, int slot, int N) {
-    return bc == 2 ? (slot + 1) >> 1 : (bc == 0 ? slot : N - 1 - slot);
+// Sample position of element n of the complex sequence, and its sign (Makhoul reordering v_n = f_{2n},
+// v_{N-1-n} = f_{2n+1}; the sine transform alternates signs; the periodic case is the plain DFT).
+template <int BC, int N>
+__device__ __forceinline__ int sample_of(int n, double &sign) {
+    sign = 1.0;
+    if (BC == 2) return n;
+    const int i = n < N / 2 ? 2 * n : 2 * (N - 1 - n) + 1;
+    if (BC == 1 && (i & 1)) sign = -1.0;
+    return i;
 }
-__device__ __forceinline__ double slot_value(int bc, int slot, cplx V, double2 t4) {
-    if (bc == 2) return (slot == 0 || (slot & 1)) ? V.x : -V.y;          // cos rows: Re X_j, sin rows: -Im X_j
-    return fma(t4.x, V.x, -t4.y * V.y);                                  // C_k = Re(e^{-i pi k / 2N} V_k)
+// slots whose basis vector has norm^2 N instead of N/2
+template <int BC, int N>
+__device__ __forceinline__ bool special_slot(int slot) {
+    return BC == 0 ? slot == 0 : (BC == 1 ? slot == N - 1 : (slot == 0 || slot == N - 1));
 }
+
+// Middle passes Q = 1 .. NP-2: in-place Stockham pass through shared memory.  Item j of a sequence: k = j mod Ns;
+// v_r = buf[j + r N/R] W^{r k}; radix-R butterfly; buf[(j - k) R + k + r Ns] = v_r.
+template <int LOGN, int INV, int Q, int NS, int UPP>
+__device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParams &p, int u) {
+    constexpr int NP = npasses(LOGN), N = 1 << LOGN;
+    if constexpr (Q < NP - 1) {
+        constexpr int R = radix_at(LOGN, Q), IT = 16 / R, PER = N / R;
+#pragma unroll
+        for (int it = 0; it < IT; ++it) {
+            const int j = u + it * UPP, k = j & (NS - 1);
+#pragma unroll
+            for (int r = 0; r < R; ++r) v[it * R + r] = seq[pad(j + r * PER)];
+            twiddle<R, INV>(v + it * R, p.Wq[Q], NS, k);
+            bfly<R, INV>(v + it * R);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < IT; ++it) {
+            const int j = u + it * UPP, k = j & (NS - 1);
+#pragma unroll
+            for (int r = 0; r < R; ++r) seq[pad((j - k) * R + k + r * NS)] = v[it * R + r];
+        }
+        __syncthreads();
+        middle_passes<LOGN, INV, Q + 1, NS * R, UPP>(seq, v, p, u);
+    }
+}
+// Items of the pass whose bins must come in conjugate pairs (k, N - k) — the last forward pass (untangling the two
+// real lines needs Z_k and Z_{N-k}) and the first inverse pass (a Hermitian spectrum is built from a_k and a_{N-k}).
+// Item j covers the bins j + r PER (PER = N/R); the partner bins N - j - r PER belong to item PER - j, r' = R-1-r.  A
+// thread therefore takes the items (u, PER - u) [and (u + UPP, PER - UPP - u) for radix 4]; the self-paired items 0 and
+// PER/2 go together to thread u = 0.
+template <int R, int PER, int UPP>
+__device__ __forceinline__ void paired_items(int u, int *j) {
+    j[0] = u;
+    j[1] = u ? PER - u : PER / 2;
+    if (R == 4) {
+        j[2] = u + UPP;
+        j[3] = PER - UPP - u;
+    }
+}
+
+// ---- per-CTA line addressing --------------------------------------------------------------------------------------
+// y: row idx of my column pair (both lines: one 16-byte access) lives at base + idx * stride on either side — natural
+//    layout: stride nx; tile-blocked layout ((idx bgroups + col/16) nz + k) 16 + col%16: stride bgroups * nz * 16.
+// x: my two lines are rows of N contiguous elements.
+template <bool YP, int LOGN>
+struct Addr {
+    using G = Geo<YP, LOGN>;
+    size_t in_base, out_base, in_stride, out_stride;
+    bool ok0, ok1;        // the two lines of my pair exist
+    __device__ __forceinline__ Addr(const FftParams &p, int pr) {
+        if (YP) {
+            const int cp = pr % (G::COLS / 2), pl = pr / (G::COLS / 2);
+            const int col = blockIdx.x * G::COLS + 2 * cp;
+            const int plane = blockIdx.y * G::PL + pl;
+            ok0 = ok1 = plane < p.planes;
+            const size_t nat = (size_t)plane * p.nx * p.ny + col;
+            const size_t blk = ((size_t)(col >> 4) * p.nz + (p.k0 + plane)) * 16 + (col & 15);
+            const size_t bstride = (size_t)p.bgroups * p.nz * 16;
+            in_base = p.blk_in ? blk : nat;
+            in_stride = p.blk_in ? bstride : (size_t)p.nx;
+            out_base = p.blk_out ? blk : nat;
+            out_stride = p.blk_out ? bstride : (size_t)p.nx;
+        } else {
+            const int l = blockIdx.x * G::LINES + 2 * pr;
+            ok0 = l < p.lines;
+            ok1 = l + 1 < p.lines;
+            in_base = out_base = (size_t)l << LOGN;
+            in_stride = out_stride = 0;
+        }
+    }
+};
 
 // Forward: out[line][slot] = s(slot) * sum_i q_slot(i) in[line][i]   (Eq. 10 with Q^-1 = Q~^T D^{1/2}, D = w I)
+//   y: the first pass reads its 16 rows straight from global memory (whole 128-byte rows per quarter-warp);
+//   x: the rows are staged once through shared memory (coalesced 16-byte loads, Makhoul scatter);
+//   last pass: paired items, the two lines untangled in registers, every result stored straight to global memory.
 template <bool YP, int LOGN, int BC>
-__global__ void __launch_bounds__(threads_of(YP, LOGN), threads_of(YP, LOGN) > 256 ? 2 : 4)
-fft_forward_kernel(const FftParams p) {
+__global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) fft_forward_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int N = 1 << LOGN, nlines = lines_of(YP, LOGN), pairs = nlines >> 1;
-    constexpr int npad = N + (N >> 3) + 1;       // padded length + 1: neighbouring sequences start in different banks
-    constexpr int bc = BC;
-    cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
-    const Lines<YP> L(p, nlines, LOGN);
-    const int steps = L.steps();
-#pragma unroll 4
-    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
-        int l, i;
-        L.decode(e2, l, i);
-        if (YP) {            // v = sample i of lines l, l+1: one complex element
-            const double2 v = *reinterpret_cast<const double2 *>(p.in + L.addr(l, i));
-            double sign;
-            const int n = seq_index(bc, i, N, sign);
-            b0[(l >> 1) * npad + pad(n)] = cplx{sign * v.x, sign * v.y};
-        } else {             // samples i (even), i+1 of lines l and l+1: two complex elements
-            double2 va = make_double2(0.0, 0.0), vb = va;
-            if (l < L.valid) va = *reinterpret_cast<const double2 *>(p.in + L.addr(l, i));
-            if (l + 1 < L.valid) vb = *reinterpret_cast<const double2 *>(p.in + L.addr(l + 1, i));
-            double s0, s1;
-            const int n0 = seq_index(bc, i, N, s0), n1 = seq_index(bc, i + 1, N, s1);
-            cplx *z = b0 + (l >> 1) * npad;
-            z[pad(n0)] = cplx{s0 * va.x, s0 * vb.x};
-            z[pad(n1)] = cplx{s1 * va.y, s1 * vb.y};
+    using G = Geo<YP, LOGN>;
+    constexpr int N = G::N, NP = npasses(LOGN), UPP = G::UPP, NPAD = G::NPAD;
+    cplx *buf = reinterpret_cast<cplx *>(smem_raw);
+    const int t = threadIdx.x;
+    const int pr = YP ? t % G::PAIRS : t / UPP;
+    const int u = YP ? t / G::PAIRS : t % UPP;
+    cplx *seq = buf + pr * NPAD;
+    const Addr<YP, LOGN> A(p, pr);
+    cplx v[16];
+
+    // ---- pass 0 (Ns = 1: no twiddles) -------------------------------------------------------------------------------
+    constexpr int R0 = radix_at(LOGN, 0), IT0 = 16 / R0, PER0 = N / R0;
+    if (YP) {
+        // all 16 loads are issued before the first use (no branch, no arithmetic on a loaded value in between)
+        if (A.ok0) {
+            const double *src = p.in + A.in_base;
+#pragma unroll
+            for (int it = 0; it < IT0; ++it)
+#pragma unroll
+                for (int r = 0; r < R0; ++r) {
+                    double sg;
+                    const int i = sample_of<BC, N>(u + it * UPP + r * PER0, sg);
+                    const double2 w = *reinterpret_cast<const double2 *>(src + (size_t)i * A.in_stride);
+                    v[it * R0 + r] = cplx{w.x, w.y};
+                }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) v[q] = cplx{0.0, 0.0};
         }
+        if (BC == 1) {
+#pragma unroll
+            for (int it = 0; it < IT0; ++it)
+#pragma unroll
+                for (int r = 0; r < R0; ++r) {
+                    double sg;
+                    sample_of<BC, N>(u + it * UPP + r * PER0, sg);
+                    v[it * R0 + r] = cplx{sg * v[it * R0 + r].x, sg * v[it * R0 + r].y};
+                }
+        }
+    } else {
+        // CTA-wide coalesced load: step e -> samples i, i+1 of the lines l, l+1 of a pair -> two complex elements.
+        // All of a thread's loads are issued before the first shared-memory store (v[] serves as the landing registers);
+        // lines past the end of the field (last CTA only) are read from the last existing line and zeroed.
+        constexpr int STEPS = G::PAIRS * (N / 2), IT = STEPS / G::THREADS;
+        static_assert(IT == 8 && STEPS % G::THREADS == 0, "16 landing registers per thread");
+        const int lmax = p.lines - 1;
+#pragma unroll
+        for (int s = 0; s < IT; ++s) {
+            const int e = t + s * G::THREADS;
+            const int q = e >> (LOGN - 1), i = (e & (N / 2 - 1)) << 1;
+            const int l = blockIdx.x * G::LINES + 2 * q;
+            const double2 va = *reinterpret_cast<const double2 *>(p.in + ((size_t)min(l, lmax) << LOGN) + i);
+            const double2 vb = *reinterpret_cast<const double2 *>(p.in + ((size_t)min(l + 1, lmax) << LOGN) + i);
+            v[2 * s] = cplx{va.x, va.y};
+            v[2 * s + 1] = cplx{vb.x, vb.y};
+        }
+#pragma unroll
+        for (int s = 0; s < IT; ++s) {
+            const int e = t + s * G::THREADS;
+            const int q = e >> (LOGN - 1), i = (e & (N / 2 - 1)) << 1;
+            const int l = blockIdx.x * G::LINES + 2 * q;
+            cplx va = v[2 * s], vb = v[2 * s + 1];
+            if (l > lmax) va = cplx{0.0, 0.0};
+            if (l + 1 > lmax) vb = cplx{0.0, 0.0};
+            cplx *z = buf + q * NPAD;
+            if (BC == 2) {
+                z[pad(i)] = cplx{va.x, vb.x};
+                z[pad(i + 1)] = cplx{va.y, vb.y};
+            } else {       // i even -> n = i/2; i + 1 odd -> n = N - 1 - i/2 (sign flips for the sine transform)
+                const double s1 = BC == 1 ? -1.0 : 1.0;
+                z[pad(i >> 1)] = cplx{va.x, vb.x};
+                z[pad(N - 1 - (i >> 1))] = cplx{s1 * va.y, s1 * vb.y};
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < IT0; ++it)
+#pragma unroll
+            for (int r = 0; r < R0; ++r) v[it * R0 + r] = seq[pad(u + it * UPP + r * PER0)];
+        __syncthreads();
+    }
+#pragma unroll
+    for (int it = 0; it < IT0; ++it) {
+        bfly<R0, 0>(v + it * R0);
+#pragma unroll
+        for (int r = 0; r < R0; ++r) seq[pad((u + it * UPP) * R0 + r)] = v[it * R0 + r];
     }
     __syncthreads();
-    run_passes<LOGN, 0>(b0, p, pairs, npad);
-    const cplx *Z = b0;
-#pragma unroll 4
-    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
-        int l, slot;
-        L.decode(e2, l, slot);
-        if (l >= L.valid) continue;
-        const cplx *z = Z + (l >> 1) * npad;
-        double2 o;
-        if (YP) {            // one slot, both lines of the pair
-            const int k = slot_bin(bc, slot, N);
-            const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
-            const double2 t4 = __ldg(p.T4 + k);
-            const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
-            o.x = sc * slot_value(bc, slot, cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, t4);
-            o.y = sc * slot_value(bc, slot, cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)}, t4);
-        } else {             // slots `slot`, `slot + 1` of both lines of the pair
-            double ra[2], rb[2];
+    middle_passes<LOGN, 0, 1, R0, UPP>(seq, v, p, u);
+
+    // ---- last pass: paired items; Ns = PER = N / R ---------------------------------------------------------------------
+    constexpr int RL = radix_at(LOGN, NP - 1), ITL = 16 / RL, NSL = N / RL;
+    int jl[4];
+    paired_items<RL, NSL, UPP>(u, jl);
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int sl = slot + h, k = slot_bin(bc, sl, N);
-                const cplx zk = z[pad(k)], zm = z[pad((N - k) & (N - 1))];
-                const double2 t4 = __ldg(p.T4 + k);
-                const double sc = special_slot(bc, sl, N) ? p.s0 : p.s1;
-                ra[h] = sc * slot_value(bc, sl, cplx{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, t4);
-                rb[h] = sc * slot_value(bc, sl, cplx{0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x)}, t4);
-            }
-            o = make_double2(ra[0], ra[1]);
-            if (l + 1 < L.valid) *reinterpret_cast<double2 *>(p.out + L.addr(l + 1, slot)) = make_double2(rb[0], rb[1]);
+    for (int it = 0; it < ITL; ++it) {
+#pragma unroll
+        for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[pad(jl[it] + r * NSL)];
+        twiddle<RL, 0>(v + it * RL, p.Wq[NP - 1], NSL, jl[it]);
+        bfly<RL, 0>(v + it * RL);
+    }
+    // v[it RL + r] = Z[jl[it] + r NSL].  Untangle (V1_k = (Z_k + conj Z_{N-k}) / 2, V2_k = (Z_k - conj Z_{N-k}) / 2i;
+    // V_{N-k} = conj V_k for real lines), apply e^{-i pi k / 2N}, scale, store.
+    auto store = [&](int slot, double o1, double o2) {
+        const double sc = special_slot<BC, N>(slot) ? p.s0 : p.s1;
+        if (YP) {
+            if (A.ok0) *reinterpret_cast<double2 *>(p.out + A.out_base + (size_t)slot * A.out_stride) = make_double2(sc * o1, sc * o2);
+        } else {
+            if (A.ok0) p.out[A.out_base + slot] = sc * o1;
+            if (A.ok1) p.out[A.out_base + N + slot] = sc * o2;
         }
-        *reinterpret_cast<double2 *>(p.out + ((YP && p.blk_out) ? L.addr_blocked(p, l, slot) : L.addr(l, slot))) = o;
+    };
+    auto emit = [&](int k, cplx zk, cplx zm) {               // bins k and N - k; zm = Z_{N-k};  0 < k < N, k != N/2
+        const cplx V1{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, V2{0.5 * (zk.y + zm.y), 0.5 * (zm.x - zk.x)};
+        if (BC == 2) {
+            const int kk = k < N / 2 ? k : N - k;
+            const double sg = k < N / 2 ? -1.0 : 1.0;           // slot 2kk-1: Re V_kk, slot 2kk: -Im V_kk
+            store(2 * kk - 1, V1.x, V2.x);
+            store(2 * kk, sg * V1.y, sg * V2.y);
+        } else {
+            const double2 tk = __ldg(p.T4 + k), tm = __ldg(p.T4 + (N - k));
+            store(BC == 0 ? k : N - 1 - k, fma(tk.x, V1.x, -tk.y * V1.y), fma(tk.x, V2.x, -tk.y * V2.y));
+            store(BC == 0 ? N - k : k - 1, fma(tm.x, V1.x, tm.y * V1.y), fma(tm.x, V2.x, tm.y * V2.y));
+        }
+    };
+    auto emit_single = [&](int k, cplx z) {                  // k = 0 or N/2: its own partner; V1 = Re Z, V2 = Im Z
+        if (BC == 2) {
+            store(k == 0 ? 0 : N - 1, z.x, z.y);
+        } else {
+            const double tx = k == 0 ? 1.0 : 0.70710678118654752440;    // Re e^{-i pi k / 2N}
+            store(BC == 0 ? k : N - 1 - k, tx * z.x, tx * z.y);
+        }
+    };
+    if (RL == 4) {
+#pragma unroll
+        for (int r = 0; r < RL; ++r) emit(jl[2] + r * NSL, v[2 * RL + r], v[3 * RL + RL - 1 - r]);
+    }
+    if (u) {
+#pragma unroll
+        for (int r = 0; r < RL; ++r) emit(jl[0] + r * NSL, v[r], v[RL + RL - 1 - r]);
+    } else {
+        emit_single(0, v[0]);
+        emit_single(N / 2, v[RL / 2]);
+#pragma unroll
+        for (int r = 1; r < RL / 2; ++r) emit(r * NSL, v[r], v[RL - r]);
+#pragma unroll
+        for (int r = 0; r < RL / 2; ++r) emit(NSL / 2 + r * NSL, v[RL + r], v[RL + RL - 1 - r]);
     }
 }
 
 // Inverse: out[line][i] = sum_slot q_slot(i) s(slot) in[line][slot]   (Eq. 12 with Q = D^{-1/2} Q~)
+//   first pass: paired items; the Hermitian-symmetrised spectrum B of each line (its inverse DFT is real; the pair rides
+//   as Z = B_1 + i B_2) is built in registers straight from the global loads of the scaled coefficients;
+//   y: the last pass stores its 16 rows straight to global memory;  x: one pass through shared memory for coalesced rows.
 template <bool YP, int LOGN, int BC>
-__global__ void __launch_bounds__(threads_of(YP, LOGN), threads_of(YP, LOGN) > 256 ? 2 : 4)
-fft_inverse_kernel(const FftParams p) {
+__global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) fft_inverse_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int N = 1 << LOGN, logN = LOGN, nlines = lines_of(YP, LOGN), pairs = nlines >> 1;
-    constexpr int npad = N + (N >> 3) + 1;
-    constexpr int bc = BC;
-    cplx *b0 = reinterpret_cast<cplx *>(smem_raw);
-    cplx *Cc = b0;                   // staged scaled coefficients [pair][slot] = (line 2 pr, line 2 pr + 1), overwritten by Z
-    constexpr int cstr = N + 1;      // pair stride: neighbouring pairs in different banks
-    // (x keeps the two lines of a pair as two real arrays, `rstr` apart: its 16-byte stores are then conflict-free)
-    double *Rr = reinterpret_cast<double *>(b0);
-    constexpr int rstr = N + 2;
-    const Lines<YP> L(p, nlines, LOGN);
-    const int steps = L.steps();
-#pragma unroll 4
-    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
-        int l, slot;
-        L.decode(e2, l, slot);
-        if (YP) {            // slot of lines l, l+1
-            const double2 v = *reinterpret_cast<const double2 *>(p.in + (p.blk_in ? L.addr_blocked(p, l, slot) : L.addr(l, slot)));
-            const double sc = special_slot(bc, slot, N) ? p.s0 : p.s1;
-            Cc[(l >> 1) * cstr + slot] = cplx{sc * v.x, sc * v.y};
-        } else {             // slots slot, slot+1 of lines l and l+1
-            double2 va = make_double2(0.0, 0.0), vb = va;
-            if (l < L.valid) va = *reinterpret_cast<const double2 *>(p.in + L.addr(l, slot));
-            if (l + 1 < L.valid) vb = *reinterpret_cast<const double2 *>(p.in + L.addr(l + 1, slot));
-            const double sc0 = special_slot(bc, slot, N) ? p.s0 : p.s1, sc1 = special_slot(bc, slot + 1, N) ? p.s0 : p.s1;
-            *reinterpret_cast<double2 *>(Rr + l * rstr + slot) = make_double2(sc0 * va.x, sc1 * va.y);
-            *reinterpret_cast<double2 *>(Rr + (l + 1) * rstr + slot) = make_double2(sc0 * vb.x, sc1 * vb.y);
-        }
-    }
-    __syncthreads();
-    // Hermitian-symmetrised spectrum B of each line (its inverse DFT is real); the pair rides as Z = B_even + i B_odd.
-    // Built in registers (at most ZITEMS elements per thread), then written over the staged coefficients.
-    constexpr int ZITEMS = 8;
-    cplx zreg[ZITEMS];
+    using G = Geo<YP, LOGN>;
+    constexpr int N = G::N, NP = npasses(LOGN), UPP = G::UPP, NPAD = G::NPAD;
+    cplx *buf = reinterpret_cast<cplx *>(smem_raw);
+    const int t = threadIdx.x;
+    const int pr = YP ? t % G::PAIRS : t / UPP;
+    const int u = YP ? t / G::PAIRS : t % UPP;
+    cplx *seq = buf + pr * NPAD;
+    const Addr<YP, LOGN> A(p, pr);
+    cplx v[16];
+
+    // ---- first pass: paired items, inputs built from the coefficients ---------------------------------------------------
+    constexpr int R0 = radix_at(LOGN, 0), IT0 = 16 / R0, PER0 = N / R0;
+    int j0[4];
+    paired_items<R0, PER0, UPP>(u, j0);
+    // Every register position first receives the coefficient its own bin contributes: bin k of a cosine / sine transform
+    // the coefficient a_k; of the real DFT, a bin below N/2 the cosine coefficient of its frequency and its partner N - k
+    // the sine coefficient.  All 16 loads are issued before the first use (no branch, no arithmetic in between); the
+    // scales follow, then the conjugate pairs are combined in place.
+    auto slot_for = [&](int k) -> int {
+        if (BC == 0) return k;
+        if (BC == 1) return N - 1 - k;
+        return k == 0 ? 0 : (k == N / 2 ? N - 1 : (k < N / 2 ? 2 * k - 1 : 2 * (N - k)));
+    };
+    if (A.ok0) {
+        const double *src = p.in + A.in_base;
+        const double *src1 = A.ok1 ? src + N : src;           // x: second line of the pair (a copy of the first if it does not exist)
 #pragma unroll
-    for (int it = 0; it < ZITEMS; ++it) {
-        const int item = threadIdx.x + it * blockDim.x;
-        if (item >= (pairs << logN)) continue;
-        const int pr = item >> logN, k = item & (N - 1);
-        cplx B[2];
-        // scaled coefficient q of both lines of the pair
-        auto c = [&](int q) -> cplx {
-            if (YP) return Cc[pr * cstr + q];
-            return cplx{Rr[2 * pr * rstr + q], Rr[(2 * pr + 1) * rstr + q]};
-        };
-        if (bc == 2) {
-            const int j = k <= N / 2 ? k : N - k;                          // B_k = b_k / 2, B_{N-k} = conj(b_k) / 2
-            if (j == 0 || j == N / 2) {
-                const cplx a = c(j == 0 ? 0 : N - 1);
-                B[0] = {a.x, 0.0};
-                B[1] = {a.y, 0.0};
-            } else {
-                const cplx ar = c(2 * j - 1), ai = c(2 * j);
-                const double sg = k < N / 2 ? -0.5 : 0.5;
-                B[0] = {0.5 * ar.x, sg * ai.x};
-                B[1] = {0.5 * ar.y, sg * ai.y};
+        for (int it = 0; it < IT0; ++it)
+#pragma unroll
+            for (int r = 0; r < R0; ++r) {
+                const int slot = slot_for(j0[it] + r * PER0);
+                if (YP) {
+                    const double2 w = *reinterpret_cast<const double2 *>(src + (size_t)slot * A.in_stride);
+                    v[it * R0 + r] = cplx{w.x, w.y};
+                } else {
+                    v[it * R0 + r] = cplx{src[slot], src1[slot]};
+                }
             }
-        } else if (k == 0) {
-            const cplx a = c(bc == 0 ? 0 : N - 1);
-            B[0] = {a.x, 0.0};
-            B[1] = {a.y, 0.0};
-        } else {
-            const cplx ak = c(bc == 0 ? k : N - 1 - k), am = c(bc == 0 ? N - k : k - 1);
-            const double2 t = __ldg(p.T4 + k);                             // e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2
-            B[0] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak.x, -am.x});
-            B[1] = cmul(cplx{0.5 * t.x, -0.5 * t.y}, cplx{ak.y, -am.y});
-        }
-        zreg[it] = cplx{B[0].x - B[1].y, B[0].y + B[1].x};
-    }
-    __syncthreads();
+    } else {
 #pragma unroll
-    for (int it = 0; it < ZITEMS; ++it) {
-        const int item = threadIdx.x + it * blockDim.x;
-        if (item >= (pairs << logN)) continue;
-        b0[(item >> logN) * npad + pad(item & (N - 1))] = zreg[it];
+        for (int q = 0; q < 16; ++q) v[q] = cplx{0.0, 0.0};
+    }
+#pragma unroll
+    for (int it = 0; it < IT0; ++it)
+#pragma unroll
+        for (int r = 0; r < R0; ++r) {
+            const double sc = special_slot<BC, N>(slot_for(j0[it] + r * PER0)) ? p.s0 : p.s1;
+            v[it * R0 + r] = cplx{sc * v[it * R0 + r].x, sc * v[it * R0 + r].y};
+        }
+    // (zk, zm) hold the coefficients of bins k and N - k on entry, Z_k and Z_{N-k} on exit;  0 < k < N, k != N/2
+    auto build = [&](int k, cplx &zk, cplx &zm) {
+        if (BC == 2) {
+            const cplx ar = k < N / 2 ? zk : zm, ai = k < N / 2 ? zm : zk;   // B_kk = (ar - i ai) / 2, B_{N-kk} = (ar + i ai) / 2 per line
+            const cplx lo{0.5 * (ar.x + ai.y), 0.5 * (ar.y - ai.x)}, hi{0.5 * (ar.x - ai.y), 0.5 * (ar.y + ai.x)};
+            zk = k < N / 2 ? lo : hi;
+            zm = k < N / 2 ? hi : lo;
+        } else {
+            const cplx ak = zk, am = zm;
+            const double2 tk = __ldg(p.T4 + k), tm = __ldg(p.T4 + (N - k));
+            // B_k = e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2 per line; Z = B_1 + i B_2
+            const cplx b1 = cmul(cplx{0.5 * tk.x, -0.5 * tk.y}, cplx{ak.x, -am.x}), b2 = cmul(cplx{0.5 * tk.x, -0.5 * tk.y}, cplx{ak.y, -am.y});
+            zk = cplx{b1.x - b2.y, b1.y + b2.x};
+            const cplx c1 = cmul(cplx{0.5 * tm.x, -0.5 * tm.y}, cplx{am.x, -ak.x}), c2 = cmul(cplx{0.5 * tm.x, -0.5 * tm.y}, cplx{am.y, -ak.y});
+            zm = cplx{c1.x - c2.y, c1.y + c2.x};
+        }
+    };
+    if (R0 == 4) {
+#pragma unroll
+        for (int r = 0; r < R0; ++r) build(j0[2] + r * PER0, v[2 * R0 + r], v[3 * R0 + R0 - 1 - r]);
+    }
+    if (u) {
+#pragma unroll
+        for (int r = 0; r < R0; ++r) build(j0[0] + r * PER0, v[r], v[R0 + R0 - 1 - r]);
+    } else {
+        // bins 0 and N/2 are their own partners: B_0 = a_0 and (cosine / sine) B_{N/2} = e^{+i pi / 4} (a - i a) / 2 = a / sqrt 2
+        if (BC != 2) v[R0 / 2] = cplx{0.70710678118654752440 * v[R0 / 2].x, 0.70710678118654752440 * v[R0 / 2].y};
+#pragma unroll
+        for (int r = 1; r < R0 / 2; ++r) build(r * PER0, v[r], v[R0 - r]);
+#pragma unroll
+        for (int r = 0; r < R0 / 2; ++r) build(PER0 / 2 + r * PER0, v[R0 + r], v[R0 + R0 - 1 - r]);
+    }
+#pragma unroll
+    for (int it = 0; it < IT0; ++it) {
+        bfly<R0, 1>(v + it * R0);
+#pragma unroll
+        for (int r = 0; r < R0; ++r) seq[pad(j0[it] * R0 + r)] = v[it * R0 + r];
     }
     __syncthreads();
-    run_passes<LOGN, 1>(b0, p, pairs, npad);
-    const cplx *Z = b0;
+    middle_passes<LOGN, 1, 1, R0, UPP>(seq, v, p, u);
+
+    // ---- last pass ------------------------------------------------------------------------------------------------------
+    constexpr int RL = radix_at(LOGN, NP - 1), ITL = 16 / RL, NSL = N / RL;
+#pragma unroll
+    for (int it = 0; it < ITL; ++it) {
+        const int j = u + it * UPP;
+#pragma unroll
+        for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[pad(j + r * NSL)];
+        twiddle<RL, 1>(v + it * RL, p.Wq[NP - 1], NSL, j);
+        bfly<RL, 1>(v + it * RL);
+    }
+    if (YP) {       // z[n] -> sample i(n) of both lines: one 16-byte store per row
+#pragma unroll
+        for (int it = 0; it < ITL; ++it)
+#pragma unroll
+            for (int r = 0; r < RL; ++r) {
+                double sg;
+                const int i = sample_of<BC, N>(u + it * UPP + r * NSL, sg);
+                if (A.ok0) *reinterpret_cast<double2 *>(p.out + A.out_base + (size_t)i * A.out_stride) = make_double2(sg * v[it * RL + r].x, sg * v[it * RL + r].y);
+            }
+    } else {
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < ITL; ++it)
+#pragma unroll
+            for (int r = 0; r < RL; ++r) seq[pad(u + it * UPP + r * NSL)] = v[it * RL + r];
+        __syncthreads();
+        constexpr int STEPS = G::PAIRS * (N / 2);
 #pragma unroll 4
-    for (int e2 = threadIdx.x; e2 < steps; e2 += blockDim.x) {
-        int l, i;
-        L.decode(e2, l, i);
-        if (l >= L.valid) continue;
-        const cplx *z = Z + (l >> 1) * npad;
-        double2 o;
-        if (YP) {
-            double sign;
-            const cplx c = z[pad(seq_index(bc, i, N, sign))];
-            o = make_double2(sign * c.x, sign * c.y);
-        } else {
-            double s0, s1;
-            const cplx c0 = z[pad(seq_index(bc, i, N, s0))], c1 = z[pad(seq_index(bc, i + 1, N, s1))];
-            o = make_double2(s0 * c0.x, s1 * c1.x);              // line l: real parts; line l + 1: imaginary parts
-            if (l + 1 < L.valid) *reinterpret_cast<double2 *>(p.out + L.addr(l + 1, i)) = make_double2(s0 * c0.y, s1 * c1.y);
+        for (int e = t; e < STEPS; e += G::THREADS) {
+            const int q = e >> (LOGN - 1), i = (e & (N / 2 - 1)) << 1;
+            const int l = blockIdx.x * G::LINES + 2 * q;
+            const cplx *z = buf + q * NPAD;
+            cplx c0, c1;
+            double s1 = 1.0;
+            if (BC == 2) {
+                c0 = z[pad(i)];
+                c1 = z[pad(i + 1)];
+            } else {
+                c0 = z[pad(i >> 1)];
+                c1 = z[pad(N - 1 - (i >> 1))];
+                if (BC == 1) s1 = -1.0;
+            }
+            if (l < p.lines) *reinterpret_cast<double2 *>(p.out + ((size_t)l << LOGN) + i) = make_double2(c0.x, s1 * c1.x);
+            if (l + 1 < p.lines) *reinterpret_cast<double2 *>(p.out + ((size_t)(l + 1) << LOGN) + i) = make_double2(c0.y, s1 * c1.y);
         }
-        *reinterpret_cast<double2 *>(p.out + L.addr(l, i)) = o;
     }
 }
 
@@ -435,9 +570,19 @@ cudaError_t fft_configure() { return cudaSuccess; }   // shared-memory opt-in ha
 namespace {
 
 template <bool YP, int LOGN, int BC>
-cudaError_t launch_bc(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
-    constexpr int N = 1 << LOGN, nl = lines_of(YP, LOGN), threads = threads_of(YP, LOGN);
-    constexpr size_t smem = (size_t)(nl / 2) * (N + (N >> 3) + 1) * 16;
+cudaError_t launch_bc(const FftParams &p, int inverse, cudaStream_t stream) {
+    using G = Geo<YP, LOGN>;
+    constexpr int threads = G::THREADS;
+    constexpr size_t smem = G::SMEM;
+    int grid_x, grid_y = 1;
+    if (YP) {
+        const int ncols = p.bgroups * 16;      // columns of this launch (set by launch_fft, a multiple of COLS)
+        if (ncols % G::COLS) return cudaErrorInvalidValue;
+        grid_x = ncols / G::COLS;
+        grid_y = (p.planes + G::PL - 1) / G::PL;
+    } else {
+        grid_x = (p.lines + G::LINES - 1) / G::LINES;
+    }
     if (smem > 48 * 1024) {
         static DeviceOnce configured;                        // per device, thread-safe (devonce.hpp)
         cudaError_t e = configured.run([&] {
@@ -454,23 +599,23 @@ cudaError_t launch_bc(const FftParams &p, int inverse, int grid_x, int grid_y, c
 }
 
 template <bool YP, int LOGN>
-cudaError_t launch_one(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
-    if (p.bc == 0) return launch_bc<YP, LOGN, 0>(p, inverse, grid_x, grid_y, stream);
-    if (p.bc == 1) return launch_bc<YP, LOGN, 1>(p, inverse, grid_x, grid_y, stream);
-    return launch_bc<YP, LOGN, 2>(p, inverse, grid_x, grid_y, stream);
+cudaError_t launch_one(const FftParams &p, int inverse, cudaStream_t stream) {
+    if (p.bc == 0) return launch_bc<YP, LOGN, 0>(p, inverse, stream);
+    if (p.bc == 1) return launch_bc<YP, LOGN, 1>(p, inverse, stream);
+    return launch_bc<YP, LOGN, 2>(p, inverse, stream);
 }
 
 template <bool YP>
-cudaError_t launch_len(const FftParams &p, int inverse, int grid_x, int grid_y, cudaStream_t stream) {
+cudaError_t launch_len(const FftParams &p, int inverse, cudaStream_t stream) {
     switch (p.logN) {
-        case 4: return launch_one<YP, 4>(p, inverse, grid_x, grid_y, stream);
-        case 5: return launch_one<YP, 5>(p, inverse, grid_x, grid_y, stream);
-        case 6: return launch_one<YP, 6>(p, inverse, grid_x, grid_y, stream);
-        case 7: return launch_one<YP, 7>(p, inverse, grid_x, grid_y, stream);
-        case 8: return launch_one<YP, 8>(p, inverse, grid_x, grid_y, stream);
-        case 9: return launch_one<YP, 9>(p, inverse, grid_x, grid_y, stream);
-        case 10: return launch_one<YP, 10>(p, inverse, grid_x, grid_y, stream);
-        case 11: return launch_one<YP, 11>(p, inverse, grid_x, grid_y, stream);
+        case 4: return launch_one<YP, 4>(p, inverse, stream);
+        case 5: return launch_one<YP, 5>(p, inverse, stream);
+        case 6: return launch_one<YP, 6>(p, inverse, stream);
+        case 7: return launch_one<YP, 7>(p, inverse, stream);
+        case 8: return launch_one<YP, 8>(p, inverse, stream);
+        case 9: return launch_one<YP, 9>(p, inverse, stream);
+        case 10: return launch_one<YP, 10>(p, inverse, stream);
+        case 11: return launch_one<YP, 11>(p, inverse, stream);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -497,14 +642,18 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
             Ns *= p.radix[q];
         }
     }
+    p.planes = a.planes;
     if (a.dir == 0) {
-        const int nl = lines_of(false, p.logN);
         p.lines = a.ny * a.planes;
-        return launch_len<false>(p, a.inverse, (p.lines + nl - 1) / nl, 1, stream);
+        return launch_len<false>(p, a.inverse, stream);
     }
-    const int cols = lines_of(true, p.logN);
-    if (a.nx % cols) return cudaErrorInvalidValue;
-    return launch_len<true>(p, a.inverse, a.nx / cols, a.planes, stream);
+    const int ncols = a.ncols ? a.ncols : a.nx;
+    if (ncols % 16 || a.x0 % 16 || a.x0 < 0 || a.x0 + ncols > a.nx) return cudaErrorInvalidValue;
+    p.bgroups = ncols / 16;
+    // the natural-layout side starts at column x0 of every row; the blocked side is indexed by the slab-local column
+    if (!p.blk_in) p.in += a.x0;
+    if (!p.blk_out) p.out += a.x0;
+    return launch_len<true>(p, a.inverse, stream);
 }
 
 }  // namespace tpt

@@ -131,6 +131,10 @@ struct FftArgs {
     // y only: the mode-space side (output of the forward, input of the inverse transform) is tile-blocked; in / out
     // then point at the FIELD on that side, nz = field depth, k0 = z index of the first plane of this launch
     int blocked = 0, nz = 0, k0 = 0;
+    // y only: transform just the columns [x0, x0 + ncols) of every plane (ncols = 0: all nx).  The natural-layout side keeps
+    // the full field addressing (row length nx); a blocked side is then a SLAB buffer of its own, ncols columns wide
+    // (element (i, m, k) at ((m (ncols/16) + (i - x0)/16) nz + k) 16 + i mod 16) — the L2-resident slab pipeline of api.cu.
+    int x0 = 0, ncols = 0;
 };
 bool fft_supported(int n);                                   // 2^m, 16 <= n <= 2048
 void fft_tables(int n, std::vector<double> &out);            // e^{-i pi k/2n} (n entries) | per-pass twiddle tables

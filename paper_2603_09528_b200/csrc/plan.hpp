@@ -23,6 +23,11 @@ struct tpt_plan {
     double *d_fft[2] = {nullptr, nullptr};   // twiddle tables
     int gemm_variant = 2;
     int thomas_variant = 1;       // 1 = on-chip partitioned kernel where supported, 0 = streaming kernel
+    int slab_groups = -1;         // L2-resident slab pipeline of steps 2.2-2.4: -1 = automatic, 0 = off, G > 0 = slabs of G 16-column groups
+    double *d_slab = nullptr;     // its two slab buffers (lazy)
+    size_t slab_elems = 0;        // doubles per slab buffer
+    cudaStream_t st_slab = nullptr;                    // second stream: odd slabs overlap the even ones
+    cudaEvent_t ev_slab_fork = nullptr, ev_slab_join = nullptr;
     int fused_small = 1;          // grids that fit on chip: the whole solve in one cluster launch (fused_small.cu)
     int sms = 0;
     int profiling = 0;
