@@ -228,3 +228,52 @@ def test_longest_lines_against_the_closed_form_basis(tpt, torch, direction, bc):
     arg = {N_: np.pi * k / (2 * N), D_: np.pi * (k + 1) / (2 * N), P_: np.pi * ((k + 1) // 2) / N}[bc]
     assert np.abs(lam + 4.0 / w**2 * np.sin(arg) ** 2).max() <= 1e-13 * 4.0 / w**2
     plan.destroy()
+
+
+# --------------------------------------------------------------------------------------------------
+# Slab pipeline of steps 2.2 -> 2.3 -> 2.4 (tpt_plan_set_slab_groups; BASELINE north_star "Fusion"):
+# same kernels, same per-column arithmetic, another schedule — bit-for-bit the unslabbed solve.
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", [
+    ("ff-singular", (64, 32, 48), (0.0, 0.0, 2.0), (N_, N_, N_), 0.0, ("f", "f"), 7),
+    ("gf-helmholtz", (128, 64, 40), (2.0, 0.0, 2.5), (N_, D_, D_), 1e-3, ("g", "f"), 7),
+    ("gg-tma", (256, 128, 24), (2.0, 2.0, 2.0), (N_, N_, D_), 0.0, ("g", "g"), 7),
+    ("fg-periodic-x", (64, 96, 33), (0.0, 1.5, 2.0), (P_, N_, N_), 0.0, ("f", "g"), 7),
+    ("yz-only", (48, 64, 20), (2.0, 0.0, 2.0), (N_, N_, D_), 5e-3, ("g", "f"), 6),
+], ids=lambda c: c[0])
+@pytest.mark.parametrize("groups", [1, 3])
+def test_slab_pipeline_is_bitwise_the_plain_solve(tpt, torch, orc, case, groups):
+    name, n, beta, bc, alpha, tr, dirs = case
+    P = I.Problem(name, n, (1.0, 1.0, 1.0), beta, bc, alpha, seed=len(name))
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    kind = {"g": tpt.TRANSFORM_GEMM, "f": tpt.TRANSFORM_FFT}
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, alpha, dirs=dirs, transform=(kind[tr[0]] if dirs & 1 else 0, kind[tr[1]]))
+    assert plan.paths()[tpt.K_THOMAS] == tpt.PATH_THOMAS_BLOCKED
+    d_f = torch.from_numpy(f).cuda()
+    d_ref = torch.empty_like(d_f)
+    plan.solve(d_f, d_ref)
+    torch.cuda.synchronize()
+    plain_launches = plan.launches_last()
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha, dirs=dirs).solve(f)
+    assert _rel(d_ref.cpu().numpy(), ref) <= PARITY_TOL
+    plan.set_slab_groups(groups)
+    nslabs = -(-(n[0] // 16) // groups)
+    for inplace in (False, True):
+        d_in = d_f.clone()
+        d_out = d_in if inplace else torch.empty_like(d_f)
+        plan.solve(d_in, d_out)
+        torch.cuda.synchronize()
+        assert plan.launches_last() == plain_launches - 3 + 3 * nslabs
+        assert torch.equal(d_out, d_ref)
+    # a batch runs the slabs field by field
+    plan.reserve_batch(2)
+    d_b = torch.stack([d_f, d_f])
+    d_o = torch.empty_like(d_b)
+    plan.solve_batch(d_b, d_o)
+    torch.cuda.synchronize()
+    assert torch.equal(d_o[0], d_ref) and torch.equal(d_o[1], d_ref)
+    plan.set_slab_groups(0)
+    plan.solve(d_f, d_o[0])
+    assert plan.launches_last() == plain_launches
+    plan.destroy()
