@@ -169,6 +169,32 @@ __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParam
         middle_passes<LOGN, INV, Q + 1, NS * R, UPP>(seq, v, p, u);
     }
 }
+// e^{-i pi r / (2 R)}: T4[j + r N/R] = T4[j] * rot<R>(r), so the post-/pre-twiddles e^{-i pi k / 2N} of all bins of an item
+// follow from ONE table entry (and T4[N - k] = -i conj T4[k] needs none): 2 table loads per thread instead of 16.
+template <int R>
+__device__ __forceinline__ cplx rot(int r) {
+    constexpr double c1 = 0.98078528040323044913, s1 = 0.19509032201612826785;   // pi/16
+    constexpr double c2 = 0.92387953251128675613, s2 = 0.38268343236508977173;   // pi/8
+    constexpr double c3 = 0.83146961230254523708, s3 = 0.55557023301960222474;   // 3 pi/16
+    constexpr double c4 = 0.70710678118654752440;                                // pi/4
+    const int q = R == 8 ? r : 2 * r;                                            // angle = q pi / 16
+    switch (q) {
+        case 0: return cplx{1.0, 0.0};
+        case 1: return cplx{c1, -s1};
+        case 2: return cplx{c2, -s2};
+        case 3: return cplx{c3, -s3};
+        case 4: return cplx{c4, -c4};
+        case 5: return cplx{s3, -c3};
+        case 6: return cplx{s2, -c2};
+        default: return cplx{s1, -c1};
+    }
+}
+// e^{-i pi / (4 R)}: T4[N / (2R)], the first bin of the self-paired item PER/2
+template <int R>
+__device__ __forceinline__ cplx rot_half() {
+    return R == 8 ? cplx{0.99518472667219688624, -0.09801714032956060199} : cplx{0.98078528040323044913, -0.19509032201612826785};
+}
+
 // Items of the pass whose bins must come in conjugate pairs (k, N - k) — the last forward pass (untangling the two
 // real lines needs Z_k and Z_{N-k}) and the first inverse pass (a Hermitian spectrum is built from a_k and a_{N-k}).
 // Item j covers the bins j + r PER (PER = N/R); the partner bins N - j - r PER belong to item PER - j, r' = R-1-r.  A
@@ -317,6 +343,15 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     constexpr int RL = radix_at(LOGN, NP - 1), ITL = 16 / RL, NSL = N / RL;
     int jl[4];
     paired_items<RL, NSL, UPP>(u, jl);
+    cplx tb0{1.0, 0.0}, tb2{1.0, 0.0};                       // e^{-i pi j / 2N} of my items (BC 0 / 1); latency hides under the pass
+    if (BC != 2) {
+        const double2 w0 = __ldg(p.T4 + jl[0]);
+        tb0 = cplx{w0.x, w0.y};
+        if (RL == 4) {
+            const double2 w2 = __ldg(p.T4 + jl[2]);
+            tb2 = cplx{w2.x, w2.y};
+        }
+    }
 #pragma unroll
     for (int it = 0; it < ITL; ++it) {
 #pragma unroll
@@ -335,7 +370,8 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
             if (A.ok1) p.out[A.out_base + N + slot] = sc * o2;
         }
     };
-    auto emit = [&](int k, cplx zk, cplx zm) {               // bins k and N - k; zm = Z_{N-k};  0 < k < N, k != N/2
+    // bins k and N - k; zm = Z_{N-k}; tk = e^{-i pi k / 2N};  0 < k < N, k != N/2
+    auto emit = [&](int k, cplx tk, cplx zk, cplx zm) {
         const cplx V1{0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y)}, V2{0.5 * (zk.y + zm.y), 0.5 * (zm.x - zk.x)};
         if (BC == 2) {
             const int kk = k < N / 2 ? k : N - k;
@@ -343,7 +379,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
             store(2 * kk - 1, V1.x, V2.x);
             store(2 * kk, sg * V1.y, sg * V2.y);
         } else {
-            const double2 tk = __ldg(p.T4 + k), tm = __ldg(p.T4 + (N - k));
+            const cplx tm{-tk.y, -tk.x};                         // e^{-i pi (N-k) / 2N} = -i conj tk
             store(BC == 0 ? k : N - 1 - k, fma(tk.x, V1.x, -tk.y * V1.y), fma(tk.x, V2.x, -tk.y * V2.y));
             store(BC == 0 ? N - k : k - 1, fma(tm.x, V1.x, tm.y * V1.y), fma(tm.x, V2.x, tm.y * V2.y));
         }
@@ -358,18 +394,18 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     };
     if (RL == 4) {
 #pragma unroll
-        for (int r = 0; r < RL; ++r) emit(jl[2] + r * NSL, v[2 * RL + r], v[3 * RL + RL - 1 - r]);
+        for (int r = 0; r < RL; ++r) emit(jl[2] + r * NSL, cmul(tb2, rot<RL>(r)), v[2 * RL + r], v[3 * RL + RL - 1 - r]);
     }
     if (u) {
 #pragma unroll
-        for (int r = 0; r < RL; ++r) emit(jl[0] + r * NSL, v[r], v[RL + RL - 1 - r]);
+        for (int r = 0; r < RL; ++r) emit(jl[0] + r * NSL, cmul(tb0, rot<RL>(r)), v[r], v[RL + RL - 1 - r]);
     } else {
         emit_single(0, v[0]);
         emit_single(N / 2, v[RL / 2]);
 #pragma unroll
-        for (int r = 1; r < RL / 2; ++r) emit(r * NSL, v[r], v[RL - r]);
+        for (int r = 1; r < RL / 2; ++r) emit(r * NSL, rot<RL>(r), v[r], v[RL - r]);
 #pragma unroll
-        for (int r = 0; r < RL / 2; ++r) emit(NSL / 2 + r * NSL, v[RL + r], v[RL + RL - 1 - r]);
+        for (int r = 0; r < RL / 2; ++r) emit(NSL / 2 + r * NSL, cmul(rot_half<RL>(), rot<RL>(r)), v[RL + r], v[RL + RL - 1 - r]);
     }
 }
 
@@ -403,6 +439,15 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
         if (BC == 1) return N - 1 - k;
         return k == 0 ? 0 : (k == N / 2 ? N - 1 : (k < N / 2 ? 2 * k - 1 : 2 * (N - k)));
     };
+    cplx tb0{1.0, 0.0}, tb2{1.0, 0.0};                       // e^{-i pi j / 2N} of my items (BC 0 / 1)
+    if (BC != 2) {
+        const double2 w0 = __ldg(p.T4 + j0[0]);
+        tb0 = cplx{w0.x, w0.y};
+        if (R0 == 4) {
+            const double2 w2 = __ldg(p.T4 + j0[2]);
+            tb2 = cplx{w2.x, w2.y};
+        }
+    }
     if (A.ok0) {
         const double *src = p.in + A.in_base;
         const double *src1 = A.ok1 ? src + N : src;           // x: second line of the pair (a copy of the first if it does not exist)
@@ -430,7 +475,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
             v[it * R0 + r] = cplx{sc * v[it * R0 + r].x, sc * v[it * R0 + r].y};
         }
     // (zk, zm) hold the coefficients of bins k and N - k on entry, Z_k and Z_{N-k} on exit;  0 < k < N, k != N/2
-    auto build = [&](int k, cplx &zk, cplx &zm) {
+    auto build = [&](int k, cplx tk, cplx &zk, cplx &zm) {
         if (BC == 2) {
             const cplx ar = k < N / 2 ? zk : zm, ai = k < N / 2 ? zm : zk;   // B_kk = (ar - i ai) / 2, B_{N-kk} = (ar + i ai) / 2 per line
             const cplx lo{0.5 * (ar.x + ai.y), 0.5 * (ar.y - ai.x)}, hi{0.5 * (ar.x - ai.y), 0.5 * (ar.y + ai.x)};
@@ -438,7 +483,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
             zm = k < N / 2 ? hi : lo;
         } else {
             const cplx ak = zk, am = zm;
-            const double2 tk = __ldg(p.T4 + k), tm = __ldg(p.T4 + (N - k));
+            const cplx tm{-tk.y, -tk.x};                         // e^{-i pi (N-k) / 2N} = -i conj tk
             // B_k = e^{+i pi k / 2N} (a_k - i a_{N-k}) / 2 per line; Z = B_1 + i B_2
             const cplx b1 = cmul(cplx{0.5 * tk.x, -0.5 * tk.y}, cplx{ak.x, -am.x}), b2 = cmul(cplx{0.5 * tk.x, -0.5 * tk.y}, cplx{ak.y, -am.y});
             zk = cplx{b1.x - b2.y, b1.y + b2.x};
@@ -448,18 +493,18 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     };
     if (R0 == 4) {
 #pragma unroll
-        for (int r = 0; r < R0; ++r) build(j0[2] + r * PER0, v[2 * R0 + r], v[3 * R0 + R0 - 1 - r]);
+        for (int r = 0; r < R0; ++r) build(j0[2] + r * PER0, cmul(tb2, rot<R0>(r)), v[2 * R0 + r], v[3 * R0 + R0 - 1 - r]);
     }
     if (u) {
 #pragma unroll
-        for (int r = 0; r < R0; ++r) build(j0[0] + r * PER0, v[r], v[R0 + R0 - 1 - r]);
+        for (int r = 0; r < R0; ++r) build(j0[0] + r * PER0, cmul(tb0, rot<R0>(r)), v[r], v[R0 + R0 - 1 - r]);
     } else {
         // bins 0 and N/2 are their own partners: B_0 = a_0 and (cosine / sine) B_{N/2} = e^{+i pi / 4} (a - i a) / 2 = a / sqrt 2
         if (BC != 2) v[R0 / 2] = cplx{0.70710678118654752440 * v[R0 / 2].x, 0.70710678118654752440 * v[R0 / 2].y};
 #pragma unroll
-        for (int r = 1; r < R0 / 2; ++r) build(r * PER0, v[r], v[R0 - r]);
+        for (int r = 1; r < R0 / 2; ++r) build(r * PER0, rot<R0>(r), v[r], v[R0 - r]);
 #pragma unroll
-        for (int r = 0; r < R0 / 2; ++r) build(PER0 / 2 + r * PER0, v[R0 + r], v[R0 + R0 - 1 - r]);
+        for (int r = 0; r < R0 / 2; ++r) build(PER0 / 2 + r * PER0, cmul(rot_half<R0>(), rot<R0>(r)), v[R0 + r], v[R0 + R0 - 1 - r]);
     }
 #pragma unroll
     for (int it = 0; it < IT0; ++it) {
