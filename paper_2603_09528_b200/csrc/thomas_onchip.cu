@@ -376,6 +376,13 @@ cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, cons
     // rounding — on a natural-layout field (tpt_solve_host, whose results equal tpt_solve's bit for bit).
     if ((blocked || blocked_shape) && nz <= 544) return TPT_GO(17, 8, 256, 2);
     if (nz <= 512) return TPT_GO(16, 16, 512, 1);
+    // 545 .. 800 rows on the blocked layout: the same 32-segment, two-CTA shape with the shortest odd segment that covers
+    // the column (768^3: 0.709 -> 0.668 ms against one 384-thread CTA of 32-row segments; 25 rows x 2 register arrays
+    // still fit 128 registers with 16 bytes of spill)
+    if ((blocked || blocked_shape) && nz <= 608) return TPT_GO(19, 8, 256, 2);
+    if ((blocked || blocked_shape) && nz <= 672) return TPT_GO(21, 8, 256, 2);
+    if ((blocked || blocked_shape) && nz <= 736) return TPT_GO(23, 8, 256, 2);
+    if ((blocked || blocked_shape) && nz <= 800) return TPT_GO(25, 8, 256, 2);
     if (nz <= 768) return TPT_GO(32, 16, 384, 1);
     // up to 1056 rows: 8-column tiles of 17-row segments, 512 threads (16 warps), two 68 KB buffers, one CTA per SM
     // (33-row segments with 256 threads and 242 registers: 4.25 instead of 3.69 ms at 1024^3)

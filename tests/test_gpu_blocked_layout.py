@@ -42,7 +42,8 @@ def _solve(torch, plan, f):
 
 
 # nz picks the sweep's launch shape: <=128: 8-row segments; <=256: 16 rows, two CTAs per SM; 257..544 (blocked):
-# 8-column tiles with 17-row segments; 545..768: 32-row segments; 769..1056: 8-column tiles with 17-row segments and 512 threads.  Ragged nz exercises the zero-filled tail rows.
+# 8-column tiles with 17-row segments; 545..800 (blocked): the same shape with 19 / 21 / 23 / 25-row segments; 801..1056: 8-column
+# tiles with 17-row segments and 512 threads.  Ragged nz exercises the zero-filled tail rows.
 SHAPES = [
     ("nz24", (128, 128, 24), (N_, N_, D_), 0.0),
     ("nz130", (128, 256, 130), (N_, N_, D_), 0.0),
@@ -51,7 +52,12 @@ SHAPES = [
     ("nz513-singular", (128, 128, 513), (N_, N_, N_), 0.0),
     ("nz544", (128, 128, 544), (D_, N_, D_), 0.0),
     ("nz545", (128, 128, 545), (N_, N_, D_), 0.0),
+    ("nz608", (128, 128, 608), (N_, N_, D_), 1e-3),
+    ("nz650", (128, 128, 650), (N_, D_, D_), 0.0),
     ("nz700-singular", (128, 128, 700), (N_, N_, N_), 0.0),
+    ("nz768", (128, 128, 768), (N_, N_, D_), 5e-4),
+    ("nz800", (128, 128, 800), (D_, D_, N_), 0.0),
+    ("nz801", (128, 128, 801), (N_, N_, D_), 0.0),
     ("nz1000", (128, 128, 1000), (N_, N_, D_), 0.0),
     ("nz1056", (128, 128, 1056), (N_, D_, N_), 0.0),
 ]
