@@ -51,6 +51,9 @@ struct TmaGemmParams {
     double *peerC[MAX_PEERS];
 };
 
+// EDGE = false: M, N multiples of 128 and K of 16 — no predicate, no skipped warp, plain stride-grid tile walk (the
+// round-1 kernel, instruction for instruction: the headline configs).  EDGE = true: everything described above.
+template <bool EDGE>
 __global__ void __launch_bounds__(THREADS, 1)
 gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
                 const TmaGemmParams p) {
@@ -80,7 +83,7 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             int slot = 0;
             uint32_t phase = 0;
             for (int round = 0, base = 0; base < p.ntiles; ++round, base += gridDim.x) {
-                const int tile = base + (int)((blockIdx.x + round) % gridDim.x);
+                const int tile = base + (EDGE ? (int)((blockIdx.x + round) % gridDim.x) : (int)blockIdx.x);
                 if (tile >= p.ntiles) continue;
                 const int b = tile / p.tiles_mn;
                 const int mn = tile - b * p.tiles_mn;
@@ -92,7 +95,7 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                     unsigned char *st = smem + (size_t)slot * STAGE_BYTES;
                     ptx::mbar_arrive_expect_tx(&full[slot], STAGE_BYTES);
                     ptx::tma_load_2d(st, &mapA, kt * BK, a_row, &full[slot]);
-                    if (!p.b_split) {
+                    if (!EDGE || !p.b_split) {
                         ptx::tma_load_4d(st + A_BYTES, &mapB, 0, kt * BK, nt * (BN / 16), b_sel, &full[slot]);
                     } else {     // same shared-memory image, built from eight boxes clipped at column N
 #pragma unroll
@@ -112,7 +115,7 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     // Warp w runs on SM sub-partition w % 4.  The 4 x 4 grid of 32 x 32 warp tiles is handed out as a Latin square: every
     // sub-partition holds one warp of each row block AND of each column block, so on an edge tile (rows or columns past
     // M / N skipped) the remaining DMMAs still spread evenly over the four FP64 tensor pipes.
-    const int wm0 = (warp >> 2) * 32, wn0 = (((warp & 3) + (warp >> 2)) & 3) * 32;
+    const int wm0 = (warp >> 2) * 32, wn0 = (EDGE ? (((warp & 3) + (warp >> 2)) & 3) : (warp & 3)) * 32;
     const int rho = ((g & 3) << 1) | (g >> 2);                 // MMA row g  <-> tile row 8i + rho
     // A fragment (row 8i + rho, k = 4kk + t):  byte = row*128 + (((k>>1) ^ rho) << 4) + (k&1)*8
     uint32_t a_off[4];
@@ -146,7 +149,7 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     // CTA would meet the same (mt, nt) every round whenever grid is a multiple of tiles_mn, i.e. some CTAs only cheap edge
     // tiles and others only full ones.
     for (int round = 0, base = 0; base < p.ntiles; ++round, base += gridDim.x) {
-        const int tile = base + (int)((blockIdx.x + round) % gridDim.x);
+        const int tile = base + (EDGE ? (int)((blockIdx.x + round) % gridDim.x) : (int)blockIdx.x);
         if (tile >= p.ntiles) continue;
         double acc[4][4][2];
 #pragma unroll
@@ -157,7 +160,7 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         const int mn = tile - b * p.tiles_mn;
         const int mt = mn / p.tiles_n, nt = mn - mt * p.tiles_n;
         // edge tiles: a warp whose sub-tile lies wholly past M or N only keeps the ring's bookkeeping going
-        const bool inside = mt * BM + wm0 < p.M && nt * BN + wn0 < p.N;
+        const bool inside = !EDGE || (mt * BM + wm0 < p.M && nt * BN + wn0 < p.N);
 
         for (int kt = 0; kt < KT; ++kt) {
             ptx::mbar_wait(&full[slot], phase);
@@ -193,14 +196,14 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int row = row0 + 8 * i;
-            if (row >= p.M) break;
+            if (EDGE && row >= p.M) break;
             // sharded solve: the owner of mode row `row` receives it straight from this epilogue (16-byte stores to
             // peer-mapped memory travel over NVLink while the next tile's DMMAs run) — no pack kernel, no collective
             double *base = p.npeers ? p.peerC[(((row >> 4) + 1) * p.npeers - 1) / p.units] : p.C;
             double *Cw = base + off + (int64_t)row * p.ldc;
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                if (col0 + (j >> 1) * 16 + (j & 1) * 4 < p.N)         // N is even: a column pair is inside or outside as a whole
+                if (!EDGE || col0 + (j >> 1) * 16 + (j & 1) * 4 < p.N)   // N is even: a column pair is inside or outside as a whole
                     *reinterpret_cast<double2 *>(Cw + (int64_t)(j >> 1) * p.ldg + (j & 1) * 4) = make_double2(acc[i][j][0], acc[i][j][1]);
         }
     }
@@ -236,10 +239,15 @@ cudaError_t gemm_tma_configure() {
     // THREADS x numRegs >= 128 x 24 + 512 x 112, i.e. 96 registers per thread at launch (what ptxas gives under
     // __launch_bounds__(640, 1) today).  A toolchain that allocated fewer would hang the kernel: refuse instead.
     cudaFuncAttributes fa;
-    cudaError_t e = cudaFuncGetAttributes(&fa, gemm_tma_kernel);
+    cudaError_t e = cudaFuncGetAttributes(&fa, gemm_tma_kernel<false>);
     if (e != cudaSuccess) return e;
     if (fa.numRegs * THREADS < 128 * 24 + CONSUMER_WARPS * 32 * 112) return cudaErrorLaunchOutOfResources;
-    return cudaFuncSetAttribute(gemm_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+    e = cudaFuncGetAttributes(&fa, gemm_tma_kernel<true>);
+    if (e != cudaSuccess) return e;
+    if (fa.numRegs * THREADS < 128 * 24 + CONSUMER_WARPS * 32 * 112) return cudaErrorLaunchOutOfResources;
+    e = cudaFuncSetAttribute(gemm_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(gemm_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
 }
 
 cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
@@ -286,7 +294,8 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
     p.units = g.M / 16 > 0 ? g.M / 16 : 1;
     for (int q = 0; q < MAX_PEERS; ++q) p.peerC[q] = q < g.npeers ? g.peerC[q] : nullptr;
     const int grid = p.ntiles < sms ? p.ntiles : sms;
-    gemm_tma_kernel<<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);
+    if (g.M % BM == 0 && g.N % BN == 0 && g.K % BK == 0) gemm_tma_kernel<false><<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);
+    else gemm_tma_kernel<true><<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);
     return cudaGetLastError();
 }
 
