@@ -269,6 +269,20 @@ def measure_config(api, torch, name, fp64_peak, hbm_gbs, steps=6, warmup=3):
     kms, launches, _ = pl0.kernel_times()
     for pl in plan_cache.values():
         pl.set_profiling(False)
+    paths = pl0.paths()
+    fused = api.PATH_FUSED_SMALL in paths
+    back_to_back = None
+    if small:      # launch-bound sizes: also the throughput of solves issued back to back (warm L2, no events in between)
+        reps = 200
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(20):
+            step()
+        a.record(stream)
+        for _ in range(reps):
+            step()
+        b.record(stream)
+        torch.cuda.synchronize()
+        back_to_back = a.elapsed_time(b) / reps
     nx, ny, nz = P0.n
     gemm = {"fwd_x": 2.0 * nx, "fwd_y": 2.0 * ny, "inv_y": 2.0 * ny, "inv_x": 2.0 * nx}
     fr = {k: gemm[k] * P0.points / (kms[i] * 1e-3) / 1e12 / fp64_peak for i, k in enumerate(api.KERNEL_NAMES) if k in gemm}
@@ -278,11 +292,16 @@ def measure_config(api, torch, name, fp64_peak, hbm_gbs, steps=6, warmup=3):
         "workload": ", ".join(P.name for P in probs), "grid": list(P0.n), "solves_per_step": len(probs),
         "ms_per_step": ms_step, "ms_per_step_min": ms[0], "gpts_per_s": sum(P.points for P in probs) / ms_step / 1e6,
         "timed_steps": steps, "warmup": warmup, "l2_flushed_between_steps": bool(small),
+        "ms_per_step_back_to_back_warm_l2": back_to_back,
+        "paths_first_plan": dict(zip(api.KERNEL_NAMES, paths)),
         "kernel_ms_first_plan": dict(zip(api.KERNEL_NAMES, kms)),
-        "gemm_frac_of_fp64_peak": {"slowest": slow, "frac": fr[slow], "all": fr},
-        "thomas_frac_of_hbm_peak_16B_per_pt": 16.0 * P0.points / (th * 1e-3) / 1e9 / hbm_gbs,
+        "gemm_frac_of_fp64_peak": None if fused else {"slowest": slow, "frac": fr[slow], "all": fr},
+        "thomas_frac_of_hbm_peak_16B_per_pt": None if fused else 16.0 * P0.points / (th * 1e-3) / 1e9 / hbm_gbs,
         "gpu_launches_first_plan": launches,
     }
+    if fused:
+        out["note"] = ("small-grid path: the whole solve is ONE cluster launch (fused_small_kernel); its time is reported in the "
+                       "fwd_x slot, the other slots are empty event intervals")
     for pl in plan_cache.values():
         pl.destroy()
     del rhs, outs, flush

@@ -395,16 +395,16 @@ int orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
                              const double *lamx, const double *qx, const double *lamy, const double *qy) {
     if (!out || !bc || !faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf)) return ORC_EINVAL;
     if (!bc_ok(bc[0]) || !bc_ok(bc[1]) || !bc_ok(bc[2]) || !(alpha >= 0.0) || !isfinite(alpha)) return ORC_EINVAL;
-    /* periodic directions are diagonalised (x, y); the z sweep is the plain Thomas algorithm */
-    if (bc[2] == ORC_BC_PERIODIC || (bc[0] == ORC_BC_PERIODIC && nx < 3) || (bc[1] == ORC_BC_PERIODIC && ny < 3)) return ORC_EINVAL;
+    /* periodic x, y are diagonalised; a periodic z makes the sweep a CYCLIC tridiagonal solve ("cyclic corner entries") [A19] */
+    if ((bc[2] == ORC_BC_PERIODIC && nz < 3) || (bc[0] == ORC_BC_PERIODIC && nx < 3) || (bc[1] == ORC_BC_PERIODIC && ny < 3)) return ORC_EINVAL;
     if (!lamx || !qx || !lamy || !qy) return ORC_EINVAL;
     orc_plan *p = (orc_plan *)calloc(1, sizeof(orc_plan));
     if (!p) return ORC_ENOMEM;
     p->nx = nx; p->ny = ny; p->nz = nz; p->alpha = alpha;
     p->dirs = ORC_DIRS_XYZ;
     p->bc[0] = bc[0]; p->bc[1] = bc[1]; p->bc[2] = bc[2];
-    /* [A7] structural detection of the null mode: all-Neumann and Poisson. */
-    p->singular = (alpha == 0.0 && bc[0] != ORC_BC_DIRICHLET && bc[1] != ORC_BC_DIRICHLET && bc[2] == ORC_BC_NEUMANN);
+    /* [A7] structural detection of the null mode: no Dirichlet direction and Poisson. */
+    p->singular = (alpha == 0.0 && bc[0] != ORC_BC_DIRICHLET && bc[1] != ORC_BC_DIRICHLET && bc[2] != ORC_BC_DIRICHLET);
     p->wx = dup_array(NULL, nx); p->wy = dup_array(NULL, ny); p->wz = dup_array(NULL, nz);
     p->az = dup_array(NULL, nz); p->bz = dup_array(NULL, nz); p->cz = dup_array(NULL, nz);
     p->lamx = dup_array(lamx, nx); p->lamy = dup_array(lamy, ny);
@@ -427,7 +427,7 @@ int orc_plan_create_with_eig(orc_plan **out, int nx, int ny, int nz,
 int orc_plan_create(orc_plan **out, int nx, int ny, int nz,
                     const double *xf, const double *yf, const double *zf, const int bc[3], double alpha) {
     if (!out || !bc || !faces_ok(nx, xf) || !faces_ok(ny, yf) || !faces_ok(nz, zf)) return ORC_EINVAL;
-    if (!bc_ok(bc[0]) || !bc_ok(bc[1]) || !bc_ok(bc[2]) || bc[2] == ORC_BC_PERIODIC) return ORC_EINVAL;
+    if (!bc_ok(bc[0]) || !bc_ok(bc[1]) || !bc_ok(bc[2])) return ORC_EINVAL;
     double *lamx = dup_array(NULL, nx), *lamy = dup_array(NULL, ny);
     double *qx = dup_array(NULL, (size_t)nx * nx), *qy = dup_array(NULL, (size_t)ny * ny);
     int rc = ORC_ENOMEM;
@@ -542,7 +542,78 @@ void orc_inverse_x(const orc_plan *p, const double *in, double *out) {
  * independent columns side by side so that memory is read along x).
  * Singular plan, column (0,0): the final pivot vanishes -> last unknown := 0, then the
  * Delta z-weighted mean of that column is removed (zero volume-weighted mean gauge) [A7]. */
+/* Textbook Thomas for one tridiagonal system of size n (sub[0], sup[n-1] unused), in place on d; cp = scratch. */
+static void thomas_line(int n, const double *sub, const double *dia, const double *sup, double *d, double *cp) {
+    double den = dia[0];
+    cp[0] = sup[0] / den;
+    d[0] = d[0] / den;
+    for (int k = 1; k < n; ++k) {
+        den = dia[k] - sub[k] * cp[k - 1];
+        cp[k] = sup[k] / den;
+        d[k] = (d[k] - sub[k] * d[k - 1]) / den;
+    }
+    for (int k = n - 2; k >= 0; --k) d[k] -= cp[k] * d[k + 1];
+}
+
+/* Periodic z [A19]: row 0 couples to x_{n-1} through sub[0], row n-1 to x_0 through sup[n-1] ("cyclic corner
+ * entries").  The paper does not say how it sweeps such a system; the textbook way is taken: the cyclic matrix is a
+ * tridiagonal matrix A' plus a rank-one term u v^T (u = (g, 0, .., 0, sup[n-1]), v = (1, 0, .., 0, sub[0]/g), g = -dia[0];
+ * A' = A with dia[0] - g and dia[n-1] - sup[n-1] sub[0] / g), so by the Sherman-Morrison formula
+ *     x = y - q (v.y) / (1 + v.q),   A' y = d,  A' q = u.
+ * Null column of a singular plan: the cyclic T_z is singular (constant null vector); following P:219 the last unknown
+ * is set to 0 — which removes both corner couplings — the remaining n-1 equations are a plain tridiagonal system, and
+ * the Delta z-weighted mean of the column is removed afterwards [A7]. */
+static int thomas_z_cyclic(const orc_plan *p, double *field) {
+    const int nx = p->nx, ny = p->ny, nz = p->nz;
+    const double alpha = p->alpha;
+    const size_t plane = (size_t)nx * ny;
+    int status = ORC_OK;
+#pragma omp parallel
+    {
+        double *buf = (double *)malloc(sizeof(double) * 7 * (size_t)nz);
+        if (!buf) {
+#pragma omp critical
+            status = ORC_ENOMEM;
+        }
+        double *sub = buf, *dia = buf + nz, *sup = buf + 2 * nz, *y = buf + 3 * nz, *q = buf + 4 * nz, *cp = buf + 5 * nz, *bb = buf + 6 * nz;
+        for (int k = 0; buf && k < nz; ++k) {
+            if (alpha == 0.0) { sub[k] = p->az[k]; dia[k] = p->bz[k]; sup[k] = p->cz[k]; }
+            else { sub[k] = -alpha * p->az[k]; dia[k] = 1.0 - alpha * p->bz[k]; sup[k] = -alpha * p->cz[k]; }
+        }
+#pragma omp for schedule(static) collapse(2)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                if (!buf) continue;
+                double *col = field + (size_t)j * nx + i;
+                double sigma = ((p->dirs & 1) ? p->lamx[i] : 0.0) + ((p->dirs & 2) ? p->lamy[j] : 0.0);
+                double shift = (alpha == 0.0) ? sigma : -alpha * sigma;
+                for (int k = 0; k < nz; ++k) { y[k] = col[k * plane]; bb[k] = dia[k] + shift; }
+                if (p->singular && i == 0 && j == 0) {
+                    thomas_line(nz - 1, sub, bb, sup, y, cp);
+                    y[nz - 1] = 0.0;
+                    double s = 0.0, L = 0.0;
+                    for (int k = 0; k < nz; ++k) { s += p->wz[k] * y[k]; L += p->wz[k]; }
+                    for (int k = 0; k < nz; ++k) col[k * plane] = y[k] - s / L;
+                    continue;
+                }
+                const double g = -bb[0];
+                bb[0] -= g;
+                bb[nz - 1] -= sup[nz - 1] * sub[0] / g;
+                for (int k = 0; k < nz; ++k) q[k] = 0.0;
+                q[0] = g;
+                q[nz - 1] = sup[nz - 1];
+                thomas_line(nz, sub, bb, sup, y, cp);
+                thomas_line(nz, sub, bb, sup, q, cp);
+                const double fact = (y[0] + sub[0] * y[nz - 1] / g) / (1.0 + q[0] + sub[0] * q[nz - 1] / g);
+                for (int k = 0; k < nz; ++k) col[k * plane] = y[k] - fact * q[k];
+            }
+        free(buf);
+    }
+    return status;
+}
+
 int orc_thomas_z(const orc_plan *p, double *field) {
+    if (p->bc[2] == ORC_BC_PERIODIC) return thomas_z_cyclic(p, field);
     const int nx = p->nx, ny = p->ny, nz = p->nz;
     const double alpha = p->alpha;
     const size_t plane = (size_t)nx * ny;

@@ -34,7 +34,8 @@
 extern "C" {
 #endif
 
-/* PERIODIC (P:102 cyclic corners, P:211 dense cyclic operator): x and y only — the z sweep is the plain Thomas algorithm. */
+/* PERIODIC (P:102 cyclic corners, P:211 dense cyclic operator): x and y are diagonalised; a periodic z makes the sweep a cyclic
+ * tridiagonal solve (Sherman-Morrison, A19). */
 enum { ORC_BC_NEUMANN = 0, ORC_BC_DIRICHLET = 1, ORC_BC_PERIODIC = 2 };
 /* Implicitly treated directions L_I of the Helmholtz problem, Eq. 2b: bit 0 = x, 1 = y, 2 = z. */
 enum { ORC_DIRS_Z = 4, ORC_DIRS_YZ = 6, ORC_DIRS_XYZ = 7 };

@@ -94,7 +94,10 @@ def test_periodic_uniform_1d_solve_equals_fft_division(orc):
 
 
 @pytest.mark.parametrize("bc,alpha", [((P_, N_, D_), 0.0), ((P_, P_, N_), 0.0), ((N_, P_, D_), 0.3), ((P_, D_, N_), 0.0),
-                                      ((P_, N_, N_), 0.0)])
+                                      ((P_, N_, N_), 0.0),
+                                      # periodic z: the sweep is a cyclic tridiagonal solve (A19)
+                                      ((N_, D_, P_), 0.0), ((N_, N_, P_), 0.0), ((P_, P_, P_), 0.0), ((D_, N_, P_), 0.4),
+                                      ((P_, N_, P_), 2e-3)])
 def test_periodic_matches_brute_force_lu(orc, bc, alpha):
     xf, yf, zf = I.tanh_faces(5, 1.0, 1.3), I.tanh_faces(7, 2.0, 1.8), I.tanh_faces(6, 0.5, 2.2)
     f = I.uniform_pm1(21, 5 * 7 * 6).reshape(6, 7, 5)
@@ -128,10 +131,37 @@ def test_periodic_flux_operator_matches_dense_rows_and_translation_invariance(or
     assert _rel(plan.solve(np.roll(f, 2, axis=1)), np.roll(plan.solve(f), 2, axis=1)) < 1e-13
 
 
-def test_periodic_z_is_rejected(orc):
-    xf = I.tanh_faces(6, 1.0, 0.0)
+def test_periodic_z_cyclic_sweep_closed_forms(orc):
+    # (1) uniform periodic z, rhs = a discrete Fourier mode in z times eigenmodes in x, y: phi = f / (lx + ly + lz) exactly
+    nx, ny, nz = 6, 5, 16
+    xf, yf, zf = I.tanh_faces(nx, 1.0, 0.0), I.tanh_faces(ny, 2.0, 0.0), I.tanh_faces(nz, 3.0, 0.0)
+    plan = orc.OraclePlan(xf, yf, zf, (N_, N_, P_), 0.0)
+    lamx, qx = plan.eigen(0)
+    lamy, qy = plan.eigen(1)
+    dz = 3.0 / nz
+    for m, (ix, iy) in ((3, (2, 1)), (8, (0, 4)), (1, (0, 0))):
+        zmode = np.cos(2 * math.pi * m * (np.arange(nz) + 0.5) / nz + 0.3)
+        f = zmode[:, None, None] * qy[:, iy][None, :, None] * qx[:, ix][None, None, :]
+        lz = -(4 / dz ** 2) * math.sin(math.pi * m / nz) ** 2
+        assert _rel(plan.solve(f), f / (lamx[ix] + lamy[iy] + lz)) < 1e-12
+    # (2) a stretched periodic z against numpy's dense solve of the assembled cyclic column systems (Helmholtz, z only)
+    zf = I.tanh_faces(11, 1.0, 1.7)
+    xf2 = I.tanh_faces(3, 1.0, 0.0)
+    w, T = _dense_T(orc, zf, P_)
+    alpha = 0.07
+    f = I.uniform_pm1(3, 11 * 3 * 3).reshape(11, 3, 3)
+    u = orc.OraclePlan(xf2, xf2, zf, (N_, N_, P_), alpha, dirs=4).solve(f)
+    ref = np.linalg.solve(np.eye(11) - alpha * T, f.reshape(11, 9)).reshape(11, 3, 3)
+    assert _rel(u, ref) < 1e-13
+    # (3) z uniform and periodic: a cyclic shift of the rhs in z shifts the solution (non-singular Helmholtz)
+    zf = I.tanh_faces(9, 1.0, 0.0)
+    xs, ys = I.tanh_faces(4, 1.0, 1.2), I.tanh_faces(5, 1.0, 0.8)
+    plan = orc.OraclePlan(xs, ys, zf, (N_, D_, P_), 0.2)
+    f = I.uniform_pm1(9, 9 * 5 * 4).reshape(9, 5, 4)
+    assert _rel(plan.solve(np.roll(f, 4, axis=0)), np.roll(plan.solve(f), 4, axis=0)) < 1e-13
+    # (4) n = 2 cells cannot be periodic (the two couplings coincide)
     with pytest.raises(RuntimeError):
-        orc.OraclePlan(xf, xf, xf, (N_, N_, P_), 0.0)
+        orc.OraclePlan(xs, ys, I.tanh_faces(2, 1.0, 0.0), (N_, N_, P_), 0.0)
 
 
 def test_paper_benchmark_bcs_residual_on_stretched_grid(orc):
