@@ -63,6 +63,8 @@ void free_plan(tpt_plan *p) {
     cudaFree(p->d_work);
     cudaFree(p->d_stage);
     cudaFree(p->d_slab);
+    cudaFree(p->d_cyc_q);
+    cudaFree(p->d_cyc_rden);
     if (p->ev_slab_fork) cudaEventDestroy(p->ev_slab_fork);
     if (p->ev_slab_join) cudaEventDestroy(p->ev_slab_join);
     if (p->st_slab) cudaStreamDestroy(p->st_slab);
@@ -126,7 +128,7 @@ cudaError_t run_gemm(const tpt_plan *p, const tpt::GemmArgs &g, cudaStream_t st)
 // The mode-space field (between steps 2.2 and 2.4) is kept tile-blocked when the kernels on both sides of it can:
 // the TMA GEMM for the y transforms and the on-chip sweep.  tpt_stage always uses the natural layout.
 bool use_blocked(const tpt_plan *p) {
-    if (p->thomas_variant != 1 || !(p->dirs & 2)) return false;
+    if (p->thomas_variant != 1 || !(p->dirs & 2) || p->cyclic) return false;   // (the cyclic correction runs in the natural layout)
     if (!tpt::blocked_layout_supported(p->nx, p->ny, p->nz) || !tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) return false;
     // the fast y transform addresses either layout (its tiles write whole 128-byte lines of the blocked field)
     if (p->transform[1] == TPT_TRANSFORM_FFT) return true;
@@ -134,12 +136,26 @@ bool use_blocked(const tpt_plan *p) {
 }
 
 // Step 2.3 on one field: in -> out (in == out allowed); `scratch` is a free field (used by the streaming kernel only).
+int run_sweep(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches, bool blocked,
+              bool blocked_shape, int singular);
+
 int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches, bool blocked = false,
                bool blocked_shape = false) {
+    int rc = run_sweep(p, in, out, scratch, st, launches, blocked, blocked_shape, p->singular);
+    if (rc != TPT_OK || !p->cyclic) return rc;
+    // periodic z: x = y - q (y_0 + r y_{n-1}) rden   (Sherman-Morrison, kernels.cu)
+    if (blocked) return TPT_ECUDA;
+    ++*launches;
+    return tpt::launch_cyclic_correct(out, p->d_cyc_q, p->d_cyc_rden, (size_t)p->nx * p->ny, p->nz, p->cyc_r, st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+}
+
+// the tridiagonal sweep proper (`singular`: treat column (0,0) as the null column)
+int run_sweep(tpt_plan *p, const double *in, double *out, double *scratch, cudaStream_t st, int *launches, bool blocked,
+              bool blocked_shape, int singular) {
     if (p->thomas_variant == 1 && tpt::thomas_onchip_supported(p->nx, p->ny, p->nz)) {
         // on-chip kernel; the null-mode gauge of a singular plan is fused into it
         cudaError_t e = tpt::launch_thomas_onchip(in, out, p->d_abc, p->d_lamx, p->d_lamy, p->d_wz, p->nx, p->ny, p->nz, p->shift0,
-                                                  p->singular, blocked, blocked_shape, p->sms, st);
+                                                  singular, blocked, blocked_shape, p->sms, st);
         ++*launches;
         return e == cudaSuccess ? TPT_OK : TPT_ECUDA;
     }
@@ -148,9 +164,9 @@ int run_thomas(tpt_plan *p, const double *in, double *out, double *scratch, cuda
     if (in != out && cudaMemcpyAsync(out, in, p->points() * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
         return TPT_ECUDA;
     cudaError_t e = tpt::launch_thomas(out, scratch, p->d_az, p->d_bz, p->d_cz, p->d_lamx, p->d_lamy, p->nx, p->ny, p->nz,
-                                       p->shift0, p->singular, st);
+                                       p->shift0, singular, p->b0_null, st);
     ++*launches;
-    if (e == cudaSuccess && p->singular) {
+    if (e == cudaSuccess && singular) {
         e = tpt::launch_gauge(out, p->d_wz, (size_t)p->nx * p->ny, p->nz, st);
         ++*launches;
     }
@@ -217,6 +233,8 @@ int slab_setup(tpt_plan *p, int groups) {
     if (p->slab_elems < need) {
         if (cudaDeviceSynchronize() != cudaSuccess) return TPT_ECUDA;
         cudaFree(p->d_slab);
+    cudaFree(p->d_cyc_q);
+    cudaFree(p->d_cyc_rden);
         p->d_slab = nullptr;
         p->slab_elems = 0;
         cudaError_t e = cudaMalloc(&p->d_slab, 2 * need * sizeof(double));
@@ -272,7 +290,7 @@ int run_slabs(tpt_plan *p, const double *src, double *dst, int groups, cudaStrea
 // Grids that fit on chip run the whole solve as one cluster launch (fused_small.cu) — with the default kernel variants
 // only, so that selecting a variant still exercises that kernel.
 bool use_fused_small(const tpt_plan *p) {
-    if (!p->fused_small || p->gemm_variant != 2 || p->thomas_variant != 1) return false;
+    if (!p->fused_small || p->gemm_variant != 2 || p->thomas_variant != 1 || p->cyclic) return false;
     if (!(p->dirs & 3)) return false;     // sweep only ("z"): already a single launch
     if (((p->dirs & 1) && p->transform[0] != TPT_TRANSFORM_GEMM) || ((p->dirs & 2) && p->transform[1] != TPT_TRANSFORM_GEMM)) return false;
     return tpt::fused_small_supported(p->nx, p->ny, p->nz);
@@ -422,8 +440,8 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
     if (implicit_dirs != TPT_DIRS_XYZ && !(helmholtz_alpha > 0.0)) return TPT_EINVAL;   // Eq. 2c carries the full L
     if (!tpt::faces_valid(nx, xf) || !tpt::faces_valid(ny, yf) || !tpt::faces_valid(nz, zf)) return TPT_EINVAL;
     if (!bc_valid(bc[0]) || !bc_valid(bc[1]) || !bc_valid(bc[2])) return TPT_EINVAL;
-    // periodic directions are diagonalised (x, y); the z sweep is the plain Thomas algorithm
-    if (bc[2] == TPT_BC_PERIODIC || (bc[0] == TPT_BC_PERIODIC && nx < 3) || (bc[1] == TPT_BC_PERIODIC && ny < 3)) return TPT_EINVAL;
+    // periodic x, y are diagonalised; a periodic z makes the sweep cyclic (A19)
+    if ((bc[2] == TPT_BC_PERIODIC && nz < 3) || (bc[0] == TPT_BC_PERIODIC && nx < 3) || (bc[1] == TPT_BC_PERIODIC && ny < 3)) return TPT_EINVAL;
     if (!(helmholtz_alpha >= 0.0) || !std::isfinite(helmholtz_alpha)) return TPT_EINVAL;
     if ((double)nx * ny * nz > 4.0e9) return TPT_EINVAL;
     // fast transforms: diagonalised, uniform, power-of-two directions only; y tiles need nx % 16 == 0
@@ -456,7 +474,8 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
     p->device = dev;
     p->sms = sm_count;
     p->singular = (helmholtz_alpha == 0.0 && bc[0] != TPT_BC_DIRICHLET && bc[1] != TPT_BC_DIRICHLET &&
-                   bc[2] == TPT_BC_NEUMANN) ? 1 : 0;
+                   bc[2] != TPT_BC_DIRICHLET) ? 1 : 0;
+    p->cyclic = bc[2] == TPT_BC_PERIODIC ? 1 : 0;
     // Helmholtz (I - alpha T) u = f  <=>  (T - I/alpha) u = -f/alpha: same z kernel with a constant
     // extra shift, the -1/alpha scale folded into the first forward matrix ("constant shift").
     // With no transform at all (the "z" choice) the sweep solves (I - alpha T_z) u = f on scaled coefficients.
@@ -478,6 +497,23 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
                 oz.b[k] = 1.0 - helmholtz_alpha * oz.b[k];
                 oz.c[k] *= -helmholtz_alpha;
             }
+        }
+        // Periodic z: the sweep kernels solve the tridiagonal A' = A - u v^T (corners b_0 - g and b_{n-1} - c_{n-1} a_0 / g with
+        // g = -b_0, which only strengthens the diagonal); the rank-one term is put back after the sweep (run_thomas).  The
+        // null column of a singular plan keeps the unmodified diagonal: with x_{n-1} = 0 both corner
+        // couplings vanish.
+        std::vector<double> bz_null;
+        double cyc_g = 0.0, cyc_cn = 0.0;
+        p->b0_null = oz.b[0];
+        if (p->cyclic) {
+            bz_null = oz.b;
+            cyc_g = -oz.b[0];
+            cyc_cn = oz.c[nz - 1];
+            p->cyc_r = oz.a[0] / cyc_g;
+            oz.b[0] -= cyc_g;
+            oz.b[nz - 1] -= cyc_cn * oz.a[0] / cyc_g;
+            oz.a[0] = 0.0;
+            oz.c[nz - 1] = 0.0;
         }
         // a direction that is not diagonalised contributes no modal shift (Eq. 9 restricted)
         p->lamx.assign(nx, 0.0);
@@ -577,8 +613,14 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
         }
         if (rc == TPT_OK) {
             std::vector<double> t;
-            tpt::thomas_onchip_tables(nz, oz.a.data(), oz.b.data(), oz.c.data(), t);
+            tpt::thomas_onchip_tables(nz, oz.a.data(), oz.b.data(), oz.c.data(), t, p->cyclic ? bz_null.data() : nullptr);
             rc = upload(&p->d_abc, t);
+        }
+        if (rc == TPT_OK && p->cyclic) {
+            cudaError_t e = cudaMalloc(&p->d_cyc_q, p->points() * sizeof(double));
+            if (e == cudaSuccess) e = cudaMalloc(&p->d_cyc_rden, (size_t)nx * ny * sizeof(double));
+            if (e != cudaSuccess) { cudaGetLastError(); rc = e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
+            p->cyc_g_tmp[0] = cyc_g; p->cyc_g_tmp[1] = cyc_cn;
         }
     } catch (const std::bad_alloc &) {
         rc = TPT_ENOMEM;
@@ -593,6 +635,16 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
                          tpt::fft_configure() != cudaSuccess)) {
         cudaGetLastError();
         rc = TPT_ECUDA;
+    }
+    if (rc == TPT_OK && p->cyclic) {
+        // q = A'^-1 u for every column (its spectral shift is all that distinguishes the columns): one sweep at plan time
+        int launches = 0;
+        const size_t cols = (size_t)nx * ny;
+        cudaError_t e = tpt::launch_cyclic_rhs(p->d_cyc_q, cols, nz, p->cyc_g_tmp[0], p->cyc_g_tmp[1], nullptr);
+        if (e == cudaSuccess) rc = run_sweep(p, p->d_cyc_q, p->d_cyc_q, p->d_work, nullptr, &launches, false, false, 0);
+        if (e == cudaSuccess && rc == TPT_OK) e = tpt::launch_cyclic_rden(p->d_cyc_q, p->d_cyc_rden, cols, nz, p->cyc_r, p->singular, nullptr);
+        if (e == cudaSuccess && rc == TPT_OK) e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) { cudaGetLastError(); rc = TPT_ECUDA; }
     }
     if (rc != TPT_OK) { free_plan(p); return rc; }
     *plan_out = p;
@@ -768,6 +820,7 @@ int tpt_solve_host_async(tpt_plan *p, const double *rhs_host, double *out_host, 
 int tpt_divergence(tpt_plan *p, const double *u_dev, const double *v_dev, const double *w_dev, double scale, double *out_dev,
                    void *cuda_stream) {
     if (!p || !u_dev || !v_dev || !w_dev || !out_dev || !std::isfinite(scale) || !on_plan_device(p)) return TPT_EINVAL;
+    if (p->cyclic) return TPT_EINVAL;   // the staggered operators close z with walls or ghost cells only
     if (!aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(out_dev)) return TPT_EINVAL;
     cudaError_t e = tpt::launch_divergence(u_dev, v_dev, w_dev, p->geo, scale, out_dev, static_cast<cudaStream_t>(cuda_stream));
     p->launches_last = 1;
@@ -778,7 +831,7 @@ static bool dirs_valid(int d) { return d == TPT_DIRS_XYZ || d == TPT_DIRS_YZ || 
 
 int tpt_gradient_correct(tpt_plan *p, const double *phi_dev, double c, double *u_dev, double *v_dev, double *w_dev, double *p_dev,
                          double alpha_p, int implicit_dirs, void *cuda_stream) {
-    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c) || !on_plan_device(p)) return TPT_EINVAL;
+    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c) || !on_plan_device(p) || p->cyclic) return TPT_EINVAL;
     if (!aligned8(phi_dev) || !aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(p_dev)) return TPT_EINVAL;
     if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
     cudaError_t e = tpt::launch_correct(phi_dev, u_dev, v_dev, w_dev, p_dev, p->geo, c, alpha_p, implicit_dirs,
@@ -791,7 +844,7 @@ int tpt_project(tpt_plan *p, double *u_dev, double *v_dev, double *w_dev, double
                 double alpha_p, int implicit_dirs, void *cuda_stream) {
     if (!p || !u_dev || !v_dev || !w_dev || !phi_dev || !aligned16(phi_dev) || !on_plan_device(p)) return TPT_EINVAL;
     if (!aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(p_dev)) return TPT_EINVAL;
-    if (p->alpha != 0.0 || p->dirs != TPT_DIRS_XYZ) return TPT_EINVAL;       // Eq. 2c carries the full Laplacian
+    if (p->alpha != 0.0 || p->dirs != TPT_DIRS_XYZ || p->cyclic) return TPT_EINVAL;       // Eq. 2c carries the full Laplacian
     if (!(gamma_dt > 0.0) || !std::isfinite(gamma_dt)) return TPT_EINVAL;
     if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);

@@ -263,7 +263,7 @@ template <int U>
 __global__ void __launch_bounds__(128)
 thomas_kernel(double *x, double *__restrict__ cprime, const double *__restrict__ az, const double *__restrict__ bz,
               const double *__restrict__ cz, const double *__restrict__ lamx, const double *__restrict__ lamy, int nx,
-              int ny, int nz, double shift0, int singular) {
+              int ny, int nz, double shift0, int singular, double b0_null) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y;
     if (i >= nx) return;
@@ -273,7 +273,7 @@ thomas_kernel(double *x, double *__restrict__ cprime, const double *__restrict__
     const double s = lamx[i] + lamy[j] + shift0;
     const bool null_col = singular && i == 0 && j == 0;
 
-    double r = 1.0 / (__ldg(bz) + s);
+    double r = 1.0 / ((null_col ? b0_null : __ldg(bz)) + s);      // (cyclic sweep: the null column keeps the unmodified corner)
     double cprev = __ldg(cz) * r;
     double dprev = xc[0] * r;
     cc[0] = cprev;
@@ -322,10 +322,57 @@ thomas_kernel(double *x, double *__restrict__ cprime, const double *__restrict__
 
 cudaError_t launch_thomas(double *x, double *cprime, const double *az, const double *bz, const double *cz,
                           const double *lamx, const double *lamy, int nx, int ny, int nz, double shift0, int singular,
-                          cudaStream_t stream) {
+                          double b0_null, cudaStream_t stream) {
     if (ny > 65535) return cudaErrorInvalidValue;
     dim3 grid((nx + 127) / 128, ny);
-    thomas_kernel<8><<<grid, 128, 0, stream>>>(x, cprime, az, bz, cz, lamx, lamy, nx, ny, nz, shift0, singular);
+    thomas_kernel<8><<<grid, 128, 0, stream>>>(x, cprime, az, bz, cz, lamx, lamy, nx, ny, nz, shift0, singular, b0_null);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Periodic z ("cyclic corner entries"; A19): the cyclic column matrix is the tridiagonal A'
+// the sweep kernels solve (corners b_0 - g, b_{n-1} - c_{n-1} a_0 / g, one g per plan) plus a rank-one term, so
+//     x = y - q (y_0 + r y_{n-1}) / (1 + q_0 + r q_{n-1}),   A' y = p,  A' q = u = (g, 0, .., 0, c_{n-1}),  r = a_0 / g
+// (Sherman-Morrison).  q depends on the column's spectral shift only, not on the right-hand side: it is swept once at
+// plan time and kept (one field), with rden = 1 / (1 + q_0 + r q_{n-1}) per column (0 for the null column of a singular
+// plan, which the sweep itself gauges).  Per solve: the ordinary sweep, then this correction (24 B/pt).  Natural layout.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) cyclic_rhs_kernel(double *u, size_t cols, int nz, double g, double cn) {
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= cols) return;
+    for (int k = 0; k < nz; ++k) u[(size_t)k * cols + col] = k == 0 ? g : (k == nz - 1 ? cn : 0.0);
+}
+
+__global__ void __launch_bounds__(256) cyclic_rden_kernel(const double *__restrict__ q, double *__restrict__ rden, size_t cols, int nz,
+                                                          double r, int singular) {
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= cols) return;
+    const double den = 1.0 + q[col] + r * q[(size_t)(nz - 1) * cols + col];
+    rden[col] = (singular && col == 0) ? 0.0 : 1.0 / den;
+}
+
+__global__ void __launch_bounds__(256) cyclic_correct_kernel(double *x, const double *__restrict__ q, const double *__restrict__ rden,
+                                                             size_t cols, int nz, double r) {
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= cols) return;
+    const double fact = (x[col] + r * x[(size_t)(nz - 1) * cols + col]) * __ldg(rden + col);
+#pragma unroll 4
+    for (int k = 0; k < nz; ++k) {
+        const size_t e = (size_t)k * cols + col;
+        x[e] = fma(-fact, __ldg(q + e), x[e]);
+    }
+}
+
+cudaError_t launch_cyclic_rhs(double *u, size_t cols, int nz, double g, double cn, cudaStream_t stream) {
+    cyclic_rhs_kernel<<<(unsigned)((cols + 255) / 256), 256, 0, stream>>>(u, cols, nz, g, cn);
+    return cudaGetLastError();
+}
+cudaError_t launch_cyclic_rden(const double *q, double *rden, size_t cols, int nz, double r, int singular, cudaStream_t stream) {
+    cyclic_rden_kernel<<<(unsigned)((cols + 255) / 256), 256, 0, stream>>>(q, rden, cols, nz, r, singular);
+    return cudaGetLastError();
+}
+cudaError_t launch_cyclic_correct(double *x, const double *q, const double *rden, size_t cols, int nz, double r, cudaStream_t stream) {
+    cyclic_correct_kernel<<<(unsigned)((cols + 255) / 256), 256, 0, stream>>>(x, q, rden, cols, nz, r);
     return cudaGetLastError();
 }
 

@@ -55,9 +55,16 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream);
 // z sweep (step 2.3): in place on x (nx*ny*nz), cprime = field-sized scratch.
 // Solves (T_z + (lamx[i] + lamy[j] + shift0) I) x = rhs for each column; on a singular plan the
 // column (0,0) gets "last unknown = 0".
+// b0_null: diagonal entry of row 0 for the null column (= bz[0] except in the cyclic sweep, see launch_cyclic_*).
 cudaError_t launch_thomas(double *x, double *cprime, const double *az, const double *bz, const double *cz,
                           const double *lamx, const double *lamy, int nx, int ny, int nz, double shift0,
-                          int singular, cudaStream_t stream);
+                          int singular, double b0_null, cudaStream_t stream);
+
+// Periodic z (A19): Sherman-Morrison correction around the tridiagonal sweep (kernels.cu).
+// Natural layout, cols = nx * ny.  rhs: u = (g, 0, .., 0, cn) in every column; rden from the swept q; correct: per solve.
+cudaError_t launch_cyclic_rhs(double *u, size_t cols, int nz, double g, double cn, cudaStream_t stream);
+cudaError_t launch_cyclic_rden(const double *q, double *rden, size_t cols, int nz, double r, int singular, cudaStream_t stream);
+cudaError_t launch_cyclic_correct(double *x, const double *q, const double *rden, size_t cols, int nz, double r, cudaStream_t stream);
 
 // Same solve with the z-columns resident on chip (thomas_onchip.cu): 16 B/pt of HBM traffic, no scratch field.
 // Reads the right-hand sides from `in` and writes the solution to `x` (in == x: in place).
@@ -65,7 +72,9 @@ cudaError_t launch_thomas(double *x, double *cprime, const double *az, const dou
 // sms = SM count.
 constexpr int THOMAS_TABLE_PAD = 160;   // >= the rows by which S*M can exceed nz in any launch shape
 bool thomas_onchip_supported(int nx, int ny, int nz);
-void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out);
+// b_null: diagonal of the null column's table when it differs from b (cyclic sweep: unmodified corners); nullptr = b.
+void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out,
+                          const double *b_null = nullptr);
 // wz: the nz cell widths of the z direction — on a singular plan the kernel itself removes the dz-weighted mean of the
 // null column (0,0) before the tile leaves the chip (A7): no separate gauge launch.
 cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, const double *wz,

@@ -205,7 +205,7 @@ int tpt_shard_layout(int nranks, int rank, int nx, int ny, int nz, tpt_shard_lay
 
 int tpt_shard_create(tpt_shard **shard_out, int rank, int nranks, int nx, int ny, int nz, const double *xf, const double *yf,
                      const double *zf, const int bc[3], double helmholtz_alpha, int transform_x) {
-    if (!shard_out) return TPT_EINVAL;
+    if (!shard_out || !bc || bc[2] == TPT_BC_PERIODIC) return TPT_EINVAL;   // (the cyclic correction is not sharded)
     tpt_shard_layout_t lay;
     int rc = tpt_shard_layout(nranks, rank, nx, ny, nz, &lay);
     if (rc != TPT_OK) return rc;

@@ -408,7 +408,7 @@ cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &pe
 // Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows
 // [0, -1, 0, 0] (pivot -1 + s < 0 for every mode since s <= 0); the second table is the null column's, with the
 // last equation replaced by "-x = p" (the kernel zeroes p there): PAPER.md:219.
-void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out) {
+void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out, const double *b_null) {
     const size_t rows = (size_t)nz + THOMAS_TABLE_PAD;
     out.assign(8 * rows, 0.0);
     for (int v = 0; v < 2; ++v) {
@@ -416,7 +416,7 @@ void thomas_onchip_tables(int nz, const double *a, const double *b, const double
         for (size_t k = 0; k < rows; ++k) t[4 * k + 1] = -1.0;
         for (int k = 0; k < nz; ++k) {
             t[4 * k] = k > 0 ? a[k] * c[k - 1] : 0.0;
-            t[4 * k + 1] = b[k];
+            t[4 * k + 1] = (v == 1 && b_null) ? b_null[k] : b[k];
             t[4 * k + 2] = a[k];
             t[4 * k + 3] = c[k];
         }

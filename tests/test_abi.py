@@ -51,7 +51,7 @@ def test_argument_validation_needs_no_gpu(tpt):
         tpt.plan_create(8, 8, 8, good, good, good, (0, 3, 1), 0.0)
     assert e.value.status == -1
     with pytest.raises(tpt.TptError) as e:
-        tpt.plan_create(8, 8, 8, good, good, good, (0, 0, 2), 0.0)      # periodic z: the sweep is the plain Thomas algorithm
+        tpt.plan_create(8, 8, 2, good, good, np.linspace(0, 1, 3), (0, 0, 2), 0.0)      # periodic z needs at least 3 cells
     assert e.value.status == -1
     with pytest.raises(tpt.TptError) as e:
         tpt.plan_create(8, 8, 8, good, good, good, (0, 0, 1), -1.0)

@@ -301,13 +301,75 @@ def test_periodic_uniform_plan_eigenpairs_are_fourier(tpt, torch):
     plan.destroy()
 
 
-def test_periodic_z_and_tiny_periodic_are_rejected(tpt, torch):
+def test_tiny_periodic_directions_are_rejected(tpt, torch):
     xf = I.tanh_faces(16, 1.0, 0.0)
-    with pytest.raises(tpt.TptError):
-        tpt.plan_create(16, 16, 16, xf, xf, xf, (N_, N_, P_), 0.0)
     x2 = I.tanh_faces(2, 1.0, 0.0)
     with pytest.raises(tpt.TptError):
         tpt.plan_create(2, 16, 16, x2, xf, xf, (P_, N_, N_), 0.0)
+    with pytest.raises(tpt.TptError):
+        tpt.plan_create(16, 16, 2, xf, xf, x2, (N_, N_, P_), 0.0)
+
+
+# Periodic z ("cyclic corner entries"; A19): the sweep becomes a cyclic tridiagonal solve —
+# ordinary sweep on a corner-modified matrix + Sherman-Morrison correction — on every sweep kernel and GEMM path.
+CYCLIC_Z = [
+    # name, n, L, beta, bc, alpha, dirs, transform                                        sweep kernel
+    ("onchip", (128, 128, 40), (1.0, 1.0, 2.0), (2.0, 2.0, 1.5), (N_, D_, P_), 0.0, 7, (0, 0)),          # on-chip, TMA GEMM
+    ("singular", (128, 64, 96), (1.0, 1.0, 1.0), (2.0, 1.5, 2.0), (N_, N_, P_), 0.0, 7, (0, 0)),        # null column: x_last = 0 + gauge
+    ("all-periodic", (64, 48, 300), (2.0, 1.0, 1.0), (0.0, 1.0, 0.0), (P_, P_, P_), 0.0, 7, (0, 0)),    # singular, 17-row segments
+    ("odd-streaming", (9, 7, 11), (1.0, 2.0, 1.5), (1.2, 2.0, 1.0), (N_, N_, P_), 0.0, 7, (0, 0)),       # streaming sweep, singular
+    ("helmholtz-ff", (64, 32, 24), (2.0, 1.0, 1.0), (0.0, 0.0, 2.0), (P_, N_, P_), 3e-3, 7, (1, 1)),     # fast transforms in x, y
+    ("yz", (48, 64, 20), (1.0, 1.0, 1.0), (2.0, 1.0, 2.0), (N_, N_, P_), 5e-3, 6, (0, 0)),
+    ("z-only", (32, 16, 33), (1.0, 1.0, 1.0), (1.0, 1.0, 2.5), (N_, D_, P_), 0.3, 4, (0, 0)),            # scaled coefficients, cyclic
+    ("tall", (16, 16, 1000), (1.0, 1.0, 4.0), (1.0, 1.0, 3.0), (D_, N_, P_), 0.0, 7, (0, 0)),            # 512-thread shape
+]
+
+
+@pytest.mark.parametrize("case", CYCLIC_Z, ids=[c[0] for c in CYCLIC_Z])
+@pytest.mark.parametrize("thomas_variant", [1, 0])
+def test_periodic_z_parity(tpt, torch, orc, case, thomas_variant):
+    name, n, L, beta, bc, alpha, dirs, tr = case
+    P = I.Problem(name, n, L, beta, bc, alpha, seed=3 + n[2])
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, alpha, dirs=dirs, transform=tr)
+    plan.set_thomas_variant(thomas_variant)
+    assert plan.singular == P.singular
+    assert tpt.PATH_FUSED_SMALL not in plan.paths() and plan.paths()[tpt.K_THOMAS] != tpt.PATH_THOMAS_BLOCKED
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha, dirs=dirs).solve(f)
+    for inplace in (False, True):
+        u = _solve(torch, plan, f, inplace)
+        assert _rel(u, ref) <= PARITY_TOL
+        r = orc.residual_norms(xf, yf, zf, bc, alpha, f, u, dirs=dirs)
+        assert r["rel2"] <= RESID_TOL and r["relL2vol"] <= RESID_TOL
+    if P.singular:
+        V = np.diff(zf)[:, None, None] * np.diff(yf)[None, :, None] * np.diff(xf)[None, None, :]
+        assert abs((V * u).sum()) <= 1e-13 * np.abs(u).max() * V.sum()
+    # host-buffer solve (slab pipeline of the copies) and a batch of two
+    out = np.empty_like(f)
+    plan.solve_host(f, out)
+    assert _rel(out, ref) <= PARITY_TOL
+    plan.reserve_batch(2)
+    d_b = torch.from_numpy(np.stack([f, f])).cuda()
+    d_o = torch.empty_like(d_b)
+    plan.solve_batch(d_b, d_o)
+    torch.cuda.synchronize()
+    assert _rel(d_o[1].cpu().numpy(), ref) <= PARITY_TOL
+    plan.destroy()
+
+
+def test_periodic_z_limits(tpt, torch):
+    P = I.Problem("lim", (128, 128, 16), (1.0, 1.0, 1.0), (1.0, 1.0, 0.0), (N_, N_, P_), 0.0, 1)
+    xf, yf, zf = P.faces()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, 0.0)
+    d = torch.zeros(P.n[::-1], dtype=torch.float64, device="cuda")
+    su, sv, sw = (16, 128, 129), (16, 129, 128), (17, 128, 128)
+    du, dv, dw = (torch.zeros(sh, dtype=torch.float64, device="cuda") for sh in (su, sv, sw))
+    with pytest.raises(tpt.TptError):
+        tpt.project(plan, du, dv, dw, 0.5, d)           # the staggered operators do not close z periodically
+    plan.destroy()
+    with pytest.raises(tpt.TptError):
+        tpt.shard_create(0, 2, *P.n, xf, yf, zf, P.bc, 0.0)
 
 
 def test_paper_benchmark_case_thin_z_parity(tpt, torch, orc):
