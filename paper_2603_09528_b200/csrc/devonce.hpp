@@ -9,6 +9,7 @@
 #include <map>
 #include <mutex>
 #include <tuple>
+#include <utility>
 
 namespace tpt {
 
@@ -58,5 +59,22 @@ class OccupancyCache {
     std::mutex m_;
     std::map<std::tuple<int, int, size_t>, int> map_;
 };
+
+// Kernel launch with programmatic dependent launch allowed (ptx.cuh pdl_wait / pdl_launch_dependents): the launch
+// latency and prologue of a solve's kernel k+1 overlap the tail of kernel k — what matters on the launch-bound grids.
+template <class K, class... Args>
+cudaError_t launch_pdl(K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args &&...args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 }  // namespace tpt

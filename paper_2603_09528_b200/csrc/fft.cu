@@ -23,6 +23,9 @@ namespace tpt {
 
 namespace {
 
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }   // see ptx.cuh
+
 struct cplx { double x, y; };
 __device__ __forceinline__ cplx operator+(cplx a, cplx b) { return {a.x + b.x, a.y + b.y}; }
 __device__ __forceinline__ cplx operator-(cplx a, cplx b) { return {a.x - b.x, a.y - b.y}; }
@@ -258,6 +261,8 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     cplx *seq = buf + pr * NPAD;
     const Addr<YP, LOGN> A(p, pr);
     cplx v[16];
+    pdl_launch_dependents();
+    pdl_wait();                   // the input is the previous kernel's output
 
     // ---- pass 0 (Ns = 1: no twiddles) -------------------------------------------------------------------------------
     constexpr int R0 = radix_at(LOGN, 0), IT0 = 16 / R0, PER0 = N / R0;
@@ -425,6 +430,8 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     cplx *seq = buf + pr * NPAD;
     const Addr<YP, LOGN> A(p, pr);
     cplx v[16];
+    pdl_launch_dependents();
+    pdl_wait();                   // the input is the previous kernel's output
 
     // ---- first pass: paired items, inputs built from the coefficients ---------------------------------------------------
     constexpr int R0 = radix_at(LOGN, 0), IT0 = 16 / R0, PER0 = N / R0;
@@ -638,9 +645,8 @@ cudaError_t launch_bc(const FftParams &p, int inverse, cudaStream_t stream) {
         if (e != cudaSuccess) return e;
     }
     const dim3 grid(grid_x, grid_y);
-    if (inverse) fft_inverse_kernel<YP, LOGN, BC><<<grid, threads, smem, stream>>>(p);
-    else fft_forward_kernel<YP, LOGN, BC><<<grid, threads, smem, stream>>>(p);
-    return cudaGetLastError();
+    if (inverse) return launch_pdl(fft_inverse_kernel<YP, LOGN, BC>, grid, dim3(threads), smem, stream, p);
+    return launch_pdl(fft_forward_kernel<YP, LOGN, BC>, grid, dim3(threads), smem, stream, p);
 }
 
 template <bool YP, int LOGN>

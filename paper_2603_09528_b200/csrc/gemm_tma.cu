@@ -16,6 +16,7 @@
 // lies wholly outside skip their DMMAs, and the epilogue stores are predicated.
 #include <cuda.h>
 
+#include "devonce.hpp"
 #include "kernels.cuh"
 #include "ptx.cuh"
 #include "tmap.hpp"
@@ -73,7 +74,9 @@ gemm_tma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         }
         ptx::fence_mbar_init();
     }
+    ptx::pdl_launch_dependents();
     __syncthreads();
+    ptx::pdl_wait();              // the operands are the previous kernel's output
 
     const int KT = p.KT;
     if (warp >= CONSUMER_WARPS) {
@@ -294,9 +297,8 @@ cudaError_t launch_gemm_tma(const GemmArgs &g, int sms, cudaStream_t stream) {
     p.units = g.M / 16 > 0 ? g.M / 16 : 1;
     for (int q = 0; q < MAX_PEERS; ++q) p.peerC[q] = q < g.npeers ? g.peerC[q] : nullptr;
     const int grid = p.ntiles < sms ? p.ntiles : sms;
-    if (g.M % BM == 0 && g.N % BN == 0 && g.K % BK == 0) gemm_tma_kernel<false><<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);
-    else gemm_tma_kernel<true><<<grid, THREADS, SMEM_BYTES, stream>>>(mapA, mapB, p);
-    return cudaGetLastError();
+    if (g.M % BM == 0 && g.N % BN == 0 && g.K % BK == 0) return launch_pdl(gemm_tma_kernel<false>, dim3(grid), dim3(THREADS), SMEM_BYTES, stream, mapA, mapB, p);
+    return launch_pdl(gemm_tma_kernel<true>, dim3(grid), dim3(THREADS), SMEM_BYTES, stream, mapA, mapB, p);
 }
 
 }  // namespace tpt

@@ -108,6 +108,13 @@ __device__ __forceinline__ void tma_prefetch_desc(const void *tmap) {
 // generic-proxy shared-memory writes -> visible to subsequent async-proxy (bulk copy) reads
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 
+// ---- programmatic dependent launch (PDL): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may
+// start (its CTAs become resident and run their prologue) while the previous kernel of the stream is still draining;
+// pdl_wait() blocks until that kernel has completed and its memory is visible — nothing it wrote may be touched before.
+// pdl_launch_dependents() lets the NEXT kernel of the stream start early in the same way.  Both are no-ops without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
+
 // ---- cp.async (LDGSTS) --------------------------------------------------------------------------
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");

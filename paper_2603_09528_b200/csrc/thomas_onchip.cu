@@ -81,7 +81,9 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
     for (int b = 0; b < nbuf; ++b)
         for (int e = nbox * box_rows * TCOLS + tid; e < (int)tile_elems; e += blockDim.x)
             bufs[(size_t)b * tile_elems + e] = 0.0;
+    ptx::pdl_launch_dependents();
     __syncthreads();
+    ptx::pdl_wait();              // the tiles are the previous kernel's output
 
     auto issue_load = [&](int tile, int b) {      // one thread: nbox boxes of box_rows x 16 doubles
         if (tid != 0) return;
@@ -342,15 +344,14 @@ cudaError_t launch_m(const double *in, double *x, const ThomasPeers *peers, cons
             if ((peers->k0[r] & 1) && TC < 16) return cudaErrorInvalidValue;
             if (!make_field_map(&dst.map[r], peers->slab[r], peers->total_cols, nzl, TC, dst.box_rows, true)) return cudaErrorUnknown;
         }
-        kern<<<grid, g.threads, g.smem, stream>>>(tmap, dst, tab, tab_null, lamx, lamy, wz, nx, nz, g.S, g.nbuf, g.box_rows, g.nbox,
-                                                  g.buf_rows, shift0, singular, ntiles);
+        return launch_pdl(kern, dim3(grid), dim3(g.threads), g.smem, stream, tmap, dst, tab, tab_null, lamx, lamy, wz, nx, nz, g.S, g.nbuf,
+                          g.box_rows, g.nbox, g.buf_rows, shift0, singular, ntiles);
     } else {
         StoreOne dst;
         if (!make_field_map(&dst.map, x, cols, nz, TC, g.box_rows, blocked)) return cudaErrorUnknown;
-        kern<<<grid, g.threads, g.smem, stream>>>(tmap, dst, tab, tab_null, lamx, lamy, wz, nx, nz, g.S, g.nbuf, g.box_rows, g.nbox,
-                                                  g.buf_rows, shift0, singular, ntiles);
+        return launch_pdl(kern, dim3(grid), dim3(g.threads), g.smem, stream, tmap, dst, tab, tab_null, lamx, lamy, wz, nx, nz, g.S, g.nbuf,
+                          g.box_rows, g.nbox, g.buf_rows, shift0, singular, ntiles);
     }
-    return cudaGetLastError();
 }
 
 }  // namespace
