@@ -41,8 +41,9 @@ SM_COUNT, FP64_FMA_PER_CLK_SM = 148, 64
 # uniform power-of-two direction.  BASELINE.json's metric is quoted on GG.
 TRANSFORMS = {"gg": (0, 0), "fg": (1, 0), "gf": (0, 1), "ff": (1, 1)}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (gemm_tma_kernel), from the one
-# `ncu --set full` capture summarised in profiles/r1c_blocked_layout_projection.md (config c3; bytes).  Other configs: null.
-NCU_TRAFFIC = {"commit": "757b0f5", "capture": "profiles/r1c_blocked_layout_projection.md", "bytes": {"c3": 1.077565e9 + 1.031300e9}}
+# `ncu --set full` capture summarised in profiles/r2_final_round2.md (config c3; bytes), taken with the kernel sources of the
+# commit named here (the round's last kernel change).  Other configs: null.
+NCU_TRAFFIC = {"commit": "2e93fea", "capture": "profiles/r2_final_round2.md", "bytes": {"c3": 1.075920e9 + 1.030197e9}}
 
 
 def _peaks():

@@ -277,3 +277,24 @@ def test_slab_pipeline_is_bitwise_the_plain_solve(tpt, torch, orc, case, groups)
     plan.solve(d_f, d_o[0])
     assert plan.launches_last() == plain_launches
     plan.destroy()
+
+
+def test_ff512_full_size_parity_in_the_bench_configuration(tpt, torch, orc):
+    # the grid bench.py --config ff512 --transform ff times (512^3, uniform x, y, stretched z): every element against a
+    # full oracle solve (the oracle knows no fast transform: its own eigen-solver and naive loops), residual and paths
+    P = I.CONFIGS["ff512"][0]
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    plan = tpt.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=(tpt.TRANSFORM_FFT, tpt.TRANSFORM_FFT))
+    assert plan.paths() == [tpt.PATH_FFT, tpt.PATH_FFT, tpt.PATH_THOMAS_BLOCKED, tpt.PATH_FFT, tpt.PATH_FFT]
+    d_f = torch.from_numpy(f).cuda()
+    d_o = torch.empty_like(d_f)
+    plan.solve(d_f, d_o)
+    torch.cuda.synchronize()
+    phi = d_o.cpu().numpy()
+    del d_f, d_o
+    plan.destroy()
+    r = orc.residual_norms(xf, yf, zf, P.bc, P.alpha, f, phi)
+    assert r["rel2"] <= 1e-11 and r["relL2vol"] <= 1e-11
+    ref = orc.OraclePlan(xf, yf, zf, P.bc, P.alpha).solve(f)
+    assert _rel(phi, ref) <= PARITY_TOL
