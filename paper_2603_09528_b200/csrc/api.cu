@@ -910,6 +910,8 @@ int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
     for (int d = 0; d < 2; ++d)
         if (p->d_fft[d]) b += (size_t)5 * (d == 0 ? p->nx : p->ny) * sizeof(double);        // twiddle tables (upper bound)
     b += p->points() * sizeof(double) * ((size_t)p->work_fields + (p->d_stage ? 1 : 0));
+    b += 2 * p->slab_elems * sizeof(double);                                                // slab pipeline buffers (lazy)
+    if (p->cyclic) b += (p->points() + (size_t)p->nx * p->ny) * sizeof(double);             // periodic z: q field + per-column factors
     *bytes_out = b;
     return TPT_OK;
 }
