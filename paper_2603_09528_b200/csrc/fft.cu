@@ -121,12 +121,32 @@ __device__ __forceinline__ void bfly(cplx *v) {
     if (R == 8) fft8<INV>(v);
     else fft4<INV>(v[0], v[1], v[2], v[3]);
 }
-template <int R, int INV>
+// v_r *= W^{r k}, W = e^{-+2 pi i / (Ns R)}, from the pass table Wq[(r-1) Ns + k].  DERIVE: load only W^k, W^2k (and W^4k) and
+// form the other powers by complex multiplication — in the x kernels consecutive lanes hold consecutive k, so every
+// table load is a full 512-byte warp access and seven of them per item cost more L1 bandwidth than the data itself.
+template <int R, int INV, bool DERIVE>
 __device__ __forceinline__ void twiddle(cplx *v, const double2 *__restrict__ Wq, int Ns, int k) {
+    if (!DERIVE) {
 #pragma unroll
-    for (int r = 1; r < R; ++r) {
-        const double2 w = __ldg(Wq + (r - 1) * Ns + k);
-        v[r] = cmul(v[r], cplx{w.x, INV ? -w.y : w.y});
+        for (int r = 1; r < R; ++r) {
+            const double2 w = __ldg(Wq + (r - 1) * Ns + k);
+            v[r] = cmul(v[r], cplx{w.x, INV ? -w.y : w.y});
+        }
+    } else {
+        const double2 a = __ldg(Wq + k), b = __ldg(Wq + Ns + k);
+        const cplx w1{a.x, INV ? -a.y : a.y}, w2{b.x, INV ? -b.y : b.y};
+        const cplx w3 = cmul(w1, w2);
+        v[1] = cmul(v[1], w1);
+        v[2] = cmul(v[2], w2);
+        v[3] = cmul(v[3], w3);
+        if (R == 8) {
+            const double2 c = __ldg(Wq + 3 * Ns + k);
+            const cplx w4{c.x, INV ? -c.y : c.y};
+            v[4] = cmul(v[4], w4);
+            v[5] = cmul(v[5], cmul(w4, w1));
+            v[6] = cmul(v[6], cmul(w4, w2));
+            v[7] = cmul(v[7], cmul(w4, w3));
+        }
     }
 }
 
@@ -148,7 +168,7 @@ __device__ __forceinline__ bool special_slot(int slot) {
 
 // Middle passes Q = 1 .. NP-2: in-place Stockham pass through shared memory.  Item j of a sequence: k = j mod Ns;
 // v_r = buf[j + r N/R] W^{r k}; radix-R butterfly; buf[(j - k) R + k + r Ns] = v_r.
-template <int LOGN, int INV, int Q, int NS, int UPP>
+template <int LOGN, int INV, int Q, int NS, int UPP, bool XDIR>
 __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParams &p, int u) {
     constexpr int NP = npasses(LOGN), N = 1 << LOGN;
     if constexpr (Q < NP - 1) {
@@ -158,7 +178,7 @@ __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParam
             const int j = u + it * UPP, k = j & (NS - 1);
 #pragma unroll
             for (int r = 0; r < R; ++r) v[it * R + r] = seq[pad(j + r * PER)];
-            twiddle<R, INV>(v + it * R, p.Wq[Q], NS, k);
+            twiddle<R, INV, (XDIR && NS >= 32)>(v + it * R, p.Wq[Q], NS, k);
             bfly<R, INV>(v + it * R);
         }
         __syncthreads();
@@ -169,7 +189,7 @@ __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParam
             for (int r = 0; r < R; ++r) seq[pad((j - k) * R + k + r * NS)] = v[it * R + r];
         }
         __syncthreads();
-        middle_passes<LOGN, INV, Q + 1, NS * R, UPP>(seq, v, p, u);
+        middle_passes<LOGN, INV, Q + 1, NS * R, UPP, XDIR>(seq, v, p, u);
     }
 }
 // e^{-i pi r / (2 R)}: T4[j + r N/R] = T4[j] * rot<R>(r), so the post-/pre-twiddles e^{-i pi k / 2N} of all bins of an item
@@ -342,7 +362,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
         for (int r = 0; r < R0; ++r) seq[pad((u + it * UPP) * R0 + r)] = v[it * R0 + r];
     }
     __syncthreads();
-    middle_passes<LOGN, 0, 1, R0, UPP>(seq, v, p, u);
+    middle_passes<LOGN, 0, 1, R0, UPP, !YP>(seq, v, p, u);
 
     // ---- last pass: paired items; Ns = PER = N / R ---------------------------------------------------------------------
     constexpr int RL = radix_at(LOGN, NP - 1), ITL = 16 / RL, NSL = N / RL;
@@ -361,7 +381,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     for (int it = 0; it < ITL; ++it) {
 #pragma unroll
         for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[pad(jl[it] + r * NSL)];
-        twiddle<RL, 0>(v + it * RL, p.Wq[NP - 1], NSL, jl[it]);
+        twiddle<RL, 0, (!YP && NSL >= 32)>(v + it * RL, p.Wq[NP - 1], NSL, jl[it]);
         bfly<RL, 0>(v + it * RL);
     }
     // v[it RL + r] = Z[jl[it] + r NSL].  Untangle (V1_k = (Z_k + conj Z_{N-k}) / 2, V2_k = (Z_k - conj Z_{N-k}) / 2i;
@@ -520,7 +540,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
         for (int r = 0; r < R0; ++r) seq[pad(j0[it] * R0 + r)] = v[it * R0 + r];
     }
     __syncthreads();
-    middle_passes<LOGN, 1, 1, R0, UPP>(seq, v, p, u);
+    middle_passes<LOGN, 1, 1, R0, UPP, !YP>(seq, v, p, u);
 
     // ---- last pass ------------------------------------------------------------------------------------------------------
     constexpr int RL = radix_at(LOGN, NP - 1), ITL = 16 / RL, NSL = N / RL;
@@ -529,7 +549,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
         const int j = u + it * UPP;
 #pragma unroll
         for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[pad(j + r * NSL)];
-        twiddle<RL, 1>(v + it * RL, p.Wq[NP - 1], NSL, j);
+        twiddle<RL, 1, (!YP && NSL >= 32)>(v + it * RL, p.Wq[NP - 1], NSL, j);
         bfly<RL, 1>(v + it * RL);
     }
     if (YP) {       // z[n] -> sample i(n) of both lines: one 16-byte store per row
