@@ -908,7 +908,7 @@ int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
     b += ((size_t)p->nx + p->ny + 4 * (size_t)p->nz + 8) * sizeof(double);
     b += (2 * ((size_t)p->nx + p->ny + p->nz) + 16) * sizeof(double);                       // staggered-grid geometry
     for (int d = 0; d < 2; ++d)
-        if (p->d_fft[d]) b += (size_t)5 * (d == 0 ? p->nx : p->ny) * sizeof(double);        // twiddle tables (upper bound)
+        if (p->d_fft[d]) b += (size_t)8 * (d == 0 ? p->nx : p->ny) * sizeof(double);        // twiddle tables (upper bound)
     b += p->points() * sizeof(double) * ((size_t)p->work_fields + (p->d_stage ? 1 : 0));
     b += 2 * p->slab_elems * sizeof(double);                                                // slab pipeline buffers (lazy)
     if (p->cyclic) b += (p->points() + (size_t)p->nx * p->ny) * sizeof(double);             // periodic z: q field + per-column factors

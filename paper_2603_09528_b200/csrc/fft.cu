@@ -86,7 +86,17 @@ struct FftParams {
 
 // Everything that depends only on the transform length is a compile-time constant of the kernel (template LOGN): the
 // pass radices, the lines per CTA, every shift, mask and padded offset.
-__host__ __device__ constexpr int radix_at(int logn, int q) {            // as many 8s as possible, then 4 (or 4, 4)
+// Pass radices.  Up to N = 512: as many 8s as possible, then 4 (or 4, 4) — at most three passes.  N = 1024 / 2048 would need
+// four radix-8/4 passes = three exchanges through shared memory, the pipe these kernels saturate first; with radix-16
+// passes (one item of 16 values per thread) they need three: 16, 16, 4 / 16, 16, 8.  The pass that works on conjugate-paired
+// items (last forward, first inverse) needs two items per thread, i.e. radix 4 or 8: the inverse runs the same radices
+// in the opposite order (4, 16, 16 / 8, 16, 16) with its own twiddle tables.
+__host__ __device__ constexpr int radix_at(int logn, int q, int inv = 0) {
+    if (logn >= 10) {
+        const int small = logn == 10 ? 4 : 8;
+        if (q > 2) return 0;
+        return inv ? (q == 0 ? small : 16) : (q == 2 ? small : 16);
+    }
     const int n8 = logn / 3, rem = logn % 3;
     if (rem == 1) return q < n8 - 1 ? 8 : (q < n8 + 1 ? 4 : 0);
     return q < n8 ? 8 : ((rem == 2 && q == n8) ? 4 : 0);
@@ -116,9 +126,32 @@ struct Geo {
     static constexpr size_t SMEM = (size_t)PAIRS * NPAD * 16;
 };
 
+// 16-point DFT in registers as 4 x 4: radix-4 over the stride-4 subsets, twiddles W16^{a b}, radix-4 across; the result
+// of frequency b + 4c lands in slot 4b + c and is renamed into natural order.
+template <int INV>
+__device__ __forceinline__ void fft16(cplx *v) {
+    constexpr double c1 = 0.92387953251128675613, s1 = 0.38268343236508977173, h = 0.70710678118654752440;
+#pragma unroll
+    for (int a = 0; a < 4; ++a) fft4<INV>(v[a], v[a + 4], v[a + 8], v[a + 12]);      // v[a + 4b] = sum_m x[a + 4m] W4^{m b}
+    auto tw = [&](cplx &z, double wr, double wi) { z = cmul(z, cplx{wr, INV ? -wi : wi}); };   // W16^q = (wr, wi), forward sign
+    tw(v[1 + 4], c1, -s1);  tw(v[2 + 4], h, -h);     tw(v[3 + 4], s1, -c1);          // b = 1: q = 1, 2, 3
+    tw(v[1 + 8], h, -h);    v[2 + 8] = mul_mi<INV>(v[2 + 8]);  tw(v[3 + 8], -h, -h); // b = 2: q = 2, 4, 6
+    tw(v[1 + 12], s1, -c1); tw(v[2 + 12], -h, -h);   tw(v[3 + 12], -c1, s1);         // b = 3: q = 3, 6, 9
+#pragma unroll
+    for (int b = 0; b < 4; ++b) fft4<INV>(v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]);   // v[4b + c] = X[b + 4c]
+    cplx t[16];
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) t[b + 4 * c] = v[4 * b + c];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) v[q] = t[q];
+}
+
 template <int R, int INV>
 __device__ __forceinline__ void bfly(cplx *v) {
-    if (R == 8) fft8<INV>(v);
+    if (R == 16) fft16<INV>(v);
+    else if (R == 8) fft8<INV>(v);
     else fft4<INV>(v[0], v[1], v[2], v[3]);
 }
 // v_r *= W^{r k}, W = e^{-+2 pi i / (Ns R)}, from the pass table Wq[(r-1) Ns + k].  DERIVE: load only W^k, W^2k (and W^4k) and
@@ -139,13 +172,26 @@ __device__ __forceinline__ void twiddle(cplx *v, const double2 *__restrict__ Wq,
         v[1] = cmul(v[1], w1);
         v[2] = cmul(v[2], w2);
         v[3] = cmul(v[3], w3);
-        if (R == 8) {
+        if (R >= 8) {
             const double2 c = __ldg(Wq + 3 * Ns + k);
             const cplx w4{c.x, INV ? -c.y : c.y};
+            const cplx w5 = cmul(w4, w1), w6 = cmul(w4, w2), w7 = cmul(w4, w3);
             v[4] = cmul(v[4], w4);
-            v[5] = cmul(v[5], cmul(w4, w1));
-            v[6] = cmul(v[6], cmul(w4, w2));
-            v[7] = cmul(v[7], cmul(w4, w3));
+            v[5] = cmul(v[5], w5);
+            v[6] = cmul(v[6], w6);
+            v[7] = cmul(v[7], w7);
+            if (R == 16) {
+                const double2 d = __ldg(Wq + 7 * Ns + k);
+                const cplx w8{d.x, INV ? -d.y : d.y};
+                v[8] = cmul(v[8], w8);
+                v[9] = cmul(v[9], cmul(w8, w1));
+                v[10] = cmul(v[10], cmul(w8, w2));
+                v[11] = cmul(v[11], cmul(w8, w3));
+                v[12] = cmul(v[12], cmul(w8, w4));
+                v[13] = cmul(v[13], cmul(w8, w5));
+                v[14] = cmul(v[14], cmul(w8, w6));
+                v[15] = cmul(v[15], cmul(w8, w7));
+            }
         }
     }
 }
@@ -172,7 +218,7 @@ template <int LOGN, int INV, int Q, int NS, int UPP, bool XDIR>
 __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParams &p, int u) {
     constexpr int NP = npasses(LOGN), N = 1 << LOGN;
     if constexpr (Q < NP - 1) {
-        constexpr int R = radix_at(LOGN, Q), IT = 16 / R, PER = N / R;
+        constexpr int R = radix_at(LOGN, Q, INV), IT = 16 / R, PER = N / R;
 #pragma unroll
         for (int it = 0; it < IT; ++it) {
             const int j = u + it * UPP, k = j & (NS - 1);
@@ -454,7 +500,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     pdl_wait();                   // the input is the previous kernel's output
 
     // ---- first pass: paired items, inputs built from the coefficients ---------------------------------------------------
-    constexpr int R0 = radix_at(LOGN, 0), IT0 = 16 / R0, PER0 = N / R0;
+    constexpr int R0 = radix_at(LOGN, 0, 1), IT0 = 16 / R0, PER0 = N / R0;
     int j0[4];
     paired_items<R0, PER0, UPP>(u, j0);
     // Every register position first receives the coefficient its own bin contributes: bin k of a cosine / sine transform
@@ -543,7 +589,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     middle_passes<LOGN, 1, 1, R0, UPP, !YP>(seq, v, p, u);
 
     // ---- last pass ------------------------------------------------------------------------------------------------------
-    constexpr int RL = radix_at(LOGN, NP - 1), ITL = 16 / RL, NSL = N / RL;
+    constexpr int RL = radix_at(LOGN, NP - 1, 1), ITL = 16 / RL, NSL = N / RL;
 #pragma unroll
     for (int it = 0; it < ITL; ++it) {
         const int j = u + it * UPP;
@@ -592,37 +638,23 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
 
 }  // namespace
 
-// pass radices of a length-2^m transform: as many 8s as possible, then 4 (or 4, 4); at most 4 passes for n <= 2048
-static int fft_radices(int n, int radix[4]) {
+// pass radices of a length-2^m transform (radix_at above), forward or inverse order
+static int fft_radices(int n, int radix[4], int inv) {
     int m = 0;
     while ((1 << m) < n) ++m;
-    int q = 0;
-    const int n8 = m / 3, rem = m % 3;
-    radix[0] = radix[1] = radix[2] = radix[3] = 0;
-    if (rem == 1) {
-        for (int r = 0; r < n8 - 1; ++r) radix[q++] = 8;
-        radix[q++] = 4; radix[q++] = 4;
-    } else {
-        for (int r = 0; r < n8; ++r) radix[q++] = 8;
-        if (rem == 2) radix[q++] = 4;
-    }
+    for (int q = 0; q < 4; ++q) radix[q] = radix_at(m, q, inv);
     return m;
 }
 
 bool fft_supported(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
 
 // Host side of the twiddle tables, interleaved (re, im): T4[k] = e^{-i pi k / 2N} (n entries), then for every pass
-// after the first its table e^{-2 pi i r k / (Ns R)}, r = 1..R-1, k = 0..Ns-1.
-void fft_tables(int n, std::vector<double> &out) {
+// after the first its table e^{-2 pi i r k / (Ns R)}, r = 1..R-1, k = 0..Ns-1 — for the forward radix order, then (where
+// it differs: n >= 1024) for the inverse order.
+static void pass_tables(int n, int inv, std::vector<double> &out) {
     const long double pi = 3.14159265358979323846264338327950288L;
-    out.clear();
-    for (int t = 0; t < n; ++t) {
-        const long double b = -pi * t / (2.0L * n);
-        out.push_back((double)cosl(b));
-        out.push_back((double)sinl(b));
-    }
     int radix[4];
-    fft_radices(n, radix);
+    fft_radices(n, radix, inv);
     int Ns = 1;
     for (int q = 0; q < 4 && radix[q]; ++q) {
         const int R = radix[q];
@@ -635,6 +667,25 @@ void fft_tables(int n, std::vector<double> &out) {
                 }
         Ns *= R;
     }
+}
+static bool orders_differ(int n) {
+    int f[4], i[4];
+    fft_radices(n, f, 0);
+    fft_radices(n, i, 1);
+    for (int q = 0; q < 4; ++q)
+        if (f[q] != i[q]) return true;
+    return false;
+}
+void fft_tables(int n, std::vector<double> &out) {
+    const long double pi = 3.14159265358979323846264338327950288L;
+    out.clear();
+    for (int t = 0; t < n; ++t) {
+        const long double b = -pi * t / (2.0L * n);
+        out.push_back((double)cosl(b));
+        out.push_back((double)sinl(b));
+    }
+    pass_tables(n, 0, out);
+    if (orders_differ(n)) pass_tables(n, 1, out);
 }
 
 cudaError_t fft_configure() { return cudaSuccess; }   // shared-memory opt-in happens per instantiation at first launch
@@ -703,14 +754,17 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
     p.s0 = a.s0; p.s1 = a.s1;
     p.blk_in = a.dir == 1 && a.inverse && a.blocked; p.blk_out = a.dir == 1 && !a.inverse && a.blocked;
     p.nz = a.nz; p.k0 = a.k0;
-    p.logN = fft_radices(N, p.radix);
     {
         const double2 *w = p.T4 + N;
-        int Ns = 1;
-        for (int q = 0; q < 4 && p.radix[q]; ++q) {
-            p.Wq[q] = w;
-            if (q > 0) w += (p.radix[q] - 1) * Ns;
-            Ns *= p.radix[q];
+        // forward-order tables first; the inverse-order set follows where the orders differ
+        for (int dir = 0; dir <= (a.inverse && orders_differ(N) ? 1 : 0); ++dir) {
+            p.logN = fft_radices(N, p.radix, dir);
+            int Ns = 1;
+            for (int q = 0; q < 4 && p.radix[q]; ++q) {
+                p.Wq[q] = w;
+                if (q > 0) w += (p.radix[q] - 1) * Ns;
+                Ns *= p.radix[q];
+            }
         }
     }
     p.planes = a.planes;
