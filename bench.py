@@ -339,7 +339,7 @@ def measure_sharded(api, torch, dist, args, probs, rank, world, stream, barrier)
         key = (P.n, P.bc, P.alpha, P.beta, P.length)
         if key not in cache:
             xf, yf, zf = P.faces()
-            sh = api.shard_create(rank, world, *P.n, xf, yf, zf, P.bc, P.alpha, TRANSFORMS[args.transform][0])
+            sh = api.shard_create(rank, world, *P.n, xf, yf, zf, P.bc, P.alpha, *TRANSFORMS[args.transform])
             exchange_ipc_handles(dist, sh)
             cache[key] = sh
         sh = cache[key]

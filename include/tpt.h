@@ -202,7 +202,9 @@ int tpt_plan_destroy(tpt_plan *plan);
  * owner's memory — peer-mapped pointers over NVLink, no pack/unpack kernel, no collective.  Per solve a rank sends
  * nvlink_bytes_per_solve bytes (2 * 8 * nx * (m1-m0) * (nz - (k1-k0))), two device-side flag barriers order the phases.
  *
- * Shapes: nx, ny multiples of 128; 2*nranks <= nz <= 1056; ny/16 >= nranks; x and y by GEMM or (x only) fast transform;
+ * Shapes: nx a multiple of 128; ny a multiple of 128 (GEMM y transform) or a power of two >= 16 (fast y transform,
+ * tpt_shard_create_ex); 2*nranks <= nz <= 1056; ny/16 >= nranks; x and y by GEMM or fast transform — all four variants
+ * GG / FG / GF / FF of PAPER.md:294, the y transform (GEMM epilogue or the fast transform's own stores) carrying exchange 1;
  * bc and alpha as tpt_plan_create (periodic z: TPT_EINVAL); anything else TPT_EINVAL.  Slab boundaries are even numbers.
  *
  * tpt_shard_layout      HOST only, needs no device: the split every rank computes identically.
@@ -245,6 +247,8 @@ typedef struct tpt_shard_layout_t {
 int tpt_shard_layout(int nranks, int rank, int nx, int ny, int nz, tpt_shard_layout_t *out);
 int tpt_shard_create(tpt_shard **shard_out, int rank, int nranks, int nx, int ny, int nz, const double *xf, const double *yf,
                      const double *zf, const int bc[3], double helmholtz_alpha, int transform_x);
+int tpt_shard_create_ex(tpt_shard **shard_out, int rank, int nranks, int nx, int ny, int nz, const double *xf, const double *yf,
+                        const double *zf, const int bc[3], double helmholtz_alpha, const int transform_xy[2]);
 int tpt_shard_get_layout(const tpt_shard *shard, tpt_shard_layout_t *out);
 int tpt_shard_sym(const tpt_shard *shard, void **sym_dev_out, size_t *bytes_out);
 int tpt_shard_set_peers(tpt_shard *shard, void *const *sym_dev);

@@ -34,7 +34,7 @@ SYMBOLS = (
     "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_launches", "tpt_plan_set_slab_groups", "tpt_plan_set_fused_small", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
     "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_fill_uniform",
-    "tpt_shard_layout", "tpt_shard_create", "tpt_shard_get_layout", "tpt_shard_sym", "tpt_shard_set_peers", "tpt_shard_ipc_export",
+    "tpt_shard_layout", "tpt_shard_create", "tpt_shard_create_ex", "tpt_shard_get_layout", "tpt_shard_sym", "tpt_shard_set_peers", "tpt_shard_ipc_export",
     "tpt_shard_ipc_import", "tpt_solve_sharded", "tpt_shard_solve_phase", "tpt_shard_barrier", "tpt_shard_barrier_all", "tpt_shard_launches", "tpt_shard_destroy",
 )
 IPC_HANDLE_BYTES = 64
@@ -98,6 +98,7 @@ def lib():
         L.tpt_fill_uniform.argtypes = [vp, C.c_size_t, C.c_ulonglong, C.c_ulonglong, vp]
         L.tpt_shard_layout.argtypes = [i, i, i, i, i, C.POINTER(ShardLayout)]
         L.tpt_shard_create.argtypes = [C.POINTER(vp), i, i, i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i]
+        L.tpt_shard_create_ex.argtypes = [C.POINTER(vp), i, i, i, i, i, _dp, _dp, _dp, C.POINTER(i), d, C.POINTER(i)]
         L.tpt_shard_get_layout.argtypes = [vp, C.POINTER(ShardLayout)]
         L.tpt_shard_sym.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_size_t)]
         L.tpt_shard_set_peers.argtypes = [vp, C.POINTER(vp)]
@@ -439,7 +440,7 @@ class Shard:
 
 
 def shard_create(rank: int, nranks: int, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha: float = 0.0,
-                 transform_x: int = TRANSFORM_GEMM) -> Shard:
+                 transform_x: int = TRANSFORM_GEMM, transform_y: int = TRANSFORM_GEMM) -> Shard:
     xa, xp = _faces(xf)
     ya, yp = _faces(yf)
     za, zp = _faces(zf)
@@ -447,8 +448,9 @@ def shard_create(rank: int, nranks: int, nx, ny, nz, xf, yf, zf, bc, helmholtz_a
         raise ValueError("face arrays must have n+1 entries per direction")
     bca = (C.c_int * 3)(*[int(b) for b in bc])
     h = C.c_void_p()
-    _check(lib().tpt_shard_create(C.byref(h), int(rank), int(nranks), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha),
-                                  int(transform_x)), "tpt_shard_create")
+    tra = (C.c_int * 2)(int(transform_x), int(transform_y))
+    _check(lib().tpt_shard_create_ex(C.byref(h), int(rank), int(nranks), nx, ny, nz, xp, yp, zp, bca, float(helmholtz_alpha),
+                                     tra), "tpt_shard_create_ex")
     return Shard(h, nx, ny, nz)
 
 

@@ -82,6 +82,8 @@ struct FftParams {
     int bgroups;          // y only: 16-column groups per mode row of the blocked side (nx/16, or the slab width / 16)
     int radix[4];         // pass radices (0-terminated)
     double s0, s1;        // forward: output scale of the two special slots / of the others; inverse: input scales
+    int npeers, units;    // sharded forward y: owner of mode row m = ((m >> 4) + 1) npeers - 1) / units, stored through peer_out
+    double *peer_out[MAX_PEERS];
 };
 
 // Everything that depends only on the transform length is a compile-time constant of the kernel (template LOGN): the
@@ -435,7 +437,9 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     auto store = [&](int slot, double o1, double o2) {
         const double sc = special_slot<BC, N>(slot) ? p.s0 : p.s1;
         if (YP) {
-            if (A.ok0) *reinterpret_cast<double2 *>(p.out + A.out_base + (size_t)slot * A.out_stride) = make_double2(sc * o1, sc * o2);
+            // sharded solve: the owner of mode row `slot` receives it straight from this store (exchange 1 of sharded.cu)
+            double *dst = p.npeers ? p.peer_out[(((slot >> 4) + 1) * p.npeers - 1) / p.units] : p.out;
+            if (A.ok0) *reinterpret_cast<double2 *>(dst + A.out_base + (size_t)slot * A.out_stride) = make_double2(sc * o1, sc * o2);
         } else {
             if (A.ok0) p.out[A.out_base + slot] = sc * o1;
             if (A.ok1) p.out[A.out_base + N + slot] = sc * o2;
@@ -753,6 +757,15 @@ cudaError_t launch_fft(const FftArgs &a, cudaStream_t stream) {
     p.N = N; p.bc = a.bc; p.nx = a.nx; p.ny = a.ny;
     p.s0 = a.s0; p.s1 = a.s1;
     p.blk_in = a.dir == 1 && a.inverse && a.blocked; p.blk_out = a.dir == 1 && !a.inverse && a.blocked;
+    if (a.npeers) {
+        if (a.npeers < 0 || a.npeers > MAX_PEERS || !p.blk_out || a.ny % 16) return cudaErrorInvalidValue;
+        p.npeers = a.npeers;
+        p.units = a.ny / 16;
+        for (int q = 0; q < a.npeers; ++q) {
+            if (!a.peer_out[q]) return cudaErrorInvalidValue;
+            p.peer_out[q] = a.peer_out[q];
+        }
+    }
     p.nz = a.nz; p.k0 = a.k0;
     {
         const double2 *w = p.T4 + N;

@@ -144,6 +144,11 @@ struct FftArgs {
     // the full field addressing (row length nx); a blocked side is then a SLAB buffer of its own, ncols columns wide
     // (element (i, m, k) at ((m (ncols/16) + (i - x0)/16) nz + k) 16 + i mod 16) — the L2-resident slab pipeline of api.cu.
     int x0 = 0, ncols = 0;
+    // Sharded solve (sharded.cu), forward y with a blocked output only: mode row m belongs to rank ((m/16 + 1) npeers - 1) / units
+    // (units = ny / 16) and is stored through peer_out[q] instead of `out` — a pointer into rank q's mode buffer with the
+    // owner's row offset folded in; nz / k0 then describe that buffer (full depth, this rank's first plane).
+    int npeers = 0;
+    double *peer_out[MAX_PEERS] = {};
 };
 bool fft_supported(int n);                                   // 2^m, 16 <= n <= 2048
 void fft_tables(int n, std::vector<double> &out);            // e^{-i pi k/2n} (n entries) | per-pass twiddle tables

@@ -56,8 +56,10 @@ int plane_start(int nz, int r, int P) {
 }
 int row_start(int ny, int q, int P) { return 16 * (int)((long long)(ny / 16) * q / P); }
 
+// the GEMM shapes (nx, ny multiples of 128) cover every transform choice; tpt_shard_create_ex accepts a fast y transform
+// on any supported power of two (ny / 16 >= P)
 bool layout_ok(int P, int nx, int ny, int nz) {
-    return P >= 1 && P <= tpt::MAX_PEERS && nx >= 128 && nx % 128 == 0 && ny >= 128 && ny % 128 == 0 && nz >= 2 * P &&
+    return P >= 1 && P <= tpt::MAX_PEERS && nx >= 128 && nx % 128 == 0 && ny >= 16 && ny % 16 == 0 && nz >= 2 * P &&
            ny / 16 >= P && nz <= 1056;
 }
 
@@ -122,6 +124,23 @@ int phase_forward(tpt_shard *s, const double *rhs, cudaStream_t st, int *launche
         if (rc != TPT_OK) return rc;
         cur = W;
     }
+    if (p->transform[1] == TPT_TRANSFORM_FFT) {
+        // fast y transform: the same scatter from the kernel's own stores (row `slot` of the blocked mode buffer of its owner)
+        tpt::FftArgs a{};
+        a.in = cur; a.out = nullptr;
+        a.tables = p->d_fft[1];
+        a.dir = 1; a.inverse = 0; a.bc = p->bc[1];
+        a.nx = p->nx; a.ny = p->ny; a.planes = nzl;
+        a.s0 = p->fft_s[1][0]; a.s1 = p->fft_s[1][1];
+        a.blocked = 1; a.nz = p->nz; a.k0 = s->k0[r];
+        a.npeers = P;
+        const int64_t row_stride = (int64_t)p->nx * p->nz;          // elements between mode rows of a blocked buffer
+        for (int q = 0; q < P; ++q)
+            a.peer_out[q] = reinterpret_cast<double *>(reinterpret_cast<intptr_t>(mode_of(s, q)) -
+                                                       (intptr_t)s->m0[q] * row_stride * (intptr_t)sizeof(double));
+        ++*launches;
+        return tpt::launch_fft(a, st) == cudaSuccess ? TPT_OK : TPT_ECUDA;
+    }
     tpt::GemmArgs g{};
     g.A = p->d_yfwd; g.lda = p->ny; g.strideA = 0;
     g.M = p->ny; g.N = p->nx; g.K = p->ny;
@@ -162,6 +181,19 @@ int phase_inverse(tpt_shard *s, double *out, cudaStream_t st, int *launches) {
     const int r = s->lay.rank, nzl = s->lay.k1 - s->lay.k0;
     double *W = p->d_work;
     double *dst = (p->dirs & 1) ? W : out;
+    if (p->transform[1] == TPT_TRANSFORM_FFT) {
+        tpt::FftArgs a{};
+        a.in = slab_of(s, r); a.out = dst;
+        a.tables = p->d_fft[1];
+        a.dir = 1; a.inverse = 1; a.bc = p->bc[1];
+        a.nx = p->nx; a.ny = p->ny; a.planes = nzl;
+        a.s0 = p->fft_s[1][2]; a.s1 = p->fft_s[1][3];
+        a.blocked = 1; a.nz = nzl; a.k0 = 0;                          // the slab buffer is blocked over the rank's own planes
+        ++*launches;
+        if (tpt::launch_fft(a, st) != cudaSuccess) return TPT_ECUDA;
+        if (p->dirs & 1) return tpt::detail::run_slot(p, TPT_K_INV_X, W, out, st, launches, 0, nzl);
+        return TPT_OK;
+    }
     tpt::GemmArgs g{};
     g.A = p->d_yinv; g.lda = p->ny; g.strideA = 0;
     g.M = p->ny; g.N = p->nx; g.K = p->ny;
@@ -205,7 +237,14 @@ int tpt_shard_layout(int nranks, int rank, int nx, int ny, int nz, tpt_shard_lay
 
 int tpt_shard_create(tpt_shard **shard_out, int rank, int nranks, int nx, int ny, int nz, const double *xf, const double *yf,
                      const double *zf, const int bc[3], double helmholtz_alpha, int transform_x) {
-    if (!shard_out || !bc || bc[2] == TPT_BC_PERIODIC) return TPT_EINVAL;   // (the cyclic correction is not sharded)
+    const int transform[2] = {transform_x, TPT_TRANSFORM_GEMM};
+    return tpt_shard_create_ex(shard_out, rank, nranks, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha, transform);
+}
+
+int tpt_shard_create_ex(tpt_shard **shard_out, int rank, int nranks, int nx, int ny, int nz, const double *xf, const double *yf,
+                        const double *zf, const int bc[3], double helmholtz_alpha, const int transform_xy[2]) {
+    if (!shard_out || !bc || !transform_xy || bc[2] == TPT_BC_PERIODIC) return TPT_EINVAL;   // (the cyclic correction is not sharded)
+    if (transform_xy[1] != TPT_TRANSFORM_FFT && ny % 128) return TPT_EINVAL;                 // the GEMM's exchange needs full 128-row tiles
     tpt_shard_layout_t lay;
     int rc = tpt_shard_layout(nranks, rank, nx, ny, nz, &lay);
     if (rc != TPT_OK) return rc;
@@ -216,7 +255,7 @@ int tpt_shard_create(tpt_shard **shard_out, int rank, int nranks, int nx, int ny
     s->mode_off = 0;
     s->slab_off = align_up(lay.mode_bytes, 256);
     s->pad_off = s->slab_off + align_up(lay.slab_bytes, 256);
-    const int transform[2] = {transform_x, TPT_TRANSFORM_GEMM};   // the y transform carries exchange 1: the TMA GEMM
+    const int transform[2] = {transform_xy[0], transform_xy[1]};  // the y transform (TMA GEMM or fast transform) carries exchange 1
     rc = tpt::detail::plan_create_sized(&s->plan, nx, ny, nz, xf, yf, zf, bc, helmholtz_alpha, TPT_DIRS_XYZ, transform,
                                         lay.slab_bytes / sizeof(double));
     if (rc != TPT_OK) { free_shard(s); return rc; }

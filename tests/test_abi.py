@@ -111,7 +111,7 @@ def test_shard_layout_partitions_planes_and_mode_rows():
     from paper_2603_09528_b200 import api
 
     for (nx, ny, nz, P) in [(512, 512, 512, 8), (1024, 256, 512, 8), (128, 128, 21, 5), (256, 128, 35, 3), (128, 256, 300, 8),
-                            (128, 128, 16, 1), (768, 768, 768, 7), (1024, 1024, 1024, 8)]:
+                            (128, 128, 16, 1), (768, 768, 768, 7), (1024, 1024, 1024, 8), (128, 64, 30, 3), (256, 32, 16, 2)]:
         lays = [api.shard_layout(P, r, nx, ny, nz) for r in range(P)]
         assert lays[0].k0 == 0 and lays[-1].k1 == nz and lays[0].m0 == 0 and lays[-1].m1 == ny
         sent = 0
@@ -131,7 +131,7 @@ def test_shard_layout_partitions_planes_and_mode_rows():
         assert max(q.m1 - q.m0 for q in lays) - min(q.m1 - q.m0 for q in lays) <= 16
         if P > 1 and nz % (2 * P) == 0 and ny % (16 * P) == 0:
             assert sent == 2 * 8 * nx * ny * nz * (P - 1) // P
-    for bad in [(9, 0, 128, 128, 64), (2, 2, 128, 128, 64), (2, 0, 96, 128, 64), (2, 0, 128, 192, 64), (8, 0, 128, 128, 12),
+    for bad in [(9, 0, 128, 128, 64), (2, 2, 128, 128, 64), (2, 0, 96, 128, 64), (2, 0, 128, 200, 64), (4, 0, 128, 32, 64), (8, 0, 128, 128, 12),
                 (2, 0, 128, 128, 2000)]:
         with pytest.raises(api.TptError):
             api.shard_layout(*bad)

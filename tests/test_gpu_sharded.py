@@ -33,9 +33,9 @@ def tpt(torch):
     return api
 
 
-def _make_shards(tpt, P, nranks, transform_x=0):
+def _make_shards(tpt, P, nranks, transform_x=0, transform_y=0):
     xf, yf, zf = P.faces()
-    shards = [tpt.shard_create(r, nranks, *P.n, xf, yf, zf, P.bc, P.alpha, transform_x) for r in range(nranks)]
+    shards = [tpt.shard_create(r, nranks, *P.n, xf, yf, zf, P.bc, P.alpha, transform_x, transform_y) for r in range(nranks)]
     syms = [s.sym()[0] for s in shards]
     for s in shards:
         s.set_peers(syms)
@@ -161,6 +161,42 @@ def test_solve_sharded_with_device_barriers(tpt, torch, orc):
             s.destroy()
 
 
+# The fast y transform carries exchange 1 from its own stores (every mode row written straight into its owner's buffer),
+# the inverse reads the slab buffer: the GF and FF variants of PAPER.md:294 sharded — against the oracle, and bit-for-bit
+# against the single-plan solve with the same transforms.
+@pytest.mark.parametrize("case", [
+    ("gf-p3", (128, 64, 30), (1.0, 2.0, 1.0), (2.0, 0.0, 2.5), (N_, D_, D_), 0.0, 3, (0, 1)),
+    ("ff-p4-singular", (256, 128, 44), (4.0, 1.0, 1.0), (0.0, 0.0, 2.0), (PER_, N_, N_), 0.0, 4, (1, 1)),
+    ("ff-p8-long-y", (128, 1024, 18), (1.0, 3.0, 1.0), (0.0, 0.0, 2.0), (N_, N_, D_), 2e-3, 8, (1, 1)),
+    ("gf-p2-small-y", (128, 32, 16), (1.0, 1.0, 1.0), (2.0, 0.0, 1.5), (D_, N_, N_), 0.0, 2, (0, 1)),
+], ids=lambda c: c[0])
+def test_fast_y_transform_in_sharded_solve(tpt, torch, orc, case):
+    name, n, L, beta, bc, alpha, nranks, tr = case
+    P = I.Problem(name, n, L, beta, bc, alpha, seed=40 + nranks)
+    xf, yf, zf = P.faces()
+    f = P.rhs()
+    shards = _make_shards(tpt, P, nranks, transform_x=tr[0], transform_y=tr[1])
+    rhs, out = _split(torch, shards, f)
+    tpt.virtual_ranks_solve(shards, rhs, out)
+    torch.cuda.synchronize()
+    phi = _gather(shards, out)
+    ref = orc.OraclePlan(xf, yf, zf, bc, alpha).solve(f)
+    assert float(np.abs(phi - ref).max() / np.abs(ref).max()) <= PARITY_TOL
+    plan = tpt.plan_create(*n, xf, yf, zf, bc, alpha, transform=tr)
+    d_f = torch.from_numpy(f).cuda()
+    d_o = torch.empty_like(d_f)
+    plan.solve(d_f, d_o)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_o.cpu().numpy(), phi)
+    plan.destroy()
+    # with the device-side flag barriers as well
+    tpt.virtual_ranks_solve(shards, rhs, out, barriers=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(_gather(shards, out), phi)
+    for s in shards:
+        s.destroy()
+
+
 def test_shard_argument_errors(tpt, torch):
     P = I.Problem("err", (128, 128, 16), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, D_), 0.0, seed=1)
     xf, yf, zf = P.faces()
@@ -170,6 +206,8 @@ def test_shard_argument_errors(tpt, torch):
         tpt.shard_create(0, 8, 128, 128, 12, xf, yf, zf[:13], P.bc)
     with pytest.raises(tpt.TptError):          # periodic z
         tpt.shard_create(0, 2, 128, 128, 16, xf, yf, zf, (N_, N_, PER_))
+    with pytest.raises(tpt.TptError):          # a GEMM y transform needs ny % 128 == 0 (a fast one any power of two >= 16)
+        tpt.shard_create(0, 2, 128, 64, 16, xf, I.tanh_faces(64, 1.0, 2.0), zf, P.bc)
     s = tpt.shard_create(0, 2, *P.n, xf, yf, zf, P.bc)
     d = torch.zeros(s.slab_points, dtype=torch.float64, device="cuda")
     with pytest.raises(tpt.TptError):          # peers not set yet
