@@ -368,7 +368,7 @@ def measure_sharded(api, torch, dist, args, probs, rank, world, stream, barrier)
     # parity of the sharded result with the single-GPU solve of the same right-hand side (first problem), slab by slab
     P = probs[0]
     xf, yf, zf = P.faces()
-    plan = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=(TRANSFORMS[args.transform][0], 0))
+    plan = api.plan_create(*P.n, xf, yf, zf, P.bc, P.alpha, transform=TRANSFORMS[args.transform])
     full = torch.from_numpy(P.rhs()).cuda()
     api.solve(plan, full, full, stream)
     torch.cuda.synchronize()
