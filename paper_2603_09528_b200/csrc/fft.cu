@@ -317,7 +317,8 @@ struct Addr {
 //   y: the first pass reads its 16 rows straight from global memory (whole 128-byte rows per quarter-warp);
 //   x: the rows are staged once through shared memory (coalesced 16-byte loads, Makhoul scatter);
 //   last pass: paired items, the two lines untangled in registers, every result stored straight to global memory.
-template <bool YP, int LOGN, int BC>
+// PEERS (y only): the sharded solve's exchange 1 — every mode row is stored through the base pointer of its owner.
+template <bool YP, int LOGN, int BC, bool PEERS = false>
 __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) fft_forward_kernel(const FftParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using G = Geo<YP, LOGN>;
@@ -362,46 +363,40 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
                 }
         }
     } else {
-        // CTA-wide coalesced load: step e -> samples i, i+1 of the lines l, l+1 of a pair -> two complex elements.
-        // All of a thread's loads are issued before the first shared-memory store (v[] serves as the landing registers);
-        // lines past the end of the field (last CTA only) are read from the last existing line and zeroed.
-        constexpr int STEPS = G::PAIRS * (N / 2), IT = STEPS / G::THREADS;
-        static_assert(IT == 8 && STEPS % G::THREADS == 0, "16 landing registers per thread");
-        const int lmax = p.lines - 1;
+        // x: sample i(n) of both lines straight into registers.  Makhoul's order makes these 8-byte loads stride-2 across the
+        // lanes (even samples ascending for the first half of the sequence, odd samples descending for the second); the
+        // other half of every 32-byte sector is asked for by the mirrored lane of the same warp a few instructions later
+        // (an L1 hit), which costs less L1 bandwidth than staging the rows through shared memory (one store + one load
+        // per element and two barriers more).
+        if (A.ok0) {
+            const double *src0 = p.in + A.in_base;
+            const double *src1 = A.ok1 ? src0 + N : src0;
 #pragma unroll
-        for (int s = 0; s < IT; ++s) {
-            const int e = t + s * G::THREADS;
-            const int q = e >> (LOGN - 1), i = (e & (N / 2 - 1)) << 1;
-            const int l = blockIdx.x * G::LINES + 2 * q;
-            const double2 va = *reinterpret_cast<const double2 *>(p.in + ((size_t)min(l, lmax) << LOGN) + i);
-            const double2 vb = *reinterpret_cast<const double2 *>(p.in + ((size_t)min(l + 1, lmax) << LOGN) + i);
-            v[2 * s] = cplx{va.x, va.y};
-            v[2 * s + 1] = cplx{vb.x, vb.y};
-        }
+            for (int it = 0; it < IT0; ++it)
 #pragma unroll
-        for (int s = 0; s < IT; ++s) {
-            const int e = t + s * G::THREADS;
-            const int q = e >> (LOGN - 1), i = (e & (N / 2 - 1)) << 1;
-            const int l = blockIdx.x * G::LINES + 2 * q;
-            cplx va = v[2 * s], vb = v[2 * s + 1];
-            if (l > lmax) va = cplx{0.0, 0.0};
-            if (l + 1 > lmax) vb = cplx{0.0, 0.0};
-            cplx *z = buf + q * NPAD;
-            if (BC == 2) {
-                z[pad(i)] = cplx{va.x, vb.x};
-                z[pad(i + 1)] = cplx{va.y, vb.y};
-            } else {       // i even -> n = i/2; i + 1 odd -> n = N - 1 - i/2 (sign flips for the sine transform)
-                const double s1 = BC == 1 ? -1.0 : 1.0;
-                z[pad(i >> 1)] = cplx{va.x, vb.x};
-                z[pad(N - 1 - (i >> 1))] = cplx{s1 * va.y, s1 * vb.y};
+                for (int r = 0; r < R0; ++r) {
+                    double sg;
+                    const int i = sample_of<BC, N>(u + it * UPP + r * PER0, sg);
+                    v[it * R0 + r] = cplx{src0[i], src1[i]};
+                }
+            if (!A.ok1) {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) v[q].y = 0.0;
             }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) v[q] = cplx{0.0, 0.0};
         }
-        __syncthreads();
+        if (BC == 1) {
 #pragma unroll
-        for (int it = 0; it < IT0; ++it)
+            for (int it = 0; it < IT0; ++it)
 #pragma unroll
-            for (int r = 0; r < R0; ++r) v[it * R0 + r] = seq[pad(u + it * UPP + r * PER0)];
-        __syncthreads();
+                for (int r = 0; r < R0; ++r) {
+                    double sg;
+                    sample_of<BC, N>(u + it * UPP + r * PER0, sg);
+                    v[it * R0 + r] = cplx{sg * v[it * R0 + r].x, sg * v[it * R0 + r].y};
+                }
+        }
     }
 #pragma unroll
     for (int it = 0; it < IT0; ++it) {
@@ -438,7 +433,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
         const double sc = special_slot<BC, N>(slot) ? p.s0 : p.s1;
         if (YP) {
             // sharded solve: the owner of mode row `slot` receives it straight from this store (exchange 1 of sharded.cu)
-            double *dst = p.npeers ? p.peer_out[(((slot >> 4) + 1) * p.npeers - 1) / p.units] : p.out;
+            double *dst = PEERS ? p.peer_out[(((slot >> 4) + 1) * p.npeers - 1) / p.units] : p.out;
             if (A.ok0) *reinterpret_cast<double2 *>(dst + A.out_base + (size_t)slot * A.out_stride) = make_double2(sc * o1, sc * o2);
         } else {
             if (A.ok0) p.out[A.out_base + slot] = sc * o1;
@@ -721,6 +716,16 @@ cudaError_t launch_bc(const FftParams &p, int inverse, cudaStream_t stream) {
     }
     const dim3 grid(grid_x, grid_y);
     if (inverse) return launch_pdl(fft_inverse_kernel<YP, LOGN, BC>, grid, dim3(threads), smem, stream, p);
+    if (YP && p.npeers) {
+        if (smem > 48 * 1024) {
+            static DeviceOnce configured_peers;
+            cudaError_t e = configured_peers.run([&] {
+                return cudaFuncSetAttribute(fft_forward_kernel<YP, LOGN, BC, YP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            });
+            if (e != cudaSuccess) return e;
+        }
+        return launch_pdl(fft_forward_kernel<YP, LOGN, BC, YP>, grid, dim3(threads), smem, stream, p);
+    }
     return launch_pdl(fft_forward_kernel<YP, LOGN, BC>, grid, dim3(threads), smem, stream, p);
 }
 
