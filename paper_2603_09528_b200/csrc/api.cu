@@ -620,7 +620,7 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
             cudaError_t e = cudaMalloc(&p->d_cyc_q, p->points() * sizeof(double));
             if (e == cudaSuccess) e = cudaMalloc(&p->d_cyc_rden, (size_t)nx * ny * sizeof(double));
             if (e != cudaSuccess) { cudaGetLastError(); rc = e == cudaErrorMemoryAllocation ? TPT_ENOMEM : TPT_ECUDA; }
-            p->cyc_g_tmp[0] = cyc_g; p->cyc_g_tmp[1] = cyc_cn;
+            p->cyc_u[0] = cyc_g; p->cyc_u[1] = cyc_cn;
         }
     } catch (const std::bad_alloc &) {
         rc = TPT_ENOMEM;
@@ -640,7 +640,7 @@ int tpt::detail::plan_create_sized(tpt_plan **plan_out, int nx, int ny, int nz, 
         // q = A'^-1 u for every column (its spectral shift is all that distinguishes the columns): one sweep at plan time
         int launches = 0;
         const size_t cols = (size_t)nx * ny;
-        cudaError_t e = tpt::launch_cyclic_rhs(p->d_cyc_q, cols, nz, p->cyc_g_tmp[0], p->cyc_g_tmp[1], nullptr);
+        cudaError_t e = tpt::launch_cyclic_rhs(p->d_cyc_q, cols, nz, p->cyc_u[0], p->cyc_u[1], nullptr);
         if (e == cudaSuccess) rc = run_sweep(p, p->d_cyc_q, p->d_cyc_q, p->d_work, nullptr, &launches, false, false, 0);
         if (e == cudaSuccess && rc == TPT_OK) e = tpt::launch_cyclic_rden(p->d_cyc_q, p->d_cyc_rden, cols, nz, p->cyc_r, p->singular, nullptr);
         if (e == cudaSuccess && rc == TPT_OK) e = cudaDeviceSynchronize();

@@ -32,7 +32,7 @@ struct tpt_plan {
     int cyclic = 0;
     double cyc_r = 0.0;           // a_0 / g
     double b0_null = 0.0;         // unmodified b_0 (row 0 of the null column)
-    double cyc_g_tmp[2] = {0.0, 0.0};   // g and c_{n-1}: the right-hand side u of the plan-time sweep
+    double cyc_u[2] = {0.0, 0.0};   // g and c_{n-1}: the right-hand side u of the plan-time sweep
     double *d_cyc_q = nullptr;    // q = A'^-1 u, one field, natural layout (swept at plan time)
     double *d_cyc_rden = nullptr; // 1 / (1 + q_0 + r q_{n-1}) per column
     int fused_small = 1;          // grids that fit on chip: the whole solve in one cluster launch (fused_small.cu)
