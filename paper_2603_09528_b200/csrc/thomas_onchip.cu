@@ -387,6 +387,10 @@ cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, cons
     if (nz <= 768) return TPT_GO(32, 16, 384, 1);
     // up to 1056 rows: 8-column tiles of 17-row segments, 512 threads (16 warps), two 68 KB buffers, one CTA per SM
     // (33-row segments with 256 threads and 242 registers: 4.25 instead of 3.69 ms at 1024^3)
+    // 801 .. 1008 rows: 21-row segments (at most 48 per column, 384 threads) — measured 0.84 / 0.86 / 1.05 / 1.05 ms at
+    // 840 / 900 / 960 / 992 rows against 0.94 / 1.07 / 1.10 / 1.11 ms with 17-row segments (512 x 512 columns); from 1009
+    // rows on the 17-row, 64-segment shape wins (1024 rows: 0.97 vs 1.18 ms)
+    if (nz <= 1008) return TPT_GO(21, 8, 416, 1);
     return TPT_GO(17, 8, 512, 1);
 #undef TPT_GO
 }

@@ -42,8 +42,8 @@ def _solve(torch, plan, f):
 
 
 # nz picks the sweep's launch shape: <=128: 8-row segments; <=256: 16 rows, two CTAs per SM; 257..544 (blocked):
-# 8-column tiles with 17-row segments; 545..800 (blocked): the same shape with 19 / 21 / 23 / 25-row segments; 801..1056: 8-column
-# tiles with 17-row segments and 512 threads.  Ragged nz exercises the zero-filled tail rows.
+# 8-column tiles with 17-row segments; 545..800 (blocked): the same shape with 19 / 21 / 23 / 25-row segments; 801..1008: 21-row
+# segments, one CTA per SM; 1009..1056: 17-row segments and 512 threads.  Ragged nz exercises the zero-filled tail rows.
 SHAPES = [
     ("nz24", (128, 128, 24), (N_, N_, D_), 0.0),
     ("nz130", (128, 256, 130), (N_, N_, D_), 0.0),
@@ -59,6 +59,8 @@ SHAPES = [
     ("nz800", (128, 128, 800), (D_, D_, N_), 0.0),
     ("nz801", (128, 128, 801), (N_, N_, D_), 0.0),
     ("nz1000", (128, 128, 1000), (N_, N_, D_), 0.0),
+    ("nz1008-singular", (128, 128, 1008), (N_, N_, N_), 0.0),
+    ("nz1009", (128, 128, 1009), (N_, D_, D_), 0.0),
     ("nz1056", (128, 128, 1056), (N_, D_, N_), 0.0),
 ]
 
