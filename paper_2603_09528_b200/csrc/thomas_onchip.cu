@@ -369,6 +369,13 @@ cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, cons
     launch_m<M, TC, MAXT, CTAS, SH>(in, x, peers, tab, lamx, lamy, wz, nx, cols, nz, shift0, singular, blocked, sms, stream)
     // Measured on the box (profiles/r1c_*.md): the sweep is bound by the FP64 + shared-memory pipes of the 16 warps the
     // register file admits per SM, so the shapes differ only in how well the phases of co-resident CTAs interleave.
+    // Short columns on the blocked layout: the 17-row / 8-column shape also wins below 257 rows wherever its segments fill
+    // the column (at most 10 % padding rows: 64, 128, 192 rows — 512 x 512 columns x 128 rows: 0.139 -> 0.107 ms);
+    // otherwise the 8- / 16-row shapes below (160, 224, 256 rows: measured equal or better)
+    if ((blocked || blocked_shape) && nz <= 204) {
+        const int S = ((nz + 16) / 17 + 3) / 4 * 4;
+        if (S * 17 * 10 <= 11 * nz) return TPT_GO(17, 8, 256, 2);
+    }
     if (nz <= 128) return TPT_GO(8, 16, 256, 2);
     if (nz <= 256) return TPT_GO(16, 16, 256, 2);
     // 8-column tiles, odd segment length (rows of the two segments of a half-warp then fall into opposite 64-byte
