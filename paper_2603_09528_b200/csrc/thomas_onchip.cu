@@ -378,19 +378,29 @@ cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, cons
     }
     if (nz <= 128) return TPT_GO(8, 16, 256, 2);
     if (nz <= 256) return TPT_GO(16, 16, 256, 2);
-    // 8-column tiles, odd segment length (rows of the two segments of a half-warp then fall into opposite 64-byte
-    // halves of the banks: conflict-free), two CTAs per SM.  Meant for the blocked layout (in the natural one an
-    // 8-column row is a 64-byte piece of a DRAM page); `blocked_shape` asks for the same partition — hence the same
-    // rounding — on a natural-layout field (tpt_solve_host, whose results equal tpt_solve's bit for bit).
-    if ((blocked || blocked_shape) && nz <= 544) return TPT_GO(17, 8, 256, 2);
+    // 257 .. 800 rows on the blocked layout: 8-column tiles, odd segment length (rows of the two segments of a half-warp
+    // then fall into opposite 64-byte halves of the banks: conflict-free), two CTAs per SM, at most 32 segments (a multiple
+    // of 4: whole warps).  `blocked_shape` asks for the same partition — hence the same rounding — on a natural-layout field
+    // (tpt_solve_host, whose results equal tpt_solve's bit for bit).  Segment length: the shortest of 17 / 19 / 21 / 23 / 25
+    // rows that covers the column (768^3: 0.709 -> 0.667 ms against one 384-thread CTA of 32-row segments), unless another
+    // one leaves at least 3 % fewer padded rows — the padding is pure waste (416 rows: 0.400 -> 0.362 ms with 21-row
+    // segments, 288 rows: 0.262 -> 0.240 ms with 25).
+    if ((blocked || blocked_shape) && nz <= 800) {
+        int defM = 17;
+        while (defM * 32 < nz) defM += 2;
+        auto rows_of = [&](int M) { return ((nz + M - 1) / M + 3) / 4 * 4 * M; };
+        int bestM = defM, bestRows = rows_of(defM);
+        for (int M = defM + 2; M <= 25; M += 2)
+            if (rows_of(M) * 100 < bestRows * 97 || (bestM != defM && rows_of(M) <= bestRows)) { bestRows = rows_of(M); bestM = M; }
+        switch (bestM) {
+            case 17: return TPT_GO(17, 8, 256, 2);
+            case 19: return TPT_GO(19, 8, 256, 2);
+            case 21: return TPT_GO(21, 8, 256, 2);
+            case 23: return TPT_GO(23, 8, 256, 2);
+            default: return TPT_GO(25, 8, 256, 2);
+        }
+    }
     if (nz <= 512) return TPT_GO(16, 16, 512, 1);
-    // 545 .. 800 rows on the blocked layout: the same 32-segment, two-CTA shape with the shortest odd segment that covers
-    // the column (768^3: 0.709 -> 0.668 ms against one 384-thread CTA of 32-row segments; 25 rows x 2 register arrays
-    // still fit 128 registers with 16 bytes of spill)
-    if ((blocked || blocked_shape) && nz <= 608) return TPT_GO(19, 8, 256, 2);
-    if ((blocked || blocked_shape) && nz <= 672) return TPT_GO(21, 8, 256, 2);
-    if ((blocked || blocked_shape) && nz <= 736) return TPT_GO(23, 8, 256, 2);
-    if ((blocked || blocked_shape) && nz <= 800) return TPT_GO(25, 8, 256, 2);
     if (nz <= 768) return TPT_GO(32, 16, 384, 1);
     // up to 1056 rows: 8-column tiles of 17-row segments, 512 threads (16 warps), two 68 KB buffers, one CTA per SM
     // (33-row segments with 256 threads and 242 registers: 4.25 instead of 3.69 ms at 1024^3)
