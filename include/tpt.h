@@ -35,8 +35,7 @@ typedef struct tpt_plan tpt_plan; /* opaque */
  * directions, take it through their eigenbasis; a periodic z makes the sweep a cyclic tridiagonal solve — the
  * ordinary sweep on a corner-modified matrix followed by a Sherman-Morrison correction whose column vectors are swept
  * once at plan time (one extra field of device memory; natural layout; >= 3 cells).  Not available with periodic z:
- * the staggered-grid operators (tpt_divergence / tpt_gradient_correct / tpt_project), the sharded solve and the
- * one-launch small-grid path (TPT_EINVAL / the separate kernels). */
+ * the sharded solve (TPT_EINVAL) and the one-launch small-grid path (the separate kernels run instead). */
 enum { TPT_BC_NEUMANN = 0, TPT_BC_DIRICHLET = 1, TPT_BC_PERIODIC = 2 };
 
 /* Implicitly treated directions L_I of the Helmholtz problem, Eq. 2b: bit 0 = x, 1 = y, 2 = z. */

@@ -993,6 +993,8 @@ int orc_project(const orc_plan *poisson, const double *xf, const double *yf, con
         if (bc[1] == ORC_BC_PERIODIC)
             for (int k = 0; k < nz; ++k)
                 for (int i = 0; i < nx; ++i) v[i + (size_t)nx * (ny + (size_t)(ny + 1) * k)] = v[i + (size_t)nx * (0 + (size_t)(ny + 1) * k)];
+        if (bc[2] == ORC_BC_PERIODIC)
+            for (size_t c = 0; c < (size_t)nx * ny; ++c) w[c + (size_t)nx * ny * nz] = w[c];
     }
     if (rc == ORC_OK && p) {                                                                      /* 2e */
         if (alpha_p == 0.0) {

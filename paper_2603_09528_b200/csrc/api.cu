@@ -820,7 +820,6 @@ int tpt_solve_host_async(tpt_plan *p, const double *rhs_host, double *out_host, 
 int tpt_divergence(tpt_plan *p, const double *u_dev, const double *v_dev, const double *w_dev, double scale, double *out_dev,
                    void *cuda_stream) {
     if (!p || !u_dev || !v_dev || !w_dev || !out_dev || !std::isfinite(scale) || !on_plan_device(p)) return TPT_EINVAL;
-    if (p->cyclic) return TPT_EINVAL;   // the staggered operators close z with walls or ghost cells only
     if (!aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(out_dev)) return TPT_EINVAL;
     cudaError_t e = tpt::launch_divergence(u_dev, v_dev, w_dev, p->geo, scale, out_dev, static_cast<cudaStream_t>(cuda_stream));
     p->launches_last = 1;
@@ -831,7 +830,7 @@ static bool dirs_valid(int d) { return d == TPT_DIRS_XYZ || d == TPT_DIRS_YZ || 
 
 int tpt_gradient_correct(tpt_plan *p, const double *phi_dev, double c, double *u_dev, double *v_dev, double *w_dev, double *p_dev,
                          double alpha_p, int implicit_dirs, void *cuda_stream) {
-    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c) || !on_plan_device(p) || p->cyclic) return TPT_EINVAL;
+    if (!p || !phi_dev || !u_dev || !v_dev || !w_dev || !std::isfinite(c) || !on_plan_device(p)) return TPT_EINVAL;
     if (!aligned8(phi_dev) || !aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(p_dev)) return TPT_EINVAL;
     if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
     cudaError_t e = tpt::launch_correct(phi_dev, u_dev, v_dev, w_dev, p_dev, p->geo, c, alpha_p, implicit_dirs,
@@ -844,7 +843,7 @@ int tpt_project(tpt_plan *p, double *u_dev, double *v_dev, double *w_dev, double
                 double alpha_p, int implicit_dirs, void *cuda_stream) {
     if (!p || !u_dev || !v_dev || !w_dev || !phi_dev || !aligned16(phi_dev) || !on_plan_device(p)) return TPT_EINVAL;
     if (!aligned8(u_dev) || !aligned8(v_dev) || !aligned8(w_dev) || !aligned8(p_dev)) return TPT_EINVAL;
-    if (p->alpha != 0.0 || p->dirs != TPT_DIRS_XYZ || p->cyclic) return TPT_EINVAL;       // Eq. 2c carries the full Laplacian
+    if (p->alpha != 0.0 || p->dirs != TPT_DIRS_XYZ) return TPT_EINVAL;       // Eq. 2c carries the full Laplacian
     if (!(gamma_dt > 0.0) || !std::isfinite(gamma_dt)) return TPT_EINVAL;
     if (p_dev && (!(alpha_p >= 0.0) || !std::isfinite(alpha_p) || !dirs_valid(implicit_dirs))) return TPT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);

@@ -23,7 +23,7 @@ constexpr int KZD = 16;   // z-levels per thread (divergence)
 __global__ void __launch_bounds__(PX, 8)
 divergence_kernel(const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w,
                   const double *__restrict__ rwx, const double *__restrict__ rwy, const double *__restrict__ rwz,
-                  double *__restrict__ out, int nx, int ny, int nz, int px, int py, double scale) {
+                  double *__restrict__ out, int nx, int ny, int nz, int px, int py, int pz, double scale) {
     const int i = blockIdx.x * PX + threadIdx.x;
     const int j = blockIdx.y;
     const int k0 = blockIdx.z * KZD;
@@ -38,7 +38,7 @@ divergence_kernel(const double *__restrict__ u, const double *__restrict__ v, co
     for (int k = k0; k < k1; ++k) {
         const size_t urow = (size_t)(nx + 1) * (j + (size_t)ny * k);
         const size_t vpl = (size_t)nx * (ny + 1) * k;
-        const double whi = w[i + (size_t)nx * j + plane * (k + 1)];
+        const double whi = w[i + (size_t)nx * j + plane * ((pz && k == nz - 1) ? 0 : k + 1)];   // periodic: face nz is face 0
         const double du = (u[urow + ih] - u[urow + i]) * rx;
         const double dv = (v[vpl + (size_t)nx * jh + i] - v[vpl + (size_t)nx * j + i]) * ry;
         const double dw = (whi - wlo) * rwz[k];
@@ -51,7 +51,7 @@ divergence_kernel(const double *__restrict__ u, const double *__restrict__ v, co
 __global__ void __launch_bounds__(PX)
 divergence2_kernel(const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w,
                    const double *__restrict__ rwx, const double *__restrict__ rwy, const double *__restrict__ rwz,
-                   double *__restrict__ out, int nx, int ny, int nz, int px, int py, double scale) {
+                   double *__restrict__ out, int nx, int ny, int nz, int px, int py, int pz, double scale) {
     const int i = 2 * (blockIdx.x * PX + threadIdx.x);
     const int j = blockIdx.y, k = blockIdx.z;
     if (i >= nx) return;
@@ -65,7 +65,7 @@ divergence2_kernel(const double *__restrict__ u, const double *__restrict__ v, c
     const double2 vl = *reinterpret_cast<const double2 *>(v + vo);
     const double2 vh = *reinterpret_cast<const double2 *>(v + vo + (ptrdiff_t)nx * jh);
     const double2 wl = *reinterpret_cast<const double2 *>(w + wo);
-    const double2 wh = *reinterpret_cast<const double2 *>(w + wo + plane);
+    const double2 wh = *reinterpret_cast<const double2 *>((pz && k == nz - 1) ? w + wo - plane * k : w + wo + plane);
     const double ry = rwy[j], rz = rwz[k];
     double2 o;
     o.x = scale * ((u1 - u0) * rwx[i] + (vh.x - vl.x) * ry + (wh.x - wl.x) * rz);
@@ -90,17 +90,17 @@ correct_kernel(const double *__restrict__ phi, double *__restrict__ u, double *_
     if (i >= nx) return;
     const int k1 = min(k0 + KZ, nz);
     const size_t plane = (size_t)nx * ny;
-    const bool px = bcx == 2, py = bcy == 2;
+    const bool px = bcx == 2, py = bcy == 2, pz = bcz == 2;
     const double gxl = gfx[i], gxh = gfx[i + 1], gyl = gfy[j], gyh = gfy[j + 1];
     const size_t col = i + (size_t)nx * j;
     double cur = phi[col + plane * k0];
-    double below = k0 > 0 ? phi[col + plane * (k0 - 1)] : ghost(bcz, cur);
+    double below = k0 > 0 ? phi[col + plane * (k0 - 1)] : (pz ? phi[col + plane * (nz - 1)] : ghost(bcz, cur));
     for (int k = k0; k < k1; ++k) {
         const double *row = phi + (size_t)nx * j + plane * k;     // this x-line
         const double *pl = phi + plane * k + i;                   // this (i, :) line of the plane
         const double xm = i > 0 ? row[i - 1] : (px ? row[nx - 1] : ghost(bcx, cur));
         const double ym = j > 0 ? pl[(size_t)nx * (j - 1)] : (py ? pl[(size_t)nx * (ny - 1)] : ghost(bcy, cur));
-        const double above = k < nz - 1 ? phi[col + plane * (k + 1)] : ghost(bcz, cur);
+        const double above = k < nz - 1 ? phi[col + plane * (k + 1)] : (pz ? phi[col] : ghost(bcz, cur));
         const double Gxl = gxl * (cur - xm), Gyl = gyl * (cur - ym), Gzl = gfz[k] * (cur - below);
         // Eq. 2d on the low faces of this cell
         const size_t uo = (size_t)(nx + 1) * (j + (size_t)ny * k) + i;
@@ -110,7 +110,9 @@ correct_kernel(const double *__restrict__ phi, double *__restrict__ u, double *_
         u[uo] = un;
         const double vn = fma(-c, Gyl, v[vo]);
         v[vo] = vn;
-        w[wo] = fma(-c, Gzl, w[wo]);
+        const double wn = fma(-c, Gzl, w[wo]);
+        w[wo] = wn;
+        if (pz && k == 0) w[wo + plane * nz] = wn;
         if (px && i == 0) u[uo + nx] = un;                        // periodic: face n is a copy of face 0
         if (py && j == 0) v[vo + (size_t)nx * ny] = vn;
         const bool xe = i == nx - 1, ye = j == ny - 1, ze = k == nz - 1;
@@ -148,7 +150,7 @@ correct2_kernel(const double *__restrict__ phi, double *__restrict__ u, double *
     const int j = blockIdx.y, k = blockIdx.z;
     if (i >= nx) return;
     const size_t plane = (size_t)nx * ny;
-    const bool px = bcx == 2, py = bcy == 2;
+    const bool px = bcx == 2, py = bcy == 2, pz = bcz == 2;
     const size_t wo = i + (size_t)nx * j + plane * k;
     const double *row = phi + (size_t)nx * j + plane * k;
     const double2 cur = *reinterpret_cast<const double2 *>(phi + wo);
@@ -158,6 +160,7 @@ correct2_kernel(const double *__restrict__ phi, double *__restrict__ u, double *
     else if (py) ym = *reinterpret_cast<const double2 *>(phi + wo + (size_t)nx * (ny - 1));
     else ym = make_double2(ghost(bcy, cur.x), ghost(bcy, cur.y));
     if (k > 0) below = *reinterpret_cast<const double2 *>(phi + wo - plane);
+    else if (pz) below = *reinterpret_cast<const double2 *>(phi + wo + plane * (nz - 1));
     else below = make_double2(ghost(bcz, cur.x), ghost(bcz, cur.y));
     const double g0 = gfx[i], g1 = gfx[i + 1], gyl = gfy[j], gzl = gfz[k];
     const double Gx0 = g0 * (cur.x - xm), Gx1 = g1 * (cur.y - cur.x);
@@ -176,6 +179,7 @@ correct2_kernel(const double *__restrict__ phi, double *__restrict__ u, double *
     ww.x = fma(-c, Gz0, ww.x);
     ww.y = fma(-c, Gz1, ww.y);
     *reinterpret_cast<double2 *>(w + wo) = ww;
+    if (pz && k == 0) *reinterpret_cast<double2 *>(w + wo + plane * nz) = ww;
     if (px && i == 0) u[uo + nx] = un0;
     if (py && j == 0) *reinterpret_cast<double2 *>(v + vo + (size_t)nx * ny) = vv;
     const bool xe = i == nx - 2, ye = j == ny - 1, ze = k == nz - 1;
@@ -186,6 +190,7 @@ correct2_kernel(const double *__restrict__ phi, double *__restrict__ u, double *
         else if (py) yp = *reinterpret_cast<const double2 *>(phi + wo - (size_t)nx * (ny - 1));
         else yp = make_double2(ghost(bcy, cur.x), ghost(bcy, cur.y));
         if (!ze) above = *reinterpret_cast<const double2 *>(phi + wo + plane);
+        else if (pz) above = *reinterpret_cast<const double2 *>(phi + wo - plane * k);
         else above = make_double2(ghost(bcz, cur.x), ghost(bcz, cur.y));
         const double gyh = gfy[j + 1], gzh = gfz[k + 1];
         const double Gx2 = gfx[i + 2] * (xp - cur.y);
@@ -228,12 +233,12 @@ cudaError_t launch_divergence(const double *u, const double *v, const double *w,
     if (g.nx % 2 == 0 && aligned16(v) && aligned16(w) && aligned16(out)) {
         dim3 grid2((g.nx / 2 + PX - 1) / PX, g.ny, g.nz);
         divergence2_kernel<<<grid2, PX, 0, stream>>>(u, v, w, g.rwx, g.rwy, g.rwz, out, g.nx, g.ny, g.nz, g.bc[0] == 2,
-                                                     g.bc[1] == 2, scale);
+                                                     g.bc[1] == 2, g.bc[2] == 2, scale);
         return cudaGetLastError();
     }
     dim3 grid((g.nx + PX - 1) / PX, g.ny, (g.nz + KZD - 1) / KZD);
     divergence_kernel<<<grid, PX, 0, stream>>>(u, v, w, g.rwx, g.rwy, g.rwz, out, g.nx, g.ny, g.nz, g.bc[0] == 2,
-                                               g.bc[1] == 2, scale);
+                                               g.bc[1] == 2, g.bc[2] == 2, scale);
     return cudaGetLastError();
 }
 

@@ -56,6 +56,8 @@ CASES = [
     ("ragged-pdn", (33, 18, 35), (0.0, 2.0, 2.0), (P_, D_, N_)),
     ("ragged-dpd", (130, 9, 17), (1.5, 0.0, 1.0), (D_, P_, D_)),
     ("wide-nnn", (300, 12, 40), (2.0, 2.0, 2.0), (N_, N_, N_)),     # several x blocks and z chunks
+    ("ragged-ndp", (35, 14, 21), (2.0, 1.5, 2.0), (N_, D_, P_)),    # periodic z (one cell per thread)
+    ("even-ppp", (64, 16, 33), (0.0, 1.0, 1.5), (P_, P_, P_)),      # periodic z (two cells per thread)
 ]
 
 
@@ -88,6 +90,8 @@ def test_divergence_and_correction_match_the_oracle(tpt, torch, orc, case):
             eu[:, :, -1] = eu[:, :, 0]
         if bc[1] == P_:
             ev[:, -1, :] = ev[:, 0, :]
+        if bc[2] == P_:
+            ew[-1] = ew[0]
         scale = max(np.abs(c * gu).max(), np.abs(c * gv).max(), np.abs(c * gw).max())
         for got, exp in ((du, eu), (dv, ev), (dw, ew)):
             assert np.abs(got.cpu().numpy() - exp).max() <= STENCIL_TOL * scale
@@ -105,6 +109,8 @@ PROJECT_CASES = [
     ("ragged", (40, 36, 33), (2.0, 1.5, 2.5), (N_, N_, D_)),
     ("singular", (128, 128, 40), (2.0, 2.0, 2.0), (N_, N_, N_)),
     ("duct", (128, 128, 48), (0.0, 2.0, 2.5), (P_, N_, N_)),
+    ("periodic-z", (128, 64, 40), (2.0, 2.0, 1.5), (N_, N_, P_)),          # cyclic sweep inside the projection
+    ("periodic-z-odd", (33, 20, 17), (1.5, 2.0, 0.0), (D_, N_, P_)),
 ]
 
 
