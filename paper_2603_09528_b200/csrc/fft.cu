@@ -65,7 +65,14 @@ __device__ __forceinline__ void fft8(cplx *v) {
 }
 
 // shared-memory index with one padding element per 8 (keeps the stride-R stores of the first pass conflict-free)
-__device__ __forceinline__ int pad(int i) { return i + (i >> 3); }
+// Radix-16 passes (N >= 1024) store with stride 16 (forward, first pass) and in blocks of 4 every 64 (inverse, second pass):
+// the forward transform then pads one element per 16, the inverse adds half a bank round per 64 (profiles: 26-30 % of the
+// shared-memory wavefronts of the 1024-long transforms were conflict replays with the plain padding).
+template <int LOGN, int INV>
+__device__ __forceinline__ int padf(int i) {
+    if (LOGN < 10) return i + (i >> 3);
+    return INV ? i + (i >> 3) + 4 * (i >> 6) : i + (i >> 4);
+}
 
 struct FftParams {
     const double *in;
@@ -124,7 +131,7 @@ struct Geo {
     static constexpr int THREADS = PAIRS * UPP;                          // y: 256, x: 128
     static constexpr int MINB = 512 / THREADS;                           // CTAs per SM the 128-register budget admits
     static constexpr int BANKSTEP = !YP ? 1 : (COLS == 16 ? 1 : (COLS == 8 ? 2 : 4));
-    static constexpr int NPAD = ((N + (N >> 3) + 7) & ~7) + BANKSTEP;    // padded sequence length (complex elements)
+    static constexpr int NPAD = ((N + (N >> 3) + (N >= 1024 ? (N >> 4) : 0) + 7) & ~7) + BANKSTEP;   // padded sequence length (complex elements; covers padf)
     static constexpr size_t SMEM = (size_t)PAIRS * NPAD * 16;
 };
 
@@ -225,7 +232,7 @@ __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParam
         for (int it = 0; it < IT; ++it) {
             const int j = u + it * UPP, k = j & (NS - 1);
 #pragma unroll
-            for (int r = 0; r < R; ++r) v[it * R + r] = seq[pad(j + r * PER)];
+            for (int r = 0; r < R; ++r) v[it * R + r] = seq[padf<LOGN, INV>(j + r * PER)];
             twiddle<R, INV, (XDIR && NS >= 32)>(v + it * R, p.Wq[Q], NS, k);
             bfly<R, INV>(v + it * R);
         }
@@ -234,7 +241,7 @@ __device__ __forceinline__ void middle_passes(cplx *seq, cplx *v, const FftParam
         for (int it = 0; it < IT; ++it) {
             const int j = u + it * UPP, k = j & (NS - 1);
 #pragma unroll
-            for (int r = 0; r < R; ++r) seq[pad((j - k) * R + k + r * NS)] = v[it * R + r];
+            for (int r = 0; r < R; ++r) seq[padf<LOGN, INV>((j - k) * R + k + r * NS)] = v[it * R + r];
         }
         __syncthreads();
         middle_passes<LOGN, INV, Q + 1, NS * R, UPP, XDIR>(seq, v, p, u);
@@ -402,7 +409,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     for (int it = 0; it < IT0; ++it) {
         bfly<R0, 0>(v + it * R0);
 #pragma unroll
-        for (int r = 0; r < R0; ++r) seq[pad((u + it * UPP) * R0 + r)] = v[it * R0 + r];
+        for (int r = 0; r < R0; ++r) seq[padf<LOGN, 0>((u + it * UPP) * R0 + r)] = v[it * R0 + r];
     }
     __syncthreads();
     middle_passes<LOGN, 0, 1, R0, UPP, !YP>(seq, v, p, u);
@@ -423,7 +430,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
 #pragma unroll
     for (int it = 0; it < ITL; ++it) {
 #pragma unroll
-        for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[pad(jl[it] + r * NSL)];
+        for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[padf<LOGN, 0>(jl[it] + r * NSL)];
         twiddle<RL, 0, (!YP && NSL >= 32)>(v + it * RL, p.Wq[NP - 1], NSL, jl[it]);
         bfly<RL, 0>(v + it * RL);
     }
@@ -582,7 +589,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     for (int it = 0; it < IT0; ++it) {
         bfly<R0, 1>(v + it * R0);
 #pragma unroll
-        for (int r = 0; r < R0; ++r) seq[pad(j0[it] * R0 + r)] = v[it * R0 + r];
+        for (int r = 0; r < R0; ++r) seq[padf<LOGN, 1>(j0[it] * R0 + r)] = v[it * R0 + r];
     }
     __syncthreads();
     middle_passes<LOGN, 1, 1, R0, UPP, !YP>(seq, v, p, u);
@@ -593,7 +600,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
     for (int it = 0; it < ITL; ++it) {
         const int j = u + it * UPP;
 #pragma unroll
-        for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[pad(j + r * NSL)];
+        for (int r = 0; r < RL; ++r) v[it * RL + r] = seq[padf<LOGN, 1>(j + r * NSL)];
         twiddle<RL, 1, (!YP && NSL >= 32)>(v + it * RL, p.Wq[NP - 1], NSL, j);
         bfly<RL, 1>(v + it * RL);
     }
@@ -623,7 +630,7 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
 #pragma unroll
         for (int it = 0; it < ITL; ++it)
 #pragma unroll
-            for (int r = 0; r < RL; ++r) seq[pad(u + it * UPP + r * NSL)] = v[it * RL + r];
+            for (int r = 0; r < RL; ++r) seq[padf<LOGN, 1>(u + it * UPP + r * NSL)] = v[it * RL + r];
         __syncthreads();
         constexpr int STEPS = G::PAIRS * (N / 2);
 #pragma unroll 4
@@ -634,11 +641,11 @@ __global__ void __launch_bounds__(Geo<YP, LOGN>::THREADS, Geo<YP, LOGN>::MINB) f
             cplx c0, c1;
             double s1 = 1.0;
             if (BC == 2) {
-                c0 = z[pad(i)];
-                c1 = z[pad(i + 1)];
+                c0 = z[padf<LOGN, 1>(i)];
+                c1 = z[padf<LOGN, 1>(i + 1)];
             } else {
-                c0 = z[pad(i >> 1)];
-                c1 = z[pad(N - 1 - (i >> 1))];
+                c0 = z[padf<LOGN, 1>(i >> 1)];
+                c1 = z[padf<LOGN, 1>(N - 1 - (i >> 1))];
                 if (BC == 1) s1 = -1.0;
             }
             if (l < p.lines) *reinterpret_cast<double2 *>(p.out + ((size_t)l << LOGN) + i) = make_double2(c0.x, s1 * c1.x);
