@@ -24,7 +24,7 @@ import numpy as np
 
 NEUMANN = 0
 DIRICHLET = 1
-PERIODIC = 2      # x and y only; the paper's benchmark BCs are periodic x, Neumann y, z
+PERIODIC = 2      # any direction (z: cyclic sweep, A19); the paper's benchmark BCs are periodic x, Neumann y, z
 
 _M1 = np.uint64(0xBF58476D1CE4E5B9)
 _M2 = np.uint64(0x94D049BB133111EB)
