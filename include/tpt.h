@@ -46,7 +46,8 @@ enum {
     TPT_EINVAL = -1,   /* bad argument (sizes, faces, bc, alpha, null/misaligned pointer) */
     TPT_ENOMEM = -2,   /* host or device allocation failed */
     TPT_ECUDA = -3,    /* CUDA runtime error (no device, launch failure, ...) */
-    TPT_ENUMERIC = -4  /* plan-time eigen-solver did not reach its accuracy rule */
+    TPT_ENUMERIC = -4, /* plan-time eigen-solver did not reach its accuracy rule */
+    TPT_ELIMIT = -5    /* grid beyond the fixed capacity of tpt_solve_static_scratch (TPT_STATIC_SCRATCH_POINTS) */
 };
 
 /* Kernel slots, in execution order (used by tpt_plan_get_kernel_times / tpt_stage). */
@@ -118,6 +119,28 @@ int tpt_plan_create_ex(tpt_plan **plan_out, int nx, int ny, int nz,
  * A plan is not re-entrant (one workspace): order concurrent solves on one stream or use two plans.
  */
 int tpt_solve(tpt_plan *plan, const double *rhs_dev, double *out_dev, void *cuda_stream);
+
+/*
+ * tpt_solve_static_scratch — the same solve (steps 2.1–2.5 + the null-mode gauge) for callers
+ * that may not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  It is
+ * the one-launch cluster kernel of the small-grid path (TPT_PATH_FUSED_SMALL) with its mode-space scratch — the field
+ * between the two changes of ownership — in a file-scope static device array instead of the plan's workspace.  Nothing
+ * on this call path calls cudaMalloc, cudaFree, or any allocating routine (no events, no streams); the plan, created
+ * earlier, is only read.
+ *   rhs_dev / out_dev / cuda_stream: as tpt_solve (DEVICE, nx*ny*nz doubles each, 16-byte aligned, rhs_dev == out_dev
+ *   allowed); asynchronous.
+ * Limits: nx*ny*nz <= TPT_STATIC_SCRATCH_POINTS (16384 points: 128 KiB, held by every GPU that loads the library until
+ *   the process exits) — TPT_ELIMIT beyond it, nothing launched (also when the two transform matrices of a very flat
+ *   grid, nx*nx + ny*ny doubles, do not fit in shared memory beside the field).  The plan must diagonalise x and/or y with GEMM
+ *   transforms and have a non-periodic z (what that kernel computes): TPT_EINVAL otherwise.  The debug switches
+ *   tpt_plan_set_fused_small / _gemm_variant / _thomas_variant do not apply; profiling records nothing for it.
+ * Sharing: ALL calls on one GPU — any plan, any stream, any host thread — use the same array.  Calls that may overlap
+ *   on the GPU race on it: order them on one stream (or with events).  The array keeps the last call's contents; no
+ *   call depends on them (every element read is written earlier in the same launch), so there is nothing to clear.
+ * Result: the same kernel and arithmetic as tpt_solve on a plan that takes the small-grid path (bitwise equal to it).
+ */
+#define TPT_STATIC_SCRATCH_POINTS 16384
+int tpt_solve_static_scratch(tpt_plan *plan, const double *rhs_dev, double *out_dev, void *cuda_stream);
 
 /*
  * tpt_solve_batch — nrhs right-hand sides of the same plan in one call ("the resulting eigenvalues and forward/inverse

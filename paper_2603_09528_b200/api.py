@@ -29,7 +29,7 @@ KERNEL_NAMES = ("fwd_x", "fwd_y", "thomas", "inv_y", "inv_x")
 TRANSFORM_GEMM, TRANSFORM_FFT = 0, 1   # per diagonalised direction: eigenbasis GEMM / fast transform
 
 SYMBOLS = (
-    "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
+    "tpt_plan_create", "tpt_plan_create_dirs", "tpt_solve", "tpt_solve_static_scratch", "tpt_solve_batch", "tpt_plan_reserve_batch", "tpt_solve_host", "tpt_plan_destroy", "tpt_plan_get_eigen",
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_launches", "tpt_plan_set_slab_groups", "tpt_plan_set_fused_small", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
@@ -38,6 +38,8 @@ SYMBOLS = (
     "tpt_shard_ipc_import", "tpt_solve_sharded", "tpt_shard_solve_phase", "tpt_shard_barrier", "tpt_shard_barrier_all", "tpt_shard_launches", "tpt_shard_destroy",
 )
 IPC_HANDLE_BYTES = 64
+STATIC_SCRATCH_POINTS = 16384   # TPT_STATIC_SCRATCH_POINTS
+ELIMIT = -5                     # TPT_ELIMIT
 
 
 class ShardLayout(C.Structure):
@@ -71,6 +73,7 @@ def lib():
         L.tpt_plan_create_dirs.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i]
         L.tpt_plan_create_ex.argtypes = [C.POINTER(vp), i, i, i, _dp, _dp, _dp, C.POINTER(i), d, i, C.POINTER(i)]
         L.tpt_solve.argtypes = [vp, vp, vp, vp]
+        L.tpt_solve_static_scratch.argtypes = [vp, vp, vp, vp]
         L.tpt_solve_batch.argtypes = [vp, vp, vp, i, vp]
         L.tpt_plan_reserve_batch.argtypes = [vp, i]
         L.tpt_solve_host.argtypes = [vp, vp, vp, vp]
@@ -195,6 +198,13 @@ class Plan:
 
     def solve(self, rhs, out, stream=None):
         return solve(self, rhs, out, stream)
+
+    def solve_static_scratch(self, rhs, out, stream=None):
+        """tpt_solve_static_scratch: the one-launch solve with its scratch in a static device array (no allocation);
+        grids of at most STATIC_SCRATCH_POINTS points."""
+        _check(lib().tpt_solve_static_scratch(self._h, _dev_ptr(rhs, self.points, "rhs"), _dev_ptr(out, self.points, "out"),
+                                              _stream_handle(stream)), "tpt_solve_static_scratch")
+        return out
 
     def solve_host(self, rhs_host, out_host, stream=None):
         return solve_host(self, rhs_host, out_host, stream)

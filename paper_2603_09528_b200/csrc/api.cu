@@ -679,6 +679,25 @@ int tpt_solve(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_st
     return TPT_OK;
 }
 
+// The one-launch solve of fused_small.cu with its scratch in a static device array: no allocation on this call path
+// (no cudaMalloc / cudaFree / event or stream creation; the plan's workspace and profiling events are not touched).
+int tpt_solve_static_scratch(tpt_plan *p, const double *rhs_dev, double *out_dev, void *cuda_stream) {
+    if (!p || !rhs_dev || !out_dev || !aligned16(rhs_dev) || !aligned16(out_dev) || !on_plan_device(p)) return TPT_EINVAL;
+    if (p->points() > (size_t)TPT_STATIC_SCRATCH_POINTS) return TPT_ELIMIT;
+    // what the fused kernel computes: GEMM transforms in at least one direction, tridiagonal (non-periodic) z
+    if (p->cyclic || !(p->dirs & 3)) return TPT_EINVAL;
+    if (((p->dirs & 1) && p->transform[0] != TPT_TRANSFORM_GEMM) || ((p->dirs & 2) && p->transform[1] != TPT_TRANSFORM_GEMM)) return TPT_EINVAL;
+    if (!tpt::fused_small_supported(p->nx, p->ny, p->nz)) return TPT_ELIMIT;
+    tpt::FusedSmallArgs a{};
+    a.rhs = rhs_dev; a.out = out_dev; a.work = nullptr;
+    a.xfwd = p->d_xfwd; a.xinv = p->d_xinv; a.yfwd = p->d_yfwd; a.yinv = p->d_yinv;
+    a.az = p->d_az; a.bz = p->d_bz; a.cz = p->d_cz; a.wz = p->d_wz; a.lamx = p->d_lamx; a.lamy = p->d_lamy;
+    a.nx = p->nx; a.ny = p->ny; a.nz = p->nz; a.dirs = p->dirs; a.singular = p->singular; a.shift0 = p->shift0;
+    if (tpt::launch_fused_small_static(a, static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) { cudaGetLastError(); return TPT_ECUDA; }
+    p->launches_last = 1;
+    return TPT_OK;
+}
+
 int tpt_plan_reserve_batch(tpt_plan *p, int nrhs) {
     if (!p || nrhs < 1 || (double)nrhs * (double)p->points() > 8.0e9 || !on_plan_device(p)) return TPT_EINVAL;
     if (nrhs <= p->work_fields) return TPT_OK;
@@ -1030,6 +1049,7 @@ const char *tpt_strerror(int status) {
         case TPT_ENOMEM: return "out of memory";
         case TPT_ECUDA: return "CUDA error (no sm_100 device, or a runtime/launch failure)";
         case TPT_ENUMERIC: return "plan-time eigen-decomposition missed its accuracy rule";
+        case TPT_ELIMIT: return "grid larger than the fixed capacity of a no-allocation entry point (TPT_STATIC_SCRATCH_POINTS)";
         default: return "unknown status";
     }
 }

@@ -12,6 +12,8 @@
 // FP64 tensor path (same 128 flop/clk/SM peak as DFMA on sm_100) would buy nothing.
 #include <cuda_runtime.h>
 
+#include <mutex>
+
 #include "devonce.hpp"
 #include "kernels.cuh"
 
@@ -360,6 +362,40 @@ cudaError_t launch_fused_small(const FusedSmallArgs &a, cudaStream_t stream) {
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return full ? cudaLaunchKernelEx(&cfg, fused_small_kernel<true>, p) : cudaLaunchKernelEx(&cfg, fused_small_kernel<false>, p);
+}
+
+// ---- the same launch with its mode-space scratch in a static device array (tpt_solve_static_scratch, tpt.h) ---------
+// For callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): nothing on
+// this call path calls cudaMalloc, cudaFree or an allocating library routine.  Every GPU that loads the library holds
+// the array (STATIC_SCRATCH_POINTS * 8 bytes = 128 KiB) until exit.  All calls on a device share it: calls that overlap
+// on the GPU (two streams, two host threads) race on it.  It keeps the last call's contents, which is harmless here:
+// every element the sweep reads was written by the same launch (each CTA stores its own z-planes before the first
+// cluster barrier, together all nx ny nz points), so nothing has to start at zero.
+static __device__ __align__(256) double static_scratch[STATIC_SCRATCH_POINTS];
+
+cudaError_t launch_fused_small_static(const FusedSmallArgs &a, cudaStream_t stream) {
+    if (a.nx < 1 || a.ny < 1 || a.nz < 1 || (size_t)a.nx * a.ny * a.nz > STATIC_SCRATCH_POINTS) return cudaErrorInvalidValue;
+    // In host code `static_scratch` is a host-side stand-in, not a device address: the address a kernel may use comes from
+    // cudaGetSymbolAddress, per device (every device has its own instance), with that device current.
+    static std::mutex m;
+    static double *addr[64] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    double *ptr = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(m);
+        if (dev >= 0 && dev < 64) ptr = addr[dev];
+        if (!ptr) {
+            e = cudaGetSymbolAddress(reinterpret_cast<void **>(&ptr), static_scratch);
+            if (e != cudaSuccess) return e;
+            if (!ptr) return cudaErrorInvalidSymbol;
+            if (dev >= 0 && dev < 64) addr[dev] = ptr;
+        }
+    }
+    FusedSmallArgs b = a;
+    b.work = ptr;
+    return launch_fused_small(b, stream);
 }
 
 }  // namespace tpt

@@ -107,6 +107,10 @@ struct FusedSmallArgs {
 };
 bool fused_small_supported(int nx, int ny, int nz);
 cudaError_t launch_fused_small(const FusedSmallArgs &a, cudaStream_t stream);
+// The same launch with `work` replaced by a static device array of STATIC_SCRATCH_POINTS doubles (a.work is ignored): no
+// allocation on the call path.  cudaErrorInvalidValue beyond that size.  Calls that overlap on one GPU race on the array.
+constexpr size_t STATIC_SCRATCH_POINTS = 16384;   // = TPT_STATIC_SCRATCH_POINTS (tpt.h)
+cudaError_t launch_fused_small_static(const FusedSmallArgs &a, cudaStream_t stream);
 
 // Null-mode gauge: subtract the dz-weighted mean of column (0,0) (zero volume-weighted mean); `stride` = distance
 // between consecutive z levels of that column (nx*ny in the natural layout, 16 in the tile-blocked one).
