@@ -47,7 +47,12 @@ struct StorePeers {
     int group0;                   // index of this rank's first 16-column group in the peers' (global) group numbering
 };
 
-template <int M, int TCOLS, int MAXT, int MINB, bool SH>
+// Coefficient tables: stored [t][segment] for the launch's partition (thomas_onchip_tables).  In row order a warp's two
+// 16-byte loads per row touched one 128-byte line per segment — 4 to 8 LSU wavefronts each, 40 % of the kernel's LSU
+// data-pipe wavefronts at 512 rows, the busiest unit (76 %, ncu) — now one line per load.  TS: the regular table is also
+// copied to shared memory once per CTA and read from there (where it fits beside the tile ring): 1-2 wavefronts per
+// load and no L1 misses.
+template <int M, int TCOLS, int MAXT, int MINB, bool SH, bool TS>
 __global__ void __launch_bounds__(MAXT, MINB)
 thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
                      const __grid_constant__ typename std::conditional<SH, StorePeers, StoreOne>::type dst,
@@ -56,10 +61,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
                      const double *__restrict__ lamy, const double *__restrict__ wz, int nx, int nz, int S, int nbuf,
                      int box_rows, int nbox, int buf_rows, double shift0, int singular, int ntiles) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const size_t tile_elems = (size_t)buf_rows * TCOLS;             // buf_rows = max(S*M, nbox*box_rows) >= nz
+    const size_t tile_elems = (size_t)buf_rows * TCOLS;             // buf_rows = nbox*box_rows >= nz (may be < S*M: see `live`)
     double *bufs = reinterpret_cast<double *>(smem_raw);            // nbuf x tile_elems
     double *scratch = bufs + (size_t)nbuf * tile_elems;             // 2 sets x 3 x S x 16
     uint64_t *full = reinterpret_cast<uint64_t *>(scratch + 6 * S * TCOLS);
+    double2 *stab = reinterpret_cast<double2 *>(reinterpret_cast<unsigned char *>(full) + 128);   // TS: 2 * S*M entries
 
     const int tid = threadIdx.x;
     constexpr int ROW_BYTES = TCOLS * (int)sizeof(double);
@@ -77,10 +83,9 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         for (int b = 0; b < nbuf; ++b) ptx::mbar_init(&full[b], 1);
         ptx::fence_mbar_init();
     }
-    // rows the TMA boxes never reach (past nbox*box_rows) must read as zero: identity rows with p = 0
-    for (int b = 0; b < nbuf; ++b)
-        for (int e = nbox * box_rows * TCOLS + tid; e < (int)tile_elems; e += blockDim.x)
-            bufs[(size_t)b * tile_elems + e] = 0.0;
+    if constexpr (TS) {           // plan data, not the previous kernel's output: copied before the dependency wait
+        for (int e = tid; e < 2 * S * M; e += blockDim.x) stab[e] = __ldg(reinterpret_cast<const double2 *>(tab_reg) + e);
+    }
     ptx::pdl_launch_dependents();
     __syncthreads();
     ptx::pdl_wait();              // the tiles are the previous kernel's output
@@ -98,6 +103,9 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
     for (int p = 0; p < nbuf - 1 && p < n_my; ++p) issue_load(first + p * (int)gridDim.x, p);
 
     const int k0 = seg * M;
+    // rows of my segment that exist in the tile buffer; the rest of the S*M rows (past nbox*box_rows) are decoupled
+    // identity rows of the padded table with p = 0: they read as zero and are never written
+    const int live = buf_rows - k0;
     const int me = seg * TCOLS + col;
     const int STR = S * TCOLS;
     double *const set0 = scratch, *const set1 = scratch + 3 * STR;
@@ -117,7 +125,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         if (it + 1 < n_my) s_next = shift_of(tile + (int)gridDim.x);
         // the null column of a singular plan reads a table whose last row is "-x = p", and zeroes p
         const bool null_col = singular && gcol == 0;
-        const double2 *tab = reinterpret_cast<const double2 *>(null_col ? tab_null : tab_reg) + 2 * k0;
+        // Global tables are stored [t][segment] for this launch's partition (thomas_onchip_tables): row k0 + t of segment
+        // `seg` at (t S + seg) 32 bytes, so the segments of a warp read one 128-byte line per load, not one line each.
+        const double2 *tab = reinterpret_cast<const double2 *>(null_col ? tab_null : tab_reg) + 2 * seg;
+        // the tile that holds the null column reads the tables from global memory (block-uniform choice)
+        const bool tab_in_smem = TS && !(singular && tile == 0);
 
         ptx::bulk_wait_read<0>();              // (thread 0) the previous tile's store has left shared memory
         ptx::mbar_wait(&full[b], parity);
@@ -126,26 +138,30 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         // ---- 1. cold forward elimination of rows k0 .. k0+M-1 ------------------------------------
         double cp[M], g[M];
         double pi = 1.0, DD = 0.0, GG = 0.0, dprev = 0.0, rprev = 0.0;
+        auto forward = [&](const double2 *tb, const int stride, auto load) {
 #pragma unroll
-        for (int t = 0; t < M; ++t) {
-            const double2 t0 = __ldg(tab + 2 * t);         // { a_k c_{k-1}, b_k }
-            const double2 t1 = __ldg(tab + 2 * t + 1);     // { a_k, c_k }
-            const double p = buf[t * TCOLS];
-            const double bb = t0.y + s;
-            const double den = t == 0 ? bb : fma(-t0.x, rprev, bb);
-            const double r = ptx::fast_rcp3(den);
-            cp[t] = t1.y * r;
-            const double d = (t == 0 ? p : fma(-t1.x, dprev, p)) * r;
-            g[t] = (t == 0 ? t1.x : -t1.x * g[t - 1]) * r;
-            buf[t * TCOLS] = d;
-            if (t < M - 1) {
-                DD = fma(pi, d, DD);
-                GG = fma(pi, g[t], GG);
-                pi = -pi * cp[t];
+            for (int t = 0; t < M; ++t) {
+                const double2 t0 = load(tb + stride * t);           // { a_k c_{k-1}, b_k }
+                const double2 t1 = load(tb + stride * t + 1);       // { a_k, c_k }
+                const double p = t < live ? buf[t * TCOLS] : 0.0;
+                const double bb = t0.y + s;
+                const double den = t == 0 ? bb : fma(-t0.x, rprev, bb);
+                const double r = ptx::fast_rcp3(den);
+                cp[t] = t1.y * r;
+                const double d = (t == 0 ? p : fma(-t1.x, dprev, p)) * r;
+                g[t] = (t == 0 ? t1.x : -t1.x * g[t - 1]) * r;
+                if (t < live) buf[t * TCOLS] = d;
+                if (t < M - 1) {
+                    DD = fma(pi, d, DD);
+                    GG = fma(pi, g[t], GG);
+                    pi = -pi * cp[t];
+                }
+                dprev = d;
+                rprev = r;
             }
-            dprev = d;
-            rprev = r;
-        }
+        };
+        if (tab_in_smem) forward(stab + 2 * seg, 2 * S, [](const double2 *q) { return *q; });
+        else forward(tab, 2 * S, [](const double2 *q) { return __ldg(q); });
         // ---- 2. reduced system for the last unknown X of each segment ------------------------------
         //   g_last X_{s-1} + (1 - c'_last GG_{s+1}) X_s + (c'_last PI_{s+1}) X_{s+1} = d_last - c'_last DD_{s+1}
         set0[me] = DD;
@@ -208,11 +224,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         const double xl = seg > 0 ? wr[me - TCOLS] : 0.0;
         // ---- 3. back substitution -------------------------------------------------------------------
         double xk = D;
-        buf[(M - 1) * TCOLS] = xk;
+        if (M - 1 < live) buf[(M - 1) * TCOLS] = xk;
 #pragma unroll
         for (int t = M - 2; t >= 0; --t) {
-            xk = fma(-cp[t], xk, fma(-g[t], xl, buf[t * TCOLS]));
-            buf[t * TCOLS] = xk;
+            xk = fma(-cp[t], xk, fma(-g[t], xl, t < live ? buf[t * TCOLS] : 0.0));
+            if (t < live) buf[t * TCOLS] = xk;
         }
         // ---- null-mode gauge (A7), fused: the tile that holds column (0,0) of a singular
         // plan subtracts the dz-weighted mean of that column before it leaves the chip (block-uniform branch)
@@ -279,40 +295,49 @@ bool make_field_map(CUtensorMap *map, const double *x, size_t plane, int nz, int
 
 constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_CTA_RESERVED = 1024, SMEM_CTA_MAX = 227 * 1024;
 
+// A launch shape: M rows per segment, TC columns per tile, at most MAXT threads per CTA, CTAS co-resident CTAs per SM
+// (their barrier phases interleave), TS: regular coefficient table in shared memory.
+struct Shape {
+    int M, TC, MAXT, CTAS;
+    bool TS;
+};
+
 // Launch geometry shared by the plain and the sharded launch.
 struct ThomasGeom {
     int S, nbox, box_rows, buf_rows, nbuf, threads;
     size_t smem;
 };
-template <int M, int TC, int MAXT, int CTAS>
-bool thomas_geometry(int nz, ThomasGeom &g) {
-    constexpr int ROW_BYTES = TC * (int)sizeof(double);
-    int S = (nz + M - 1) / M;
-    while ((S * TC) % 32) ++S;                               // whole warps
+bool thomas_geometry(const Shape &sh, int nz, ThomasGeom &g) {
+    const int row_bytes = sh.TC * (int)sizeof(double);
+    int S = (nz + sh.M - 1) / sh.M;
+    while ((S * sh.TC) % 32) ++S;                            // whole warps
+    if (S * sh.M > nz + THOMAS_TABLE_PAD) return false;      // the tables hold nz + THOMAS_TABLE_PAD rows
     const int nbox = (nz + 255) / 256;                       // TMA boxes are at most 256 rows tall
     int box_rows = (nz + nbox - 1) / nbox;
-    if ((box_rows * ROW_BYTES) % 128) ++box_rows;            // TMA wants 128-byte aligned shared-memory boxes
-    const int buf_rows = S * M > nbox * box_rows ? S * M : nbox * box_rows;
-    const size_t tile_bytes = (size_t)buf_rows * ROW_BYTES;
-    const size_t fixed = (size_t)6 * S * TC * sizeof(double) + 64;
-    size_t budget = SMEM_PER_SM / CTAS - SMEM_CTA_RESERVED;
+    const int rows_128 = row_bytes >= 128 ? 1 : 128 / row_bytes;
+    box_rows = (box_rows + rows_128 - 1) / rows_128 * rows_128;   // TMA wants 128-byte aligned shared-memory boxes
+    const int buf_rows = nbox * box_rows;                    // >= nz; segments may reach past it (kernel: `live`)
+    const size_t tile_bytes = (size_t)buf_rows * row_bytes;
+    const size_t fixed = (size_t)6 * S * sh.TC * sizeof(double) + 128 + (sh.TS ? (size_t)S * sh.M * 32 : 0);
+    size_t budget = SMEM_PER_SM / sh.CTAS - SMEM_CTA_RESERVED;
     if (budget > SMEM_CTA_MAX) budget = SMEM_CTA_MAX;
+    if (budget < fixed + 2 * tile_bytes) return false;
     int nbuf = (int)((budget - fixed) / tile_bytes);
     if (nbuf > 3) nbuf = 3;
-    if (nbuf < 2 || TC * S > MAXT) return false;
-    g = {S, nbox, box_rows, buf_rows, nbuf, TC * S, (size_t)nbuf * tile_bytes + fixed};
+    if (sh.TC * S > sh.MAXT) return false;
+    g = {S, nbox, box_rows, buf_rows, nbuf, sh.TC * S, (size_t)nbuf * tile_bytes + fixed};
     return true;
 }
 
-// M rows per segment, TC columns per tile, CTAS co-resident CTAs per SM (their barrier phases interleave).
 // `cols` = number of (kx,ky) columns of the field at `in` (nx*ny, or the rows a rank owns times nx).
 // peers == nullptr: plain solve into the field x (same layout as `in`); else the sharded store of StorePeers.
-template <int M, int TC, int MAXT, int CTAS, bool SH>
-cudaError_t launch_m(const double *in, double *x, const ThomasPeers *peers, const double *tab, const double *lamx, const double *lamy,
+// tab: the tables of thomas_onchip_tables; part = 0 / 1: the partition (blocked / natural launch shape) this launch is.
+template <int M, int TC, int MAXT, int CTAS, bool SH, bool TS>
+cudaError_t launch_m(const double *in, double *x, const ThomasPeers *peers, const double *tab, int part, const double *lamx, const double *lamy,
                      const double *wz, int nx, size_t cols, int nz, double shift0, int singular, bool blocked, int sms, cudaStream_t stream) {
     ThomasGeom g;
-    if (!thomas_geometry<M, TC, MAXT, CTAS>(nz, g)) return cudaErrorInvalidConfiguration;
-    auto kern = thomas_onchip_kernel<M, TC, MAXT, CTAS, SH>;
+    if (!thomas_geometry(Shape{M, TC, MAXT, CTAS, TS}, nz, g)) return cudaErrorInvalidConfiguration;
+    auto kern = thomas_onchip_kernel<M, TC, MAXT, CTAS, SH, TS>;
     static DeviceOnce configured;                            // per device, thread-safe (devonce.hpp)
     static OccupancyCache occupancy;
     cudaError_t e = configured.run([&] { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CTA_MAX); });
@@ -326,7 +351,9 @@ cudaError_t launch_m(const double *in, double *x, const ThomasPeers *peers, cons
     const int ntiles = (int)(cols / TC);
     int grid = sms * per_sm;
     if (grid > ntiles) grid = ntiles;
-    const double *tab_null = tab + 4 * ((size_t)nz + THOMAS_TABLE_PAD);
+    const size_t tab_block = 4 * ((size_t)nz + THOMAS_TABLE_PAD);
+    tab += (size_t)(2 * part) * tab_block;                   // this partition's [t][segment] tables: regular, null
+    const double *tab_null = tab + tab_block;
     if constexpr (SH) {
         StorePeers dst{};
         dst.npeers = peers->npeers;
@@ -361,55 +388,89 @@ bool thomas_onchip_supported(int nx, int ny, int nz) {
 }
 
 namespace {
-template <bool SH>
-cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, const double *tab, const double *lamx, const double *lamy,
-                     const double *wz, int nx, size_t cols, int nz, double shift0, int singular, bool blocked, bool blocked_shape,
-                     int sms, cudaStream_t stream) {
-#define TPT_GO(M, TC, MAXT, CTAS) \
-    launch_m<M, TC, MAXT, CTAS, SH>(in, x, peers, tab, lamx, lamy, wz, nx, cols, nz, shift0, singular, blocked, sms, stream)
-    // Measured on the box (profiles/r1c_*.md): the sweep is bound by the FP64 + shared-memory pipes of the 16 warps the
-    // register file admits per SM, so the shapes differ only in how well the phases of co-resident CTAs interleave.
+
+// The launch shape for columns of nz rows.  blocked_any: the field is tile-blocked, or a natural-layout launch asks for
+// the same partition (tpt_solve_host, whose results equal tpt_solve's bit for bit).  allow4: 4-column tiles permitted.
+// Measured on the box (profiles/): the sweep is bound by the LSU data pipe and the dependent FP64 chains of the 16 warps
+// the register file admits per SM, so the shapes differ in wavefronts per row and in how well the phases of
+// co-resident CTAs interleave.
+Shape choose_shape(int nz, bool blocked_any, bool allow4) {
     // Short columns on the blocked layout: the 17-row / 8-column shape also wins below 257 rows wherever its segments fill
     // the column (at most 10 % padding rows: 64, 128, 192 rows — 512 x 512 columns x 128 rows: 0.139 -> 0.107 ms);
     // otherwise the 8- / 16-row shapes below (160, 224, 256 rows: measured equal or better)
-    if ((blocked || blocked_shape) && nz <= 204) {
+    if (blocked_any && nz <= 204) {
         const int S = ((nz + 16) / 17 + 3) / 4 * 4;
-        if (S * 17 * 10 <= 11 * nz) return TPT_GO(17, 8, 256, 2);
+        if (S * 17 * 10 <= 11 * nz) return {17, 8, 256, 2, false};
     }
-    if (nz <= 128) return TPT_GO(8, 16, 256, 2);
-    if (nz <= 256) return TPT_GO(16, 16, 256, 2);
-    // 257 .. 800 rows on the blocked layout: 8-column tiles, odd segment length (rows of the two segments of a half-warp
-    // then fall into opposite 64-byte halves of the banks: conflict-free), two CTAs per SM, at most 32 segments (a multiple
-    // of 4: whole warps).  `blocked_shape` asks for the same partition — hence the same rounding — on a natural-layout field
-    // (tpt_solve_host, whose results equal tpt_solve's bit for bit).  Segment length: the shortest of 17 / 19 / 21 / 23 / 25
-    // rows that covers the column (768^3: 0.709 -> 0.667 ms against one 384-thread CTA of 32-row segments), unless another
-    // one leaves at least 3 % fewer padded rows — the padding is pure waste (416 rows: 0.400 -> 0.362 ms with 21-row
-    // segments, 288 rows: 0.262 -> 0.240 ms with 25).
-    if ((blocked || blocked_shape) && nz <= 800) {
+    if (nz <= 128) return {8, 16, 256, 2, false};
+    if (nz <= 256) return {16, 16, 256, 2, false};
+    // 257 .. 800 rows on the blocked layout: narrow tiles, odd segment length (the segments of a warp then fall into
+    // different banks: conflict-free), several CTAs per SM, at most 32 segments.  Segment length: the shortest of 17 / 19 /
+    // 21 / 23 / 25 rows that covers the column (768^3: 0.709 -> 0.667 ms against one 384-thread CTA of 32-row segments),
+    // unless another one leaves at least 3 % fewer padded rows — the padding is pure waste (416 rows: 0.400 -> 0.362 ms
+    // with 21-row segments, 288 rows: 0.262 -> 0.240 ms with 25).
+    if (blocked_any && nz <= 800) {
         int defM = 17;
         while (defM * 32 < nz) defM += 2;
         auto rows_of = [&](int M) { return ((nz + M - 1) / M + 3) / 4 * 4 * M; };
         int bestM = defM, bestRows = rows_of(defM);
         for (int M = defM + 2; M <= 25; M += 2)
             if (rows_of(M) * 100 < bestRows * 97 || (bestM != defM && rows_of(M) <= bestRows)) { bestRows = rows_of(M); bestM = M; }
-        switch (bestM) {
-            case 17: return TPT_GO(17, 8, 256, 2);
-            case 19: return TPT_GO(19, 8, 256, 2);
-            case 21: return TPT_GO(21, 8, 256, 2);
-            case 23: return TPT_GO(23, 8, 256, 2);
-            default: return TPT_GO(25, 8, 256, 2);
+        ThomasGeom g;
+        // 4-column tiles, four CTAs of 4 warps per SM (same segments, so the same arithmetic): smaller barrier domains and
+        // twice as many independent tile rings — where the segment count is a multiple of 8 anyway (no extra padding)
+        // and M <= 19 (measured, interleaved runs at 512 x 512 columns: 384 / 448 rows 7-8 % faster, 512 rows 4 %, 608 rows
+        // 3.5 %, 576 rows equal; 21-row segments — 640, 672 rows — equal or slower).
+        // The coefficient table goes to shared memory where it fits beside two tile buffers and the CTAs fill the register
+        // file anyway (512 threads per SM; below that a smaller footprint lets more CTAs in: 320 rows 0.29 vs 0.35 ms):
+        // 512 rows with 4-column tiles 0.440 vs 0.454 ms, with 8-column tiles 0.458 vs 0.476 ms.
+        const int segs = (nz + bestM - 1) / bestM;
+        const int S8 = (segs + 3) / 4 * 4;
+        const bool ts_ok = S8 * 16 >= 512;
+        if (allow4 && bestM <= 19 && S8 == (segs + 7) / 8 * 8) {
+            Shape s4{bestM, 4, 128, 4, ts_ok};
+            if (thomas_geometry(s4, nz, g)) return s4;
+            s4.TS = false;
+            if (thomas_geometry(s4, nz, g)) return s4;
         }
+        Shape s8{bestM, 8, 256, 2, ts_ok};
+        if (thomas_geometry(s8, nz, g)) return s8;
+        s8.TS = false;
+        return s8;
     }
-    if (nz <= 512) return TPT_GO(16, 16, 512, 1);
-    if (nz <= 768) return TPT_GO(32, 16, 384, 1);
+    if (nz <= 512) return {16, 16, 512, 1, false};
+    if (nz <= 768) return {32, 16, 384, 1, false};
     // up to 1056 rows: 8-column tiles of 17-row segments, 512 threads (16 warps), two 68 KB buffers, one CTA per SM
     // (33-row segments with 256 threads and 242 registers: 4.25 instead of 3.69 ms at 1024^3)
     // 801 .. 1008 rows: 21-row segments (at most 48 per column, 384 threads) — measured 0.84 / 0.86 / 1.05 / 1.05 ms at
     // 840 / 900 / 960 / 992 rows against 0.94 / 1.07 / 1.10 / 1.11 ms with 17-row segments (512 x 512 columns); from 1009
     // rows on the 17-row, 64-segment shape wins (1024 rows: 0.97 vs 1.18 ms)
-    if (nz <= 1008) return TPT_GO(21, 8, 416, 1);
-    return TPT_GO(17, 8, 512, 1);
-#undef TPT_GO
+    if (nz <= 1008) return {21, 8, 416, 1, false};
+    return {17, 8, 512, 1, false};
+}
+
+template <bool SH>
+cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, const double *tab, const double *lamx, const double *lamy,
+                     const double *wz, int nx, size_t cols, int nz, double shift0, int singular, bool blocked, bool blocked_shape,
+                     int sms, cudaStream_t stream) {
+    const bool blocked_any = blocked || blocked_shape;
+    // the sharded store cuts tiles at the z-slab boundaries (even numbers): 4-column rows would lose their 128-byte alignment
+    const Shape sh = choose_shape(nz, blocked_any, !SH);
+    const int part = blocked_any ? 0 : 1;
+#define TPT_TRY(M_, TC_, MAXT_, CTAS_, TS_)                                                                                    \
+    if (sh.M == M_ && sh.TC == TC_ && sh.MAXT == MAXT_ && sh.CTAS == CTAS_ && sh.TS == TS_)                                    \
+        return launch_m<M_, TC_, MAXT_, CTAS_, SH, TS_>(in, x, peers, tab, part, lamx, lamy, wz, nx, cols, nz, shift0, singular, \
+                                                        blocked, sms, stream);
+    TPT_TRY(17, 8, 256, 2, false) TPT_TRY(19, 8, 256, 2, false) TPT_TRY(21, 8, 256, 2, false) TPT_TRY(23, 8, 256, 2, false)
+    TPT_TRY(25, 8, 256, 2, false)
+    TPT_TRY(17, 8, 256, 2, true) TPT_TRY(19, 8, 256, 2, true) TPT_TRY(21, 8, 256, 2, true)   // 23, 25: never fits
+    if constexpr (!SH) {
+        TPT_TRY(17, 4, 128, 4, true) TPT_TRY(19, 4, 128, 4, true) TPT_TRY(17, 4, 128, 4, false) TPT_TRY(19, 4, 128, 4, false)
+    }
+    TPT_TRY(8, 16, 256, 2, false) TPT_TRY(16, 16, 256, 2, false) TPT_TRY(16, 16, 512, 1, false) TPT_TRY(32, 16, 384, 1, false)
+    TPT_TRY(21, 8, 416, 1, false) TPT_TRY(17, 8, 512, 1, false)
+#undef TPT_TRY
+    return cudaErrorInvalidConfiguration;
 }
 }  // namespace
 
@@ -429,12 +490,14 @@ cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &pe
 
 // Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows
 // [0, -1, 0, 0] (pivot -1 + s < 0 for every mode since s <= 0); the second table is the null column's, with the
-// last equation replaced by "-x = p" (the kernel zeroes p there): PAPER.md:219.
+// last equation replaced by "-x = p" (the kernel zeroes p there): PAPER.md:219.  Both are stored once per partition the
+// launches of this nz can have (0: blocked layout / blocked_shape, 1: natural layout), in the order the kernel reads
+// them: row t of segment seg — row seg M + t of the column — at (t S + seg) * 4.  Four blocks of 4 (nz + THOMAS_TABLE_PAD).
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out, const double *b_null) {
     const size_t rows = (size_t)nz + THOMAS_TABLE_PAD;
-    out.assign(8 * rows, 0.0);
+    std::vector<double> nat(8 * rows, 0.0);
     for (int v = 0; v < 2; ++v) {
-        double *t = out.data() + (size_t)v * 4 * rows;
+        double *t = nat.data() + (size_t)v * 4 * rows;
         for (size_t k = 0; k < rows; ++k) t[4 * k + 1] = -1.0;
         for (int k = 0; k < nz; ++k) {
             t[4 * k] = k > 0 ? a[k] * c[k - 1] : 0.0;
@@ -445,6 +508,19 @@ void thomas_onchip_tables(int nz, const double *a, const double *b, const double
         if (v == 1) {
             double *last = t + 4 * (size_t)(nz - 1);
             last[0] = 0.0; last[1] = -1.0; last[2] = 0.0; last[3] = 0.0;
+        }
+    }
+    out.assign(16 * rows, 0.0);
+    for (int part = 0; part < 2; ++part) {
+        const Shape sh = choose_shape(nz, part == 0, true);    // 4- and 8-column shapes of one nz share M and S
+        ThomasGeom g;
+        if (!thomas_geometry(sh, nz, g)) continue;
+        for (int v = 0; v < 2; ++v) {
+            const double *src = nat.data() + (size_t)v * 4 * rows;
+            double *dst = out.data() + (size_t)(2 * part + v) * 4 * rows;
+            for (int seg = 0; seg < g.S; ++seg)
+                for (int t = 0; t < sh.M; ++t)
+                    for (int j = 0; j < 4; ++j) dst[((size_t)t * g.S + seg) * 4 + j] = src[((size_t)seg * sh.M + t) * 4 + j];
         }
     }
 }
