@@ -69,7 +69,7 @@ cudaError_t launch_cyclic_correct(double *x, const double *q, const double *rden
 // Same solve with the z-columns resident on chip (thomas_onchip.cu): 16 B/pt of HBM traffic, no scratch field.
 // Reads the right-hand sides from `in` and writes the solution to `x` (in == x: in place).
 // tab: device copy of the tables thomas_onchip_tables() builds (16 * (nz + THOMAS_TABLE_PAD) doubles: regular and null-column
-// table for each of the two partitions — blocked / natural launch shape — in the kernel's [row of segment][segment] order).
+// table for each of the two partitions — blocked / natural launch shape — in the kernel's order: groups of 4 segments, row-interleaved).
 // sms = SM count.
 constexpr int THOMAS_TABLE_PAD = 160;   // >= the rows by which S*M can exceed nz in any launch shape
 bool thomas_onchip_supported(int nx, int ny, int nz);

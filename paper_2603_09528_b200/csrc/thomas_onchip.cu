@@ -47,7 +47,7 @@ struct StorePeers {
     int group0;                   // index of this rank's first 16-column group in the peers' (global) group numbering
 };
 
-// Coefficient tables: stored [t][segment] for the launch's partition (thomas_onchip_tables).  In row order a warp's two
+// Coefficient tables: stored [group of 4 segments][t][segment] for the launch's partition (thomas_onchip_tables).  In row order a warp's two
 // 16-byte loads per row touched one 128-byte line per segment — 4 to 8 LSU wavefronts each, 40 % of the kernel's LSU
 // data-pipe wavefronts at 512 rows, the busiest unit (76 %, ncu) — now one line per load.  TS: the regular table is also
 // copied to shared memory once per CTA and read from there (where it fits beside the tile ring): 1-2 wavefronts per
@@ -61,7 +61,8 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
                      const double *__restrict__ lamy, const double *__restrict__ wz, int nx, int nz, int S, int nbuf,
                      int box_rows, int nbox, int buf_rows, double shift0, int singular, int ntiles) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const size_t tile_elems = (size_t)buf_rows * TCOLS;             // buf_rows = nbox*box_rows >= nz (may be < S*M: see `live`)
+    const size_t tile_elems = (size_t)buf_rows * TCOLS;             // buf_rows >= nbox*box_rows >= nz; PRED: may be < S*M
+    constexpr bool PRED = MINB > 1;                                 // thomas_geometry: which shapes keep fewer than S*M rows
     double *bufs = reinterpret_cast<double *>(smem_raw);            // nbuf x tile_elems
     double *scratch = bufs + (size_t)nbuf * tile_elems;             // 2 sets x 3 x S x 16
     uint64_t *full = reinterpret_cast<uint64_t *>(scratch + 6 * S * TCOLS);
@@ -83,8 +84,12 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         for (int b = 0; b < nbuf; ++b) ptx::mbar_init(&full[b], 1);
         ptx::fence_mbar_init();
     }
+    if constexpr (!PRED) {        // rows the TMA boxes never reach (past nbox*box_rows) read as zero: identity rows with p = 0
+        for (int b = 0; b < nbuf; ++b)
+            for (int e = nbox * box_rows * TCOLS + tid; e < (int)tile_elems; e += blockDim.x) bufs[(size_t)b * tile_elems + e] = 0.0;
+    }
     if constexpr (TS) {           // plan data, not the previous kernel's output: copied before the dependency wait
-        for (int e = tid; e < 2 * S * M; e += blockDim.x) stab[e] = __ldg(reinterpret_cast<const double2 *>(tab_reg) + e);
+        for (int e = tid; e < 2 * ((S + 3) & ~3) * M; e += blockDim.x) stab[e] = __ldg(reinterpret_cast<const double2 *>(tab_reg) + e);
     }
     ptx::pdl_launch_dependents();
     __syncthreads();
@@ -105,7 +110,7 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
     const int k0 = seg * M;
     // rows of my segment that exist in the tile buffer; the rest of the S*M rows (past nbox*box_rows) are decoupled
     // identity rows of the padded table with p = 0: they read as zero and are never written
-    const int live = buf_rows - k0;
+    const int live = PRED ? buf_rows - k0 : M;
     const int me = seg * TCOLS + col;
     const int STR = S * TCOLS;
     double *const set0 = scratch, *const set1 = scratch + 3 * STR;
@@ -125,9 +130,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         if (it + 1 < n_my) s_next = shift_of(tile + (int)gridDim.x);
         // the null column of a singular plan reads a table whose last row is "-x = p", and zeroes p
         const bool null_col = singular && gcol == 0;
-        // Global tables are stored [t][segment] for this launch's partition (thomas_onchip_tables): row k0 + t of segment
-        // `seg` at (t S + seg) 32 bytes, so the segments of a warp read one 128-byte line per load, not one line each.
-        const double2 *tab = reinterpret_cast<const double2 *>(null_col ? tab_null : tab_reg) + 2 * seg;
+        // Global tables of this launch's partition (thomas_onchip_tables), stored [group of 4 segments][t][segment of the
+        // group]: row k0 + t of segment `seg` at (((seg / 4) M + t) 4 + seg % 4) 32 bytes.  The (4 or 8) segments of a warp
+        // then read one or two 128-byte lines per load, not one line each, at compile-time offsets (128 t bytes).
+        const int tab_off = 2 * (((seg >> 2) * M) * 4 + (seg & 3));
+        const double2 *tab = reinterpret_cast<const double2 *>(null_col ? tab_null : tab_reg) + tab_off;
         // the tile that holds the null column reads the tables from global memory (block-uniform choice)
         const bool tab_in_smem = TS && !(singular && tile == 0);
 
@@ -138,11 +145,11 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
         // ---- 1. cold forward elimination of rows k0 .. k0+M-1 ------------------------------------
         double cp[M], g[M];
         double pi = 1.0, DD = 0.0, GG = 0.0, dprev = 0.0, rprev = 0.0;
-        auto forward = [&](const double2 *tb, const int stride, auto load) {
+        auto forward = [&](const double2 *tb, auto load) {
 #pragma unroll
             for (int t = 0; t < M; ++t) {
-                const double2 t0 = load(tb + stride * t);           // { a_k c_{k-1}, b_k }
-                const double2 t1 = load(tb + stride * t + 1);       // { a_k, c_k }
+                const double2 t0 = load(tb + 8 * t);                // { a_k c_{k-1}, b_k }
+                const double2 t1 = load(tb + 8 * t + 1);            // { a_k, c_k }
                 const double p = t < live ? buf[t * TCOLS] : 0.0;
                 const double bb = t0.y + s;
                 const double den = t == 0 ? bb : fma(-t0.x, rprev, bb);
@@ -160,8 +167,8 @@ thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
                 rprev = r;
             }
         };
-        if (tab_in_smem) forward(stab + 2 * seg, 2 * S, [](const double2 *q) { return *q; });
-        else forward(tab, 2 * S, [](const double2 *q) { return __ldg(q); });
+        if (tab_in_smem) forward(stab + tab_off, [](const double2 *q) { return *q; });
+        else forward(tab, [](const double2 *q) { return __ldg(q); });
         // ---- 2. reduced system for the last unknown X of each segment ------------------------------
         //   g_last X_{s-1} + (1 - c'_last GG_{s+1}) X_s + (c'_last PI_{s+1}) X_{s+1} = d_last - c'_last DD_{s+1}
         set0[me] = DD;
@@ -311,19 +318,27 @@ bool thomas_geometry(const Shape &sh, int nz, ThomasGeom &g) {
     const int row_bytes = sh.TC * (int)sizeof(double);
     int S = (nz + sh.M - 1) / sh.M;
     while ((S * sh.TC) % 32) ++S;                            // whole warps
-    if (S * sh.M > nz + THOMAS_TABLE_PAD) return false;      // the tables hold nz + THOMAS_TABLE_PAD rows
+    const int S4 = (S + 3) / 4 * 4;                          // the tables hold whole groups of 4 segments,
+    if (S4 * sh.M > nz + THOMAS_TABLE_PAD) return false;     // nz + THOMAS_TABLE_PAD rows in all
     const int nbox = (nz + 255) / 256;                       // TMA boxes are at most 256 rows tall
     int box_rows = (nz + nbox - 1) / nbox;
     const int rows_128 = row_bytes >= 128 ? 1 : 128 / row_bytes;
     box_rows = (box_rows + rows_128 - 1) / rows_128 * rows_128;   // TMA wants 128-byte aligned shared-memory boxes
-    const int buf_rows = nbox * box_rows;                    // >= nz; segments may reach past it (kernel: `live`)
+    // Shapes with several CTAs per SM keep only the rows the TMA boxes fill (>= nz): their segments may reach past the
+    // buffer (kernel: `live`), which buys a third ring slot or the coefficient table in shared memory.  One-CTA shapes
+    // have the room for all S*M rows and skip the predicates (their 16 warps run phase 1 together: issue-bound there;
+    // 1024 rows: 1.00 -> 0.92 ms per 512 x 512 columns).
+    const int buf_rows = (sh.CTAS > 1 || S * sh.M < nbox * box_rows) ? nbox * box_rows : S * sh.M;
     const size_t tile_bytes = (size_t)buf_rows * row_bytes;
-    const size_t fixed = (size_t)6 * S * sh.TC * sizeof(double) + 128 + (sh.TS ? (size_t)S * sh.M * 32 : 0);
+    const size_t fixed = (size_t)6 * S * sh.TC * sizeof(double) + 128 + (sh.TS ? (size_t)S4 * sh.M * 32 : 0);
     size_t budget = SMEM_PER_SM / sh.CTAS - SMEM_CTA_RESERVED;
     if (budget > SMEM_CTA_MAX) budget = SMEM_CTA_MAX;
     if (budget < fixed + 2 * tile_bytes) return false;
     int nbuf = (int)((budget - fixed) / tile_bytes);
     if (nbuf > 3) nbuf = 3;
+    // one-CTA shapes: a third ring slot would take the shared-memory carve-out to its maximum and leave the L1 too small for
+    // the coefficient table (up to 35 KB) — measured equal at 840 / 900 rows, 7 % slower at 960 / 1008 rows
+    if (sh.CTAS == 1 && nbuf > 2) nbuf = 2;
     if (sh.TC * S > sh.MAXT) return false;
     g = {S, nbox, box_rows, buf_rows, nbuf, sh.TC * S, (size_t)nbuf * tile_bytes + fixed};
     return true;
@@ -352,7 +367,7 @@ cudaError_t launch_m(const double *in, double *x, const ThomasPeers *peers, cons
     int grid = sms * per_sm;
     if (grid > ntiles) grid = ntiles;
     const size_t tab_block = 4 * ((size_t)nz + THOMAS_TABLE_PAD);
-    tab += (size_t)(2 * part) * tab_block;                   // this partition's [t][segment] tables: regular, null
+    tab += (size_t)(2 * part) * tab_block;                   // this partition's tables: regular, null
     const double *tab_null = tab + tab_block;
     if constexpr (SH) {
         StorePeers dst{};
@@ -492,7 +507,8 @@ cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &pe
 // [0, -1, 0, 0] (pivot -1 + s < 0 for every mode since s <= 0); the second table is the null column's, with the
 // last equation replaced by "-x = p" (the kernel zeroes p there): PAPER.md:219.  Both are stored once per partition the
 // launches of this nz can have (0: blocked layout / blocked_shape, 1: natural layout), in the order the kernel reads
-// them: row t of segment seg — row seg M + t of the column — at (t S + seg) * 4.  Four blocks of 4 (nz + THOMAS_TABLE_PAD).
+// them: row t of segment seg — row seg M + t of the column — at (((seg / 4) M + t) 4 + seg % 4) * 4 (groups of 4 segments,
+// row-interleaved).  Four blocks of 4 (nz + THOMAS_TABLE_PAD) doubles.
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out, const double *b_null) {
     const size_t rows = (size_t)nz + THOMAS_TABLE_PAD;
     std::vector<double> nat(8 * rows, 0.0);
@@ -520,7 +536,8 @@ void thomas_onchip_tables(int nz, const double *a, const double *b, const double
             double *dst = out.data() + (size_t)(2 * part + v) * 4 * rows;
             for (int seg = 0; seg < g.S; ++seg)
                 for (int t = 0; t < sh.M; ++t)
-                    for (int j = 0; j < 4; ++j) dst[((size_t)t * g.S + seg) * 4 + j] = src[((size_t)seg * sh.M + t) * 4 + j];
+                    for (int j = 0; j < 4; ++j)
+                        dst[(((size_t)(seg >> 2) * sh.M + t) * 4 + (seg & 3)) * 4 + j] = src[((size_t)seg * sh.M + t) * 4 + j];
         }
     }
 }
