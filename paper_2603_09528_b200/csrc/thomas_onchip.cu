@@ -480,7 +480,7 @@ cudaError_t dispatch(const double *in, double *x, const ThomasPeers *peers, cons
     TPT_TRY(25, 8, 256, 2, false)
     TPT_TRY(17, 8, 256, 2, true) TPT_TRY(19, 8, 256, 2, true) TPT_TRY(21, 8, 256, 2, true)   // 23, 25: never fits
     if constexpr (!SH) {
-        TPT_TRY(17, 4, 128, 4, true) TPT_TRY(19, 4, 128, 4, true) TPT_TRY(17, 4, 128, 4, false) TPT_TRY(19, 4, 128, 4, false)
+        TPT_TRY(17, 4, 128, 4, true) TPT_TRY(17, 4, 128, 4, false) TPT_TRY(19, 4, 128, 4, false)   // 19 rows: the table never fits
     }
     TPT_TRY(8, 16, 256, 2, false) TPT_TRY(16, 16, 256, 2, false) TPT_TRY(16, 16, 512, 1, false) TPT_TRY(32, 16, 384, 1, false)
     TPT_TRY(21, 8, 416, 1, false) TPT_TRY(17, 8, 512, 1, false)

@@ -41,15 +41,22 @@ def _solve(torch, plan, f):
     return d_o.cpu().numpy()
 
 
-# nz picks the sweep's launch shape: <=128: 8-row segments; <=256: 16 rows, two CTAs per SM; 257..544 (blocked):
-# 8-column tiles with 17-row segments; 545..800 (blocked): the same shape with 19 / 21 / 23 / 25-row segments; 801..1008: 21-row
-# segments, one CTA per SM; 1009..1056: 17-row segments and 512 threads.  Ragged nz exercises the zero-filled tail rows.
+# nz picks the sweep's launch shape (thomas_onchip.cu, choose_shape): <=128: 8-row segments; <=256: 16 rows, two CTAs per SM;
+# 257..800 (blocked): 17 / 19 / 21 / 23 / 25-row segments in 8-column tiles (two CTAs) or — 17 and 19 rows, segment count a
+# multiple of 8 — 4-column tiles (four CTAs), with the coefficient table in shared memory where it fits; 801..1008: 21-row
+# segments, one CTA per SM; 1009..1056: 17-row segments and 512 threads.  Ragged nz exercises the predicated / zero-filled
+# tail rows.
 SHAPES = [
     ("nz24", (128, 128, 24), (N_, N_, D_), 0.0),
     ("nz130", (128, 256, 130), (N_, N_, D_), 0.0),
     ("nz256", (256, 128, 256), (N_, D_, N_), 0.0),
     ("nz300", (128, 128, 300), (N_, N_, D_), 2e-3),
+    ("nz384", (128, 128, 384), (N_, N_, D_), 0.0),              # 4-column tiles, 24 segments: table through L1
+    ("nz500-singular", (128, 128, 500), (N_, N_, N_), 0.0),     # 4-column tiles, table in shared memory; null column from global
+    ("nz512", (256, 128, 512), (N_, D_, D_), 1e-3),             # the bench shape (c3, c4)
     ("nz513-singular", (128, 128, 513), (N_, N_, N_), 0.0),
+    ("nz576", (128, 128, 576), (D_, N_, N_), 0.0),              # 19-row segments, 4-column tiles
+    ("nz616", (128, 128, 616), (N_, N_, D_), 0.0),              # 21-row segments, 8-column tiles, table in shared memory
     ("nz544", (128, 128, 544), (D_, N_, D_), 0.0),
     ("nz545", (128, 128, 545), (N_, N_, D_), 0.0),
     ("nz608", (128, 128, 608), (N_, N_, D_), 1e-3),

@@ -64,6 +64,8 @@ CASES = [
     ("p4-sing", (256, 256, 130), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, 4),        # second sweep shape (nz > 128)
     ("p8", (128, 128, 66), (1.0, 2.0, 1.0), (2.0, 2.0, 2.5), (D_, N_, D_), 0.0, 8),              # one 16-row unit per rank
     ("p8-sing-tall", (128, 256, 300), (1.0, 1.0, 1.0), (2.0, 2.0, 3.0), (N_, N_, N_), 0.0, 8),
+    ("p4-512", (128, 128, 512), (1.0, 1.0, 1.0), (2.0, 2.0, 2.5), (N_, N_, D_), 0.0, 4),        # 8-column tiles with the table in shared memory
+    ("p2-576-sing", (128, 128, 576), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, 2),   # 19-row segments
     ("p5-periodic", (128, 128, 21), (1.0, 1.0, 1.0), (0.0, 2.0, 2.0), (PER_, N_, D_), 0.0, 5),  # ragged: 21 planes, 5 ranks
     ("p1", (128, 128, 16), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, D_), 0.0, 1),
 ]
