@@ -299,6 +299,13 @@ int tpt_plan_get_eigen(const tpt_plan *plan, int dir, double *lambda_host, doubl
 int tpt_host_eigen(int n, const double *faces_host, int bc, int base_kind, double *lambda_host, double *qtilde_host);
 int tpt_debug_set_eigen_base(int base_kind);
 
+/* Launch geometry of the on-chip z sweep (step 2.3) for columns of nz rows, on the HOST (no device needed;
+ * test only): blocked != 0: the tile-blocked mode-space layout (or a launch that asks for its partition), sharded != 0:
+ * the sharded store (needs blocked).  out12 (HOST, 12 ints) = { rows per segment M, columns per tile, thread limit, CTAs per
+ * SM, coefficient table in shared memory (0/1), segments S, TMA boxes per tile, rows per box, rows per tile buffer, ring
+ * slots, threads per CTA, dynamic shared memory bytes }.  TPT_EINVAL: nz outside 2..1056, no shape, or a null pointer. */
+int tpt_debug_sweep_geometry(int nz, int blocked, int sharded, int *out12);
+
 /* 1 if the plan is singular (all-Neumann Poisson), 0 if not, < 0 on error. */
 int tpt_plan_is_singular(const tpt_plan *plan);
 

@@ -33,7 +33,7 @@ SYMBOLS = (
     "tpt_plan_is_singular", "tpt_plan_device_bytes", "tpt_stage", "tpt_plan_set_profiling",
     "tpt_plan_get_kernel_times", "tpt_plan_get_paths", "tpt_plan_launches", "tpt_plan_set_slab_groups", "tpt_plan_set_fused_small", "tpt_plan_set_gemm_variant", "tpt_plan_set_thomas_variant", "tpt_fp64_peak", "tpt_strerror", "tpt_version",
     "tpt_divergence", "tpt_gradient_correct", "tpt_project", "tpt_plan_create_ex", "tpt_solve_host_async", "tpt_plan_wait",
-    "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_fill_uniform",
+    "tpt_host_eigen", "tpt_debug_set_eigen_base", "tpt_debug_sweep_geometry", "tpt_fill_uniform",
     "tpt_shard_layout", "tpt_shard_create", "tpt_shard_create_ex", "tpt_shard_get_layout", "tpt_shard_sym", "tpt_shard_set_peers", "tpt_shard_ipc_export",
     "tpt_shard_ipc_import", "tpt_solve_sharded", "tpt_shard_solve_phase", "tpt_shard_barrier", "tpt_shard_barrier_all", "tpt_shard_launches", "tpt_shard_destroy",
 )
@@ -87,6 +87,7 @@ def lib():
         L.tpt_plan_is_singular.argtypes = [vp]
         L.tpt_host_eigen.argtypes = [i, _dp, i, i, _dp, _dp]
         L.tpt_debug_set_eigen_base.argtypes = [i]
+        L.tpt_debug_sweep_geometry.argtypes = [i, i, i, C.POINTER(i)]
         L.tpt_plan_device_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
         L.tpt_stage.argtypes = [vp, i, vp, vp, vp]
         L.tpt_plan_set_profiling.argtypes = [vp, i]
@@ -489,6 +490,18 @@ def host_eigen(faces, bc: int, base_kind: int = 0):
     lam, q = np.empty(n), np.empty((n, n))
     _check(lib().tpt_host_eigen(n, fp, int(bc), int(base_kind), lam.ctypes.data_as(_dp), q.ctypes.data_as(_dp)), "tpt_host_eigen")
     return lam, q
+
+
+SWEEP_GEOMETRY_KEYS = ("M", "cols", "max_threads", "ctas_per_sm", "table_in_smem", "S", "nbox", "box_rows", "buf_rows", "nbuf",
+                       "threads", "smem")
+
+
+def debug_sweep_geometry(nz: int, blocked: bool, sharded: bool = False):
+    """tpt_debug_sweep_geometry as a dict (SWEEP_GEOMETRY_KEYS), or None where the on-chip sweep has no shape.  Host only."""
+    out = (C.c_int * 12)()
+    if lib().tpt_debug_sweep_geometry(int(nz), int(bool(blocked)), int(bool(sharded)), out) != 0:
+        return None
+    return dict(zip(SWEEP_GEOMETRY_KEYS, [int(v) for v in out]))
 
 
 def debug_set_eigen_base(base_kind: int):

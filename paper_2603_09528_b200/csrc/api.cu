@@ -914,6 +914,11 @@ int tpt_host_eigen(int n, const double *faces, int bc, int base_kind, double *la
     return TPT_OK;
 }
 
+int tpt_debug_sweep_geometry(int nz, int blocked, int sharded, int *out12) {
+    if (!out12 || (sharded && !blocked)) return TPT_EINVAL;
+    return tpt::thomas_onchip_geometry(nz, blocked != 0, sharded != 0, out12) ? TPT_OK : TPT_EINVAL;
+}
+
 int tpt_debug_set_eigen_base(int base_kind) {
     if (base_kind != 0 && base_kind != 1) return TPT_EINVAL;
     g_eigen_base = base_kind;

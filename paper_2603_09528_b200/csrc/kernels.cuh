@@ -76,6 +76,7 @@ bool thomas_onchip_supported(int nx, int ny, int nz);
 // b_null: diagonal of the null column's table when it differs from b (cyclic sweep: unmodified corners); nullptr = b.
 void thomas_onchip_tables(int nz, const double *a, const double *b, const double *c, std::vector<double> &out,
                           const double *b_null = nullptr);
+bool thomas_onchip_geometry(int nz, bool blocked_any, bool sharded, int out[12]);   // launch shape of an nz (thomas_onchip.cu)
 // wz: the nz cell widths of the z direction — on a singular plan the kernel itself removes the dz-weighted mean of the
 // null column (0,0) before the tile leaves the chip (A7): no separate gauge launch.
 cudaError_t launch_thomas_onchip(const double *in, double *x, const double *tab, const double *lamx, const double *lamy, const double *wz,

@@ -503,6 +503,19 @@ cudaError_t launch_thomas_onchip_sharded(const double *in, const ThomasPeers &pe
     return dispatch<true>(in, nullptr, &peers, tab, lamx, lamy_owned, wz, nx, (size_t)nx * rows, nz, shift0, singular, true, false, sms, stream);
 }
 
+// The launch geometry dispatch() would use, for inspection (tests sweep every nz): out = { M, columns per tile, thread limit,
+// CTAs per SM, table in shared memory, S, TMA boxes per tile, rows per box, rows per tile buffer, ring slots, threads, dynamic
+// shared memory bytes }.  false: this nz has no on-chip shape in that layout.
+bool thomas_onchip_geometry(int nz, bool blocked_any, bool sharded, int out[12]) {
+    if (nz < 2 || nz > 1056) return false;
+    const Shape sh = choose_shape(nz, blocked_any, !sharded);
+    ThomasGeom g;
+    if (!thomas_geometry(sh, nz, g)) return false;
+    const int v[12] = {sh.M, sh.TC, sh.MAXT, sh.CTAS, sh.TS ? 1 : 0, g.S, g.nbox, g.box_rows, g.buf_rows, g.nbuf, g.threads, (int)g.smem};
+    for (int i = 0; i < 12; ++i) out[i] = v[i];
+    return true;
+}
+
 // Host side of the coefficient tables: rows [a_k c_{k-1}, b_k, a_k, c_k], padded with decoupled rows
 // [0, -1, 0, 0] (pivot -1 + s < 0 for every mode since s <= 0); the second table is the null column's, with the
 // last equation replaced by "-x = p" (the kernel zeroes p there): PAPER.md:219.  Both are stored once per partition the

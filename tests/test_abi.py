@@ -35,7 +35,7 @@ def test_header_cites_the_paper_for_each_entry_point():
 
 def test_status_strings(tpt):
     assert tpt.strerror(0) == "ok"
-    for s in (-1, -2, -3, -4):
+    for s in (-1, -2, -3, -4, -5):
         assert tpt.strerror(s) not in ("ok", "unknown status")
     assert tpt.strerror(-99) == "unknown status"
 
