@@ -1,11 +1,11 @@
 // thomas_onchip.cu — step 2.3 (Eq. 11 at PAPER.md:161–163) with the whole z-column resident on chip:
 // every point of the field is read from HBM once and written once (16 B/pt, the algorithmic minimum).
 //
-// A CTA owns tiles of 16 (or 8) neighbouring (kx,ky) columns x nz rows, staged in shared memory by tiled TMA
-// (boxes of up to 256 rows of 128 or 64 bytes) through an NBUF-deep ring, so the load of the next tile and the
+// A CTA owns tiles of 16 (or 8, or 4) neighbouring (kx,ky) columns x nz rows, staged in shared memory by tiled TMA
+// (boxes of up to 256 rows of 128, 64 or 32 bytes) through an NBUF-deep ring, so the load of the next tile and the
 // store of the previous one overlap the arithmetic of the current one (persistent CTAs).  The field may be in the
 // natural layout (rows nx*ny apart) or in the tile-blocked mode-space layout of kernels.cuh, where a 16-column tile
-// is one dense block of nz*128 bytes; the tensor map hides the difference.  Launch shapes: launch_thomas_onchip.
+// is one dense block of nz*128 bytes; the tensor map hides the difference.  Launch shapes: choose_shape.
 // (Row-by-row 1-D bulk copies were measured first: the TMA unit then sustains only ~1 copy / 17 cycles per SM,
 // 2.2 TB/s chip-wide — hence the tensor map.)
 //
@@ -47,11 +47,10 @@ struct StorePeers {
     int group0;                   // index of this rank's first 16-column group in the peers' (global) group numbering
 };
 
-// Coefficient tables: stored [group of 4 segments][t][segment] for the launch's partition (thomas_onchip_tables).  In row order a warp's two
-// 16-byte loads per row touched one 128-byte line per segment — 4 to 8 LSU wavefronts each, 40 % of the kernel's LSU
-// data-pipe wavefronts at 512 rows, the busiest unit (76 %, ncu) — now one line per load.  TS: the regular table is also
-// copied to shared memory once per CTA and read from there (where it fits beside the tile ring): 1-2 wavefronts per
-// load and no L1 misses.
+// Coefficient tables: stored [group of 4 segments][t][segment] for the launch's partition (thomas_onchip_tables).  In row
+// order a warp's two 16-byte loads per row touched one 128-byte line per segment: 36 M sectors per launch at 512^3, 40 %
+// of the kernel's LSU data-pipe wavefronts — the busiest unit (76 %, ncu); now one or two lines per load.  TS: the
+// regular table is also copied to shared memory once per CTA and read from there (where it fits beside the tile ring).
 template <int M, int TCOLS, int MAXT, int MINB, bool SH, bool TS>
 __global__ void __launch_bounds__(MAXT, MINB)
 thomas_onchip_kernel(const __grid_constant__ CUtensorMap tmap,
