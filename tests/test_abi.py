@@ -74,6 +74,9 @@ def test_argument_validation_needs_no_gpu(tpt):
     assert L.tpt_project(None, None, None, None, 1.0, None, None, 0.0, 7, None) == -1
     assert L.tpt_divergence(None, None, None, None, 1.0, None, None) == -1
     assert L.tpt_solve(None, None, None, None) == -1
+    assert L.tpt_solve_static_scratch(None, None, None, None) == -1
+    assert tpt.STATIC_SCRATCH_POINTS == 16384 and "#define TPT_STATIC_SCRATCH_POINTS 16384" in open(os.path.join(ROOT, "include", "tpt.h")).read()
+    assert L.tpt_debug_sweep_geometry(512, 1, 0, None) == -1
     assert L.tpt_plan_destroy(None) == 0
     assert L.tpt_plan_is_singular(None) == -1
 
