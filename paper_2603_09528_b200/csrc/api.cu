@@ -930,6 +930,7 @@ int tpt_plan_device_bytes(const tpt_plan *p, size_t *bytes_out) {
     size_t b = 2 * ((size_t)p->nx * p->nx + (size_t)p->ny * p->ny) * sizeof(double);
     b += ((size_t)p->nx + p->ny + 4 * (size_t)p->nz + 8) * sizeof(double);
     b += (2 * ((size_t)p->nx + p->ny + p->nz) + 16) * sizeof(double);                       // staggered-grid geometry
+    if (p->d_abc) b += 16 * ((size_t)p->nz + tpt::THOMAS_TABLE_PAD) * sizeof(double);       // sweep tables (thomas_onchip_tables)
     for (int d = 0; d < 2; ++d)
         if (p->d_fft[d]) b += (size_t)8 * (d == 0 ? p->nx : p->ny) * sizeof(double);        // twiddle tables (upper bound)
     b += p->points() * sizeof(double) * ((size_t)p->work_fields + (p->d_stage ? 1 : 0));
