@@ -137,6 +137,9 @@ int tpt_solve(tpt_plan *plan, const double *rhs_dev, double *out_dev, void *cuda
  * Sharing: ALL calls on one GPU — any plan, any stream, any host thread — use the same array.  Calls that may overlap
  *   on the GPU race on it: order them on one stream (or with events).  The array keeps the last call's contents; no
  *   call depends on them (every element read is written earlier in the same launch), so there is nothing to clear.
+ * First call on a device: resolves the array's device address (cudaGetSymbolAddress) and sets the kernel's dynamic
+ *   shared-memory attribute, once, thread-safe; neither allocates, but both are set-up calls — a caller that captures
+ *   a CUDA graph makes one call before the capture starts.
  * Result: the same kernel and arithmetic as tpt_solve on a plan that takes the small-grid path (bitwise equal to it).
  */
 #define TPT_STATIC_SCRATCH_POINTS 16384
