@@ -252,6 +252,38 @@ def test_residual_at_roundoff_on_baseline_configs(orc, cfg):
     assert r["rel2"] < 2e-13                                                        # expected level (SURVEY c.6)
 
 
+def test_residual_norms_special_cases(orc):
+    # orc_residual_norms pinned by cases with a closed form: phi = 0 (residual = f: every relative norm is exactly 1);
+    # f = 0 with phi a unit vector (residual = minus one column of the operator — the diagonal b_x + b_y + b_z of that cell and
+    # six neighbour coefficients — whose largest entry the backward error divides by the sum of the 1-D absolute row sums);
+    # invariance under a common scaling of f and phi.
+    P = I.Problem("norms", (7, 5, 6), (1.0, 2.0, 1.5), (2.0, 1.0, 2.5), (N_, D_, N_), 0.0, 3)
+    xf, yf, zf = P.faces()
+    f = I.uniform_pm1(11, P.points).reshape(6, 5, 7)
+    zero = np.zeros_like(f)
+    r = orc.residual_norms(xf, yf, zf, P.bc, 0.0, f, zero)
+    assert r["rel2"] == 1.0 and r["relL2vol"] == 1.0 and r["relmax"] == 1.0 and r["backward"] == 1.0
+    ops = [orc.operator_1d(g, b) for g, b in zip((xf, yf, zf), P.bc)]          # (w, a, b, c) per direction
+    rowsum = sum(float(np.max(np.abs(a) + np.abs(b) + np.abs(c))) for (_, a, b, c) in ops)
+    i, j, k = 3, 2, 4
+    e = zero.copy(); e[k, j, i] = 1.0
+    # column (i, j, k) of the operator: the diagonal and, per direction, c of the row before and a of the row after
+    col = [abs(ops[0][2][i] + ops[1][2][j] + ops[2][2][k])]
+    for (_, a, b, c), m in zip(ops, (i, j, k)):
+        col += [abs(c[m - 1]), abs(a[m + 1])]
+    tiny = np.full_like(f, 1e-300)                                             # f = 0 would divide by zero in the relative norms
+    r = orc.residual_norms(xf, yf, zf, P.bc, 0.0, tiny, e)
+    assert abs(r["backward"] - max(col) / rowsum) <= 1e-12 * max(col) / rowsum
+    assert 0.0 < r["backward"] < 1.0
+    # a genuine solution: backward error at round-off, never above the max-norm residual; both scale-invariant
+    phi = orc.OraclePlan(xf, yf, zf, P.bc, 0.0).solve(f)
+    r1 = orc.residual_norms(xf, yf, zf, P.bc, 0.0, f, phi)
+    r2 = orc.residual_norms(xf, yf, zf, P.bc, 0.0, 8.0 * f, 8.0 * phi)
+    assert r1["backward"] <= r1["relmax"] < 1e-12 and r1["backward"] < 1e-15
+    for key in r1:                                                             # (the OpenMP reductions may reorder the sums)
+        assert abs(r1[key] - r2[key]) <= 1e-12 * r1[key], key
+
+
 def test_residual_singular_stretched(orc):
     P = I.Problem("t", (64, 48, 56), (1.0, 1.0, 1.0), (2.0, 2.0, 2.0), (N_, N_, N_), 0.0, 2)
     xf, yf, zf = P.faces()
