@@ -75,3 +75,24 @@ def test_known_shapes(tpt):
     assert (g["M"], g["cols"], g["ctas_per_sm"]) == (16, 16, 1)
     assert tpt.debug_sweep_geometry(1, True) is None and tpt.debug_sweep_geometry(1057, True) is None
     assert tpt.lib().tpt_debug_sweep_geometry(512, 0, 1, (__import__("ctypes").c_int * 12)()) == -1   # sharded needs blocked
+
+
+def test_every_shape_the_dispatcher_can_choose_is_instantiated(tpt):
+    # dispatch() matches the chosen shape against a list of template instantiations (TPT_TRY in thomas_onchip.cu) and fails
+    # with cudaErrorInvalidConfiguration on a miss: every reachable (M, columns, thread limit, CTAs, table in shared memory)
+    # must be in that list — for the sharded store, outside the `if constexpr (!SH)` block of 4-column shapes
+    import os
+    import re
+
+    src = open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2603_09528_b200", "csrc",
+                            "thomas_onchip.cu")).read()
+    body = src[src.index("#define TPT_TRY"):src.index("#undef TPT_TRY")]
+    listed = {(int(m), int(tc), int(mt), int(c), ts == "true")
+              for m, tc, mt, c, ts in re.findall(r"TPT_TRY\((\d+), (\d+), (\d+), (\d+), (true|false)\)", body)}
+    assert len(listed) >= 15
+    plain_only = {s for s in listed if s[1] == 4}
+    for nz, blocked, sharded, g in _all(tpt):
+        shape = (g["M"], g["cols"], g["max_threads"], g["ctas_per_sm"], bool(g["table_in_smem"]))
+        assert shape in listed, (nz, blocked, sharded, shape)
+        if sharded:
+            assert shape not in plain_only, (nz, shape)
